@@ -1,0 +1,189 @@
+/*
+ * tddp4.h -- C-ABI boundary of the B200-native time-dependent four-body amplitude likelihood.
+ *
+ * What it computes: the per-event time-dependent D0 -> K+ pi- pi+ pi- decay rate of arXiv:1702.06735
+ * eq. (1) with the two amplitudes A_f, Abar_f modelled as coherent sums of
+ * quasi-two-body decay chains, eq. (2), its Monte-Carlo normalisation over a
+ * phase-space sample, the negative log-likelihood handed to a host-side minimiser
+ * (PAPER.md lines 14, 18, 95), and the companion pseudo-event generator (phase-space generation followed
+ * by accept/reject against the same rate).  Formulas the paper does not print
+ * (spin factors, lineshapes, barrier factors, time integrals, Raubold-Lynch generation, Philox streams)
+ * follow the readings O-1 .. O-9 of SURVEY.md 8(c), restated in DESIGN.md.
+ *
+ * Conventions
+ *   - Units GeV and ps.  Metric (+,-,-,-).  Four-vectors are (E, px, py, pz).
+ *   - Final-state order: 0 = K+, 1 = pi-, 2 = pi+, 3 = pi-.
+ *   - Event layout is SoA fp64: p4[(4*particle + component) * ld + event], ld = row stride in doubles.
+ *   - Every function returns TDDP4_OK (0) or a negative tddp4_status; no exception crosses the boundary;
+ *     tddp4_last_error() gives a text for the last failure of that handle.
+ *   - "host" / "device" on a pointer says where the memory must live.  The caller owns every buffer it
+ *     passes; the handle owns only its internal caches.  Device buffers must belong to the CUDA device
+ *     that was current at tddp4_create().
+ *   - All work is enqueued on the handle's stream (tddp4_set_stream; default: a private non-blocking
+ *     stream).  Calls that return a value to the host synchronise that stream; *_async calls do not.
+ *   - A handle is not thread-safe; use one per host thread.
+ *   - There is no CPU fallback: without a usable CUDA device tddp4_create() fails with TDDP4_ERR_CUDA.
+ */
+#ifndef TDDP4_H
+#define TDDP4_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct tddp4 tddp4; /* opaque handle */
+
+typedef enum {
+  TDDP4_OK = 0,
+  TDDP4_ERR_ARG = -1,       /* bad argument / model description                                  */
+  TDDP4_ERR_CUDA = -2,      /* CUDA runtime error (text in tddp4_last_error)                     */
+  TDDP4_ERR_CAPACITY = -3,  /* generate: more accepted events than `capacity` (counts are exact) */
+  TDDP4_ERR_DOMAIN = -4,    /* a resonance pole mass is below its own decay threshold            */
+  TDDP4_ERR_NONFINITE = -5, /* some P_i <= 0 or non-finite: *nll_out = +inf                       */
+  TDDP4_ERR_STATE = -6      /* call order: events or parameters missing                          */
+} tddp4_status;
+
+/* limits of one model */
+#define TDDP4_MAX_RES 16
+#define TDDP4_MAX_TERMS 32
+#define TDDP4_MAX_COUPLINGS 16
+
+/* Spin-factor kinds.  The two topologies of PAPER.md Fig. 2 (lines 40-44):
+ *   VV_*   : D -> R1 R2, R1 -> (perm[0] perm[1]), R2 -> (perm[2] perm[3]);   res = {R1, R2}
+ *   AP_S   : D -> X perm[3], X -> V perm[2] (S-wave), V -> (perm[0] perm[1]); res = {X, V}, X axial
+ *   TP_D   : same cascade, X a tensor, both X vertices in D-wave;            res = {X, V}
+ *   NONRES : constant amplitude 1;                                           res = {-1, -1}          */
+enum {
+  TDDP4_SF_NONRES = 0, TDDP4_SF_VV_S = 1, TDDP4_SF_VV_P = 2, TDDP4_SF_VV_D = 3,
+  TDDP4_SF_AP_S = 4, TDDP4_SF_TP_D = 5
+};
+
+typedef struct {
+  int L; /* orbital angular momentum of the resonance's own decay: exponent 2L+1 of the running width
+            and order of its Blatt-Weisskopf factor (O-5, O-6).  m0, Gamma0 come via tddp4_set_params. */
+} tddp4_res;
+
+typedef struct {
+  int spin_factor; /* TDDP4_SF_*                                                       */
+  int res[2];      /* resonance indices, see above; -1 = none                          */
+  int perm[4];     /* role -> final-state index; a permutation of 0..3                 */
+  int coupling;    /* kappa(k): which complex coupling multiplies this chain, eq. (2); *
+                    * Bose-symmetrised orderings share one coupling  */
+} tddp4_term;
+
+typedef struct {
+  double m_parent;     /* nominal D0 mass; used by the generator only (event kinematics use p^2)     */
+  double m_final[4];
+  double r_res;        /* Blatt-Weisskopf radius of resonance vertices, GeV^-1                       */
+  double r_parent;     /* ... of the D0 vertex                                                       */
+  int n_res;
+  const tddp4_res *res;    /* host [n_res]                                                           */
+  int n_terms;
+  const tddp4_term *terms; /* host [n_terms]                                                         */
+  int n_couplings;         /* K_c                                                                    */
+  double t_lo, t_hi;       /* decay-time window of the normalisation; t_hi = +INFINITY allowed       */
+  int use_resolution;      /* 0: eq. (1) as printed; 1: per-event Gaussian sigma_t   */
+} tddp4_model_desc;
+
+/* ---- life cycle -------------------------------------------------------------------------------- */
+/* Builds a handle on the current CUDA device from a host-side description (copied).  Recurring
+ * lineshapes are de-duplicated into "instances" ("substituted by a link to a single
+ * instance").                                                                                        */
+int tddp4_create(const tddp4_model_desc *desc, tddp4 **out);
+int tddp4_destroy(tddp4 *h);
+/* cuda_stream: a cudaStream_t (0 = legacy default stream).  The handle does not own it.              */
+int tddp4_set_stream(tddp4 *h, void *cuda_stream);
+const char *tddp4_last_error(const tddp4 *h);
+const char *tddp4_version(void);
+
+/* ---- step 0/1: event store, kinematics + spin factors, once per event set ------------------------ */
+/* which: 0 = data sample, 1 = normalisation sample.  p4: [16][ld] SoA as above (ld >= n); t: decay
+ * times [n] (data; may be NULL for the normalisation sample); sigma_t: per-event resolution [n] or
+ * NULL; weight: normalisation weights w_j [n] or NULL (= 1).  on_device = 0: host pointers, copied
+ * with cudaMemcpyAsync; 1: device pointers, read once.  The call builds the parameter-independent
+ * caches (invariant masses, lineshape shape functions, spin x barrier factors) and does not keep p4. */
+int tddp4_load_events(tddp4 *h, int which, int64_t n, int64_t ld, const double *p4, const double *t,
+                      const double *sigma_t, const double *weight, int on_device);
+
+/* ---- per minimiser call -------------------------------------------------------------------------- */
+/* c, cbar: host [K_c][2] (re, im) couplings of A_f and Abar_f (eq. 2); mass_width: host [n_res][2]
+ * (m0, Gamma0); x, y mixing parameters, tau lifetime in ps (Gamma = 1/tau) of eq. (1).  Compares with
+ * the previous values to find which lineshape instances, hence which coupling columns, are dirty.    */
+int tddp4_set_params(tddp4 *h, const double *c, const double *cbar, const double *mass_width, double x,
+                     double y, double tau);
+
+/* NLL = -sum_i log( R_i / N ) over the data sample (steps 2-7).  nll_out: host.  prob_out: device [n]
+ * or NULL; receives P_i = R_i / N.  Synchronous.  TDDP4_ERR_NONFINITE if some P_i <= 0 or non-finite. */
+int tddp4_nll(tddp4 *h, double *nll_out, double *prob_out);
+/* Pipelined form: enqueue the evaluation for the current parameters into result slot 0..63 and return;
+ * tddp4_nll_result waits for that slot.  Parameters are captured at enqueue time.                    */
+int tddp4_nll_async(tddp4 *h, int slot);
+int tddp4_nll_result(tddp4 *h, int slot, double *nll_out);
+/* The pieces of the last completed evaluation in `slot`, for sharded (multi-GPU) use and parity:
+ * out[0] = sum_i log B_i, out[1] = sum_i t_i, out[2] = N (normalisation), out[3] = NLL, out[4] = number
+ * of events with non-positive / non-finite rate.                                                     */
+int tddp4_nll_parts(tddp4 *h, int slot, double out[5]);
+
+/* ---- step 6: normalisation through the Gram matrix ----------------------------------------------- */
+/* G_sum[k][l] = sum_j w_j a_k(p_j) conj(a_l(p_j)) over THIS handle's normalisation sample for the
+ * current masses/widths (recomputed if dirty); host [K_c][K_c][2]; *n_norm = its event count.         */
+int tddp4_gram(tddp4 *h, double *G_sum, int64_t *n_norm);
+/* Replace the Gram matrix used for N by G_sum / n_norm given by the caller (e.g. the all-reduced sum of
+ * all ranks' matrices).  Stays in force until the masses/widths change again.                         */
+int tddp4_gram_override(tddp4 *h, const double *G_sum, int64_t n_norm);
+/* N for the current parameters from the Gram matrix in force; host out.                              */
+int tddp4_norm(tddp4 *h, double *norm_out);
+
+/* ---- companion path: generation (G1-G6) ---------------------------------------------------------- */
+/* Candidates first .. first+n_candidates-1 of Philox stream (seed, stream_id) are generated by
+ * Raubold-Lynch with t ~ Exp(tau), weighted by w B (eq. 1 with the current parameters) and accepted
+ * iff u E < w B.  Envelope E = envelope_scale * max of w B over candidates 0 .. n_pilot-1 of the same
+ * stream; n_pilot = 0: E = envelope_scale.  Accepted events are written compacted, in candidate order:
+ * out_p4 device [16][capacity] (row stride = capacity), out_t device [capacity], out_index device
+ * [capacity] int64 candidate indices or NULL.  n_accepted, n_overflow (ratio above envelope; accepted),
+ * envelope_out: host.  TDDP4_ERR_CAPACITY if n_accepted > capacity (first `capacity` are written).    */
+int tddp4_generate(tddp4 *h, uint64_t seed, uint32_t stream_id, int64_t first, int64_t n_candidates,
+                   int64_t n_pilot, double envelope_scale, int64_t capacity, double *out_p4, double *out_t,
+                   int64_t *out_index, int64_t *n_accepted, int64_t *n_overflow, double *envelope_out);
+/* Rigorous upper bound on the Raubold-Lynch weight w of this model's final state (host out): the product
+ * of the three breakup momenta at their individual maxima.  With a constant-amplitude model, B = 2, so
+ * tddp4_generate(n_pilot = 0, envelope_scale = 2 * bound) un-weights candidates to flat phase space.  */
+int tddp4_weight_bound(const tddp4 *h, double *bound_out);
+/* Raw candidates (no accept step) for parity: device out_p4 [16][n], out_t [n], out_w [n] (phase-space
+ * weight), out_ratio [n] (w B), out_u [n] (accept uniform); any may be NULL.                          */
+int tddp4_candidates(tddp4 *h, uint64_t seed, uint32_t stream_id, int64_t first, int64_t n, double *out_p4,
+                     double *out_t, double *out_w, double *out_ratio, double *out_u);
+
+/* ---- inspection (per-layer parity, profiling) ---------------------------------------------------- */
+enum {
+  TDDP4_GET_S = 0,       /* invariant masses squared, [n_sys][n]                                     */
+  TDDP4_GET_SHAPE = 1,   /* parameter-free lineshape shape g = q^(2L+1) F_L(z)^2 / sqrt(s), [n_inst][n] */
+  TDDP4_GET_STATIC = 2,  /* spin factor x barrier factors per term, [n_terms][n] (caller's term order) */
+  TDDP4_GET_COLUMNS = 3, /* coupling columns a_kappa, [K_c][n][2] (data sample, current parameters)   */
+  TDDP4_GET_TERMS = 4    /* per-term amplitudes a_k, [n_terms][n][2], recomputed (caller's term order) */
+};
+/* Copies a cache of event set `which` into the caller's device buffer `out` (row stride n).          */
+int tddp4_get(tddp4 *h, int which, int what, double *out);
+/* Layout of the caches: systems (bit mask of final-state particles) and lineshape instances.  Arrays
+ * must hold 16 resp. 32 ints.                                                                        */
+int tddp4_layout(const tddp4 *h, int *n_sys, int *sys_mask, int *n_inst, int *inst_res, int *inst_sys,
+                 int *inst_sub);
+
+/* Per-kernel CUDA-event timing on the handle's stream.  kernel ids: */
+enum {
+  TDDP4_K_KIN = 0, TDDP4_K_COLUMNS = 1, TDDP4_K_GRAM = 2, TDDP4_K_NLL = 3, TDDP4_K_GEN_RATIO = 4,
+  TDDP4_K_GEN_EMIT = 5, TDDP4_K_COUNT = 6
+};
+int tddp4_profile(tddp4 *h, int enable);
+/* total_ms, launches since the last reset, for one kernel id; synchronises.                          */
+int tddp4_profile_read(tddp4 *h, int kernel_id, double *total_ms, int64_t *launches);
+int tddp4_profile_reset(tddp4 *h);
+/* Number of kernels this handle has launched since creation (all kinds).                            */
+int64_t tddp4_launch_count(const tddp4 *h);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* TDDP4_H */

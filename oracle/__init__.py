@@ -201,6 +201,18 @@ def candidates(mdl, tau, seed, stream, first, n):
     return p4, t, w, ua
 
 
+def candidates_at(mdl, tau, seed, stream, index):
+    """Candidates with the given indices (int64 array) -> p4[16][n], t, w, u_acc."""
+    m = c_model(mdl)
+    index = np.ascontiguousarray(index, dtype=np.int64)
+    n = len(index)
+    p4 = np.empty((16, n)); t = np.empty(n); w = np.empty(n); ua = np.empty(n)
+    lib().orc_candidates_at(_ref(m), C.c_double(tau), C.c_uint64(seed), C.c_uint32(stream), C.c_int64(n),
+                            index.ctypes.data_as(C.c_void_p), p4.ctypes.data_as(C.c_void_p),
+                            t.ctypes.data_as(C.c_void_p), w.ctypes.data_as(C.c_void_p), ua.ctypes.data_as(C.c_void_p))
+    return p4, t, w, ua
+
+
 def candidate_ratio(mdl, par, seed, stream, first, n):
     m, p = c_model(mdl), c_params(par)
     rho = np.empty(n); ua = np.empty(n)

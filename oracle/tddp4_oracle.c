@@ -562,6 +562,23 @@ void orc_candidates(const orc_model *m, double tau, uint64_t seed, uint32_t stre
   }
 }
 
+/* same for an explicit list of candidate indices (full-size parity: the oracle regenerates the  */
+/* events itself from (seed, index) instead of being handed momenta)                            */
+void orc_candidates_at(const orc_model *m, double tau, uint64_t seed, uint32_t stream, int64_t n,
+                       const int64_t *index, double *p4, double *t, double *w, double *u_acc) {
+#pragma omp parallel for schedule(static)
+  for (int64_t j = 0; j < n; ++j) {
+    double p[4][4], tj, wj, uj;
+    orc_candidate(m, tau, seed, stream, (uint64_t)index[j], p, &tj, &wj, &uj);
+    if (p4)
+      for (int a = 0; a < 4; ++a)
+        for (int mu = 0; mu < 4; ++mu) p4[(int64_t)(4 * a + mu) * n + j] = p[a][mu];
+    if (t) t[j] = tj;
+    if (w) w[j] = wj;
+    if (u_acc) u_acc[j] = uj;
+  }
+}
+
 /* O-9 / G4: ratio rho_i = w_i B(p_i, t_i) for candidates first .. first+n-1                */
 int orc_candidate_ratio(const orc_model *m, const orc_params *par, uint64_t seed, uint32_t stream,
                         uint64_t first, int64_t n, double *rho, double *u_acc) {

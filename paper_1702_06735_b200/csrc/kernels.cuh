@@ -1,0 +1,492 @@
+// kernels.cuh -- the CUDA kernels of the hot path, sm_100a, fp64.
+// All kernels take their tables by value (__grid_constant__): no global state, any stream, any handle.
+#pragma once
+#include <stdint.h>
+#include "device_math.cuh"
+
+namespace tddp4k {
+
+// ------------------------------------------------------------------------------------------------
+// deterministic block reductions (fixed shuffle tree, then warp 0 over the warp partials)
+__device__ __forceinline__ double warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  return v;
+}
+template <int BLOCK>
+__device__ __forceinline__ double block_sum(double v, double *red /* [BLOCK/32] shared */) {
+  v = warp_sum(v);
+  __syncthreads();
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = v;
+  __syncthreads();
+  double r = 0.0;
+  if (threadIdx.x < 32) {
+    r = threadIdx.x < BLOCK / 32 ? red[threadIdx.x] : 0.0;
+    r = warp_sum(r);
+  }
+  return r;  // valid in warp 0
+}
+
+// ------------------------------------------------------------------------------------------------
+// step 1: kinematics + spin factors, once per event set.  One thread per event.
+// in : p4 rows [16][ld_in];  out: s[n_sys][ld], g[n_inst][ld], f[n_terms][ld]
+constexpr int KIN_BLOCK = 128;
+struct KinSink {
+  double *sp, *gp, *fp;
+  int64_t ld, i;
+  __device__ __forceinline__ void s(int r, double v) { sp[r * ld + i] = v; }
+  __device__ __forceinline__ void g(int r, double v) { gp[r * ld + i] = v; }
+  __device__ __forceinline__ void f(int r, double v) { fp[r * ld + i] = v; }
+};
+__global__ void __launch_bounds__(KIN_BLOCK)
+kin_kernel(const __grid_constant__ ModelTab M, const double *__restrict__ p4, int64_t ld_in, int64_t n,
+           double *__restrict__ s, double *__restrict__ g, double *__restrict__ f, int64_t ld) {
+  extern __shared__ double smem[];
+  Scratch sc{smem, smem + 16 * KIN_BLOCK, smem + (16 + M.n_sys) * KIN_BLOCK, KIN_BLOCK};
+  int tid = threadIdx.x;
+  int64_t i = (int64_t)blockIdx.x * KIN_BLOCK + tid;
+  if (i >= n) return;
+#pragma unroll
+  for (int r = 0; r < 16; ++r) sc.P(r, tid) = p4[r * ld_in + i];
+  KinSink sink{s, g, f, ld, i};
+  kinematics(M, sc, tid, sink);
+}
+
+// ------------------------------------------------------------------------------------------------
+// steps 2+3: lineshapes of the instances feeding the dirty coupling columns, component products,
+// Bose orderings summed into one column per coupling.  One thread per event; T_R staged in shared
+// memory so that chains index it dynamically (each recurring lineshape evaluated once).
+constexpr int COL_BLOCK = 128;
+__global__ void __launch_bounds__(COL_BLOCK)
+columns_kernel(const __grid_constant__ ModelTab M, const __grid_constant__ LineParams LP, uint32_t inst_mask,
+               uint32_t col_mask, const double *__restrict__ s, const double *__restrict__ g,
+               const double *__restrict__ f, int64_t ld, int64_t n, double2 *__restrict__ a) {
+  extern __shared__ double2 sT[];   // [n_inst][COL_BLOCK]
+  int tid = threadIdx.x;
+  int64_t i = (int64_t)blockIdx.x * COL_BLOCK + tid;
+  if (i >= n) return;
+  for (int j = 0; j < M.n_inst; ++j) {
+    if (!(inst_mask & (1u << j))) continue;
+    double sv = __ldg(s + M.inst[j].sys * ld + i);
+    double gv = __ldg(g + j * ld + i);
+    sT[j * COL_BLOCK + tid] = breit_wigner(LP.m0sq[j], LP.gam[j], sv, gv);
+  }
+  for (int kap = 0; kap < M.n_kc; ++kap) {
+    if (!(col_mask & (1u << kap))) continue;
+    double2 acc = make_double2(0.0, 0.0);
+    for (int k = M.col_begin[kap]; k < M.col_begin[kap + 1]; ++k) {
+      const TermTab &tm = M.term[k];
+      double fv = __ldg(f + k * ld + i);
+      double2 T = make_double2(1.0, 0.0);
+      if (tm.inst0 >= 0) T = cmul(sT[tm.inst0 * COL_BLOCK + tid], sT[tm.inst1 * COL_BLOCK + tid]);
+      acc.x += fv * T.x;
+      acc.y += fv * T.y;
+    }
+    a[kap * ld + i] = acc;
+  }
+}
+
+// per-term amplitudes a_k (un-summed), for per-layer parity only (TDDP4_GET_TERMS)
+__global__ void __launch_bounds__(COL_BLOCK)
+terms_kernel(const __grid_constant__ ModelTab M, const __grid_constant__ LineParams LP, const double *__restrict__ s,
+             const double *__restrict__ g, const double *__restrict__ f, int64_t ld, int64_t n,
+             double2 *__restrict__ out /* [n_terms][n], caller's term order */) {
+  extern __shared__ double2 sT[];
+  int tid = threadIdx.x;
+  int64_t i = (int64_t)blockIdx.x * COL_BLOCK + tid;
+  if (i >= n) return;
+  for (int j = 0; j < M.n_inst; ++j)
+    sT[j * COL_BLOCK + tid] = breit_wigner(LP.m0sq[j], LP.gam[j], s[M.inst[j].sys * ld + i], g[j * ld + i]);
+  for (int k = 0; k < M.n_terms; ++k) {
+    const TermTab &tm = M.term[k];
+    double fv = f[k * ld + i];
+    double2 T = make_double2(1.0, 0.0);
+    if (tm.inst0 >= 0) T = cmul(sT[tm.inst0 * COL_BLOCK + tid], sT[tm.inst1 * COL_BLOCK + tid]);
+    out[(int64_t)M.user_term[k] * n + i] = make_double2(fv * T.x, fv * T.y);
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// step 6: Hermitian Gram matrix G_kl = sum_j w_j a_k conj(a_l) over the normalisation sample.
+// Thread-per-event grid-stride loop with KC*KC real accumulators in registers (k<=l: re, k<l: im),
+// fixed-order block reduction, one partial matrix per block, summed in block order by the last block.
+constexpr int GRAM_BLOCK = 128;
+template <int KC>
+__global__ void __launch_bounds__(GRAM_BLOCK)
+gram_kernel(const double2 *__restrict__ a, int64_t ld, const double *__restrict__ w, int64_t n,
+            double *__restrict__ partials /* [grid][KC*KC] */, unsigned int *ticket,
+            double *__restrict__ G /* [KC][KC][2] sums, Hermitian, full */) {
+  constexpr int NA = KC * KC;
+  double acc[NA];
+#pragma unroll
+  for (int q = 0; q < NA; ++q) acc[q] = 0.0;
+  for (int64_t i = (int64_t)blockIdx.x * GRAM_BLOCK + threadIdx.x; i < n; i += (int64_t)gridDim.x * GRAM_BLOCK) {
+    double2 v[KC];
+#pragma unroll
+    for (int k = 0; k < KC; ++k) v[k] = __ldg(a + k * ld + i);
+    double wj = w ? __ldg(w + i) : 1.0;
+#pragma unroll
+    for (int k = 0; k < KC; ++k) {
+      double wr = wj * v[k].x, wi = wj * v[k].y;
+      acc[k * KC + k] += wr * v[k].x + wi * v[k].y;
+#pragma unroll
+      for (int l = k + 1; l < KC; ++l) {
+        acc[k * KC + l] += wr * v[l].x + wi * v[l].y;   // Re a_k conj(a_l)
+        acc[l * KC + k] += wi * v[l].x - wr * v[l].y;   // Im a_k conj(a_l)
+      }
+    }
+  }
+  __shared__ double red[GRAM_BLOCK / 32];
+  __shared__ bool last;
+#pragma unroll
+  for (int q = 0; q < NA; ++q) {
+    double r = block_sum<GRAM_BLOCK>(acc[q], red);
+    if (threadIdx.x == 0) partials[(int64_t)blockIdx.x * NA + q] = r;
+  }
+  __threadfence();
+  if (threadIdx.x == 0) last = atomicAdd(ticket, 1u) == gridDim.x - 1;
+  __syncthreads();
+  if (!last) return;
+  __threadfence();
+  for (int q = threadIdx.x; q < NA; q += GRAM_BLOCK) {
+    double sum = 0.0;
+    for (unsigned b = 0; b < gridDim.x; ++b) sum += __ldcg(partials + (int64_t)b * NA + q);
+    int k = q / KC, l = q % KC;
+    if (k <= l) {        // real part of G_kl and G_lk
+      G[(k * KC + l) * 2] = sum;
+      G[(l * KC + k) * 2] = sum;
+      if (k == l) G[(k * KC + k) * 2 + 1] = 0.0;
+    } else {             // slot (l', k') with l' > k' holds Im G_{k'l'}: here k' = l, l' = k
+      G[(l * KC + k) * 2 + 1] = sum;
+      G[(k * KC + l) * 2 + 1] = -sum;
+    }
+  }
+  if (threadIdx.x == 0) *ticket = 0;
+}
+
+// Fallback for K_c > 8 (accumulators no longer fit in registers): tile of events staged in shared memory,
+// one (k <= l) pair per thread.  Same partial/last-block scheme, same result layout.
+constexpr int GRAMG_TILE = 128;
+__global__ void __launch_bounds__(GRAM_BLOCK)
+gram_generic_kernel(int KC, const double2 *__restrict__ a, int64_t ld, const double *__restrict__ w, int64_t n,
+                    double *__restrict__ partials /* [grid][KC*KC] */, unsigned int *ticket,
+                    double *__restrict__ G) {
+  __shared__ double2 tile[MAX_KC][GRAMG_TILE];
+  __shared__ double tw[GRAMG_TILE];
+  __shared__ bool last;
+  const int NP = KC * (KC + 1) / 2;
+  // pairs handled by this thread: p = threadIdx.x, threadIdx.x + GRAM_BLOCK (NP <= 136)
+  double re[2] = {0.0, 0.0}, im[2] = {0.0, 0.0};
+  int pk[2], pl[2];
+  for (int u = 0; u < 2; ++u) {
+    int p = threadIdx.x + u * GRAM_BLOCK, k = 0;
+    pk[u] = pl[u] = -1;
+    if (p < NP) {
+      int rem = p;
+      while (rem >= KC - k) { rem -= KC - k; ++k; }
+      pk[u] = k; pl[u] = k + rem;
+    }
+  }
+  for (int64_t base = (int64_t)blockIdx.x * GRAMG_TILE; base < n; base += (int64_t)gridDim.x * GRAMG_TILE) {
+    int64_t i = base + threadIdx.x;
+    __syncthreads();
+    for (int k = 0; k < KC; ++k) tile[k][threadIdx.x] = i < n ? a[k * ld + i] : make_double2(0.0, 0.0);
+    tw[threadIdx.x] = i < n ? (w ? w[i] : 1.0) : 0.0;
+    __syncthreads();
+    for (int u = 0; u < 2; ++u) {
+      if (pk[u] < 0) continue;
+      for (int e = 0; e < GRAMG_TILE; ++e) {
+        double2 x = tile[pk[u]][e], y = tile[pl[u]][e];
+        double wj = tw[e];
+        re[u] += wj * (x.x * y.x + x.y * y.y);
+        im[u] += wj * (x.y * y.x - x.x * y.y);
+      }
+    }
+  }
+  for (int u = 0; u < 2; ++u)
+    if (pk[u] >= 0) {
+      partials[(int64_t)blockIdx.x * KC * KC + pk[u] * KC + pl[u]] = re[u];
+      if (pk[u] != pl[u]) partials[(int64_t)blockIdx.x * KC * KC + pl[u] * KC + pk[u]] = im[u];
+    }
+  __threadfence();
+  __syncthreads();
+  if (threadIdx.x == 0) last = atomicAdd(ticket, 1u) == gridDim.x - 1;
+  __syncthreads();
+  if (!last) return;
+  __threadfence();
+  for (int q = threadIdx.x; q < KC * KC; q += GRAM_BLOCK) {
+    double sum = 0.0;
+    for (unsigned b = 0; b < gridDim.x; ++b) sum += __ldcg(partials + (int64_t)b * KC * KC + q);
+    int k = q / KC, l = q % KC;
+    if (k <= l) {
+      G[(k * KC + l) * 2] = sum;
+      G[(l * KC + k) * 2] = sum;
+      if (k == l) G[(k * KC + k) * 2 + 1] = 0.0;
+    } else {
+      G[(l * KC + k) * 2 + 1] = sum;
+      G[(k * KC + l) * 2 + 1] = -sum;
+    }
+  }
+  if (threadIdx.x == 0) *ticket = 0;
+}
+
+// ------------------------------------------------------------------------------------------------
+// steps 4+5+7: amplitude sums (eq. 2), mixing rate (eq. 1), -log reduction.
+// Streams the K_c coupling columns (16 B / event / column, coalesced 128-bit loads) and t.
+// result slot layout (doubles): [0] sum log B, [1] unused, [2] N, [3] NLL, [4] #bad events
+constexpr int NLL_BLOCK = 256;
+
+// N from the Gram matrix in force: N = T1 (nAA + nBB) + T2 (nAA - nBB) - 2 T3 Re X - 2 T4 Im X,
+// nAA = c^T G conj(c), nBB likewise for cbar, X = sum_kl c_k conj(cbar_l) G_kl   (O-8, step 6)
+__device__ __forceinline__ double norm_from_gram(const RateParams &R, const double *__restrict__ G, int KC,
+                                                 double inv_n) {
+  double nAA = 0.0, nBB = 0.0, xr = 0.0, xi = 0.0;
+  for (int k = 0; k < KC; ++k)
+    for (int l = 0; l < KC; ++l) {
+      double gr = G[(k * KC + l) * 2] * inv_n, gi = G[(k * KC + l) * 2 + 1] * inv_n;
+      // c_k conj(c_l)
+      double pr = R.c[k][0] * R.c[l][0] + R.c[k][1] * R.c[l][1], pi = R.c[k][1] * R.c[l][0] - R.c[k][0] * R.c[l][1];
+      nAA += pr * gr - pi * gi;
+      pr = R.cbar[k][0] * R.cbar[l][0] + R.cbar[k][1] * R.cbar[l][1];
+      pi = R.cbar[k][1] * R.cbar[l][0] - R.cbar[k][0] * R.cbar[l][1];
+      nBB += pr * gr - pi * gi;
+      pr = R.c[k][0] * R.cbar[l][0] + R.c[k][1] * R.cbar[l][1];
+      pi = R.c[k][1] * R.cbar[l][0] - R.c[k][0] * R.cbar[l][1];
+      xr += pr * gr - pi * gi;
+      xi += pr * gi + pi * gr;
+    }
+  return R.T[0] * (nAA + nBB) + R.T[1] * (nAA - nBB) - 2.0 * R.T[2] * xr - 2.0 * R.T[3] * xi;
+}
+
+template <int KC, bool PROB>
+__global__ void __launch_bounds__(NLL_BLOCK)
+nll_kernel(const double2 *__restrict__ a, int64_t ld, const double *__restrict__ t, int64_t n,
+           const __grid_constant__ RateParams R, const double *__restrict__ G, double inv_n_norm, double sum_t,
+           double *__restrict__ partials, unsigned int *ticket, double *__restrict__ result,
+           double *__restrict__ prob_out) {
+  __shared__ double red[NLL_BLOCK / 32];
+  __shared__ double s_norm;
+  __shared__ bool last;
+  if (PROB) {
+    if (threadIdx.x == 0) s_norm = norm_from_gram(R, G, KC, inv_n_norm);
+    __syncthreads();
+  }
+  double acc = 0.0, bad = 0.0;
+  const double yG = R.y * R.Gamma, xG = R.x * R.Gamma;
+  for (int64_t i = (int64_t)blockIdx.x * NLL_BLOCK + threadIdx.x; i < n; i += (int64_t)gridDim.x * NLL_BLOCK) {
+    double2 v[KC];
+#pragma unroll
+    for (int k = 0; k < KC; ++k) v[k] = __ldcs(a + k * ld + i);
+    double ti = __ldcs(t + i);
+    double2 A = make_double2(0.0, 0.0), Ab = make_double2(0.0, 0.0);
+#pragma unroll
+    for (int k = 0; k < KC; ++k) {
+      A.x += R.c[k][0] * v[k].x - R.c[k][1] * v[k].y;
+      A.y += R.c[k][0] * v[k].y + R.c[k][1] * v[k].x;
+      Ab.x += R.cbar[k][0] * v[k].x - R.cbar[k][1] * v[k].y;
+      Ab.y += R.cbar[k][0] * v[k].y + R.cbar[k][1] * v[k].x;
+    }
+    double B = bracket(A, Ab, yG * ti, xG * ti);
+    if (!(B > 0.0) || isinf(B)) { bad += 1.0; } else { acc += log(B); }
+    if (PROB) prob_out[i] = exp(-R.Gamma * ti) * B / s_norm;
+  }
+  double r = block_sum<NLL_BLOCK>(acc, red);
+  double rb = block_sum<NLL_BLOCK>(bad, red);
+  if (threadIdx.x == 0) {
+    partials[2 * blockIdx.x] = r;
+    partials[2 * blockIdx.x + 1] = rb;
+  }
+  __threadfence();
+  if (threadIdx.x == 0) last = atomicAdd(ticket, 1u) == gridDim.x - 1;
+  __syncthreads();
+  if (!last) return;
+  __threadfence();
+  // fixed-order second pass over the block partials
+  double s0 = 0.0, s1 = 0.0;
+  for (unsigned b = threadIdx.x; b < gridDim.x; b += NLL_BLOCK) {
+    s0 += __ldcg(partials + 2 * b);
+    s1 += __ldcg(partials + 2 * b + 1);
+  }
+  s0 = block_sum<NLL_BLOCK>(s0, red);
+  s1 = block_sum<NLL_BLOCK>(s1, red);
+  if (threadIdx.x == 0) {
+    double norm = norm_from_gram(R, G, KC, inv_n_norm);
+    // -sum log(e^{-Gamma t} B / N) = Gamma sum t - sum log B + n log N
+    double nll = R.Gamma * sum_t - s0 + (double)n * log(norm);
+    if (s1 > 0.0 || !(norm > 0.0)) nll = INFINITY;
+    result[0] = s0; result[1] = sum_t; result[2] = norm; result[3] = nll; result[4] = s1;
+    *ticket = 0;
+  }
+}
+
+// plain deterministic sum of a vector (sum of decay times at load)
+__global__ void __launch_bounds__(256) sum_kernel(const double *__restrict__ v, int64_t n, double *out) {
+  __shared__ double red[8];
+  double acc = 0.0;
+  for (int64_t i = threadIdx.x; i < n; i += 256) acc += v[i];
+  acc = block_sum<256>(acc, red);
+  if (threadIdx.x == 0) *out = acc;
+}
+
+// ------------------------------------------------------------------------------------------------
+// G1-G4: candidate generation and rate on the fly (no caches).  One thread per candidate.
+constexpr int GEN_BLOCK = 128;
+// The sink turns each shape function into T_R at once and folds each static factor into the coupling
+// column it belongs to, so only p, s, q^2 and T_R live in shared memory (terms are sorted by coupling).
+struct GenSink {
+  const ModelTab &M; const LineParams &LP; const RateParams &R; const Scratch &sc;
+  double2 *sT;
+  int tid, kap;
+  double2 A, Ab, col;
+  __device__ __forceinline__ void s(int, double) {}
+  __device__ __forceinline__ void g(int j, double gv) {
+    sT[j * GEN_BLOCK + tid] = breit_wigner(LP.m0sq[j], LP.gam[j], sc.S(M.inst[j].sys, tid), gv);
+  }
+  __device__ __forceinline__ void flush() {
+    A.x += R.c[kap][0] * col.x - R.c[kap][1] * col.y;
+    A.y += R.c[kap][0] * col.y + R.c[kap][1] * col.x;
+    Ab.x += R.cbar[kap][0] * col.x - R.cbar[kap][1] * col.y;
+    Ab.y += R.cbar[kap][0] * col.y + R.cbar[kap][1] * col.x;
+    col = make_double2(0.0, 0.0);
+    ++kap;
+  }
+  __device__ __forceinline__ void f(int k, double fv) {
+    while (k >= M.col_begin[kap + 1]) flush();
+    const TermTab &tm = M.term[k];
+    double2 T = make_double2(1.0, 0.0);
+    if (tm.inst0 >= 0) T = cmul(sT[tm.inst0 * GEN_BLOCK + tid], sT[tm.inst1 * GEN_BLOCK + tid]);
+    col.x += fv * T.x; col.y += fv * T.y;
+  }
+};
+// shared memory per block: p[16], s[n_sys], q2[n_inst] (double rows), T[n_inst] (double2 rows)
+__host__ __device__ inline size_t gen_smem_bytes(int n_sys, int n_inst) {
+  return sizeof(double) * (size_t)(16 + n_sys + 3 * n_inst) * GEN_BLOCK;
+}
+
+__device__ __forceinline__ double candidate_ratio(const ModelTab &M, const LineParams &LP, const RateParams &R,
+                                                  double *smem, int tid, const V4 p[4], double t, double w) {
+  Scratch sc{smem, smem + 16 * GEN_BLOCK, smem + (16 + M.n_sys) * GEN_BLOCK, GEN_BLOCK};
+  double2 *sT = reinterpret_cast<double2 *>(smem + (16 + M.n_sys + M.n_inst) * GEN_BLOCK);
+#pragma unroll
+  for (int a = 0; a < 4; ++a) {
+    sc.P(4 * a, tid) = p[a].e; sc.P(4 * a + 1, tid) = p[a].x; sc.P(4 * a + 2, tid) = p[a].y; sc.P(4 * a + 3, tid) = p[a].z;
+  }
+  GenSink sink{M, LP, R, sc, sT, tid, 0, make_double2(0.0, 0.0), make_double2(0.0, 0.0), make_double2(0.0, 0.0)};
+  kinematics(M, sc, tid, sink);
+  sink.flush();
+  return w * bracket(sink.A, sink.Ab, R.y * R.Gamma * t, R.x * R.Gamma * t);
+}
+
+// mode 0: raw candidate dump (parity); mode 1: pilot maximum (G5); mode 2: accept flags + block counts (G6)
+__global__ void __launch_bounds__(GEN_BLOCK)
+gen_ratio_kernel(const __grid_constant__ ModelTab M, const __grid_constant__ LineParams LP,
+                 const __grid_constant__ RateParams R, double tau, uint64_t seed, uint32_t stream, uint64_t first,
+                 int64_t n, int mode, double envelope,
+                 double *__restrict__ out_p4, double *__restrict__ out_t, double *__restrict__ out_w,
+                 double *__restrict__ out_ratio, double *__restrict__ out_u,
+                 unsigned long long *pilot_max_bits, uint32_t *__restrict__ flags /* one bit per candidate */,
+                 uint32_t *__restrict__ block_count, unsigned long long *overflow) {
+  extern __shared__ double smem[];
+  __shared__ int s_cnt[GEN_BLOCK / 32];
+  int tid = threadIdx.x;
+  int64_t j = (int64_t)blockIdx.x * GEN_BLOCK + tid;
+  bool live = j < n;
+  V4 p[4];
+  double t = 0.0, w = 0.0, u = 1.0, rho = 0.0;
+  if (live) {
+    rl_candidate(M, tau, seed, stream, first + (uint64_t)j, p, t, w, u);
+    rho = candidate_ratio(M, LP, R, smem, tid, p, t, w);
+  }
+  if (mode == 0) {
+    if (!live) return;
+    if (out_p4) {
+#pragma unroll
+      for (int a = 0; a < 4; ++a) {
+        out_p4[(4 * a) * n + j] = p[a].e; out_p4[(4 * a + 1) * n + j] = p[a].x;
+        out_p4[(4 * a + 2) * n + j] = p[a].y; out_p4[(4 * a + 3) * n + j] = p[a].z;
+      }
+    }
+    if (out_t) out_t[j] = t;
+    if (out_w) out_w[j] = w;
+    if (out_ratio) out_ratio[j] = rho;
+    if (out_u) out_u[j] = u;
+    return;
+  }
+  if (mode == 1) {
+    // rho >= 0: the IEEE bit pattern is monotone, so an integer max is the exact fp64 max
+    double m = live && rho > 0.0 ? rho : 0.0;
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
+    if ((tid & 31) == 0) atomicMax(pilot_max_bits, (unsigned long long)__double_as_longlong(m));
+    return;
+  }
+  bool acc = live && (u * envelope < rho);
+  unsigned ballot = __ballot_sync(0xffffffffu, acc);
+  unsigned over = __ballot_sync(0xffffffffu, live && rho > envelope);
+  if ((tid & 31) == 0) {
+    flags[j >> 5] = ballot;
+    s_cnt[tid >> 5] = __popc(ballot);
+    if (over) atomicAdd(overflow, (unsigned long long)__popc(over));
+  }
+  __syncthreads();
+  if (tid == 0) {
+    int c = 0;
+#pragma unroll
+    for (int k = 0; k < GEN_BLOCK / 32; ++k) c += s_cnt[k];
+    block_count[blockIdx.x] = c;
+  }
+}
+
+// exclusive scan of the block counts (single block; counts fit in 32 bits per launch chunk)
+__global__ void __launch_bounds__(1024) scan_kernel(const uint32_t *__restrict__ cnt, int64_t nb,
+                                                    unsigned long long *__restrict__ offs /* [nb+1] */) {
+  __shared__ unsigned long long part[1024];
+  int tid = threadIdx.x;
+  int64_t per = (nb + 1023) / 1024, lo = tid * per, hi = lo + per < nb ? lo + per : nb;
+  unsigned long long s = 0;
+  for (int64_t b = lo; b < hi; ++b) s += cnt[b];
+  part[tid] = s;
+  __syncthreads();
+  if (tid == 0) {
+    unsigned long long run = 0;
+    for (int k = 0; k < 1024; ++k) { unsigned long long v = part[k]; part[k] = run; run += v; }
+    offs[nb] = run;
+  }
+  __syncthreads();
+  unsigned long long run = part[tid];
+  for (int64_t b = lo; b < hi; ++b) { offs[b] = run; run += cnt[b]; }
+}
+
+// G6: regenerate the accepted candidates (Philox is counter based: no state to carry) and write them
+// compacted, in candidate order.
+__global__ void __launch_bounds__(GEN_BLOCK)
+gen_emit_kernel(const __grid_constant__ ModelTab M, double tau, uint64_t seed, uint32_t stream, uint64_t first,
+                int64_t n, const uint32_t *__restrict__ flags, const unsigned long long *__restrict__ offs,
+                int64_t base, int64_t capacity, double *__restrict__ out_p4, double *__restrict__ out_t,
+                int64_t *__restrict__ out_index) {
+  __shared__ int s_cnt[GEN_BLOCK / 32];
+  int tid = threadIdx.x, wid = tid >> 5, lane = tid & 31;
+  int64_t j = (int64_t)blockIdx.x * GEN_BLOCK + tid;
+  unsigned word = (j - lane) < n ? flags[j >> 5] : 0u;
+  if (lane == 0) s_cnt[wid] = __popc(word);
+  __syncthreads();
+  if (!((word >> lane) & 1u)) return;
+  int64_t pos = base + (int64_t)offs[blockIdx.x];
+  for (int k = 0; k < wid; ++k) pos += s_cnt[k];
+  pos += __popc(word & ((1u << lane) - 1u));
+  if (pos >= capacity) return;
+  V4 p[4];
+  double t, w, u;
+  rl_candidate(M, tau, seed, stream, first + (uint64_t)j, p, t, w, u);
+  if (out_p4) {
+#pragma unroll
+    for (int a = 0; a < 4; ++a) {
+      out_p4[(4 * a) * capacity + pos] = p[a].e; out_p4[(4 * a + 1) * capacity + pos] = p[a].x;
+      out_p4[(4 * a + 2) * capacity + pos] = p[a].y; out_p4[(4 * a + 3) * capacity + pos] = p[a].z;
+    }
+  }
+  if (out_t) out_t[pos] = t;
+  if (out_index) out_index[pos] = (int64_t)first + j;
+}
+
+}  // namespace tddp4k

@@ -1,0 +1,61 @@
+// tables.h -- plain-data tables handed to the kernels by value (they live in the constant bank).
+// Internal to csrc/; the public boundary is include/tddp4.h.
+#pragma once
+#include <stdint.h>
+
+namespace tddp4k {
+
+constexpr int MAX_SYS = 12;    // distinct particle systems (2-, 3- and the 4-body one)
+constexpr int MAX_INST = 24;   // de-duplicated lineshape instances
+constexpr int MAX_TERMS = 32;
+constexpr int MAX_KC = 16;
+constexpr int MAX_RES = 16;
+
+enum { SF_NONRES = 0, SF_VV_S = 1, SF_VV_P = 2, SF_VV_D = 3, SF_AP_S = 4, SF_TP_D = 5 };
+
+struct InstTab {     // one lineshape instance = (resonance, system it sits on, running daughter)
+  int8_t res;        // resonance index
+  int8_t sys;        // index of the system whose s is the running mass squared
+  int8_t sub;        // system index of the running daughter (cascade X -> V c), -1: two stable daughters
+  int8_t L;          // L of the resonance's decay vertex
+  int8_t dres;       // daughter resonance (its current m0 enters q0), -1 none
+  int8_t pad[3];
+  double ma, mb;     // fixed daughter masses (ma unused when sub >= 0)
+};
+
+struct TermTab {     // one decay chain (one Bose ordering)
+  int8_t sf;         // spin-factor kind
+  int8_t LD;         // L of the D vertex
+  int8_t inst0;      // VV: R1; cascade: X.  -1 none
+  int8_t inst1;      // VV: R2; cascade: V.  -1 none
+  int8_t perm[4];    // role -> particle
+};
+
+struct ModelTab {
+  int n_sys, n_inst, n_terms, n_kc;
+  int sysD;                        // index of the four-body system
+  uint8_t sys_mask[MAX_SYS];
+  int8_t col_begin[MAX_KC + 1];    // terms (sorted by coupling) of column kappa: [col_begin[k], col_begin[k+1])
+  int8_t user_term[MAX_TERMS];     // sorted position -> caller's term index
+  InstTab inst[MAX_INST];
+  TermTab term[MAX_TERMS];
+  double m_final[4];
+  double m_parent;
+  double r_res2, r_parent2;        // radii squared, GeV^-2
+};
+
+struct LineParams {                // per set_params: T = 1 / (m0sq - s - i gam g(s)),  O-6
+  double m0sq[MAX_INST];
+  double gam[MAX_INST];            // m0^2 Gamma0 / (q0^(2L+1) F_L(z0)^2)
+};
+
+struct RateParams {                // eq. (1) and O-8
+  double c[MAX_KC][2];
+  double cbar[MAX_KC][2];
+  double x, y, Gamma;
+  double T[4];                     // time integrals of cosh, cos, sinh, sin terms over the window
+  double t_lo, t_hi;
+  int use_resolution;
+};
+
+}  // namespace tddp4k

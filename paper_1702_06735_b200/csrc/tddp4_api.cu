@@ -1,0 +1,811 @@
+// tddp4_api.cu -- the C-ABI of include/tddp4.h: handle, host-side model analysis, dirty tracking,
+// launch sequencing.  Every arithmetic step of the hot path runs in the kernels of kernels.cuh; the host
+// only derives per-call scalars (pole constants of the lineshapes, time integrals) in fp64.
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cmath>
+#include <complex>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <limits>
+#include <string>
+#include <vector>
+
+#include "../../include/tddp4.h"
+#include "kernels.cuh"
+
+using namespace tddp4k;
+
+namespace {
+
+constexpr int N_SLOTS = 64;
+constexpr int SLOT_DOUBLES = 8;
+
+struct EventSet {
+  int64_t n = 0, ld = 0;
+  double *s = nullptr, *g = nullptr, *f = nullptr;   // static caches [rows][ld]
+  double2 *a = nullptr;                              // coupling columns [K_c][ld]
+  double *t = nullptr, *sigma_t = nullptr, *w = nullptr;
+  double sum_t = 0.0;
+  uint32_t dirty_cols = 0;                           // columns to recompute before next use
+  bool loaded = false;
+};
+
+struct ProfEvent { int id; cudaEvent_t a, b; };
+
+}  // namespace
+
+struct tddp4 {
+  int device = 0;
+  cudaStream_t stream = nullptr;
+  bool own_stream = false;
+  ModelTab M{};
+  std::vector<tddp4_res> res;
+  std::vector<tddp4_term> terms;   // caller's order
+  double t_lo = 0.0, t_hi = INFINITY;
+  int use_resolution = 0;
+  // parameters
+  bool have_params = false;
+  LineParams LP{};
+  RateParams RP{};
+  std::vector<double> mass, width;
+  uint32_t col_of_inst[MAX_INST] = {0};   // columns fed by each instance
+  EventSet set[2];
+  // normalisation
+  double *G = nullptr;               // device [K_c][K_c][2] sums
+  bool gram_valid = false;           // G matches the current masses/widths
+  bool gram_overridden = false;
+  int64_t gram_n = 0;                // event count G is normalised by
+  // scratch
+  double *partials = nullptr;
+  size_t partials_cap = 0;
+  unsigned int *ticket = nullptr;
+  double *results = nullptr;         // device [N_SLOTS][SLOT_DOUBLES]
+  double *results_host = nullptr;    // pinned mirror
+  cudaEvent_t slot_event[N_SLOTS] = {nullptr};
+  bool slot_used[N_SLOTS] = {false};
+  // generator scratch
+  uint32_t *gen_flags = nullptr, *gen_counts = nullptr;
+  unsigned long long *gen_offs = nullptr, *gen_scalars = nullptr;   // [0] pilot max bits, [1] overflow
+  int64_t gen_cap = 0;
+  // profiling
+  bool profiling = false;
+  std::vector<ProfEvent> pending;
+  std::vector<cudaEvent_t> pool;
+  double prof_ms[TDDP4_K_COUNT] = {0};
+  int64_t prof_n[TDDP4_K_COUNT] = {0};
+  int64_t launches = 0;
+  int sm_count = 148;
+  std::string err;
+};
+
+namespace {
+
+int fail(tddp4 *h, int code, const char *fmt, ...) {
+  if (h) {
+    char buf[512];
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(buf, sizeof buf, fmt, ap);
+    va_end(ap);
+    h->err = buf;
+  }
+  return code;
+}
+
+#define CU(call)                                                                                   \
+  do {                                                                                             \
+    cudaError_t e_ = (call);                                                                       \
+    if (e_ != cudaSuccess) return fail(h, TDDP4_ERR_CUDA, "%s: %s", #call, cudaGetErrorString(e_)); \
+  } while (0)
+
+struct Prof {   // RAII: CUDA events around one launch when profiling is on
+  tddp4 *h; int id; cudaEvent_t a = nullptr, b = nullptr;
+  Prof(tddp4 *h_, int id_) : h(h_), id(id_) {
+    ++h->launches;
+    if (!h->profiling) return;
+    auto get = [&]() { cudaEvent_t e; if (!h->pool.empty()) { e = h->pool.back(); h->pool.pop_back(); } else cudaEventCreate(&e); return e; };
+    a = get(); b = get();
+    cudaEventRecord(a, h->stream);
+  }
+  ~Prof() {
+    if (!a) return;
+    cudaEventRecord(b, h->stream);
+    h->pending.push_back({id, a, b});
+  }
+};
+
+void drain_profile(tddp4 *h) {
+  for (auto &p : h->pending) {
+    cudaEventSynchronize(p.b);
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, p.a, p.b);
+    h->prof_ms[p.id] += ms;
+    h->prof_n[p.id] += 1;
+    h->pool.push_back(p.a);
+    h->pool.push_back(p.b);
+  }
+  h->pending.clear();
+}
+
+int parent_L(int sf) {
+  switch (sf) {
+    case SF_VV_S: return 0; case SF_VV_P: return 1; case SF_VV_D: return 2;
+    case SF_AP_S: return 1; case SF_TP_D: return 2; default: return 0;
+  }
+}
+
+int find_or_add_sys(ModelTab &M, unsigned mask) {
+  for (int i = 0; i < M.n_sys; ++i)
+    if (M.sys_mask[i] == mask) return i;
+  if (M.n_sys >= MAX_SYS) return -1;
+  M.sys_mask[M.n_sys] = (uint8_t)mask;
+  return M.n_sys++;
+}
+
+int find_or_add_inst(ModelTab &M, const InstTab &in) {
+  for (int i = 0; i < M.n_inst; ++i) {
+    const InstTab &o = M.inst[i];
+    if (o.res == in.res && o.sys == in.sys && o.sub == in.sub && o.dres == in.dres && o.ma == in.ma && o.mb == in.mb)
+      return i;
+  }
+  if (M.n_inst >= MAX_INST) return -1;
+  M.inst[M.n_inst] = in;
+  return M.n_inst++;
+}
+
+double host_breakup(double M, double ma, double mb) {
+  double rad = (M - ma - mb) * (M + ma + mb) * (M + ma - mb) * (M - ma + mb);
+  return rad > 0.0 ? std::sqrt(rad) / (2.0 * M) : 0.0;
+}
+double host_barrier2(int L, double z) {   // F_L(z)^2
+  if (L == 0) return 1.0;
+  if (L == 1) return 1.0 / (1.0 + z);
+  return 1.0 / (9.0 + 3.0 * z + z * z);
+}
+
+// O-8: window integrals of e^{-Gamma t}{cosh, cos, sinh, sin}
+void time_integrals(double x, double y, double Gamma, double lo, double hi, double T[4]) {
+  using cd = std::complex<double>;
+  auto I = [&](cd lam) {
+    cd a = std::exp(-lam * lo);
+    cd b = std::isinf(hi) ? cd(0.0, 0.0) : std::exp(-lam * hi);
+    return (a - b) / lam;
+  };
+  cd Im = I(cd(Gamma * (1.0 - y), 0.0)), Ip = I(cd(Gamma * (1.0 + y), 0.0)), Ix = I(cd(Gamma, -Gamma * x));
+  T[0] = 0.5 * (Im.real() + Ip.real());
+  T[1] = Ix.real();
+  T[2] = 0.5 * (Im.real() - Ip.real());
+  T[3] = Ix.imag();
+}
+
+int ensure_partials(tddp4 *h, size_t doubles) {
+  if (doubles <= h->partials_cap) return TDDP4_OK;
+  if (h->partials) cudaFree(h->partials);
+  h->partials = nullptr;
+  h->partials_cap = 0;
+  CU(cudaMalloc(&h->partials, doubles * sizeof(double)));
+  h->partials_cap = doubles;
+  return TDDP4_OK;
+}
+
+void free_set(EventSet &e) {
+  cudaFree(e.s); cudaFree(e.g); cudaFree(e.f); cudaFree(e.a); cudaFree(e.t); cudaFree(e.sigma_t); cudaFree(e.w);
+  e = EventSet{};
+}
+
+uint32_t all_cols(const tddp4 *h) { return h->M.n_kc >= 32 ? 0xffffffffu : ((1u << h->M.n_kc) - 1u); }
+
+// steps 2+3 on one event set for the columns in its dirty mask
+int run_columns(tddp4 *h, EventSet &e) {
+  if (!e.dirty_cols || e.n == 0) { e.dirty_cols = 0; return TDDP4_OK; }
+  uint32_t inst_mask = 0;
+  for (int j = 0; j < h->M.n_inst; ++j)
+    if (h->col_of_inst[j] & e.dirty_cols) inst_mask |= 1u << j;
+  int grid = (int)((e.n + COL_BLOCK - 1) / COL_BLOCK);
+  size_t smem = (size_t)std::max(1, h->M.n_inst) * COL_BLOCK * sizeof(double2);
+  {
+    Prof p(h, TDDP4_K_COLUMNS);
+    columns_kernel<<<grid, COL_BLOCK, smem, h->stream>>>(h->M, h->LP, inst_mask, e.dirty_cols, e.s, e.g, e.f, e.ld,
+                                                         e.n, e.a);
+  }
+  CU(cudaGetLastError());
+  e.dirty_cols = 0;
+  return TDDP4_OK;
+}
+
+template <int KC>
+void launch_gram(tddp4 *h, const EventSet &e, int grid) {
+  gram_kernel<KC><<<grid, GRAM_BLOCK, 0, h->stream>>>(e.a, e.ld, e.w, e.n, h->partials, h->ticket, h->G);
+}
+
+// step 6: refresh the Gram matrix of this handle's normalisation sample if masses/widths changed
+int ensure_gram(tddp4 *h) {
+  if (h->gram_valid) return TDDP4_OK;
+  EventSet &e = h->set[1];
+  if (!e.loaded) return fail(h, TDDP4_ERR_STATE, "normalisation sample not loaded");
+  int rc = run_columns(h, e);
+  if (rc) return rc;
+  int KC = h->M.n_kc;
+  int grid = (int)std::min<int64_t>((e.n + GRAM_BLOCK - 1) / GRAM_BLOCK, (int64_t)h->sm_count * 3);
+  grid = std::max(grid, 1);
+  rc = ensure_partials(h, (size_t)grid * KC * KC + 16);
+  if (rc) return rc;
+  {
+    Prof p(h, TDDP4_K_GRAM);
+    switch (KC) {
+      case 1: launch_gram<1>(h, e, grid); break;
+      case 2: launch_gram<2>(h, e, grid); break;
+      case 3: launch_gram<3>(h, e, grid); break;
+      case 4: launch_gram<4>(h, e, grid); break;
+      case 5: launch_gram<5>(h, e, grid); break;
+      case 6: launch_gram<6>(h, e, grid); break;
+      case 7: launch_gram<7>(h, e, grid); break;
+      case 8: launch_gram<8>(h, e, grid); break;
+      default:
+        gram_generic_kernel<<<grid, GRAM_BLOCK, 0, h->stream>>>(KC, e.a, e.ld, e.w, e.n, h->partials, h->ticket, h->G);
+    }
+  }
+  CU(cudaGetLastError());
+  h->gram_valid = true;
+  h->gram_overridden = false;
+  h->gram_n = e.n;
+  return TDDP4_OK;
+}
+
+template <int KC>
+void launch_nll(tddp4 *h, const EventSet &e, int grid, double inv_n, double *result, double *prob) {
+  if (prob)
+    nll_kernel<KC, true><<<grid, NLL_BLOCK, 0, h->stream>>>(e.a, e.ld, e.t, e.n, h->RP, h->G, inv_n, e.sum_t,
+                                                            h->partials, h->ticket, result, prob);
+  else
+    nll_kernel<KC, false><<<grid, NLL_BLOCK, 0, h->stream>>>(e.a, e.ld, e.t, e.n, h->RP, h->G, inv_n, e.sum_t,
+                                                             h->partials, h->ticket, result, prob);
+}
+
+int enqueue_nll(tddp4 *h, int slot, double *prob) {
+  if (!h->have_params) return fail(h, TDDP4_ERR_STATE, "tddp4_set_params has not been called");
+  EventSet &d = h->set[0];
+  if (!d.loaded) return fail(h, TDDP4_ERR_STATE, "data sample not loaded");
+  if (h->use_resolution) return fail(h, TDDP4_ERR_ARG, "use_resolution = 1 is not implemented yet");
+  int rc = ensure_gram(h);
+  if (rc) return rc;
+  rc = run_columns(h, d);
+  if (rc) return rc;
+  int KC = h->M.n_kc;
+  int64_t blocks = (d.n + NLL_BLOCK - 1) / NLL_BLOCK;
+  int grid = (int)std::max<int64_t>(1, std::min<int64_t>(blocks, (int64_t)h->sm_count * 8));
+  rc = ensure_partials(h, (size_t)2 * grid + 16);
+  if (rc) return rc;
+  double inv_n = h->gram_n > 0 ? 1.0 / (double)h->gram_n : 0.0;
+  double *result = h->results + (size_t)slot * SLOT_DOUBLES;
+  {
+    Prof p(h, TDDP4_K_NLL);
+    switch (KC) {
+#define CASE(k) case k: launch_nll<k>(h, d, grid, inv_n, result, prob); break;
+      CASE(1) CASE(2) CASE(3) CASE(4) CASE(5) CASE(6) CASE(7) CASE(8) CASE(9) CASE(10) CASE(11) CASE(12)
+      CASE(13) CASE(14) CASE(15) CASE(16)
+#undef CASE
+      default: return fail(h, TDDP4_ERR_ARG, "unsupported number of couplings %d", KC);
+    }
+  }
+  CU(cudaGetLastError());
+  CU(cudaMemcpyAsync(h->results_host + (size_t)slot * SLOT_DOUBLES, result, SLOT_DOUBLES * sizeof(double),
+                     cudaMemcpyDeviceToHost, h->stream));
+  CU(cudaEventRecord(h->slot_event[slot], h->stream));
+  h->slot_used[slot] = true;
+  return TDDP4_OK;
+}
+
+}  // namespace
+
+// =====================================================================================================
+extern "C" {
+
+const char *tddp4_version(void) { return "tddp4 0.1 (sm_100a, fp64)"; }
+
+const char *tddp4_last_error(const tddp4 *h) { return h ? h->err.c_str() : "null handle"; }
+
+int tddp4_create(const tddp4_model_desc *desc, tddp4 **out) {
+  if (!desc || !out) return TDDP4_ERR_ARG;
+  *out = nullptr;
+  tddp4 *h = new tddp4;
+  auto bail = [&](int code) { *out = h; return code; };   // handle kept so the caller can read the error text
+  if (desc->n_res < 0 || desc->n_res > TDDP4_MAX_RES || desc->n_terms < 1 || desc->n_terms > TDDP4_MAX_TERMS ||
+      desc->n_couplings < 1 || desc->n_couplings > TDDP4_MAX_COUPLINGS)
+    return bail(fail(h, TDDP4_ERR_ARG, "model size out of range"));
+  if (!(desc->t_hi > desc->t_lo)) return bail(fail(h, TDDP4_ERR_ARG, "empty decay-time window"));
+  h->res.assign(desc->res, desc->res + desc->n_res);
+  h->terms.assign(desc->terms, desc->terms + desc->n_terms);
+  h->t_lo = desc->t_lo; h->t_hi = desc->t_hi; h->use_resolution = desc->use_resolution;
+  ModelTab &M = h->M;
+  memset(&M, 0, sizeof M);
+  M.n_kc = desc->n_couplings;
+  M.m_parent = desc->m_parent;
+  for (int i = 0; i < 4; ++i) M.m_final[i] = desc->m_final[i];
+  M.r_res2 = desc->r_res * desc->r_res;
+  M.r_parent2 = desc->r_parent * desc->r_parent;
+  M.sysD = find_or_add_sys(M, 0xF);
+  // terms sorted by coupling (stable), so that each column is a contiguous range
+  std::vector<int> order(desc->n_terms);
+  for (int k = 0; k < desc->n_terms; ++k) order[k] = k;
+  std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return desc->terms[a].coupling < desc->terms[b].coupling; });
+  for (int r = 0; r < desc->n_res; ++r)
+    if (desc->res[r].L < 0 || desc->res[r].L > 2) return bail(fail(h, TDDP4_ERR_ARG, "resonance %d: L must be 0, 1 or 2", r));
+  int pos = 0;
+  for (int kap = 0; kap <= M.n_kc; ++kap) {
+    M.col_begin[kap] = (int8_t)pos;
+    while (kap < M.n_kc && pos < desc->n_terms && desc->terms[order[pos]].coupling == kap) ++pos;
+  }
+  if (pos != desc->n_terms) return bail(fail(h, TDDP4_ERR_ARG, "term coupling index out of range"));
+  M.n_terms = desc->n_terms;
+  for (int k = 0; k < M.n_terms; ++k) {
+    const tddp4_term &t = desc->terms[order[k]];
+    TermTab &tm = M.term[k];
+    M.user_term[k] = (int8_t)order[k];
+    unsigned seen = 0;
+    for (int r = 0; r < 4; ++r) {
+      if (t.perm[r] < 0 || t.perm[r] > 3) return bail(fail(h, TDDP4_ERR_ARG, "term %d: bad permutation", order[k]));
+      seen |= 1u << t.perm[r];
+      tm.perm[r] = (int8_t)t.perm[r];
+    }
+    if (seen != 0xF) return bail(fail(h, TDDP4_ERR_ARG, "term %d: perm is not a permutation", order[k]));
+    if (t.spin_factor < SF_NONRES || t.spin_factor > SF_TP_D)
+      return bail(fail(h, TDDP4_ERR_ARG, "term %d: unknown spin factor", order[k]));
+    tm.sf = (int8_t)t.spin_factor;
+    tm.LD = (int8_t)parent_L(t.spin_factor);
+    tm.inst0 = tm.inst1 = -1;
+    if (t.spin_factor == SF_NONRES) continue;
+    for (int r = 0; r < 2; ++r)
+      if (t.res[r] < 0 || t.res[r] >= desc->n_res) return bail(fail(h, TDDP4_ERR_ARG, "term %d: bad resonance index", order[k]));
+    const int *pm = t.perm;
+    InstTab a{}, b{};
+    a.dres = b.dres = -1;
+    if (t.spin_factor <= SF_VV_D) {
+      a.res = (int8_t)t.res[0]; a.sys = (int8_t)find_or_add_sys(M, (1u << pm[0]) | (1u << pm[1])); a.sub = -1;
+      a.ma = M.m_final[pm[0]]; a.mb = M.m_final[pm[1]];
+      b.res = (int8_t)t.res[1]; b.sys = (int8_t)find_or_add_sys(M, (1u << pm[2]) | (1u << pm[3])); b.sub = -1;
+      b.ma = M.m_final[pm[2]]; b.mb = M.m_final[pm[3]];
+    } else {
+      int sysV = find_or_add_sys(M, (1u << pm[0]) | (1u << pm[1]));
+      a.res = (int8_t)t.res[0]; a.sys = (int8_t)find_or_add_sys(M, (1u << pm[0]) | (1u << pm[1]) | (1u << pm[2]));
+      a.sub = (int8_t)sysV; a.dres = (int8_t)t.res[1]; a.ma = 0.0; a.mb = M.m_final[pm[2]];
+      b.res = (int8_t)t.res[1]; b.sys = (int8_t)sysV; b.sub = -1; b.ma = M.m_final[pm[0]]; b.mb = M.m_final[pm[1]];
+    }
+    a.L = (int8_t)desc->res[a.res].L;
+    b.L = (int8_t)desc->res[b.res].L;
+    if (a.sys < 0 || b.sys < 0) return bail(fail(h, TDDP4_ERR_ARG, "too many particle systems"));
+    int ia = find_or_add_inst(M, a), ib = find_or_add_inst(M, b);
+    if (ia < 0 || ib < 0) return bail(fail(h, TDDP4_ERR_ARG, "too many lineshape instances"));
+    tm.inst0 = (int8_t)ia; tm.inst1 = (int8_t)ib;
+  }
+  for (int kap = 0; kap < M.n_kc; ++kap)
+    for (int k = M.col_begin[kap]; k < M.col_begin[kap + 1]; ++k) {
+      if (M.term[k].inst0 >= 0) h->col_of_inst[M.term[k].inst0] |= 1u << kap;
+      if (M.term[k].inst1 >= 0) h->col_of_inst[M.term[k].inst1] |= 1u << kap;
+    }
+  h->mass.assign(desc->n_res, 0.0);
+  h->width.assign(desc->n_res, 0.0);
+
+  cudaError_t e = cudaGetDevice(&h->device);
+  if (e != cudaSuccess) return bail(fail(h, TDDP4_ERR_CUDA, "cudaGetDevice: %s (no CPU fallback exists)", cudaGetErrorString(e)));
+  cudaDeviceProp prop;
+  e = cudaGetDeviceProperties(&prop, h->device);
+  if (e != cudaSuccess) return bail(fail(h, TDDP4_ERR_CUDA, "cudaGetDeviceProperties: %s", cudaGetErrorString(e)));
+  h->sm_count = prop.multiProcessorCount;
+  e = cudaStreamCreateWithFlags(&h->stream, cudaStreamNonBlocking);
+  if (e != cudaSuccess) return bail(fail(h, TDDP4_ERR_CUDA, "cudaStreamCreate: %s", cudaGetErrorString(e)));
+  h->own_stream = true;
+  int KC = M.n_kc;
+  bool ok = cudaMalloc(&h->G, sizeof(double) * 2 * KC * KC) == cudaSuccess &&
+            cudaMalloc(&h->ticket, sizeof(unsigned int)) == cudaSuccess &&
+            cudaMalloc(&h->results, sizeof(double) * N_SLOTS * SLOT_DOUBLES) == cudaSuccess &&
+            cudaMallocHost(&h->results_host, sizeof(double) * N_SLOTS * SLOT_DOUBLES) == cudaSuccess &&
+            cudaMalloc(&h->gen_scalars, sizeof(unsigned long long) * 2) == cudaSuccess &&
+            cudaMemset(h->ticket, 0, sizeof(unsigned int)) == cudaSuccess &&
+            cudaMemset(h->G, 0, sizeof(double) * 2 * KC * KC) == cudaSuccess;
+  for (int s = 0; ok && s < N_SLOTS; ++s) ok = cudaEventCreateWithFlags(&h->slot_event[s], cudaEventDisableTiming) == cudaSuccess;
+  if (!ok) return bail(fail(h, TDDP4_ERR_CUDA, "allocation failed: %s", cudaGetErrorString(cudaGetLastError())));
+  // kernels that need more than 48 KB of dynamic shared memory
+  cudaFuncSetAttribute(gen_ratio_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gen_smem_bytes(MAX_SYS, MAX_INST));
+  cudaFuncSetAttribute(columns_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(MAX_INST * COL_BLOCK * sizeof(double2)));
+  cudaFuncSetAttribute(terms_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(MAX_INST * COL_BLOCK * sizeof(double2)));
+  *out = h;
+  return TDDP4_OK;
+}
+
+int tddp4_destroy(tddp4 *h) {
+  if (!h) return TDDP4_OK;
+  if (h->stream) cudaStreamSynchronize(h->stream);
+  drain_profile(h);
+  for (auto e : h->pool) cudaEventDestroy(e);
+  free_set(h->set[0]);
+  free_set(h->set[1]);
+  cudaFree(h->G); cudaFree(h->partials); cudaFree(h->ticket); cudaFree(h->results);
+  if (h->results_host) cudaFreeHost(h->results_host);
+  cudaFree(h->gen_flags); cudaFree(h->gen_counts); cudaFree(h->gen_offs); cudaFree(h->gen_scalars);
+  for (int s = 0; s < N_SLOTS; ++s)
+    if (h->slot_event[s]) cudaEventDestroy(h->slot_event[s]);
+  if (h->own_stream && h->stream) cudaStreamDestroy(h->stream);
+  delete h;
+  return TDDP4_OK;
+}
+
+int tddp4_set_stream(tddp4 *h, void *cuda_stream) {
+  if (!h) return TDDP4_ERR_ARG;
+  if (h->stream) CU(cudaStreamSynchronize(h->stream));
+  if (h->own_stream) { cudaStreamDestroy(h->stream); h->own_stream = false; }
+  h->stream = (cudaStream_t)cuda_stream;
+  return TDDP4_OK;
+}
+
+int tddp4_load_events(tddp4 *h, int which, int64_t n, int64_t ld_in, const double *p4, const double *t,
+                      const double *sigma_t, const double *weight, int on_device) {
+  if (!h) return TDDP4_ERR_ARG;
+  if (which < 0 || which > 1 || n < 0 || ld_in < n || (n > 0 && !p4)) return fail(h, TDDP4_ERR_ARG, "bad load_events argument");
+  if (which == 0 && n > 0 && !t) return fail(h, TDDP4_ERR_ARG, "the data sample needs decay times");
+  CU(cudaStreamSynchronize(h->stream));
+  EventSet &e = h->set[which];
+  free_set(e);
+  e.n = n;
+  e.ld = std::max<int64_t>(32, (n + 31) / 32 * 32);   // rows start 256-byte aligned
+  const ModelTab &M = h->M;
+  CU(cudaMalloc(&e.s, sizeof(double) * M.n_sys * e.ld));
+  CU(cudaMalloc(&e.g, sizeof(double) * std::max(1, M.n_inst) * e.ld));
+  CU(cudaMalloc(&e.f, sizeof(double) * M.n_terms * e.ld));
+  CU(cudaMalloc(&e.a, sizeof(double2) * M.n_kc * e.ld));
+  cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
+  auto copy_vec = [&](double **dst, const double *src) -> cudaError_t {
+    if (!src || n == 0) return cudaSuccess;
+    cudaError_t e_ = cudaMalloc(dst, sizeof(double) * e.ld);
+    if (e_ != cudaSuccess) return e_;
+    return cudaMemcpyAsync(*dst, src, sizeof(double) * n, kind, h->stream);
+  };
+  CU(copy_vec(&e.t, t));
+  CU(copy_vec(&e.sigma_t, sigma_t));
+  CU(copy_vec(&e.w, weight));
+  if (n > 0) {
+    const double *dp4 = p4;
+    double *staging = nullptr;
+    int64_t ld_dev = ld_in;
+    if (!on_device) {
+      CU(cudaMalloc(&staging, sizeof(double) * 16 * n));
+      CU(cudaMemcpy2DAsync(staging, sizeof(double) * n, p4, sizeof(double) * ld_in, sizeof(double) * n, 16,
+                           cudaMemcpyHostToDevice, h->stream));
+      dp4 = staging;
+      ld_dev = n;
+    }
+    int grid = (int)((n + KIN_BLOCK - 1) / KIN_BLOCK);
+    size_t smem = sizeof(double) * (16 + M.n_sys + M.n_inst) * KIN_BLOCK;
+    {
+      Prof p(h, TDDP4_K_KIN);
+      kin_kernel<<<grid, KIN_BLOCK, smem, h->stream>>>(M, dp4, ld_dev, n, e.s, e.g, e.f, e.ld);
+    }
+    CU(cudaGetLastError());
+    if (e.t) {
+      sum_kernel<<<1, 256, 0, h->stream>>>(e.t, n, h->results);   // slot 0 word 0 as scratch
+      ++h->launches;
+      CU(cudaMemcpyAsync(&e.sum_t, h->results, sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    }
+    CU(cudaStreamSynchronize(h->stream));
+    if (staging) cudaFree(staging);
+  }
+  e.dirty_cols = all_cols(h);
+  e.loaded = true;
+  if (which == 1) { h->gram_valid = false; h->gram_overridden = false; }
+  return TDDP4_OK;
+}
+
+int tddp4_set_params(tddp4 *h, const double *c, const double *cbar, const double *mass_width, double x, double y,
+                     double tau) {
+  if (!h || !c || !cbar || (h->res.size() && !mass_width)) return fail(h, TDDP4_ERR_ARG, "null parameter block");
+  if (!(tau > 0.0) || !(std::fabs(y) < 1.0)) return fail(h, TDDP4_ERR_ARG, "need tau > 0 and |y| < 1");
+  const ModelTab &M = h->M;
+  LineParams lp{};
+  int nres = (int)h->res.size();
+  for (int j = 0; j < M.n_inst; ++j) {
+    const InstTab &in = M.inst[j];
+    double m0 = mass_width[2 * in.res], g0 = mass_width[2 * in.res + 1];
+    double ma0 = in.dres >= 0 ? mass_width[2 * in.dres] : in.ma;
+    if (!(m0 > ma0 + in.mb) || !(g0 > 0.0))
+      return fail(h, TDDP4_ERR_DOMAIN, "resonance %d: pole mass %.6g below its decay threshold %.6g (or width <= 0)",
+                  (int)in.res, m0, ma0 + in.mb);
+    double q0 = host_breakup(m0, ma0, in.mb);
+    double z0 = q0 * q0 * M.r_res2;
+    lp.m0sq[j] = m0 * m0;
+    lp.gam[j] = m0 * m0 * g0 / (std::pow(q0, 2 * in.L + 1) * host_barrier2(in.L, z0));
+  }
+  uint32_t dirty = 0;
+  for (int j = 0; j < M.n_inst; ++j)
+    if (!h->have_params || lp.m0sq[j] != h->LP.m0sq[j] || lp.gam[j] != h->LP.gam[j]) dirty |= h->col_of_inst[j];
+  if (!h->have_params) dirty = all_cols(h);
+  h->LP = lp;
+  for (int r = 0; r < nres; ++r) { h->mass[r] = mass_width[2 * r]; h->width[r] = mass_width[2 * r + 1]; }
+  RateParams &R = h->RP;
+  for (int k = 0; k < M.n_kc; ++k) {
+    R.c[k][0] = c[2 * k]; R.c[k][1] = c[2 * k + 1];
+    R.cbar[k][0] = cbar[2 * k]; R.cbar[k][1] = cbar[2 * k + 1];
+  }
+  R.x = x; R.y = y; R.Gamma = 1.0 / tau;
+  R.t_lo = h->t_lo; R.t_hi = h->t_hi; R.use_resolution = h->use_resolution;
+  time_integrals(x, y, R.Gamma, h->t_lo, h->t_hi, R.T);
+  if (dirty) {
+    h->set[0].dirty_cols |= dirty;
+    h->set[1].dirty_cols |= dirty;
+    h->gram_valid = false;
+    h->gram_overridden = false;
+  }
+  h->have_params = true;
+  return TDDP4_OK;
+}
+
+int tddp4_nll_async(tddp4 *h, int slot) {
+  if (!h || slot < 0 || slot >= N_SLOTS) return fail(h, TDDP4_ERR_ARG, "bad slot");
+  return enqueue_nll(h, slot, nullptr);
+}
+
+int tddp4_nll_result(tddp4 *h, int slot, double *nll_out) {
+  if (!h || slot < 0 || slot >= N_SLOTS || !nll_out) return fail(h, TDDP4_ERR_ARG, "bad slot");
+  if (!h->slot_used[slot]) return fail(h, TDDP4_ERR_STATE, "slot %d holds no evaluation", slot);
+  CU(cudaEventSynchronize(h->slot_event[slot]));
+  const double *r = h->results_host + (size_t)slot * SLOT_DOUBLES;
+  *nll_out = r[3];
+  if (r[4] > 0.0 || !std::isfinite(r[3])) {
+    *nll_out = INFINITY;
+    return fail(h, TDDP4_ERR_NONFINITE, "%g events with non-positive or non-finite rate (N = %g)", r[4], r[2]);
+  }
+  return TDDP4_OK;
+}
+
+int tddp4_nll(tddp4 *h, double *nll_out, double *prob_out) {
+  if (!h || !nll_out) return fail(h, TDDP4_ERR_ARG, "null argument");
+  int rc = enqueue_nll(h, 0, prob_out);
+  if (rc) return rc;
+  return tddp4_nll_result(h, 0, nll_out);
+}
+
+int tddp4_nll_parts(tddp4 *h, int slot, double out[5]) {
+  if (!h || slot < 0 || slot >= N_SLOTS || !out) return fail(h, TDDP4_ERR_ARG, "bad slot");
+  if (!h->slot_used[slot]) return fail(h, TDDP4_ERR_STATE, "slot %d holds no evaluation", slot);
+  CU(cudaEventSynchronize(h->slot_event[slot]));
+  memcpy(out, h->results_host + (size_t)slot * SLOT_DOUBLES, 5 * sizeof(double));
+  return TDDP4_OK;
+}
+
+int tddp4_gram(tddp4 *h, double *G_sum, int64_t *n_norm) {
+  if (!h || !G_sum || !n_norm) return fail(h, TDDP4_ERR_ARG, "null argument");
+  if (!h->have_params) return fail(h, TDDP4_ERR_STATE, "tddp4_set_params has not been called");
+  if (h->gram_overridden) { h->gram_valid = false; h->gram_overridden = false; }
+  int rc = ensure_gram(h);
+  if (rc) return rc;
+  int KC = h->M.n_kc;
+  CU(cudaMemcpyAsync(G_sum, h->G, sizeof(double) * 2 * KC * KC, cudaMemcpyDeviceToHost, h->stream));
+  CU(cudaStreamSynchronize(h->stream));
+  *n_norm = h->gram_n;
+  return TDDP4_OK;
+}
+
+int tddp4_gram_override(tddp4 *h, const double *G_sum, int64_t n_norm) {
+  if (!h || !G_sum || n_norm <= 0) return fail(h, TDDP4_ERR_ARG, "bad argument");
+  int KC = h->M.n_kc;
+  CU(cudaMemcpyAsync(h->G, G_sum, sizeof(double) * 2 * KC * KC, cudaMemcpyHostToDevice, h->stream));
+  CU(cudaStreamSynchronize(h->stream));
+  h->gram_valid = true;
+  h->gram_overridden = true;
+  h->gram_n = n_norm;
+  return TDDP4_OK;
+}
+
+int tddp4_norm(tddp4 *h, double *norm_out) {
+  if (!h || !norm_out) return fail(h, TDDP4_ERR_ARG, "null argument");
+  if (!h->have_params) return fail(h, TDDP4_ERR_STATE, "tddp4_set_params has not been called");
+  int rc = ensure_gram(h);
+  if (rc) return rc;
+  int KC = h->M.n_kc;
+  std::vector<double> G(2 * KC * KC);
+  CU(cudaMemcpyAsync(G.data(), h->G, sizeof(double) * G.size(), cudaMemcpyDeviceToHost, h->stream));
+  CU(cudaStreamSynchronize(h->stream));
+  // same contraction as norm_from_gram() in the kernels, on the host copy
+  const RateParams &R = h->RP;
+  double inv_n = 1.0 / (double)h->gram_n, nAA = 0, nBB = 0, xr = 0, xi = 0;
+  for (int k = 0; k < KC; ++k)
+    for (int l = 0; l < KC; ++l) {
+      double gr = G[(k * KC + l) * 2] * inv_n, gi = G[(k * KC + l) * 2 + 1] * inv_n;
+      double pr = R.c[k][0] * R.c[l][0] + R.c[k][1] * R.c[l][1], pi = R.c[k][1] * R.c[l][0] - R.c[k][0] * R.c[l][1];
+      nAA += pr * gr - pi * gi;
+      pr = R.cbar[k][0] * R.cbar[l][0] + R.cbar[k][1] * R.cbar[l][1];
+      pi = R.cbar[k][1] * R.cbar[l][0] - R.cbar[k][0] * R.cbar[l][1];
+      nBB += pr * gr - pi * gi;
+      pr = R.c[k][0] * R.cbar[l][0] + R.c[k][1] * R.cbar[l][1];
+      pi = R.c[k][1] * R.cbar[l][0] - R.c[k][0] * R.cbar[l][1];
+      xr += pr * gr - pi * gi;
+      xi += pr * gi + pi * gr;
+    }
+  *norm_out = R.T[0] * (nAA + nBB) + R.T[1] * (nAA - nBB) - 2.0 * R.T[2] * xr - 2.0 * R.T[3] * xi;
+  return TDDP4_OK;
+}
+
+// ---- generation ---------------------------------------------------------------------------------------
+static int ensure_gen(tddp4 *h, int64_t n) {
+  if (n <= h->gen_cap) return TDDP4_OK;
+  cudaFree(h->gen_flags); cudaFree(h->gen_counts); cudaFree(h->gen_offs);
+  h->gen_flags = nullptr; h->gen_counts = nullptr; h->gen_offs = nullptr; h->gen_cap = 0;
+  int64_t blocks = (n + GEN_BLOCK - 1) / GEN_BLOCK;
+  CU(cudaMalloc(&h->gen_flags, sizeof(uint32_t) * blocks * (GEN_BLOCK / 32)));
+  CU(cudaMalloc(&h->gen_counts, sizeof(uint32_t) * blocks));
+  CU(cudaMalloc(&h->gen_offs, sizeof(unsigned long long) * (blocks + 1)));
+  h->gen_cap = n;
+  return TDDP4_OK;
+}
+
+static int launch_ratio(tddp4 *h, uint64_t seed, uint32_t stream_id, uint64_t first, int64_t n, int mode, double env,
+                        double *p4, double *t, double *w, double *ratio, double *u) {
+  int grid = (int)((n + GEN_BLOCK - 1) / GEN_BLOCK);
+  {
+    Prof p(h, TDDP4_K_GEN_RATIO);
+    gen_ratio_kernel<<<grid, GEN_BLOCK, gen_smem_bytes(h->M.n_sys, h->M.n_inst), h->stream>>>(
+        h->M, h->LP, h->RP, 1.0 / h->RP.Gamma, seed, stream_id, first, n, mode, env, p4, t, w, ratio, u,
+        h->gen_scalars, h->gen_flags, h->gen_counts, h->gen_scalars + 1);
+  }
+  CU(cudaGetLastError());
+  return TDDP4_OK;
+}
+
+int tddp4_candidates(tddp4 *h, uint64_t seed, uint32_t stream_id, int64_t first, int64_t n, double *out_p4,
+                     double *out_t, double *out_w, double *out_ratio, double *out_u) {
+  if (!h || n < 0 || first < 0) return fail(h, TDDP4_ERR_ARG, "bad argument");
+  if (!h->have_params) return fail(h, TDDP4_ERR_STATE, "tddp4_set_params has not been called");
+  if (n == 0) return TDDP4_OK;
+  int rc = launch_ratio(h, seed, stream_id, (uint64_t)first, n, 0, 0.0, out_p4, out_t, out_w, out_ratio, out_u);
+  if (rc) return rc;
+  CU(cudaStreamSynchronize(h->stream));
+  return TDDP4_OK;
+}
+
+int tddp4_generate(tddp4 *h, uint64_t seed, uint32_t stream_id, int64_t first, int64_t n_candidates, int64_t n_pilot,
+                   double envelope_scale, int64_t capacity, double *out_p4, double *out_t, int64_t *out_index,
+                   int64_t *n_accepted, int64_t *n_overflow, double *envelope_out) {
+  if (!h || n_candidates < 0 || n_pilot < 0 || capacity < 0 || first < 0 || !n_accepted || !n_overflow || !envelope_out)
+    return fail(h, TDDP4_ERR_ARG, "bad argument");
+  if (!h->have_params) return fail(h, TDDP4_ERR_STATE, "tddp4_set_params has not been called");
+  const int64_t CHUNK = (int64_t)1 << 25;
+  int rc = ensure_gen(h, std::min<int64_t>(std::max<int64_t>(n_candidates, n_pilot), CHUNK));
+  if (rc) return rc;
+  CU(cudaMemsetAsync(h->gen_scalars, 0, 2 * sizeof(unsigned long long), h->stream));
+  double env = envelope_scale;
+  if (n_pilot > 0) {   // G5: exact, order-independent maximum over the pilot
+    for (int64_t f = 0; f < n_pilot; f += CHUNK) {
+      rc = launch_ratio(h, seed, stream_id, (uint64_t)f, std::min(CHUNK, n_pilot - f), 1, 0.0, nullptr, nullptr, nullptr,
+                        nullptr, nullptr);
+      if (rc) return rc;
+    }
+    unsigned long long bits = 0;
+    CU(cudaMemcpyAsync(&bits, h->gen_scalars, sizeof bits, cudaMemcpyDeviceToHost, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    double mx;
+    memcpy(&mx, &bits, sizeof mx);
+    env = envelope_scale * mx;
+  }
+  int64_t total = 0;
+  for (int64_t f = 0; f < n_candidates; f += CHUNK) {   // G6
+    int64_t n = std::min(CHUNK, n_candidates - f);
+    int64_t blocks = (n + GEN_BLOCK - 1) / GEN_BLOCK;
+    rc = launch_ratio(h, seed, stream_id, (uint64_t)(first + f), n, 2, env, nullptr, nullptr, nullptr, nullptr, nullptr);
+    if (rc) return rc;
+    scan_kernel<<<1, 1024, 0, h->stream>>>(h->gen_counts, blocks, h->gen_offs);
+    ++h->launches;
+    CU(cudaGetLastError());
+    {
+      Prof p(h, TDDP4_K_GEN_EMIT);
+      gen_emit_kernel<<<(int)blocks, GEN_BLOCK, 0, h->stream>>>(h->M, 1.0 / h->RP.Gamma, seed, stream_id,
+                                                                (uint64_t)(first + f), n, h->gen_flags, h->gen_offs, total,
+                                                                capacity, out_p4, out_t, out_index);
+    }
+    CU(cudaGetLastError());
+    unsigned long long cnt = 0;
+    CU(cudaMemcpyAsync(&cnt, h->gen_offs + blocks, sizeof cnt, cudaMemcpyDeviceToHost, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    total += (int64_t)cnt;
+  }
+  unsigned long long over = 0;
+  CU(cudaMemcpyAsync(&over, h->gen_scalars + 1, sizeof over, cudaMemcpyDeviceToHost, h->stream));
+  CU(cudaStreamSynchronize(h->stream));
+  *n_accepted = total;
+  *n_overflow = (int64_t)over;
+  *envelope_out = env;
+  if (total > capacity) return fail(h, TDDP4_ERR_CAPACITY, "%lld accepted events exceed capacity %lld", (long long)total, (long long)capacity);
+  return TDDP4_OK;
+}
+
+int tddp4_weight_bound(const tddp4 *h, double *bound_out) {
+  if (!h || !bound_out) return TDDP4_ERR_ARG;
+  const double *m = h->M.m_final;
+  double M = h->M.m_parent;
+  *bound_out = host_breakup(M, m[0] + m[1] + m[2], m[3]) * host_breakup(M - m[3], m[0] + m[1], m[2]) *
+               host_breakup(M - m[2] - m[3], m[0], m[1]);
+  return TDDP4_OK;
+}
+
+// ---- inspection ---------------------------------------------------------------------------------------
+int tddp4_get(tddp4 *h, int which, int what, double *out) {
+  if (!h || which < 0 || which > 1 || !out) return fail(h, TDDP4_ERR_ARG, "bad argument");
+  EventSet &e = h->set[which];
+  if (!e.loaded) return fail(h, TDDP4_ERR_STATE, "event set %d not loaded", which);
+  const ModelTab &M = h->M;
+  auto rows = [&](const double *src, int nrows, size_t elem) -> int {
+    CU(cudaMemcpy2DAsync(out, elem * e.n, src, elem * e.ld, elem * e.n, nrows, cudaMemcpyDeviceToDevice, h->stream));
+    CU(cudaStreamSynchronize(h->stream));
+    return TDDP4_OK;
+  };
+  switch (what) {
+    case TDDP4_GET_S: return rows(e.s, M.n_sys, sizeof(double));
+    case TDDP4_GET_SHAPE: return rows(e.g, M.n_inst, sizeof(double));
+    case TDDP4_GET_STATIC: {
+      for (int k = 0; k < M.n_terms; ++k)
+        CU(cudaMemcpyAsync(out + (int64_t)M.user_term[k] * e.n, e.f + (int64_t)k * e.ld, sizeof(double) * e.n,
+                           cudaMemcpyDeviceToDevice, h->stream));
+      CU(cudaStreamSynchronize(h->stream));
+      return TDDP4_OK;
+    }
+    case TDDP4_GET_COLUMNS: {
+      if (!h->have_params) return fail(h, TDDP4_ERR_STATE, "tddp4_set_params has not been called");
+      int rc = run_columns(h, e);
+      if (rc) return rc;
+      return rows(reinterpret_cast<const double *>(e.a), M.n_kc, sizeof(double2));
+    }
+    case TDDP4_GET_TERMS: {
+      if (!h->have_params) return fail(h, TDDP4_ERR_STATE, "tddp4_set_params has not been called");
+      if (e.n == 0) return TDDP4_OK;
+      int grid = (int)((e.n + COL_BLOCK - 1) / COL_BLOCK);
+      size_t smem = (size_t)std::max(1, M.n_inst) * COL_BLOCK * sizeof(double2);
+      terms_kernel<<<grid, COL_BLOCK, smem, h->stream>>>(M, h->LP, e.s, e.g, e.f, e.ld, e.n, reinterpret_cast<double2 *>(out));
+      ++h->launches;
+      CU(cudaGetLastError());
+      CU(cudaStreamSynchronize(h->stream));
+      return TDDP4_OK;
+    }
+  }
+  return fail(h, TDDP4_ERR_ARG, "unknown cache id %d", what);
+}
+
+int tddp4_layout(const tddp4 *h, int *n_sys, int *sys_mask, int *n_inst, int *inst_res, int *inst_sys, int *inst_sub) {
+  if (!h) return TDDP4_ERR_ARG;
+  const ModelTab &M = h->M;
+  if (n_sys) *n_sys = M.n_sys;
+  if (n_inst) *n_inst = M.n_inst;
+  for (int i = 0; i < M.n_sys; ++i)
+    if (sys_mask) sys_mask[i] = M.sys_mask[i];
+  for (int j = 0; j < M.n_inst; ++j) {
+    if (inst_res) inst_res[j] = M.inst[j].res;
+    if (inst_sys) inst_sys[j] = M.inst[j].sys;
+    if (inst_sub) inst_sub[j] = M.inst[j].sub;
+  }
+  return TDDP4_OK;
+}
+
+int tddp4_profile(tddp4 *h, int enable) {
+  if (!h) return TDDP4_ERR_ARG;
+  h->profiling = enable != 0;
+  return TDDP4_OK;
+}
+
+int tddp4_profile_read(tddp4 *h, int kernel_id, double *total_ms, int64_t *launches) {
+  if (!h || kernel_id < 0 || kernel_id >= TDDP4_K_COUNT || !total_ms || !launches) return fail(h, TDDP4_ERR_ARG, "bad argument");
+  drain_profile(h);
+  *total_ms = h->prof_ms[kernel_id];
+  *launches = h->prof_n[kernel_id];
+  return TDDP4_OK;
+}
+
+int tddp4_profile_reset(tddp4 *h) {
+  if (!h) return TDDP4_ERR_ARG;
+  drain_profile(h);
+  for (int i = 0; i < TDDP4_K_COUNT; ++i) { h->prof_ms[i] = 0; h->prof_n[i] = 0; }
+  return TDDP4_OK;
+}
+
+int64_t tddp4_launch_count(const tddp4 *h) { return h ? h->launches : 0; }
+
+}  // extern "C"
