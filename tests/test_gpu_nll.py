@@ -1,0 +1,309 @@
+"""GPU parity: the NLL path (steps 0-7 of SURVEY.md 8(a)) through the C-ABI against the CPU oracle.
+
+Tolerances are BASELINE.json's north_star: relative 1e-10 per event probability, 1e-11 on the NLL
+(relative to max(|NLL|, 1e-3 sum |log P_i|)).  Inputs come from the oracle's own generator
+(tests/samples.py); nothing the oracle sees was produced by the CUDA path."""
+import math
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_1702_06735_b200 import workloads as W
+
+import samples
+
+pytestmark = pytest.mark.gpu
+
+TOL_P = 1e-10
+TOL_NLL = 1e-11
+TOL_LAYER = 1e-11
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_1702_06735_b200 import binding
+    binding.load_library()
+    return binding
+
+
+def nll_close(got, ref, logs):
+    scale = max(abs(ref), 1e-3 * float(np.sum(np.abs(logs))))
+    return abs(got - ref) <= TOL_NLL * scale
+
+
+def run_case(B, mdl, par, p4, t, p4n, w=None, from_host=True):
+    import torch
+    h = B.Tddp4(mdl)
+    if from_host:
+        h.load_events(0, p4, t)
+        h.load_events(1, p4n, None, weight=w)
+    else:
+        dev = lambda a: None if a is None else torch.from_numpy(np.ascontiguousarray(a)).cuda()
+        h.load_events(0, dev(p4), dev(t))
+        h.load_events(1, dev(p4n), None, weight=dev(w))
+    h.set_params(par)
+    prob = h.empty(max(1, p4.shape[1]))
+    nll = h.nll(prob)
+    return h, nll, prob[:p4.shape[1]].cpu().numpy()
+
+
+def check_against_oracle(B, mdl, par, p4, t, p4n, w=None, from_host=True):
+    ref_nll, ref_norm, ref_P, st = oracle.nll(mdl, par, p4, t, p4n, w)
+    assert st == 0
+    h, nll, P = run_case(B, mdl, par, p4, t, p4n, w, from_host)
+    assert samples.rel_err(P, ref_P) < TOL_P
+    assert abs(h.nll_parts()["norm"] / ref_norm - 1.0) < 1e-12
+    assert nll_close(nll, ref_nll, np.log(ref_P))
+    assert h.nll() == nll                      # without prob_out: same value bit for bit
+    return h
+
+
+def test_config1_full(B):
+    """BASELINE config 1 at full size: 1 000 model-drawn events, 10 000 flat events, K = 3."""
+    cfg = W.config(1)
+    p4, t, _ = samples.data_sample(("C", 1), cfg.n_data)
+    p4n, _ = samples.flat_sample(cfg.n_norm)
+    check_against_oracle(B, cfg.model, W.initial_params(cfg.model), p4, t, p4n)
+
+
+@pytest.mark.parametrize("from_host", [True, False])
+def test_config2_model_ragged(B, from_host):
+    """8 chains (all six spin-factor kinds); sizes that span several tiles and leave a ragged tail."""
+    mdl = samples.model_of(("C", 2))
+    p4, t, _ = samples.data_sample(("C", 2), 4_133)
+    p4n, _ = samples.flat_sample(20_011)
+    check_against_oracle(B, mdl, W.initial_params(mdl), p4, t, p4n, from_host=from_host)
+
+
+def test_config3_model_bose_weights(B):
+    """16 Bose-symmetrised terms on 8 couplings, efficiency weights on the normalisation sample."""
+    mdl = samples.model_of(("C", 3))
+    p4, t, _ = samples.data_sample(("C", 3), 3_001)
+    p4n, _ = samples.flat_sample(10_007)
+    w = np.random.default_rng(7).uniform(0.5, 1.0, p4n.shape[1])
+    check_against_oracle(B, mdl, W.initial_params(mdl), p4, t, p4n, w)
+
+
+def test_layers(B):
+    """Per-layer parity: s-values, static factors S_k F, per-term amplitudes, columns."""
+    import torch
+    mdl = samples.model_of(("C", 3))
+    par = W.initial_params(mdl)
+    p4, _, _, _ = oracle.candidates(mdl, par.tau, 42, 5, 0, 2_077)     # raw candidates: whole phase space
+    t = np.full(p4.shape[1], 0.3)
+    h = B.Tddp4(mdl)
+    h.load_events(0, p4, t)
+    h.set_params(par)
+    S, F, a = oracle.terms(mdl, par, p4)
+    lay = h.layout()
+    s_gpu = h.get(0, B.GET_S).cpu().numpy()
+    P = p4.reshape(4, 4, -1)
+    for row, mask in enumerate(lay["sys_mask"]):
+        q = sum(P[i] for i in range(4) if mask >> i & 1)
+        s_ref = q[0] ** 2 - q[1] ** 2 - q[2] ** 2 - q[3] ** 2
+        assert samples.rel_err(s_gpu[row], s_ref) < 1e-13
+    f_gpu = h.get(0, B.GET_STATIC).cpu().numpy()
+    scale = np.abs(S * F).max(axis=1, keepdims=True)
+    assert np.max(np.abs(f_gpu - S * F) / scale) < TOL_LAYER
+    a_gpu = h.get(0, B.GET_TERMS).cpu().numpy()
+    scale = np.abs(a).max(axis=1, keepdims=True)
+    assert np.max(np.abs(a_gpu - a) / scale) < TOL_LAYER
+    col = h.get(0, B.GET_COLUMNS).cpu().numpy()
+    ref_col = np.zeros_like(col)
+    for k, kap in enumerate(mdl.term_coupling):
+        ref_col[kap] += a[k]
+    scale = np.abs(ref_col).max(axis=1, keepdims=True)
+    assert np.max(np.abs(col - ref_col) / scale) < TOL_LAYER
+
+
+def test_trajectory_dirty_tracking(B):
+    """Parameter steps as the minimiser would make them: every call is checked against a from-scratch oracle
+    evaluation, so stale caches (lineshapes not refreshed, Gram matrix not rebuilt) cannot hide."""
+    mdl = samples.model_of(("C", 3))
+    p0 = W.initial_params(mdl)
+    p4, t, _ = samples.data_sample(("C", 3), 1_500)
+    p4n, _ = samples.flat_sample(6_000)
+    h = B.Tddp4(mdl)
+    h.load_events(0, p4, t)
+    h.load_events(1, p4n)
+    steps = W.trajectory(mdl, p0, 12, "minuit", rel=1e-2) + W.trajectory(mdl, p0, 4, "coupling_only") + \
+        W.trajectory(mdl, p0, 3, "all", rel=1e-2)
+    prob = h.empty(p4.shape[1])
+    for par in [p0] + steps:
+        h.set_params(par)
+        nll = h.nll(prob)
+        ref_nll, ref_norm, ref_P, st = oracle.nll(mdl, par, p4, t, p4n)
+        assert st == 0
+        assert samples.rel_err(prob.cpu().numpy(), ref_P) < TOL_P
+        assert nll_close(nll, ref_nll, np.log(ref_P))
+
+
+def test_bit_reproducible_and_async_slots(B):
+    mdl = samples.model_of(("C", 2))
+    par = W.initial_params(mdl)
+    p4, t, _ = samples.data_sample(("C", 2), 4_133)
+    p4n, _ = samples.flat_sample(20_011)
+    h = B.Tddp4(mdl)
+    h.load_events(0, p4, t)
+    h.load_events(1, p4n)
+    h.set_params(par)
+    first = h.nll()
+    assert all(h.nll() == first for _ in range(5))
+    steps = W.trajectory(mdl, par, 8, "couplings_xy")
+    sync = []
+    for p in steps:
+        h.set_params(p)
+        sync.append(h.nll())
+    for s, p in enumerate(steps):              # pipelined: enqueue all, then collect
+        h.set_params(p)
+        h.nll_async(s)
+    assert [h.nll_result(s) for s in range(len(steps))] == sync
+    h2 = B.Tddp4(mdl)                          # a second handle gives the same bits
+    h2.load_events(0, p4, t)
+    h2.load_events(1, p4n)
+    h2.set_params(par)
+    assert h2.nll() == first
+
+
+@pytest.mark.parametrize("n", [1, 31, 32, 33, 255, 257, 1025])
+def test_ragged_sizes(B, n):
+    mdl = samples.model_of(("C", 1))
+    p4, t, _ = samples.data_sample(("C", 1), 1_025)
+    p4n, _ = samples.flat_sample(777)
+    check_against_oracle(B, mdl, W.initial_params(mdl), p4[:, :n].copy(), t[:n].copy(), p4n[:, :max(1, n // 2)].copy())
+
+
+def test_strided_device_input(B):
+    """load_events with ld > n: rows of a larger device buffer are read in place."""
+    import torch
+    mdl = samples.model_of(("C", 1))
+    par = W.initial_params(mdl)
+    p4, t, _ = samples.data_sample(("C", 1), 600)
+    p4n, _ = samples.flat_sample(777)
+    big = torch.zeros(16, 1000, dtype=torch.float64, device="cuda")
+    big[:, :600] = torch.from_numpy(p4).cuda()
+    h = B.Tddp4(mdl)
+    h.load_events(0, big[:, :600], torch.from_numpy(t).cuda())
+    h.load_events(1, p4n)
+    h.set_params(par)
+    ref = oracle.nll(mdl, par, p4, t, p4n)
+    assert nll_close(h.nll(), ref[0], np.log(ref[2]))
+
+
+def test_empty_data_sample(B):
+    mdl = samples.model_of(("C", 1))
+    p4n, _ = samples.flat_sample(777)
+    h = B.Tddp4(mdl)
+    h.load_events(0, np.zeros((16, 0)), np.zeros(0))
+    h.load_events(1, p4n)
+    h.set_params(W.initial_params(mdl))
+    assert h.nll() == 0.0                       # empty sum
+
+
+def test_special_cases_of_eq1(B):
+    """x = y = 0 -> P independent of cbar; common global phase and common real scale leave the NLL unchanged."""
+    mdl = samples.model_of(("C", 2))
+    par = W.initial_params(mdl)
+    p4, t, _ = samples.data_sample(("C", 2), 2_000)
+    p4n, _ = samples.flat_sample(5_000)
+    h = B.Tddp4(mdl)
+    h.load_events(0, p4, t)
+    h.load_events(1, p4n)
+    h.set_params(par)
+    base = h.nll()
+    q = par.copy(); q.c = par.c * np.exp(0.7j); q.cbar = par.cbar * np.exp(0.7j)
+    h.set_params(q)
+    assert abs(h.nll() - base) < 1e-9 * abs(base)
+    q = par.copy(); q.c = par.c * 3.0; q.cbar = par.cbar * 3.0
+    h.set_params(q)
+    assert abs(h.nll() - base) < 1e-9 * abs(base)
+    q = par.copy(); q.x = 0.0; q.y = 0.0
+    h.set_params(q)
+    a = h.nll()
+    q.cbar = par.cbar[::-1].copy() * 0.3
+    h.set_params(q)
+    assert abs(h.nll() - a) < 1e-10 * abs(a)
+
+
+def test_errors(B):
+    mdl = samples.model_of(("C", 1))
+    par = W.initial_params(mdl)
+    p4, t, _ = samples.data_sample(("C", 1), 100)
+    p4n, _ = samples.flat_sample(777)
+    h = B.Tddp4(mdl)
+    with pytest.raises(B.Tddp4Error) as e:
+        h.nll()
+    assert e.value.code == B.ERR_STATE
+    h.load_events(0, p4, t)
+    h.set_params(par)
+    with pytest.raises(B.Tddp4Error) as e:      # normalisation sample missing
+        h.nll()
+    assert e.value.code == B.ERR_STATE
+    h.load_events(1, p4n)
+    bad = par.copy(); bad.mass = par.mass.copy(); bad.mass[0] = 0.3     # K* pole below the K pi threshold
+    with pytest.raises(B.Tddp4Error) as e:
+        h.set_params(bad)
+    assert e.value.code == B.ERR_DOMAIN
+    zero = par.copy(); zero.c = par.c * 0; zero.cbar = par.cbar * 0    # rate vanishes: P_i = 0/0
+    h.set_params(zero)
+    with pytest.raises(B.Tddp4Error) as e:
+        h.nll()
+    assert e.value.code == B.ERR_NONFINITE
+    assert h.nll(strict=False) == math.inf
+    h.set_params(par)                           # the handle recovers
+    ref = oracle.nll(mdl, par, p4, t, p4n)
+    assert nll_close(h.nll(), ref[0], np.log(ref[2]))
+
+
+def test_gram_matches_direct_normalisation(B):
+    """Step 6 both ways: N from the Gram matrix (GPU) equals the direct sum over the sample (oracle), and the
+    Gram matrix itself equals sum_j w_j a_k conj(a_l) built from the oracle's per-term amplitudes."""
+    mdl = samples.model_of(("C", 3))
+    par = W.initial_params(mdl)
+    p4n, _ = samples.flat_sample(10_007)
+    w = np.random.default_rng(3).uniform(0.5, 1.0, p4n.shape[1])
+    h = B.Tddp4(mdl)
+    h.load_events(1, p4n, None, weight=w)
+    h.set_params(par)
+    G, n = h.gram()
+    assert n == p4n.shape[1]
+    _, _, a = oracle.terms(mdl, par, p4n)
+    col = np.zeros((mdl.n_couplings, p4n.shape[1]), complex)
+    for k, kap in enumerate(mdl.term_coupling):
+        col[kap] += a[k]
+    G_ref = (col * w) @ col.conj().T
+    assert np.max(np.abs(G - G_ref)) < 1e-12 * np.abs(G_ref).max()
+    ref_norm, _ = oracle.norm(mdl, par, p4n, w)
+    assert abs(h.norm() / ref_norm - 1.0) < 1e-12
+
+
+def test_sharded_evaluation_adds_up(B):
+    """SURVEY.md 8(e) on one GPU: two handles hold halves of both samples; summing their Gram matrices and
+    their (sum log B, sum t) parts in rank order reproduces the single-handle NLL."""
+    mdl = samples.model_of(("C", 2))
+    par = W.initial_params(mdl)
+    p4, t, _ = samples.data_sample(("C", 2), 4_133)
+    p4n, _ = samples.flat_sample(20_011)
+    one = B.Tddp4(mdl)
+    one.load_events(0, p4, t); one.load_events(1, p4n); one.set_params(par)
+    full = one.nll()
+    cut, cutn = 2_000, 9_000
+    hs = [B.Tddp4(mdl), B.Tddp4(mdl)]
+    hs[0].load_events(0, p4[:, :cut].copy(), t[:cut].copy()); hs[0].load_events(1, p4n[:, :cutn].copy())
+    hs[1].load_events(0, p4[:, cut:].copy(), t[cut:].copy()); hs[1].load_events(1, p4n[:, cutn:].copy())
+    Gs = []
+    for h in hs:
+        h.set_params(par)
+        Gs.append(h.gram())
+    G = Gs[0][0] + Gs[1][0]
+    n = Gs[0][1] + Gs[1][1]
+    sum_log_b = sum_t = 0.0
+    for h in hs:
+        h.gram_override(G, n)
+        h.nll(strict=True)
+        parts = h.nll_parts()
+        sum_log_b += parts["sum_log_B"]; sum_t += parts["sum_t"]
+        norm = parts["norm"]
+    nll = sum_t / par.tau - sum_log_b + p4.shape[1] * math.log(norm)
+    assert abs(nll - full) < 1e-12 * abs(full)
