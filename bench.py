@@ -1,0 +1,355 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the hot path on BASELINE.json's headline workload (configs[2], "C3" in SURVEY.md 8):
+1 000 000 data events, 4 000 000 flat normalisation events, 16 Bose-symmetrised terms on 8 couplings, masses and
+widths floating, consecutive NLL evaluations along a seeded MINUIT-like parameter trajectory.
+
+One "step" = one NLL evaluation (tddp4_set_params + tddp4_nll): lineshapes and coupling columns are refreshed for
+whatever that step's parameter change made dirty, the Gram matrix of the normalisation sample is rebuilt if a
+mass or width moved, then the amplitude-sum + rate + -log pass runs over the data sample.  Kinematics and spin
+factors (step 1) run once per event set, at load, as the paper's de-duplication licence allows.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+
+Prints ONE JSON line (see DESIGN.md "Measurement" for every key).  Metric: events x NLL evaluations per second.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+from paper_1702_06735_b200 import workloads as W  # noqa: E402
+
+METRIC = "nll_events_x_evals_per_s"
+UNIT = "events*evals/s"
+WORKLOAD = "C3"
+TRAJECTORY = "minuit"
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            p = json.load(f)
+        return float(p["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)"
+    return 6650.0, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler(threading.Thread):
+    """Samples SM clock and throttle reasons through NVML while the timed region runs."""
+
+    def __init__(self, index, period=0.01):
+        super().__init__(daemon=True)
+        self.index, self.period = index, period
+        self.sm, self.reasons, self.stop_flag = [], set(), False
+        self.max_mhz = None
+        try:
+            import pynvml
+            pynvml.nvmlInit()
+            self.nv = pynvml
+            self.dev = pynvml.nvmlDeviceGetHandleByIndex(index)
+            self.max_mhz = pynvml.nvmlDeviceGetMaxClockInfo(self.dev, pynvml.NVML_CLOCK_SM)
+        except Exception:
+            self.nv = None
+
+    NAMES = {0x8: "hw_slowdown", 0x40: "hw_thermal_slowdown", 0x20: "sw_thermal_slowdown", 0x4: "sw_power_cap",
+             0x80: "hw_power_brake_slowdown", 0x2: "applications_clocks_setting", 0x100: "display_clock_setting"}
+
+    def run(self):
+        if self.nv is None:
+            return
+        while not self.stop_flag:
+            try:
+                self.sm.append(self.nv.nvmlDeviceGetClockInfo(self.dev, self.nv.NVML_CLOCK_SM))
+                r = self.nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.dev)
+                for bit, name in self.NAMES.items():
+                    if r & bit:
+                        self.reasons.add(name)
+            except Exception:
+                pass
+            time.sleep(self.period)
+
+    def summary(self):
+        self.stop_flag = True
+        if self.is_alive():
+            self.join()
+        return {"sm_mhz": float(np.median(self.sm)) if self.sm else None, "sm_max_mhz": self.max_mhz,
+                "reasons": sorted(self.reasons), "samples": len(self.sm)}
+
+
+def build_workload(binding, cfg, device, seed):
+    """Seeded synthetic samples of the config, produced on the device by the CUDA generator:
+    flat normalisation sample = hit-or-miss on the Raubold-Lynch weight; data = accept-reject against the model."""
+    flat = W.flat_model()
+    hf = binding.Tddp4(flat, device)
+    hf.set_params(W.flat_params(flat))
+    p4n, _, _, _ = hf.generate_n(seed, W.STREAM_NORM, cfg.n_norm, 0, 2.0 * hf.weight_bound(), chunk=1 << 24)
+    hf.close()
+    hg = binding.Tddp4(cfg.model, device)
+    hg.set_params(W.initial_params(cfg.model))
+    p4, t, _, info = hg.generate_n(seed, W.STREAM_DATA, cfg.n_data, cfg.n_pilot, cfg.envelope_scale, chunk=1 << 24)
+    hg.close()
+    return p4, t, p4n, info
+
+
+def kernel_table(prof, total_ms):
+    hbm, which = peaks()
+    out = {}
+    for name, (ms, n, by) in prof.items():
+        if n == 0:
+            continue
+        gbs = by / (ms * 1e-3) / 1e9 if ms > 0 else 0.0
+        out[name] = {"launches": n, "ms": round(ms, 4), "share": round(ms / total_ms, 4) if total_ms > 0 else None,
+                     "us_per_launch": round(1e3 * ms / n, 3), "alg_MB_per_launch": round(by / n / 1e6, 3),
+                     "achieved_GBs": round(gbs, 1), "frac": round(gbs / hbm, 4)}
+    return out
+
+
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    from paper_1702_06735_b200 import binding
+
+    rank, world = int(os.environ.get("RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
+    local = int(os.environ.get("LOCAL_RANK", 0))
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device(f"cuda:{local}"))
+    device = f"cuda:{local}"
+    torch.cuda.set_device(device)
+    binding.load_library()          # fails loudly if the CUDA extension is missing: there is no fallback
+
+    cfg = W.config(3)
+    mdl = cfg.model
+    N, Nn, KC = cfg.n_data, cfg.n_norm, mdl.n_couplings
+    # weak scaling: every rank evaluates its own independent replica of the workload (own seed), SURVEY.md 8(e)
+    p4, t, p4n, ginfo = build_workload(binding, cfg, device, W.BASE_SEED + rank)
+    p0 = W.initial_params(mdl)
+    traj = W.trajectory(mdl, p0, args.warmup + args.steps, TRAJECTORY)
+
+    stream = torch.cuda.Stream(device)
+    h = binding.Tddp4(mdl, device)
+    h.set_stream(stream)
+    h.load_events(0, p4, t)
+    h.load_events(1, p4n)
+    packed = h.pack_params(traj)
+    torch.cuda.synchronize()
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # ---- device-timed region: K steps enqueued back to back through tddp4_nll_batch ---------------------------
+    h.set_params(p0)
+    h.nll()
+    h.nll_batch(packed[:args.warmup])
+    h.profile(True)
+    h.profile_reset()
+    launches0 = h.launch_count()
+    sampler = ClockSampler(local)
+    ev0, ev1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    sampler.start()
+    ev0.record(stream)
+    nll_vals, _ = h.nll_batch(packed[args.warmup:])
+    ev1.record(stream)
+    barrier()
+    clocks = sampler.summary()
+    ms = ev0.elapsed_time(ev1)
+    launches = h.launch_count() - launches0
+    prof = h.profile_read()
+    h.profile(False)
+    if world > 1:
+        tms = torch.tensor([ms], device=device, dtype=torch.float64)
+        dist.all_reduce(tms, op=dist.ReduceOp.MAX)
+        ms = float(tms.item())
+    value = world * N * args.steps / (ms * 1e-3)
+
+    # ---- the same K steps without per-kernel events (what the events cost) -----------------------------------
+    ev2, ev3 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    h.set_params(p0)
+    h.nll_batch(packed[:args.warmup])
+    torch.cuda.synchronize()
+    ev2.record(stream)
+    h.nll_batch(packed[args.warmup:])
+    ev3.record(stream)
+    torch.cuda.synchronize()
+    ms_noprof = ev2.elapsed_time(ev3)
+
+    # ---- sub-cases reported next to the mixture ---------------------------------------------
+    sub = {}
+    for kind in ("coupling_only", "all"):
+        tr = h.pack_params(W.trajectory(mdl, p0, args.warmup + args.steps, kind))
+        h.set_params(p0)
+        h.nll_batch(tr[:args.warmup])
+        torch.cuda.synchronize()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record(stream)
+        h.nll_batch(tr[args.warmup:])
+        b.record(stream)
+        torch.cuda.synchronize()
+        m = a.elapsed_time(b)
+        sub[kind] = {"ms_per_step": round(m / args.steps, 5), "value": N * args.steps / (m * 1e-3)}
+
+    # ---- end to end through the C-ABI with HOST buffers: load both samples from pinned host memory, then K
+    #      synchronous tddp4_set_params + tddp4_nll calls, all inside the timed region ------------------------
+    host = [torch.empty(x.shape, dtype=torch.float64, pin_memory=True).copy_(x) for x in (p4, t, p4n)]
+    hp4, ht, hp4n = [x.numpy() for x in host]
+    torch.cuda.synchronize()
+    h2 = binding.Tddp4(mdl, device)
+    barrier()
+    t0 = time.perf_counter()
+    h2.load_events(0, hp4, ht)
+    h2.load_events(1, hp4n)
+    t_load = time.perf_counter() - t0
+    e2e_vals = []
+    for par in traj[args.warmup:]:
+        h2.set_params(par)
+        e2e_vals.append(h2.nll())
+    torch.cuda.synchronize()
+    t_e2e = time.perf_counter() - t0
+    if world > 1:
+        tt = torch.tensor([t_e2e], device=device, dtype=torch.float64)
+        dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+        t_e2e = float(tt.item())
+    assert np.array_equal(np.asarray(e2e_vals), nll_vals), "batched and synchronous evaluations differ"
+    load_bytes = hp4.nbytes + ht.nbytes + hp4n.nbytes
+    e2e = {"value": world * N * args.steps / t_e2e, "unit": UNIT,
+           "h2d_bytes_per_step": load_bytes / args.steps + h2.h2d_bytes_per_call, "d2h_bytes_per_step": 64,
+           "load_events_ms": round(1e3 * t_load, 3), "ms_per_step_after_load": round(1e3 * (t_e2e - t_load) / args.steps, 5),
+           "note": "timed region = tddp4_load_events of both samples from pinned host memory (one-time, amortised "
+                   "over the K steps) + K synchronous tddp4_set_params/tddp4_nll calls"}
+    h2.close()
+
+    if rank != 0:
+        if world > 1:
+            dist.destroy_process_group()
+        return
+
+    total_kernel_ms = sum(v[0] for v in prof.values())
+    ktab = kernel_table(prof, total_kernel_ms)
+    dominant = max(ktab, key=lambda k: ktab[k]["ms"])
+    hbm, which = peaks()
+    roof = {"kernel": dominant, "bound": "hbm", "achieved": ktab[dominant]["achieved_GBs"], "peak": hbm, "unit": "GB/s",
+            "frac": ktab[dominant]["frac"], "peak_source": which, "traffic": None,
+            "alg_bytes_per_launch": ktab[dominant]["alg_MB_per_launch"] * 1e6, "us_per_launch": ktab[dominant]["us_per_launch"]}
+    traffic_file = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(traffic_file):
+        with open(traffic_file) as f:
+            tr = json.load(f)
+        roof["traffic"] = tr.get(dominant, {}).get("dram_bytes_per_launch")
+        for k in ktab:
+            ktab[k]["traffic"] = tr.get(k, {}).get("dram_bytes_per_launch")
+
+    cpu = cpu_baseline(mdl, p0, p4, t, p4n)
+    line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
+            "config": {"workload": WORKLOAD, "n_data": N, "n_norm": Nn, "n_terms": mdl.n_terms, "n_couplings": KC,
+                       "trajectory": TRAJECTORY + " (p=0.8 one of 46 floating parameters moves, p=0.2 all move)",
+                       "l2": "inputs larger than L2: a coupling-only step streams 136 MB, a dirty step 1.5+ GB; no flush",
+                       "generation": {"data_candidates": ginfo["n_candidates"], "envelope": ginfo["envelope"]}},
+            "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roof, "kernels": ktab,
+            "ms_per_step_without_kernel_events": ms_noprof / args.steps,
+            "coupling_only": sub["coupling_only"], "all_dirty": sub["all"], "cpu_baseline": cpu,
+            "nll_first_last": [float(nll_vals[0]), float(nll_vals[-1])]}
+    print(json.dumps(line))
+    if world > 1:
+        dist.destroy_process_group()
+
+
+def cpu_baseline(mdl, par, p4, t, p4n, n_data=100_000):
+    """The oracle as it stands, timed on this box's host cores on a bounded sample of the same workload."""
+    import oracle
+    n_norm = 4 * n_data
+    a, b, c = p4[:, :n_data].cpu().numpy(), t[:n_data].cpu().numpy(), p4n[:, :n_norm].cpu().numpy()
+    a, c = np.ascontiguousarray(a), np.ascontiguousarray(c)
+    best = float("inf")
+    for _ in range(3):
+        t0 = time.perf_counter()
+        oracle.nll(mdl, par, a, b, c, want_prob=False)
+        best = min(best, time.perf_counter() - t0)
+    return {"value": n_data / best, "unit": UNIT, "cores": oracle.threads(), "kind": "oracle",
+            "sample": f"first {n_data} data + {n_norm} normalisation events of the same samples, 1 full-recompute NLL "
+                      f"evaluation, best of 3 ({best:.3f} s)"}
+
+
+def run_reference(args):
+    """`--impl reference`: the CPU oracle, as it stands, on this box's host cores; same metric, config and trajectory.
+    Each step is one full-recompute NLL evaluation on a bounded sample of the workload (same 1:4 data:normalisation
+    ratio, same model), sized from a calibration call so that the W + K steps end within a few minutes.  No CUDA."""
+    rank = int(os.environ.get("RANK", 0))
+    if rank != 0:
+        return
+    import oracle
+    import math
+    cfg = W.config(3)
+    mdl = cfg.model
+    p0 = W.initial_params(mdl)
+    traj = W.trajectory(mdl, p0, args.warmup + args.steps, TRAJECTORY)
+    flat, fpar = W.flat_model(), W.flat_params(W.flat_model())
+    bound = math.prod(oracle.breakup(*tr) for tr in W.flat_envelope_inputs(flat))
+
+    def sample(n_data):
+        n_norm = 4 * n_data
+        g = oracle.generate(flat, fpar, W.BASE_SEED, W.STREAM_NORM, int(n_norm / 0.06) + 5000, 0, 2.0 * bound, n_norm)
+        assert g["n_accepted"] >= n_norm
+        n_cand = 80 * n_data + 20000
+        while True:
+            d = oracle.generate(mdl, p0, W.BASE_SEED, W.STREAM_DATA, n_cand, min(cfg.n_pilot, n_cand // 4), cfg.envelope_scale, n_data)
+            if d["n_accepted"] >= n_data:
+                return d["p4"][:, :n_data].copy(), d["t"][:n_data].copy(), g["p4"][:, :n_norm].copy()
+            n_cand *= 2
+
+    p4, t, p4n = sample(2000)
+    t0 = time.perf_counter()
+    oracle.nll(mdl, p0, p4, t, p4n, want_prob=False)
+    rate = 2000 / (time.perf_counter() - t0)                    # data events per second of one evaluation
+    budget_s = 90.0
+    n_data = int(max(500, min(50_000, rate * budget_s / (args.warmup + args.steps))))   # cap bounds the (untimed) generation
+    if n_data != 2000:
+        p4, t, p4n = sample(n_data)
+    for par in traj[:args.warmup]:
+        oracle.nll(mdl, par, p4, t, p4n, want_prob=False)
+    t0 = time.perf_counter()
+    vals = [oracle.nll(mdl, par, p4, t, p4n, want_prob=False)[0] for par in traj[args.warmup:]]
+    dt = time.perf_counter() - t0
+    value = n_data * args.steps / dt
+    samp = (f"{n_data} data + {4 * n_data} normalisation events per step (oracle-generated with the workload's recipe), "
+            f"{args.steps} full-recompute NLL evaluations along the same trajectory")
+    line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": 1, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+            "config": {"workload": WORKLOAD, "n_data": cfg.n_data, "n_norm": cfg.n_norm, "n_terms": mdl.n_terms,
+                       "n_couplings": mdl.n_couplings, "trajectory": TRAJECTORY, "sample": samp},
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": oracle.threads(), "kind": "oracle", "sample": samp},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0, "nll_first_last": [vals[0], vals[-1]]}
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=1000)     # BASELINE.json configs[2]: 1 000 consecutive evaluations
+    ap.add_argument("--warmup", type=int, default=10)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3 if args.impl == "ours" else 0)
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

@@ -126,6 +126,16 @@ int tddp4_nll_result(tddp4 *h, int slot, double *nll_out);
  * of events with non-positive / non-finite rate.                                                     */
 int tddp4_nll_parts(tddp4 *h, int slot, double out[5]);
 
+/* Batched form for independent parameter points (the 2 n_par points of a numerical gradient, a scan, a
+ * replayed minimiser trajectory): equivalent to tddp4_set_params + tddp4_nll for each point in order, with all
+ * evaluations enqueued back to back and ONE synchronisation at the end.  params: host [n_points][stride],
+ * stride = tddp4_param_stride(h) = 4 K_c + 2 n_res + 3, one point laid out as c[K_c][2], cbar[K_c][2],
+ * mass_width[n_res][2], x, y, tau.  nll_out: host [n_points]; status_out: host [n_points] or NULL, per-point
+ * tddp4_status (a failed point gets NaN, or +inf for TDDP4_ERR_NONFINITE).  Returns the first non-OK status.
+ * The handle is left holding the last valid point's parameters.                                        */
+int tddp4_param_stride(const tddp4 *h);
+int tddp4_nll_batch(tddp4 *h, int64_t n_points, const double *params, double *nll_out, int *status_out);
+
 /* ---- step 6: normalisation through the Gram matrix ----------------------------------------------- */
 /* G_sum[k][l] = sum_j w_j a_k(p_j) conj(a_l(p_j)) over THIS handle's normalisation sample for the
  * current masses/widths (recomputed if dirty); host [K_c][K_c][2]; *n_norm = its event count.         */
@@ -177,8 +187,10 @@ enum {
   TDDP4_K_GEN_EMIT = 5, TDDP4_K_COUNT = 6
 };
 int tddp4_profile(tddp4 *h, int enable);
-/* total_ms, launches since the last reset, for one kernel id; synchronises.                          */
-int tddp4_profile_read(tddp4 *h, int kernel_id, double *total_ms, int64_t *launches);
+/* total_ms, launches and (alg_bytes may be NULL) the algorithmic bytes of those launches -- the rows each launch
+ * had to read and write, counted on the host from its dirty masks, DESIGN.md "Kernels" -- since the last reset,
+ * for one kernel id; synchronises.                                                                     */
+int tddp4_profile_read(tddp4 *h, int kernel_id, double *total_ms, int64_t *launches, double *alg_bytes);
 int tddp4_profile_reset(tddp4 *h);
 /* Number of kernels this handle has launched since creation (all kinds).                            */
 int64_t tddp4_launch_count(const tddp4 *h);

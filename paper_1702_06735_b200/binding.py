@@ -23,7 +23,7 @@ KERNEL_NAMES = ["kin", "columns", "gram", "nll", "gen_ratio", "gen_emit"]
 # every symbol include/tddp4.h declares
 SYMBOLS = ["tddp4_create", "tddp4_destroy", "tddp4_set_stream", "tddp4_last_error", "tddp4_version",
            "tddp4_load_events", "tddp4_set_params", "tddp4_nll", "tddp4_nll_async", "tddp4_nll_result",
-           "tddp4_nll_parts", "tddp4_gram", "tddp4_gram_override", "tddp4_norm", "tddp4_generate", "tddp4_weight_bound",
+           "tddp4_nll_parts", "tddp4_param_stride", "tddp4_nll_batch", "tddp4_gram", "tddp4_gram_override", "tddp4_norm", "tddp4_generate", "tddp4_weight_bound",
            "tddp4_candidates", "tddp4_get", "tddp4_layout", "tddp4_profile", "tddp4_profile_read",
            "tddp4_profile_reset", "tddp4_launch_count"]
 
@@ -74,6 +74,8 @@ def load_library():
     L.tddp4_nll_async.argtypes = [vp, C.c_int]
     L.tddp4_nll_result.argtypes = [vp, C.c_int, dp]
     L.tddp4_nll_parts.argtypes = [vp, C.c_int, dp]
+    L.tddp4_param_stride.argtypes = [vp]
+    L.tddp4_nll_batch.argtypes = [vp, i64, vp, vp, vp]
     L.tddp4_gram.argtypes = [vp, vp, C.POINTER(i64)]
     L.tddp4_gram_override.argtypes = [vp, vp, i64]
     L.tddp4_norm.argtypes = [vp, dp]
@@ -84,7 +86,7 @@ def load_library():
     L.tddp4_get.argtypes = [vp, C.c_int, C.c_int, vp]
     L.tddp4_layout.argtypes = [vp] + [C.POINTER(C.c_int)] * 6
     L.tddp4_profile.argtypes = [vp, C.c_int]
-    L.tddp4_profile_read.argtypes = [vp, C.c_int, dp, C.POINTER(i64)]
+    L.tddp4_profile_read.argtypes = [vp, C.c_int, dp, C.POINTER(i64), dp]
     L.tddp4_profile_reset.argtypes = [vp]
     L.tddp4_launch_count.argtypes = [vp]
     L.tddp4_launch_count.restype = i64
@@ -220,6 +222,30 @@ class Tddp4:
         self._check(self.lib.tddp4_nll_parts(self._h, slot, out))
         return dict(sum_log_B=out[0], sum_t=out[1], norm=out[2], nll=out[3], n_bad=out[4])
 
+    def pack_params(self, points):
+        """[Params-like] -> host array [n_points][stride] in the layout tddp4_nll_batch reads."""
+        stride = self.lib.tddp4_param_stride(self._h)
+        out = np.empty((len(points), stride))
+        kc, nr = self.kc, self.n_res
+        for i, p in enumerate(points):
+            out[i, 0:2 * kc] = np.asarray(p.c, dtype=np.complex128).view(np.float64)
+            out[i, 2 * kc:4 * kc] = np.asarray(p.cbar, dtype=np.complex128).view(np.float64)
+            out[i, 4 * kc:4 * kc + 2 * nr:2] = p.mass
+            out[i, 4 * kc + 1:4 * kc + 2 * nr:2] = p.width
+            out[i, -3:] = (p.x, p.y, p.tau)
+        return out
+
+    def nll_batch(self, packed, strict=True):
+        """packed: pack_params() output.  Returns (nll[n_points], status[n_points])."""
+        packed = np.ascontiguousarray(packed, dtype=np.float64)
+        n = packed.shape[0]
+        out = np.empty(n)
+        st = np.zeros(n, dtype=np.int32)
+        rc = self.lib.tddp4_nll_batch(self._h, n, packed.ctypes.data, out.ctypes.data, st.ctypes.data)
+        if strict:
+            self._check(rc)
+        return out, st
+
     def gram(self):
         G = np.empty((self.kc, self.kc, 2))
         n = C.c_int64()
@@ -311,12 +337,12 @@ class Tddp4:
         self._check(self.lib.tddp4_profile_reset(self._h))
 
     def profile_read(self):
-        """{kernel: (total_ms, launches)} since the last reset."""
+        """{kernel: (total_ms, launches, algorithmic bytes)} since the last reset."""
         out = {}
         for k, name in enumerate(KERNEL_NAMES):
-            ms, n = C.c_double(), C.c_int64()
-            self._check(self.lib.tddp4_profile_read(self._h, k, C.byref(ms), C.byref(n)))
-            out[name] = (ms.value, n.value)
+            ms, n, by = C.c_double(), C.c_int64(), C.c_double()
+            self._check(self.lib.tddp4_profile_read(self._h, k, C.byref(ms), C.byref(n), C.byref(by)))
+            out[name] = (ms.value, n.value, by.value)
         return out
 
     def launch_count(self):

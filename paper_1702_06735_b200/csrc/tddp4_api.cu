@@ -33,7 +33,7 @@ struct EventSet {
   bool loaded = false;
 };
 
-struct ProfEvent { int id; cudaEvent_t a, b; };
+struct ProfEvent { int id; cudaEvent_t a, b; double bytes; };
 
 }  // namespace
 
@@ -66,6 +66,9 @@ struct tddp4 {
   double *results_host = nullptr;    // pinned mirror
   cudaEvent_t slot_event[N_SLOTS] = {nullptr};
   bool slot_used[N_SLOTS] = {false};
+  double *batch_res = nullptr;       // device [batch_cap][SLOT_DOUBLES]
+  double *batch_res_host = nullptr;  // pinned mirror
+  int64_t batch_cap = 0;
   // generator scratch
   uint32_t *gen_flags = nullptr, *gen_counts = nullptr;
   unsigned long long *gen_offs = nullptr, *gen_scalars = nullptr;   // [0] pilot max bits, [1] overflow
@@ -75,6 +78,7 @@ struct tddp4 {
   std::vector<ProfEvent> pending;
   std::vector<cudaEvent_t> pool;
   double prof_ms[TDDP4_K_COUNT] = {0};
+  double prof_bytes[TDDP4_K_COUNT] = {0};   // algorithmic bytes of the profiled launches
   int64_t prof_n[TDDP4_K_COUNT] = {0};
   int64_t launches = 0;
   int sm_count = 148;
@@ -102,8 +106,8 @@ int fail(tddp4 *h, int code, const char *fmt, ...) {
   } while (0)
 
 struct Prof {   // RAII: CUDA events around one launch when profiling is on
-  tddp4 *h; int id; cudaEvent_t a = nullptr, b = nullptr;
-  Prof(tddp4 *h_, int id_) : h(h_), id(id_) {
+  tddp4 *h; int id; double bytes; cudaEvent_t a = nullptr, b = nullptr;
+  Prof(tddp4 *h_, int id_, double bytes_ = 0.0) : h(h_), id(id_), bytes(bytes_) {
     ++h->launches;
     if (!h->profiling) return;
     auto get = [&]() { cudaEvent_t e; if (!h->pool.empty()) { e = h->pool.back(); h->pool.pop_back(); } else cudaEventCreate(&e); return e; };
@@ -113,7 +117,7 @@ struct Prof {   // RAII: CUDA events around one launch when profiling is on
   ~Prof() {
     if (!a) return;
     cudaEventRecord(b, h->stream);
-    h->pending.push_back({id, a, b});
+    h->pending.push_back({id, a, b, bytes});
   }
 };
 
@@ -124,6 +128,7 @@ void drain_profile(tddp4 *h) {
     cudaEventElapsedTime(&ms, p.a, p.b);
     h->prof_ms[p.id] += ms;
     h->prof_n[p.id] += 1;
+    h->prof_bytes[p.id] += p.bytes;
     h->pool.push_back(p.a);
     h->pool.push_back(p.b);
   }
@@ -206,8 +211,16 @@ int run_columns(tddp4 *h, EventSet &e) {
     if (h->col_of_inst[j] & e.dirty_cols) inst_mask |= 1u << j;
   int grid = (int)((e.n + COL_BLOCK - 1) / COL_BLOCK);
   size_t smem = (size_t)std::max(1, h->M.n_inst) * COL_BLOCK * sizeof(double2);
+  // algorithmic bytes: s rows and g rows of the dirty instances, f rows of the dirty columns' terms, columns written
+  unsigned sys_seen = 0;
+  int rows = 0;
+  for (int j = 0; j < h->M.n_inst; ++j)
+    if (inst_mask & (1u << j)) { ++rows; if (!(sys_seen & (1u << h->M.inst[j].sys))) { sys_seen |= 1u << h->M.inst[j].sys; ++rows; } }
+  int ncol = 0;
+  for (int kap = 0; kap < h->M.n_kc; ++kap)
+    if (e.dirty_cols & (1u << kap)) { ++ncol; rows += h->M.col_begin[kap + 1] - h->M.col_begin[kap]; }
   {
-    Prof p(h, TDDP4_K_COLUMNS);
+    Prof p(h, TDDP4_K_COLUMNS, (double)e.n * (8.0 * rows + 16.0 * ncol));
     columns_kernel<<<grid, COL_BLOCK, smem, h->stream>>>(h->M, h->LP, inst_mask, e.dirty_cols, e.s, e.g, e.f, e.ld,
                                                          e.n, e.a);
   }
@@ -234,7 +247,7 @@ int ensure_gram(tddp4 *h) {
   rc = ensure_partials(h, (size_t)grid * KC * KC + 16);
   if (rc) return rc;
   {
-    Prof p(h, TDDP4_K_GRAM);
+    Prof p(h, TDDP4_K_GRAM, (double)e.n * (16.0 * KC + (e.w ? 8.0 : 0.0)));
     switch (KC) {
       case 1: launch_gram<1>(h, e, grid); break;
       case 2: launch_gram<2>(h, e, grid); break;
@@ -265,7 +278,7 @@ void launch_nll(tddp4 *h, const EventSet &e, int grid, double inv_n, double *res
                                                              h->partials, h->ticket, result, prob);
 }
 
-int enqueue_nll(tddp4 *h, int slot, double *prob) {
+int enqueue_nll(tddp4 *h, double *result, double *prob) {
   if (!h->have_params) return fail(h, TDDP4_ERR_STATE, "tddp4_set_params has not been called");
   EventSet &d = h->set[0];
   if (!d.loaded) return fail(h, TDDP4_ERR_STATE, "data sample not loaded");
@@ -280,9 +293,8 @@ int enqueue_nll(tddp4 *h, int slot, double *prob) {
   rc = ensure_partials(h, (size_t)2 * grid + 16);
   if (rc) return rc;
   double inv_n = h->gram_n > 0 ? 1.0 / (double)h->gram_n : 0.0;
-  double *result = h->results + (size_t)slot * SLOT_DOUBLES;
   {
-    Prof p(h, TDDP4_K_NLL);
+    Prof p(h, TDDP4_K_NLL, (double)d.n * (16.0 * KC + 8.0 + (prob ? 8.0 : 0.0)));
     switch (KC) {
 #define CASE(k) case k: launch_nll<k>(h, d, grid, inv_n, result, prob); break;
       CASE(1) CASE(2) CASE(3) CASE(4) CASE(5) CASE(6) CASE(7) CASE(8) CASE(9) CASE(10) CASE(11) CASE(12)
@@ -292,6 +304,13 @@ int enqueue_nll(tddp4 *h, int slot, double *prob) {
     }
   }
   CU(cudaGetLastError());
+  return TDDP4_OK;
+}
+
+int enqueue_nll_slot(tddp4 *h, int slot, double *prob) {
+  double *result = h->results + (size_t)slot * SLOT_DOUBLES;
+  int rc = enqueue_nll(h, result, prob);
+  if (rc) return rc;
   CU(cudaMemcpyAsync(h->results_host + (size_t)slot * SLOT_DOUBLES, result, SLOT_DOUBLES * sizeof(double),
                      cudaMemcpyDeviceToHost, h->stream));
   CU(cudaEventRecord(h->slot_event[slot], h->stream));
@@ -423,7 +442,8 @@ int tddp4_destroy(tddp4 *h) {
   for (auto e : h->pool) cudaEventDestroy(e);
   free_set(h->set[0]);
   free_set(h->set[1]);
-  cudaFree(h->G); cudaFree(h->partials); cudaFree(h->ticket); cudaFree(h->results);
+  cudaFree(h->G); cudaFree(h->partials); cudaFree(h->ticket); cudaFree(h->results); cudaFree(h->batch_res);
+  if (h->batch_res_host) cudaFreeHost(h->batch_res_host);
   if (h->results_host) cudaFreeHost(h->results_host);
   cudaFree(h->gen_flags); cudaFree(h->gen_counts); cudaFree(h->gen_offs); cudaFree(h->gen_scalars);
   for (int s = 0; s < N_SLOTS; ++s)
@@ -480,7 +500,7 @@ int tddp4_load_events(tddp4 *h, int which, int64_t n, int64_t ld_in, const doubl
     int grid = (int)((n + KIN_BLOCK - 1) / KIN_BLOCK);
     size_t smem = sizeof(double) * (16 + M.n_sys + M.n_inst) * KIN_BLOCK;
     {
-      Prof p(h, TDDP4_K_KIN);
+      Prof p(h, TDDP4_K_KIN, (double)n * 8.0 * (16 + M.n_sys + M.n_inst + M.n_terms));
       kin_kernel<<<grid, KIN_BLOCK, smem, h->stream>>>(M, dp4, ld_dev, n, e.s, e.g, e.f, e.ld);
     }
     CU(cudaGetLastError());
@@ -543,7 +563,7 @@ int tddp4_set_params(tddp4 *h, const double *c, const double *cbar, const double
 
 int tddp4_nll_async(tddp4 *h, int slot) {
   if (!h || slot < 0 || slot >= N_SLOTS) return fail(h, TDDP4_ERR_ARG, "bad slot");
-  return enqueue_nll(h, slot, nullptr);
+  return enqueue_nll_slot(h, slot, nullptr);
 }
 
 int tddp4_nll_result(tddp4 *h, int slot, double *nll_out) {
@@ -561,7 +581,7 @@ int tddp4_nll_result(tddp4 *h, int slot, double *nll_out) {
 
 int tddp4_nll(tddp4 *h, double *nll_out, double *prob_out) {
   if (!h || !nll_out) return fail(h, TDDP4_ERR_ARG, "null argument");
-  int rc = enqueue_nll(h, 0, prob_out);
+  int rc = enqueue_nll_slot(h, 0, prob_out);
   if (rc) return rc;
   return tddp4_nll_result(h, 0, nll_out);
 }
@@ -572,6 +592,51 @@ int tddp4_nll_parts(tddp4 *h, int slot, double out[5]) {
   CU(cudaEventSynchronize(h->slot_event[slot]));
   memcpy(out, h->results_host + (size_t)slot * SLOT_DOUBLES, 5 * sizeof(double));
   return TDDP4_OK;
+}
+
+int tddp4_param_stride(const tddp4 *h) { return h ? 4 * h->M.n_kc + 2 * (int)h->res.size() + 3 : TDDP4_ERR_ARG; }
+
+int tddp4_nll_batch(tddp4 *h, int64_t n_points, const double *params, double *nll_out, int *status_out) {
+  if (!h || n_points < 0 || (n_points > 0 && (!params || !nll_out))) return fail(h, TDDP4_ERR_ARG, "bad argument");
+  if (n_points == 0) return TDDP4_OK;
+  if (n_points > h->batch_cap) {
+    cudaFree(h->batch_res);
+    if (h->batch_res_host) cudaFreeHost(h->batch_res_host);
+    h->batch_res = nullptr; h->batch_res_host = nullptr; h->batch_cap = 0;
+    CU(cudaMalloc(&h->batch_res, sizeof(double) * SLOT_DOUBLES * n_points));
+    CU(cudaMallocHost(&h->batch_res_host, sizeof(double) * SLOT_DOUBLES * n_points));
+    h->batch_cap = n_points;
+  }
+  const int KC = h->M.n_kc, nres = (int)h->res.size(), stride = 4 * KC + 2 * nres + 3;
+  int first_err = TDDP4_OK;
+  std::vector<int> st((size_t)n_points, TDDP4_OK);
+  for (int64_t i = 0; i < n_points; ++i) {
+    const double *p = params + i * stride;
+    const double *tail = p + 4 * KC + 2 * nres;
+    int rc = tddp4_set_params(h, p, p + 2 * KC, p + 4 * KC, tail[0], tail[1], tail[2]);
+    if (!rc) rc = enqueue_nll(h, h->batch_res + i * SLOT_DOUBLES, nullptr);
+    st[i] = rc;
+    if (rc == TDDP4_ERR_CUDA) return rc;
+  }
+  CU(cudaMemcpyAsync(h->batch_res_host, h->batch_res, sizeof(double) * SLOT_DOUBLES * n_points, cudaMemcpyDeviceToHost,
+                     h->stream));
+  CU(cudaStreamSynchronize(h->stream));
+  for (int64_t i = 0; i < n_points; ++i) {
+    const double *r = h->batch_res_host + i * SLOT_DOUBLES;
+    if (st[i] == TDDP4_OK) {
+      nll_out[i] = r[3];
+      if (r[4] > 0.0 || !std::isfinite(r[3])) {
+        nll_out[i] = INFINITY;
+        st[i] = fail(h, TDDP4_ERR_NONFINITE, "point %lld: %g events with non-positive or non-finite rate (N = %g)",
+                     (long long)i, r[4], r[2]);
+      }
+    } else {
+      nll_out[i] = std::numeric_limits<double>::quiet_NaN();
+    }
+    if (status_out) status_out[i] = st[i];
+    if (st[i] && !first_err) first_err = st[i];
+  }
+  return first_err;
 }
 
 int tddp4_gram(tddp4 *h, double *G_sum, int64_t *n_norm) {
@@ -791,18 +856,19 @@ int tddp4_profile(tddp4 *h, int enable) {
   return TDDP4_OK;
 }
 
-int tddp4_profile_read(tddp4 *h, int kernel_id, double *total_ms, int64_t *launches) {
+int tddp4_profile_read(tddp4 *h, int kernel_id, double *total_ms, int64_t *launches, double *alg_bytes) {
   if (!h || kernel_id < 0 || kernel_id >= TDDP4_K_COUNT || !total_ms || !launches) return fail(h, TDDP4_ERR_ARG, "bad argument");
   drain_profile(h);
   *total_ms = h->prof_ms[kernel_id];
   *launches = h->prof_n[kernel_id];
+  if (alg_bytes) *alg_bytes = h->prof_bytes[kernel_id];
   return TDDP4_OK;
 }
 
 int tddp4_profile_reset(tddp4 *h) {
   if (!h) return TDDP4_ERR_ARG;
   drain_profile(h);
-  for (int i = 0; i < TDDP4_K_COUNT; ++i) { h->prof_ms[i] = 0; h->prof_n[i] = 0; }
+  for (int i = 0; i < TDDP4_K_COUNT; ++i) { h->prof_ms[i] = 0; h->prof_n[i] = 0; h->prof_bytes[i] = 0; }
   return TDDP4_OK;
 }
 
