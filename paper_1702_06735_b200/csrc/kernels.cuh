@@ -107,210 +107,257 @@ terms_kernel(const __grid_constant__ ModelTab M, const __grid_constant__ LinePar
 }
 
 // ------------------------------------------------------------------------------------------------
-// step 6: Hermitian Gram matrix G_kl = sum_j w_j a_k conj(a_l) over the normalisation sample.
-// Thread-per-event grid-stride loop with KC*KC real accumulators in registers (k<=l: re, k<l: im),
-// fixed-order block reduction, one partial matrix per block, summed in block order by the last block.
-constexpr int GRAM_BLOCK = 128;
-template <int KC>
-__global__ void __launch_bounds__(GRAM_BLOCK)
-gram_kernel(const double2 *__restrict__ a, int64_t ld, const double *__restrict__ w, int64_t n,
-            double *__restrict__ partials /* [grid][KC*KC] */, unsigned int *ticket,
-            double *__restrict__ G /* [KC][KC][2] sums, Hermitian, full */) {
-  constexpr int NA = KC * KC;
-  double acc[NA];
+// Lineshapes + component products of ONE event from the step-1 caches (steps 2+3): T_R of every instance into
+// the thread's shared-memory slots, then the K_c coupling columns into col[].  Rows are read with streaming
+// loads; each is touched once per pass.
+template <int KC, int BLOCK>
+__device__ __forceinline__ void event_columns(const ModelTab &M, const LineParams &LP, const double *__restrict__ s,
+                                              const double *__restrict__ g, const double *__restrict__ f, int64_t ld,
+                                              int64_t i, double2 *sT, int tid, double2 col[KC]) {
+  for (int j = 0; j < M.n_inst; ++j) {
+    double sv = __ldcs(s + M.inst[j].sys * ld + i);
+    double gv = __ldcs(g + j * ld + i);
+    sT[j * BLOCK + tid] = breit_wigner(LP.m0sq[j], LP.gam[j], sv, gv);
+  }
 #pragma unroll
-  for (int q = 0; q < NA; ++q) acc[q] = 0.0;
-  for (int64_t i = (int64_t)blockIdx.x * GRAM_BLOCK + threadIdx.x; i < n; i += (int64_t)gridDim.x * GRAM_BLOCK) {
-    double2 v[KC];
-#pragma unroll
-    for (int k = 0; k < KC; ++k) v[k] = __ldg(a + k * ld + i);
-    double wj = w ? __ldg(w + i) : 1.0;
-#pragma unroll
-    for (int k = 0; k < KC; ++k) {
-      double wr = wj * v[k].x, wi = wj * v[k].y;
-      acc[k * KC + k] += wr * v[k].x + wi * v[k].y;
-#pragma unroll
-      for (int l = k + 1; l < KC; ++l) {
-        acc[k * KC + l] += wr * v[l].x + wi * v[l].y;   // Re a_k conj(a_l)
-        acc[l * KC + k] += wi * v[l].x - wr * v[l].y;   // Im a_k conj(a_l)
-      }
+  for (int kap = 0; kap < KC; ++kap) {
+    double2 acc = make_double2(0.0, 0.0);
+    for (int k = M.col_begin[kap]; k < M.col_begin[kap + 1]; ++k) {
+      const TermTab &tm = M.term[k];
+      double fv = __ldcs(f + k * ld + i);
+      double2 T = make_double2(1.0, 0.0);
+      if (tm.inst0 >= 0) T = cmul(sT[tm.inst0 * BLOCK + tid], sT[tm.inst1 * BLOCK + tid]);
+      acc.x += fv * T.x;
+      acc.y += fv * T.y;
     }
+    col[kap] = acc;
   }
-  __shared__ double red[GRAM_BLOCK / 32];
-  __shared__ bool last;
-#pragma unroll
-  for (int q = 0; q < NA; ++q) {
-    double r = block_sum<GRAM_BLOCK>(acc[q], red);
-    if (threadIdx.x == 0) partials[(int64_t)blockIdx.x * NA + q] = r;
-  }
-  __threadfence();
-  if (threadIdx.x == 0) last = atomicAdd(ticket, 1u) == gridDim.x - 1;
-  __syncthreads();
-  if (!last) return;
-  __threadfence();
-  for (int q = threadIdx.x; q < NA; q += GRAM_BLOCK) {
-    double sum = 0.0;
-    for (unsigned b = 0; b < gridDim.x; ++b) sum += __ldcg(partials + (int64_t)b * NA + q);
-    int k = q / KC, l = q % KC;
-    if (k <= l) {        // real part of G_kl and G_lk
-      G[(k * KC + l) * 2] = sum;
-      G[(l * KC + k) * 2] = sum;
-      if (k == l) G[(k * KC + k) * 2 + 1] = 0.0;
-    } else {             // slot (l', k') with l' > k' holds Im G_{k'l'}: here k' = l, l' = k
-      G[(l * KC + k) * 2 + 1] = sum;
-      G[(k * KC + l) * 2 + 1] = -sum;
-    }
-  }
-  if (threadIdx.x == 0) *ticket = 0;
 }
 
-// Fallback for K_c > 8 (accumulators no longer fit in registers): tile of events staged in shared memory,
-// one (k <= l) pair per thread.  Same partial/last-block scheme, same result layout.
-constexpr int GRAMG_TILE = 128;
+// ------------------------------------------------------------------------------------------------
+// step 6: Hermitian Gram matrix G_kl = sum_j w_j a_k(p_j) conj(a_l(p_j)) over the normalisation sample, fused with
+// steps 2+3: the columns of the normalisation sample are never stored.  With x_j = (Re a_0, Im a_0, Re a_1, ...)
+// the real matrix X^T diag(w) X holds every Re/Im piece of G, and it is a dense contraction over events: it runs on
+// the fp64 tensor cores (mma.sync m8n8k4 DMMA), the only place of the path where they apply (north_star).
+//   G_kl.re = XtX[2k][2l] + XtX[2k+1][2l+1],   G_kl.im = XtX[2k+1][2l] - XtX[2k][2l+1].
+// One thread per event computes the columns; each warp then feeds its own 32 events, 4 at a time, through the
+// MMA from a padded shared-memory tile (no block barrier inside the loop).  NB = number of 8-feature blocks.
+// Deterministic: per-warp accumulation in event order, warps then blocks summed in index order.
+constexpr int GRAM_BLOCK = 128;
+__host__ __device__ constexpr int gram_stride(int NB) { return NB <= 2 ? 20 : 36; }   // = 4 mod 16: conflict-free fragments
+__host__ __device__ inline size_t gram_smem_bytes(int NB, int n_inst) {
+  return sizeof(double2) * (size_t)(n_inst > 0 ? n_inst : 1) * GRAM_BLOCK + sizeof(double) * GRAM_BLOCK * gram_stride(NB) +
+         sizeof(double) * (GRAM_BLOCK / 32) * 64 * NB * NB;
+}
+
+__device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double b) {
+  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+               : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
+}
+
+template <int NB>
 __global__ void __launch_bounds__(GRAM_BLOCK)
-gram_generic_kernel(int KC, const double2 *__restrict__ a, int64_t ld, const double *__restrict__ w, int64_t n,
-                    double *__restrict__ partials /* [grid][KC*KC] */, unsigned int *ticket,
-                    double *__restrict__ G) {
-  __shared__ double2 tile[MAX_KC][GRAMG_TILE];
-  __shared__ double tw[GRAMG_TILE];
+gram_fused_kernel(const __grid_constant__ ModelTab M, const __grid_constant__ LineParams LP,
+                  const double *__restrict__ s, const double *__restrict__ g, const double *__restrict__ f, int64_t ld,
+                  const double *__restrict__ w, int64_t n, double *__restrict__ partials /* [grid][64 NB NB] */,
+                  unsigned int *ticket, double *__restrict__ G /* [KC][KC][2] sums, Hermitian, full */) {
+  constexpr int KCMAX = 4 * NB, F = 8 * NB, STRIDE = gram_stride(NB), NP = NB * (NB + 1) / 2;
+  extern __shared__ double2 smem2[];
+  double2 *sT = smem2;                                                        // [n_inst][GRAM_BLOCK]
+  double *Xs = reinterpret_cast<double *>(smem2 + (M.n_inst > 0 ? M.n_inst : 1) * GRAM_BLOCK);   // [GRAM_BLOCK][STRIDE]
+  double *Ws = Xs + GRAM_BLOCK * STRIDE;                                      // [warps][NB*NB][64] block reduction
   __shared__ bool last;
-  const int NP = KC * (KC + 1) / 2;
-  // pairs handled by this thread: p = threadIdx.x, threadIdx.x + GRAM_BLOCK (NP <= 136)
-  double re[2] = {0.0, 0.0}, im[2] = {0.0, 0.0};
-  int pk[2], pl[2];
-  for (int u = 0; u < 2; ++u) {
-    int p = threadIdx.x + u * GRAM_BLOCK, k = 0;
-    pk[u] = pl[u] = -1;
-    if (p < NP) {
-      int rem = p;
-      while (rem >= KC - k) { rem -= KC - k; ++k; }
-      pk[u] = k; pl[u] = k + rem;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int KC = M.n_kc;
+  double acc[NP][2];
+#pragma unroll
+  for (int q = 0; q < NP; ++q) acc[q][0] = acc[q][1] = 0.0;
+  double *row = Xs + tid * STRIDE;
+  const int64_t n_tiles = (n + GRAM_BLOCK - 1) / GRAM_BLOCK;
+  for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
+    int64_t i = tile * GRAM_BLOCK + tid;
+    double2 col[KCMAX];
+    double wj = 0.0;
+    if (i < n) {
+      event_columns<KCMAX, GRAM_BLOCK>(M, LP, s, g, f, ld, i, sT, tid, col);   // columns >= KC have no terms: zero
+      wj = w ? __ldcs(w + i) : 1.0;
+    } else {
+#pragma unroll
+      for (int k = 0; k < KCMAX; ++k) col[k] = make_double2(0.0, 0.0);
     }
-  }
-  for (int64_t base = (int64_t)blockIdx.x * GRAMG_TILE; base < n; base += (int64_t)gridDim.x * GRAMG_TILE) {
-    int64_t i = base + threadIdx.x;
-    __syncthreads();
-    for (int k = 0; k < KC; ++k) tile[k][threadIdx.x] = i < n ? a[k * ld + i] : make_double2(0.0, 0.0);
-    tw[threadIdx.x] = i < n ? (w ? w[i] : 1.0) : 0.0;
-    __syncthreads();
-    for (int u = 0; u < 2; ++u) {
-      if (pk[u] < 0) continue;
-      for (int e = 0; e < GRAMG_TILE; ++e) {
-        double2 x = tile[pk[u]][e], y = tile[pl[u]][e];
-        double wj = tw[e];
-        re[u] += wj * (x.x * y.x + x.y * y.y);
-        im[u] += wj * (x.y * y.x - x.x * y.y);
+    __syncwarp();                                       // previous tile's fragments of this warp are consumed
+#pragma unroll
+    for (int k = 0; k < KCMAX; ++k) *reinterpret_cast<double2 *>(row + 2 * k) = col[k];
+    row[F] = wj;
+    __syncwarp();
+    const double *base = Xs + (warp * 32 + (lane & 3)) * STRIDE + (lane >> 2);
+#pragma unroll
+    for (int grp = 0; grp < 8; ++grp) {                  // 4 events per MMA, 8 groups per warp tile
+      const double *r = base + grp * 4 * STRIDE;
+      double wv = r[F - (lane >> 2)];
+      double x[NB];
+#pragma unroll
+      for (int b = 0; b < NB; ++b) x[b] = r[8 * b];
+      int q = 0;
+#pragma unroll
+      for (int bi = 0; bi < NB; ++bi) {
+        double aw = wv * x[bi];
+#pragma unroll
+        for (int bj = bi; bj < NB; ++bj, ++q) dmma884(acc[q][0], acc[q][1], aw, x[bj]);
       }
     }
   }
-  for (int u = 0; u < 2; ++u)
-    if (pk[u] >= 0) {
-      partials[(int64_t)blockIdx.x * KC * KC + pk[u] * KC + pl[u]] = re[u];
-      if (pk[u] != pl[u]) partials[(int64_t)blockIdx.x * KC * KC + pl[u] * KC + pk[u]] = im[u];
-    }
+  // block reduction in warp order, block partial [NB*NB block pairs as full F x F upper blocks]
+  {
+    int q = 0;
+#pragma unroll
+    for (int bi = 0; bi < NB; ++bi)
+#pragma unroll
+      for (int bj = bi; bj < NB; ++bj, ++q) {
+        double *dst = Ws + ((warp * NB + bi) * NB + bj) * 64;
+        dst[(lane >> 2) * 8 + 2 * (lane & 3)] = acc[q][0];      // C fragment: row lane/4, cols 2 (lane%4) + {0,1}
+        dst[(lane >> 2) * 8 + 2 * (lane & 3) + 1] = acc[q][1];
+      }
+  }
+  __syncthreads();
+  for (int e = tid; e < NB * NB * 64; e += GRAM_BLOCK) {
+    int bi = e / (NB * 64), bj = (e / 64) % NB;
+    if (bi > bj) continue;
+    double sum = 0.0;
+#pragma unroll
+    for (int wp = 0; wp < GRAM_BLOCK / 32; ++wp) sum += Ws[wp * NB * NB * 64 + e];
+    partials[(int64_t)blockIdx.x * NB * NB * 64 + e] = sum;
+  }
   __threadfence();
   __syncthreads();
-  if (threadIdx.x == 0) last = atomicAdd(ticket, 1u) == gridDim.x - 1;
+  if (tid == 0) last = atomicAdd(ticket, 1u) == gridDim.x - 1;
   __syncthreads();
   if (!last) return;
   __threadfence();
-  for (int q = threadIdx.x; q < KC * KC; q += GRAM_BLOCK) {
+  // final pass: XtX (upper blocks) summed over blocks in index order, staged in shared memory, then G
+  double *XtX = Ws;                                      // [NB][NB][64], reused
+  for (int e = tid; e < NB * NB * 64; e += GRAM_BLOCK) {
+    int bi = e / (NB * 64), bj = (e / 64) % NB;
+    if (bi > bj) continue;
     double sum = 0.0;
-    for (unsigned b = 0; b < gridDim.x; ++b) sum += __ldcg(partials + (int64_t)b * KC * KC + q);
-    int k = q / KC, l = q % KC;
-    if (k <= l) {
-      G[(k * KC + l) * 2] = sum;
-      G[(l * KC + k) * 2] = sum;
-      if (k == l) G[(k * KC + k) * 2 + 1] = 0.0;
-    } else {
-      G[(l * KC + k) * 2 + 1] = sum;
-      G[(k * KC + l) * 2 + 1] = -sum;
-    }
+    for (unsigned b = 0; b < gridDim.x; ++b) sum += __ldcg(partials + (int64_t)b * NB * NB * 64 + e);
+    XtX[e] = sum;
   }
-  if (threadIdx.x == 0) *ticket = 0;
+  __syncthreads();
+  auto xtx = [&](int m, int nn) {                        // symmetric: only the upper triangle is ever read
+    if (m > nn) { int tmp = m; m = nn; nn = tmp; }
+    return XtX[((m >> 3) * NB + (nn >> 3)) * 64 + (m & 7) * 8 + (nn & 7)];
+  };
+  for (int q = tid; q < KC * KC; q += GRAM_BLOCK) {
+    int k = q / KC, l = q % KC;
+    double re = xtx(2 * k, 2 * l) + xtx(2 * k + 1, 2 * l + 1);
+    double im = xtx(2 * k + 1, 2 * l) - xtx(2 * k, 2 * l + 1);
+    if (k == l) im = 0.0;
+    G[q * 2] = re;
+    G[q * 2 + 1] = im;
+  }
+  if (tid == 0) *ticket = 0;
 }
 
 // ------------------------------------------------------------------------------------------------
 // steps 4+5+7: amplitude sums (eq. 2), mixing rate (eq. 1), -log reduction.
-// Streams the K_c coupling columns (16 B / event / column, coalesced 128-bit loads) and t.
-// result slot layout (doubles): [0] sum log B, [1] unused, [2] N, [3] NLL, [4] #bad events
+// result slot layout (doubles): [0] sum log B, [1] sum t, [2] N, [3] NLL, [4] #bad events
 constexpr int NLL_BLOCK = 256;
 
 // N from the Gram matrix in force: N = T1 (nAA + nBB) + T2 (nAA - nBB) - 2 T3 Re X - 2 T4 Im X,
-// nAA = c^T G conj(c), nBB likewise for cbar, X = sum_kl c_k conj(cbar_l) G_kl   (O-8, step 6)
+// nAA = c^T G conj(c), nBB likewise for cbar, X = sum_kl c_k conj(cbar_l) G_kl   (O-8, step 6).
+// One (k,l) pair per thread, fixed-order block reduction; every thread of the block must call; valid in thread 0.
+template <int BLOCK>
 __device__ __forceinline__ double norm_from_gram(const RateParams &R, const double *__restrict__ G, int KC,
-                                                 double inv_n) {
+                                                 double inv_n, double *red) {
   double nAA = 0.0, nBB = 0.0, xr = 0.0, xi = 0.0;
-  for (int k = 0; k < KC; ++k)
-    for (int l = 0; l < KC; ++l) {
-      double gr = G[(k * KC + l) * 2] * inv_n, gi = G[(k * KC + l) * 2 + 1] * inv_n;
-      // c_k conj(c_l)
-      double pr = R.c[k][0] * R.c[l][0] + R.c[k][1] * R.c[l][1], pi = R.c[k][1] * R.c[l][0] - R.c[k][0] * R.c[l][1];
-      nAA += pr * gr - pi * gi;
-      pr = R.cbar[k][0] * R.cbar[l][0] + R.cbar[k][1] * R.cbar[l][1];
-      pi = R.cbar[k][1] * R.cbar[l][0] - R.cbar[k][0] * R.cbar[l][1];
-      nBB += pr * gr - pi * gi;
-      pr = R.c[k][0] * R.cbar[l][0] + R.c[k][1] * R.cbar[l][1];
-      pi = R.c[k][1] * R.cbar[l][0] - R.c[k][0] * R.cbar[l][1];
-      xr += pr * gr - pi * gi;
-      xi += pr * gi + pi * gr;
-    }
+  for (int q = threadIdx.x; q < KC * KC; q += BLOCK) {
+    int k = q / KC, l = q % KC;
+    double gr = __ldcg(G + q * 2) * inv_n, gi = __ldcg(G + q * 2 + 1) * inv_n;
+    double pr = R.c[k][0] * R.c[l][0] + R.c[k][1] * R.c[l][1], pi = R.c[k][1] * R.c[l][0] - R.c[k][0] * R.c[l][1];
+    nAA += pr * gr - pi * gi;
+    pr = R.cbar[k][0] * R.cbar[l][0] + R.cbar[k][1] * R.cbar[l][1];
+    pi = R.cbar[k][1] * R.cbar[l][0] - R.cbar[k][0] * R.cbar[l][1];
+    nBB += pr * gr - pi * gi;
+    pr = R.c[k][0] * R.cbar[l][0] + R.c[k][1] * R.cbar[l][1];
+    pi = R.c[k][1] * R.cbar[l][0] - R.c[k][0] * R.cbar[l][1];
+    xr += pr * gr - pi * gi;
+    xi += pr * gi + pi * gr;
+  }
+  nAA = block_sum<BLOCK>(nAA, red);
+  nBB = block_sum<BLOCK>(nBB, red);
+  xr = block_sum<BLOCK>(xr, red);
+  xi = block_sum<BLOCK>(xi, red);
   return R.T[0] * (nAA + nBB) + R.T[1] * (nAA - nBB) - 2.0 * R.T[2] * xr - 2.0 * R.T[3] * xi;
 }
 
-template <int KC, bool PROB>
-__global__ void __launch_bounds__(NLL_BLOCK)
-nll_kernel(const double2 *__restrict__ a, int64_t ld, const double *__restrict__ t, int64_t n,
-           const __grid_constant__ RateParams R, const double *__restrict__ G, double inv_n_norm, double sum_t,
-           double *__restrict__ partials, unsigned int *ticket, double *__restrict__ result,
-           double *__restrict__ prob_out) {
-  __shared__ double red[NLL_BLOCK / 32];
-  __shared__ double s_norm;
-  __shared__ bool last;
-  if (PROB) {
-    if (threadIdx.x == 0) s_norm = norm_from_gram(R, G, KC, inv_n_norm);
-    __syncthreads();
-  }
-  double acc = 0.0, bad = 0.0;
-  const double yG = R.y * R.Gamma, xG = R.x * R.Gamma;
-  for (int64_t i = (int64_t)blockIdx.x * NLL_BLOCK + threadIdx.x; i < n; i += (int64_t)gridDim.x * NLL_BLOCK) {
-    double2 v[KC];
-#pragma unroll
-    for (int k = 0; k < KC; ++k) v[k] = __ldcs(a + k * ld + i);
-    double ti = __ldcs(t + i);
-    double2 A = make_double2(0.0, 0.0), Ab = make_double2(0.0, 0.0);
-#pragma unroll
-    for (int k = 0; k < KC; ++k) {
-      A.x += R.c[k][0] * v[k].x - R.c[k][1] * v[k].y;
-      A.y += R.c[k][0] * v[k].y + R.c[k][1] * v[k].x;
-      Ab.x += R.cbar[k][0] * v[k].x - R.cbar[k][1] * v[k].y;
-      Ab.y += R.cbar[k][0] * v[k].y + R.cbar[k][1] * v[k].x;
+// sum_i log B_i without a log per event: B = m 2^e with m in [1,2); the mantissas are multiplied up, the exponents
+// added as integers, and one log is taken per thread at the end:  sum log B = log(prod m) + ln2 * sum e.
+struct LogAcc {
+  double prod = 1.0;
+  long long esum = 0;
+  int bad = 0, since = 0;
+  __device__ __forceinline__ void add(double B) {
+    long long bits = __double_as_longlong(B);
+    int e = (int)((bits >> 52) & 0x7ff);
+    if (bits <= 0 || e == 0x7ff) { ++bad; return; }              // B <= 0 (sign bit or zero), inf, nan
+    if (e == 0) {                                                 // subnormal: rescale first
+      bits = __double_as_longlong(B * 0x1.0p64);
+      e = (int)((bits >> 52) & 0x7ff) - 64;
     }
-    double B = bracket(A, Ab, yG * ti, xG * ti);
-    if (!(B > 0.0) || isinf(B)) { bad += 1.0; } else { acc += log(B); }
-    if (PROB) prob_out[i] = exp(-R.Gamma * ti) * B / s_norm;
+    esum += e - 1023;
+    prod *= __longlong_as_double((bits & 0x000fffffffffffffLL) | 0x3ff0000000000000LL);
+    if (++since == 512) renorm();
   }
-  double r = block_sum<NLL_BLOCK>(acc, red);
-  double rb = block_sum<NLL_BLOCK>(bad, red);
+  __device__ __forceinline__ void renorm() {
+    long long bits = __double_as_longlong(prod);
+    esum += (int)((bits >> 52) & 0x7ff) - 1023;
+    prod = __longlong_as_double((bits & 0x000fffffffffffffLL) | 0x3ff0000000000000LL);
+    since = 0;
+  }
+  __device__ __forceinline__ double value() const { return log(prod) + 0.693147180559945309417 * (double)esum; }
+};
+
+// A, Abar from the K_c columns of one event (eq. 2)
+template <int KC>
+__device__ __forceinline__ void amplitude_sums(const RateParams &R, const double2 v[KC], double2 &A, double2 &Ab) {
+  A = make_double2(0.0, 0.0);
+  Ab = make_double2(0.0, 0.0);
+#pragma unroll
+  for (int k = 0; k < KC; ++k) {
+    A.x += R.c[k][0] * v[k].x - R.c[k][1] * v[k].y;
+    A.y += R.c[k][0] * v[k].y + R.c[k][1] * v[k].x;
+    Ab.x += R.cbar[k][0] * v[k].x - R.cbar[k][1] * v[k].y;
+    Ab.y += R.cbar[k][0] * v[k].y + R.cbar[k][1] * v[k].x;
+  }
+}
+
+// common tail of the two NLL kernels: block partials, last block adds them in index order and finishes the NLL
+template <int BLOCK>
+__device__ __forceinline__ void nll_finish(const RateParams &R, int64_t n, double sum_t, double acc, double bad,
+                                           double norm_block0, double *__restrict__ partials, unsigned int *ticket,
+                                           double *__restrict__ result, double *red, bool *last) {
+  double r = block_sum<BLOCK>(acc, red);
+  double rb = block_sum<BLOCK>(bad, red);
   if (threadIdx.x == 0) {
     partials[2 * blockIdx.x] = r;
     partials[2 * blockIdx.x + 1] = rb;
+    if (blockIdx.x == 0) partials[2 * gridDim.x] = norm_block0;
   }
   __threadfence();
-  if (threadIdx.x == 0) last = atomicAdd(ticket, 1u) == gridDim.x - 1;
+  if (threadIdx.x == 0) *last = atomicAdd(ticket, 1u) == gridDim.x - 1;
   __syncthreads();
-  if (!last) return;
+  if (!*last) return;
   __threadfence();
-  // fixed-order second pass over the block partials
   double s0 = 0.0, s1 = 0.0;
-  for (unsigned b = threadIdx.x; b < gridDim.x; b += NLL_BLOCK) {
+  for (unsigned b = threadIdx.x; b < gridDim.x; b += BLOCK) {
     s0 += __ldcg(partials + 2 * b);
     s1 += __ldcg(partials + 2 * b + 1);
   }
-  s0 = block_sum<NLL_BLOCK>(s0, red);
-  s1 = block_sum<NLL_BLOCK>(s1, red);
+  s0 = block_sum<BLOCK>(s0, red);
+  s1 = block_sum<BLOCK>(s1, red);
   if (threadIdx.x == 0) {
-    double norm = norm_from_gram(R, G, KC, inv_n_norm);
+    double norm = __ldcg(partials + 2 * gridDim.x);
     // -sum log(e^{-Gamma t} B / N) = Gamma sum t - sum log B + n log N
     double nll = R.Gamma * sum_t - s0 + (double)n * log(norm);
     if (s1 > 0.0 || !(norm > 0.0)) nll = INFINITY;
@@ -319,13 +366,93 @@ nll_kernel(const double2 *__restrict__ a, int64_t ld, const double *__restrict__
   }
 }
 
-// plain deterministic sum of a vector (sum of decay times at load)
-__global__ void __launch_bounds__(256) sum_kernel(const double *__restrict__ v, int64_t n, double *out) {
-  __shared__ double red[8];
-  double acc = 0.0;
-  for (int64_t i = threadIdx.x; i < n; i += 256) acc += v[i];
-  acc = block_sum<256>(acc, red);
-  if (threadIdx.x == 0) *out = acc;
+// Coupling-only call: streams the K_c cached columns (16 B / event / column, 128-bit coalesced loads) and t.
+// SMALL: |y Gamma t|, |x Gamma t| < 1/4 for every event of the sample (checked on the host from max |t|): the four
+// time functions are short Taylor polynomials instead of exp / sincos.
+template <int KC, bool PROB, bool SMALL>
+__global__ void __launch_bounds__(NLL_BLOCK, KC <= 8 ? 4 : 1)
+nll_kernel(const double2 *__restrict__ a, int64_t ld, const double *__restrict__ t, int64_t n,
+           const __grid_constant__ RateParams R, const double *__restrict__ G, double inv_n_norm, double sum_t,
+           double *__restrict__ partials, unsigned int *ticket, double *__restrict__ result,
+           double *__restrict__ prob_out) {
+  __shared__ double red[NLL_BLOCK / 32];
+  __shared__ double s_norm;
+  __shared__ bool last;
+  double norm0 = 0.0;
+  if (PROB || blockIdx.x == 0) {                         // block 0 evaluates N while the others already stream
+    norm0 = norm_from_gram<NLL_BLOCK>(R, G, KC, inv_n_norm, red);
+    if (PROB) {
+      if (threadIdx.x == 0) s_norm = norm0;
+      __syncthreads();
+    }
+  }
+  LogAcc la;
+  const double yG = R.y * R.Gamma, xG = R.x * R.Gamma;
+  for (int64_t i = (int64_t)blockIdx.x * NLL_BLOCK + threadIdx.x; i < n; i += (int64_t)gridDim.x * NLL_BLOCK) {
+    double2 v[KC];
+#pragma unroll
+    for (int k = 0; k < KC; ++k) v[k] = __ldcs(a + k * ld + i);
+    double ti = __ldcs(t + i);
+    double2 A, Ab;
+    amplitude_sums<KC>(R, v, A, Ab);
+    double B = bracket<SMALL>(A, Ab, yG * ti, xG * ti);
+    la.add(B);
+    if (PROB) prob_out[i] = exp(-R.Gamma * ti) * B / s_norm;
+  }
+  nll_finish<NLL_BLOCK>(R, n, sum_t, la.value(), (double)la.bad, norm0, partials, ticket, result, red, &last);
+}
+
+// Call after a mass or width moved: steps 2+3 for every column from the step-1 caches, columns written back for the
+// coupling-only calls that follow, and steps 4+5+7 in the same pass (the fresh columns never leave registers).
+constexpr int CNLL_BLOCK = NLL_BLOCK;   // same block size and grid as nll_kernel: the two paths then add the same
+                                        // per-thread terms in the same order and return bit-identical NLLs
+template <int KC, bool SMALL>
+__global__ void __launch_bounds__(CNLL_BLOCK, KC <= 8 ? 4 : 1)
+columns_nll_kernel(const __grid_constant__ ModelTab M, const __grid_constant__ LineParams LP,
+                   const double *__restrict__ s, const double *__restrict__ g, const double *__restrict__ f, int64_t ld,
+                   const double *__restrict__ t, int64_t n, double2 *__restrict__ a,
+                   const __grid_constant__ RateParams R, const double *__restrict__ G, double inv_n_norm, double sum_t,
+                   double *__restrict__ partials, unsigned int *ticket, double *__restrict__ result) {
+  extern __shared__ double2 sT[];                        // [n_inst][CNLL_BLOCK]
+  __shared__ double red[CNLL_BLOCK / 32];
+  __shared__ bool last;
+  double norm0 = 0.0;
+  if (blockIdx.x == 0) norm0 = norm_from_gram<CNLL_BLOCK>(R, G, KC, inv_n_norm, red);
+  LogAcc la;
+  const double yG = R.y * R.Gamma, xG = R.x * R.Gamma;
+  for (int64_t i = (int64_t)blockIdx.x * CNLL_BLOCK + threadIdx.x; i < n; i += (int64_t)gridDim.x * CNLL_BLOCK) {
+    double2 v[KC];
+    event_columns<KC, CNLL_BLOCK>(M, LP, s, g, f, ld, i, sT, threadIdx.x, v);
+    double ti = __ldcs(t + i);
+#pragma unroll
+    for (int k = 0; k < KC; ++k) a[k * ld + i] = v[k];
+    double2 A, Ab;
+    amplitude_sums<KC>(R, v, A, Ab);
+    la.add(bracket<SMALL>(A, Ab, yG * ti, xG * ti));
+  }
+  nll_finish<CNLL_BLOCK>(R, n, sum_t, la.value(), (double)la.bad, norm0, partials, ticket, result, red, &last);
+}
+
+// deterministic sum and max |.| of a vector (decay times at load): one block, fixed order
+__global__ void __launch_bounds__(1024) stat_kernel(const double *__restrict__ v, int64_t n, double *out /* [2] */) {
+  __shared__ double red[32];
+  double acc = 0.0, mx = 0.0;
+  for (int64_t i = threadIdx.x; i < n; i += 1024) {
+    double x = v[i];
+    acc += x;
+    mx = fmax(mx, fabs(x));
+  }
+  acc = block_sum<1024>(acc, red);
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+  __syncthreads();
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = mx;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int k = 1; k < 32; ++k) mx = fmax(mx, red[k]);
+    out[0] = acc;
+    out[1] = mx;
+  }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -374,7 +501,7 @@ __device__ __forceinline__ double candidate_ratio(const ModelTab &M, const LineP
   GenSink sink{M, LP, R, sc, sT, tid, 0, make_double2(0.0, 0.0), make_double2(0.0, 0.0), make_double2(0.0, 0.0)};
   kinematics(M, sc, tid, sink);
   sink.flush();
-  return w * bracket(sink.A, sink.Ab, R.y * R.Gamma * t, R.x * R.Gamma * t);
+  return w * bracket<false>(sink.A, sink.Ab, R.y * R.Gamma * t, R.x * R.Gamma * t);
 }
 
 // mode 0: raw candidate dump (parity); mode 1: pilot maximum (G5); mode 2: accept flags + block counts (G6)

@@ -28,7 +28,7 @@ struct EventSet {
   double *s = nullptr, *g = nullptr, *f = nullptr;   // static caches [rows][ld]
   double2 *a = nullptr;                              // coupling columns [K_c][ld]
   double *t = nullptr, *sigma_t = nullptr, *w = nullptr;
-  double sum_t = 0.0;
+  double sum_t = 0.0, t_max = 0.0;                   // sum and max |t| of the decay times (fixed-order kernel)
   uint32_t dirty_cols = 0;                           // columns to recompute before next use
   bool loaded = false;
 };
@@ -229,9 +229,36 @@ int run_columns(tddp4 *h, EventSet &e) {
   return TDDP4_OK;
 }
 
-template <int KC>
-void launch_gram(tddp4 *h, const EventSet &e, int grid) {
-  gram_kernel<KC><<<grid, GRAM_BLOCK, 0, h->stream>>>(e.a, e.ld, e.w, e.n, h->partials, h->ticket, h->G);
+// number of distinct s rows the lineshape instances read
+int used_sys_rows(const ModelTab &M) {
+  unsigned seen = 0;
+  int rows = 0;
+  for (int j = 0; j < M.n_inst; ++j)
+    if (!(seen & (1u << M.inst[j].sys))) { seen |= 1u << M.inst[j].sys; ++rows; }
+  return rows;
+}
+
+// persistent grid: one wave of resident blocks (or fewer if the sample is small)
+template <class K>
+int one_wave(tddp4 *h, K kernel, int block, size_t smem, int64_t n_items_per_block_unit) {
+  int per_sm = 1;
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, block, smem) != cudaSuccess || per_sm < 1) per_sm = 1;
+  int64_t need = (n_items_per_block_unit + block - 1) / block;
+  return (int)std::max<int64_t>(1, std::min<int64_t>(need, (int64_t)h->sm_count * per_sm));
+}
+
+template <int NB>
+int launch_gram(tddp4 *h, const EventSet &e) {
+  size_t smem = gram_smem_bytes(NB, h->M.n_inst);
+  cudaFuncSetAttribute(gram_fused_kernel<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  int grid = one_wave(h, gram_fused_kernel<NB>, GRAM_BLOCK, smem, e.n);
+  int rc = ensure_partials(h, (size_t)grid * 64 * NB * NB + 16);
+  if (rc) return rc;
+  const ModelTab &M = h->M;
+  Prof p(h, TDDP4_K_GRAM, (double)e.n * 8.0 * (used_sys_rows(M) + M.n_inst + M.n_terms + (e.w ? 1 : 0)));
+  gram_fused_kernel<NB><<<grid, GRAM_BLOCK, smem, h->stream>>>(M, h->LP, e.s, e.g, e.f, e.ld, e.w, e.n, h->partials,
+                                                              h->ticket, h->G);
+  return TDDP4_OK;
 }
 
 // step 6: refresh the Gram matrix of this handle's normalisation sample if masses/widths changed
@@ -239,28 +266,12 @@ int ensure_gram(tddp4 *h) {
   if (h->gram_valid) return TDDP4_OK;
   EventSet &e = h->set[1];
   if (!e.loaded) return fail(h, TDDP4_ERR_STATE, "normalisation sample not loaded");
-  int rc = run_columns(h, e);
+  int KC = h->M.n_kc, rc;
+  if (KC <= 4) rc = launch_gram<1>(h, e);
+  else if (KC <= 8) rc = launch_gram<2>(h, e);
+  else if (KC <= 12) rc = launch_gram<3>(h, e);
+  else rc = launch_gram<4>(h, e);
   if (rc) return rc;
-  int KC = h->M.n_kc;
-  int grid = (int)std::min<int64_t>((e.n + GRAM_BLOCK - 1) / GRAM_BLOCK, (int64_t)h->sm_count * 3);
-  grid = std::max(grid, 1);
-  rc = ensure_partials(h, (size_t)grid * KC * KC + 16);
-  if (rc) return rc;
-  {
-    Prof p(h, TDDP4_K_GRAM, (double)e.n * (16.0 * KC + (e.w ? 8.0 : 0.0)));
-    switch (KC) {
-      case 1: launch_gram<1>(h, e, grid); break;
-      case 2: launch_gram<2>(h, e, grid); break;
-      case 3: launch_gram<3>(h, e, grid); break;
-      case 4: launch_gram<4>(h, e, grid); break;
-      case 5: launch_gram<5>(h, e, grid); break;
-      case 6: launch_gram<6>(h, e, grid); break;
-      case 7: launch_gram<7>(h, e, grid); break;
-      case 8: launch_gram<8>(h, e, grid); break;
-      default:
-        gram_generic_kernel<<<grid, GRAM_BLOCK, 0, h->stream>>>(KC, e.a, e.ld, e.w, e.n, h->partials, h->ticket, h->G);
-    }
-  }
   CU(cudaGetLastError());
   h->gram_valid = true;
   h->gram_overridden = false;
@@ -268,14 +279,46 @@ int ensure_gram(tddp4 *h) {
   return TDDP4_OK;
 }
 
+// One grid policy for nll_kernel and columns_nll_kernel (both NLL_BLOCK threads, launch bounds of 4 resident blocks
+// per SM up to K_c = 8, 1 above): the same events meet the same threads on either path, so the fixed-order
+// reduction returns the same bits whether the columns were cached or rebuilt in the call.
+int nll_grid(const tddp4 *h, int64_t n) {
+  int per_sm = h->M.n_kc <= 8 ? 4 : 1;
+  return (int)std::max<int64_t>(1, std::min<int64_t>((n + NLL_BLOCK - 1) / NLL_BLOCK, (int64_t)h->sm_count * per_sm));
+}
+
+template <int KC, bool PROB, bool SMALL>
+int launch_nll_t(tddp4 *h, const EventSet &e, double inv_n, double *result, double *prob) {
+  int grid = nll_grid(h, e.n);
+  int rc = ensure_partials(h, (size_t)2 * grid + 16);
+  if (rc) return rc;
+  Prof p(h, TDDP4_K_NLL, (double)e.n * (16.0 * KC + 8.0 + (PROB ? 8.0 : 0.0)));
+  nll_kernel<KC, PROB, SMALL><<<grid, NLL_BLOCK, 0, h->stream>>>(e.a, e.ld, e.t, e.n, h->RP, h->G, inv_n, e.sum_t,
+                                                                 h->partials, h->ticket, result, prob);
+  return TDDP4_OK;
+}
 template <int KC>
-void launch_nll(tddp4 *h, const EventSet &e, int grid, double inv_n, double *result, double *prob) {
-  if (prob)
-    nll_kernel<KC, true><<<grid, NLL_BLOCK, 0, h->stream>>>(e.a, e.ld, e.t, e.n, h->RP, h->G, inv_n, e.sum_t,
-                                                            h->partials, h->ticket, result, prob);
-  else
-    nll_kernel<KC, false><<<grid, NLL_BLOCK, 0, h->stream>>>(e.a, e.ld, e.t, e.n, h->RP, h->G, inv_n, e.sum_t,
-                                                             h->partials, h->ticket, result, prob);
+int launch_nll(tddp4 *h, const EventSet &e, double inv_n, double *result, double *prob, bool small) {
+  if (prob) return small ? launch_nll_t<KC, true, true>(h, e, inv_n, result, prob) : launch_nll_t<KC, true, false>(h, e, inv_n, result, prob);
+  return small ? launch_nll_t<KC, false, true>(h, e, inv_n, result, prob) : launch_nll_t<KC, false, false>(h, e, inv_n, result, prob);
+}
+
+template <int KC, bool SMALL>
+int launch_colnll_t(tddp4 *h, const EventSet &e, double inv_n, double *result) {
+  const ModelTab &M = h->M;
+  size_t smem = (size_t)std::max(1, M.n_inst) * CNLL_BLOCK * sizeof(double2);
+  cudaFuncSetAttribute(columns_nll_kernel<KC, SMALL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+  int grid = nll_grid(h, e.n);
+  int rc = ensure_partials(h, (size_t)2 * grid + 16);
+  if (rc) return rc;
+  Prof p(h, TDDP4_K_COLNLL, (double)e.n * (8.0 * (used_sys_rows(M) + M.n_inst + M.n_terms + 1) + 16.0 * KC));
+  columns_nll_kernel<KC, SMALL><<<grid, CNLL_BLOCK, smem, h->stream>>>(M, h->LP, e.s, e.g, e.f, e.ld, e.t, e.n, e.a, h->RP,
+                                                                       h->G, inv_n, e.sum_t, h->partials, h->ticket, result);
+  return TDDP4_OK;
+}
+template <int KC>
+int launch_colnll(tddp4 *h, const EventSet &e, double inv_n, double *result, bool small) {
+  return small ? launch_colnll_t<KC, true>(h, e, inv_n, result) : launch_colnll_t<KC, false>(h, e, inv_n, result);
 }
 
 int enqueue_nll(tddp4 *h, double *result, double *prob) {
@@ -285,25 +328,26 @@ int enqueue_nll(tddp4 *h, double *result, double *prob) {
   if (h->use_resolution) return fail(h, TDDP4_ERR_ARG, "use_resolution = 1 is not implemented yet");
   int rc = ensure_gram(h);
   if (rc) return rc;
-  rc = run_columns(h, d);
-  if (rc) return rc;
   int KC = h->M.n_kc;
-  int64_t blocks = (d.n + NLL_BLOCK - 1) / NLL_BLOCK;
-  int grid = (int)std::max<int64_t>(1, std::min<int64_t>(blocks, (int64_t)h->sm_count * 8));
-  rc = ensure_partials(h, (size_t)2 * grid + 16);
-  if (rc) return rc;
   double inv_n = h->gram_n > 0 ? 1.0 / (double)h->gram_n : 0.0;
-  {
-    Prof p(h, TDDP4_K_NLL, (double)d.n * (16.0 * KC + 8.0 + (prob ? 8.0 : 0.0)));
-    switch (KC) {
-#define CASE(k) case k: launch_nll<k>(h, d, grid, inv_n, result, prob); break;
-      CASE(1) CASE(2) CASE(3) CASE(4) CASE(5) CASE(6) CASE(7) CASE(8) CASE(9) CASE(10) CASE(11) CASE(12)
-      CASE(13) CASE(14) CASE(15) CASE(16)
-#undef CASE
-      default: return fail(h, TDDP4_ERR_ARG, "unsupported number of couplings %d", KC);
-    }
+  // Taylor forms of the four time functions are valid when both mixing phases stay below 1/4 on this sample
+  const RateParams &R = h->RP;
+  bool small = std::fabs(R.y) * R.Gamma * d.t_max < 0.25 && std::fabs(R.x) * R.Gamma * d.t_max < 0.25;
+  bool fused = !prob && d.dirty_cols != 0 && d.n > 0;
+  if (!fused) {
+    rc = run_columns(h, d);
+    if (rc) return rc;
   }
+  switch (KC) {
+#define CASE(k) case k: rc = fused ? launch_colnll<k>(h, d, inv_n, result, small) : launch_nll<k>(h, d, inv_n, result, prob, small); break;
+    CASE(1) CASE(2) CASE(3) CASE(4) CASE(5) CASE(6) CASE(7) CASE(8) CASE(9) CASE(10) CASE(11) CASE(12)
+    CASE(13) CASE(14) CASE(15) CASE(16)
+#undef CASE
+    default: return fail(h, TDDP4_ERR_ARG, "unsupported number of couplings %d", KC);
+  }
+  if (rc) return rc;
   CU(cudaGetLastError());
+  if (fused) d.dirty_cols = 0;
   return TDDP4_OK;
 }
 
@@ -475,7 +519,7 @@ int tddp4_load_events(tddp4 *h, int which, int64_t n, int64_t ld_in, const doubl
   CU(cudaMalloc(&e.s, sizeof(double) * M.n_sys * e.ld));
   CU(cudaMalloc(&e.g, sizeof(double) * std::max(1, M.n_inst) * e.ld));
   CU(cudaMalloc(&e.f, sizeof(double) * M.n_terms * e.ld));
-  CU(cudaMalloc(&e.a, sizeof(double2) * M.n_kc * e.ld));
+  if (which == 0) CU(cudaMalloc(&e.a, sizeof(double2) * M.n_kc * e.ld));   // the normalisation sample keeps no columns
   cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
   auto copy_vec = [&](double **dst, const double *src) -> cudaError_t {
     if (!src || n == 0) return cudaSuccess;
@@ -505,9 +549,13 @@ int tddp4_load_events(tddp4 *h, int which, int64_t n, int64_t ld_in, const doubl
     }
     CU(cudaGetLastError());
     if (e.t) {
-      sum_kernel<<<1, 256, 0, h->stream>>>(e.t, n, h->results);   // slot 0 word 0 as scratch
+      double st[2];
+      stat_kernel<<<1, 1024, 0, h->stream>>>(e.t, n, h->results);   // slot 0 words 0, 1 as scratch
       ++h->launches;
-      CU(cudaMemcpyAsync(&e.sum_t, h->results, sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+      CU(cudaMemcpyAsync(st, h->results, 2 * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+      CU(cudaStreamSynchronize(h->stream));
+      e.sum_t = st[0];
+      e.t_max = st[1];
     }
     CU(cudaStreamSynchronize(h->stream));
     if (staging) cudaFree(staging);
@@ -815,6 +863,7 @@ int tddp4_get(tddp4 *h, int which, int what, double *out) {
       return TDDP4_OK;
     }
     case TDDP4_GET_COLUMNS: {
+      if (which != 0) return fail(h, TDDP4_ERR_ARG, "the normalisation sample keeps no coupling columns");
       if (!h->have_params) return fail(h, TDDP4_ERR_STATE, "tddp4_set_params has not been called");
       int rc = run_columns(h, e);
       if (rc) return rc;

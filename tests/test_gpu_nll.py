@@ -307,3 +307,37 @@ def test_sharded_evaluation_adds_up(B):
         norm = parts["norm"]
     nll = sum_t / par.tau - sum_log_b + p4.shape[1] * math.log(norm)
     assert abs(nll - full) < 1e-12 * abs(full)
+
+
+def test_large_mixing_phases_use_the_full_range_functions(B):
+    """x, y far from the small-phase regime: the kernels switch from Taylor polynomials to exp / sincos."""
+    mdl = samples.model_of(("C", 2))
+    par = W.initial_params(mdl)
+    par.x, par.y = 0.83, -0.41
+    p4, t, _ = samples.data_sample(("C", 2), 2_000)
+    p4n, _ = samples.flat_sample(5_000)
+    h = check_against_oracle(B, mdl, par, p4, t, p4n)
+    step = par.copy(); step.mass = par.mass * 1.001          # same regime through the fused columns+NLL kernel
+    h.set_params(step)
+    ref = oracle.nll(mdl, step, p4, t, p4n)
+    assert nll_close(h.nll(), ref[0], np.log(ref[2]))
+    # just below / above the switch-over (|phase| = 1/4 at the largest decay time) both agree with the oracle
+    for scale in (0.999, 1.001):
+        q = par.copy(); q.y = 0.0061; q.x = scale * 0.25 * par.tau / t.max()
+        h.set_params(q)
+        ref = oracle.nll(mdl, q, p4, t, p4n)
+        assert nll_close(h.nll(), ref[0], np.log(ref[2]))
+
+
+@pytest.mark.parametrize("chains", [(1, 2, 3, 4, 5, 6, 7, 8, 1, 3), (1, 2, 3, 4, 5, 6, 7, 8, 2, 3, 4, 5, 6)])
+def test_more_than_eight_couplings(B, chains):
+    """K_c = 10 and 13: the Gram kernel's 3- and 4-block tensor-core tilings and the wide NLL kernels."""
+    mdl = samples.model_of(("chains", chains, False))
+    par = W.initial_params(mdl)
+    p4, t, _ = samples.data_sample(("C", 2), 1_111)
+    p4n, _ = samples.flat_sample(3_333)
+    h = check_against_oracle(B, mdl, par, p4, t, p4n)
+    step = par.copy(); step.width = par.width * 1.01
+    h.set_params(step)
+    ref = oracle.nll(mdl, step, p4, t, p4n)
+    assert nll_close(h.nll(), ref[0], np.log(ref[2]))
