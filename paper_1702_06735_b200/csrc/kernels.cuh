@@ -53,39 +53,7 @@ kin_kernel(const __grid_constant__ ModelTab M, const double *__restrict__ p4, in
 }
 
 // ------------------------------------------------------------------------------------------------
-// steps 2+3: lineshapes of the instances feeding the dirty coupling columns, component products,
-// Bose orderings summed into one column per coupling.  One thread per event; T_R staged in shared
-// memory so that chains index it dynamically (each recurring lineshape evaluated once).
 constexpr int COL_BLOCK = 128;
-__global__ void __launch_bounds__(COL_BLOCK)
-columns_kernel(const __grid_constant__ ModelTab M, const __grid_constant__ LineParams LP, uint32_t inst_mask,
-               uint32_t col_mask, const double *__restrict__ s, const double *__restrict__ g,
-               const double *__restrict__ f, int64_t ld, int64_t n, double2 *__restrict__ a) {
-  extern __shared__ double2 sT[];   // [n_inst][COL_BLOCK]
-  int tid = threadIdx.x;
-  int64_t i = (int64_t)blockIdx.x * COL_BLOCK + tid;
-  if (i >= n) return;
-  for (int j = 0; j < M.n_inst; ++j) {
-    if (!(inst_mask & (1u << j))) continue;
-    double sv = __ldg(s + M.inst[j].sys * ld + i);
-    double gv = __ldg(g + j * ld + i);
-    sT[j * COL_BLOCK + tid] = breit_wigner(LP.m0sq[j], LP.gam[j], sv, gv);
-  }
-  for (int kap = 0; kap < M.n_kc; ++kap) {
-    if (!(col_mask & (1u << kap))) continue;
-    double2 acc = make_double2(0.0, 0.0);
-    for (int k = M.col_begin[kap]; k < M.col_begin[kap + 1]; ++k) {
-      const TermTab &tm = M.term[k];
-      double fv = __ldg(f + k * ld + i);
-      double2 T = make_double2(1.0, 0.0);
-      if (tm.inst0 >= 0) T = cmul(sT[tm.inst0 * COL_BLOCK + tid], sT[tm.inst1 * COL_BLOCK + tid]);
-      acc.x += fv * T.x;
-      acc.y += fv * T.y;
-    }
-    a[kap * ld + i] = acc;
-  }
-}
-
 // per-term amplitudes a_k (un-summed), for per-layer parity only (TDDP4_GET_TERMS)
 __global__ void __launch_bounds__(COL_BLOCK)
 terms_kernel(const __grid_constant__ ModelTab M, const __grid_constant__ LineParams LP, const double *__restrict__ s,
@@ -107,162 +75,8 @@ terms_kernel(const __grid_constant__ ModelTab M, const __grid_constant__ LinePar
 }
 
 // ------------------------------------------------------------------------------------------------
-// Lineshapes + component products of ONE event from the step-1 caches (steps 2+3): T_R of every instance into
-// the thread's shared-memory slots, then the K_c coupling columns into col[].  Rows are read with streaming
-// loads; each is touched once per pass.
-template <int KC, int BLOCK>
-__device__ __forceinline__ void event_columns(const ModelTab &M, const LineParams &LP, const double *__restrict__ s,
-                                              const double *__restrict__ g, const double *__restrict__ f, int64_t ld,
-                                              int64_t i, double2 *sT, int tid, double2 col[KC]) {
-  for (int j = 0; j < M.n_inst; ++j) {
-    double sv = __ldcs(s + M.inst[j].sys * ld + i);
-    double gv = __ldcs(g + j * ld + i);
-    sT[j * BLOCK + tid] = breit_wigner(LP.m0sq[j], LP.gam[j], sv, gv);
-  }
-#pragma unroll
-  for (int kap = 0; kap < KC; ++kap) {
-    double2 acc = make_double2(0.0, 0.0);
-    for (int k = M.col_begin[kap]; k < M.col_begin[kap + 1]; ++k) {
-      const TermTab &tm = M.term[k];
-      double fv = __ldcs(f + k * ld + i);
-      double2 T = make_double2(1.0, 0.0);
-      if (tm.inst0 >= 0) T = cmul(sT[tm.inst0 * BLOCK + tid], sT[tm.inst1 * BLOCK + tid]);
-      acc.x += fv * T.x;
-      acc.y += fv * T.y;
-    }
-    col[kap] = acc;
-  }
-}
-
-// ------------------------------------------------------------------------------------------------
-// step 6: Hermitian Gram matrix G_kl = sum_j w_j a_k(p_j) conj(a_l(p_j)) over the normalisation sample, fused with
-// steps 2+3: the columns of the normalisation sample are never stored.  With x_j = (Re a_0, Im a_0, Re a_1, ...)
-// the real matrix X^T diag(w) X holds every Re/Im piece of G, and it is a dense contraction over events: it runs on
-// the fp64 tensor cores (mma.sync m8n8k4 DMMA), the only place of the path where they apply (north_star).
-//   G_kl.re = XtX[2k][2l] + XtX[2k+1][2l+1],   G_kl.im = XtX[2k+1][2l] - XtX[2k][2l+1].
-// One thread per event computes the columns; each warp then feeds its own 32 events, 4 at a time, through the
-// MMA from a padded shared-memory tile (no block barrier inside the loop).  NB = number of 8-feature blocks.
-// Deterministic: per-warp accumulation in event order, warps then blocks summed in index order.
-constexpr int GRAM_BLOCK = 128;
-__host__ __device__ constexpr int gram_stride(int NB) { return NB <= 2 ? 20 : 36; }   // = 4 mod 16: conflict-free fragments
-__host__ __device__ inline size_t gram_smem_bytes(int NB, int n_inst) {
-  return sizeof(double2) * (size_t)(n_inst > 0 ? n_inst : 1) * GRAM_BLOCK + sizeof(double) * GRAM_BLOCK * gram_stride(NB) +
-         sizeof(double) * (GRAM_BLOCK / 32) * 64 * NB * NB;
-}
-
-__device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double b) {
-  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
-               : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
-}
-
-template <int NB>
-__global__ void __launch_bounds__(GRAM_BLOCK)
-gram_fused_kernel(const __grid_constant__ ModelTab M, const __grid_constant__ LineParams LP,
-                  const double *__restrict__ s, const double *__restrict__ g, const double *__restrict__ f, int64_t ld,
-                  const double *__restrict__ w, int64_t n, double *__restrict__ partials /* [grid][64 NB NB] */,
-                  unsigned int *ticket, double *__restrict__ G /* [KC][KC][2] sums, Hermitian, full */) {
-  constexpr int KCMAX = 4 * NB, F = 8 * NB, STRIDE = gram_stride(NB), NP = NB * (NB + 1) / 2;
-  extern __shared__ double2 smem2[];
-  double2 *sT = smem2;                                                        // [n_inst][GRAM_BLOCK]
-  double *Xs = reinterpret_cast<double *>(smem2 + (M.n_inst > 0 ? M.n_inst : 1) * GRAM_BLOCK);   // [GRAM_BLOCK][STRIDE]
-  double *Ws = Xs + GRAM_BLOCK * STRIDE;                                      // [warps][NB*NB][64] block reduction
-  __shared__ bool last;
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int KC = M.n_kc;
-  double acc[NP][2];
-#pragma unroll
-  for (int q = 0; q < NP; ++q) acc[q][0] = acc[q][1] = 0.0;
-  double *row = Xs + tid * STRIDE;
-  const int64_t n_tiles = (n + GRAM_BLOCK - 1) / GRAM_BLOCK;
-  for (int64_t tile = blockIdx.x; tile < n_tiles; tile += gridDim.x) {
-    int64_t i = tile * GRAM_BLOCK + tid;
-    double2 col[KCMAX];
-    double wj = 0.0;
-    if (i < n) {
-      event_columns<KCMAX, GRAM_BLOCK>(M, LP, s, g, f, ld, i, sT, tid, col);   // columns >= KC have no terms: zero
-      wj = w ? __ldcs(w + i) : 1.0;
-    } else {
-#pragma unroll
-      for (int k = 0; k < KCMAX; ++k) col[k] = make_double2(0.0, 0.0);
-    }
-    __syncwarp();                                       // previous tile's fragments of this warp are consumed
-#pragma unroll
-    for (int k = 0; k < KCMAX; ++k) *reinterpret_cast<double2 *>(row + 2 * k) = col[k];
-    row[F] = wj;
-    __syncwarp();
-    const double *base = Xs + (warp * 32 + (lane & 3)) * STRIDE + (lane >> 2);
-#pragma unroll
-    for (int grp = 0; grp < 8; ++grp) {                  // 4 events per MMA, 8 groups per warp tile
-      const double *r = base + grp * 4 * STRIDE;
-      double wv = r[F - (lane >> 2)];
-      double x[NB];
-#pragma unroll
-      for (int b = 0; b < NB; ++b) x[b] = r[8 * b];
-      int q = 0;
-#pragma unroll
-      for (int bi = 0; bi < NB; ++bi) {
-        double aw = wv * x[bi];
-#pragma unroll
-        for (int bj = bi; bj < NB; ++bj, ++q) dmma884(acc[q][0], acc[q][1], aw, x[bj]);
-      }
-    }
-  }
-  // block reduction in warp order, block partial [NB*NB block pairs as full F x F upper blocks]
-  {
-    int q = 0;
-#pragma unroll
-    for (int bi = 0; bi < NB; ++bi)
-#pragma unroll
-      for (int bj = bi; bj < NB; ++bj, ++q) {
-        double *dst = Ws + ((warp * NB + bi) * NB + bj) * 64;
-        dst[(lane >> 2) * 8 + 2 * (lane & 3)] = acc[q][0];      // C fragment: row lane/4, cols 2 (lane%4) + {0,1}
-        dst[(lane >> 2) * 8 + 2 * (lane & 3) + 1] = acc[q][1];
-      }
-  }
-  __syncthreads();
-  for (int e = tid; e < NB * NB * 64; e += GRAM_BLOCK) {
-    int bi = e / (NB * 64), bj = (e / 64) % NB;
-    if (bi > bj) continue;
-    double sum = 0.0;
-#pragma unroll
-    for (int wp = 0; wp < GRAM_BLOCK / 32; ++wp) sum += Ws[wp * NB * NB * 64 + e];
-    partials[(int64_t)blockIdx.x * NB * NB * 64 + e] = sum;
-  }
-  __threadfence();
-  __syncthreads();
-  if (tid == 0) last = atomicAdd(ticket, 1u) == gridDim.x - 1;
-  __syncthreads();
-  if (!last) return;
-  __threadfence();
-  // final pass: XtX (upper blocks) summed over blocks in index order, staged in shared memory, then G
-  double *XtX = Ws;                                      // [NB][NB][64], reused
-  for (int e = tid; e < NB * NB * 64; e += GRAM_BLOCK) {
-    int bi = e / (NB * 64), bj = (e / 64) % NB;
-    if (bi > bj) continue;
-    double sum = 0.0;
-    for (unsigned b = 0; b < gridDim.x; ++b) sum += __ldcg(partials + (int64_t)b * NB * NB * 64 + e);
-    XtX[e] = sum;
-  }
-  __syncthreads();
-  auto xtx = [&](int m, int nn) {                        // symmetric: only the upper triangle is ever read
-    if (m > nn) { int tmp = m; m = nn; nn = tmp; }
-    return XtX[((m >> 3) * NB + (nn >> 3)) * 64 + (m & 7) * 8 + (nn & 7)];
-  };
-  for (int q = tid; q < KC * KC; q += GRAM_BLOCK) {
-    int k = q / KC, l = q % KC;
-    double re = xtx(2 * k, 2 * l) + xtx(2 * k + 1, 2 * l + 1);
-    double im = xtx(2 * k + 1, 2 * l) - xtx(2 * k, 2 * l + 1);
-    if (k == l) im = 0.0;
-    G[q * 2] = re;
-    G[q * 2 + 1] = im;
-  }
-  if (tid == 0) *ticket = 0;
-}
-
-// ------------------------------------------------------------------------------------------------
 // steps 4+5+7: amplitude sums (eq. 2), mixing rate (eq. 1), -log reduction.
 // result slot layout (doubles): [0] sum log B, [1] sum t, [2] N, [3] NLL, [4] #bad events
-constexpr int NLL_BLOCK = 256;
 
 // N from the Gram matrix in force: N = T1 (nAA + nBB) + T2 (nAA - nBB) - 2 T3 Re X - 2 T4 Im X,
 // nAA = c^T G conj(c), nBB likewise for cbar, X = sum_kl c_k conj(cbar_l) G_kl   (O-8, step 6).
@@ -366,73 +180,6 @@ __device__ __forceinline__ void nll_finish(const RateParams &R, int64_t n, doubl
   }
 }
 
-// Coupling-only call: streams the K_c cached columns (16 B / event / column, 128-bit coalesced loads) and t.
-// SMALL: |y Gamma t|, |x Gamma t| < 1/4 for every event of the sample (checked on the host from max |t|): the four
-// time functions are short Taylor polynomials instead of exp / sincos.
-template <int KC, bool PROB, bool SMALL>
-__global__ void __launch_bounds__(NLL_BLOCK, KC <= 8 ? 4 : 1)
-nll_kernel(const double2 *__restrict__ a, int64_t ld, const double *__restrict__ t, int64_t n,
-           const __grid_constant__ RateParams R, const double *__restrict__ G, double inv_n_norm, double sum_t,
-           double *__restrict__ partials, unsigned int *ticket, double *__restrict__ result,
-           double *__restrict__ prob_out) {
-  __shared__ double red[NLL_BLOCK / 32];
-  __shared__ double s_norm;
-  __shared__ bool last;
-  double norm0 = 0.0;
-  if (PROB || blockIdx.x == 0) {                         // block 0 evaluates N while the others already stream
-    norm0 = norm_from_gram<NLL_BLOCK>(R, G, KC, inv_n_norm, red);
-    if (PROB) {
-      if (threadIdx.x == 0) s_norm = norm0;
-      __syncthreads();
-    }
-  }
-  LogAcc la;
-  const double yG = R.y * R.Gamma, xG = R.x * R.Gamma;
-  for (int64_t i = (int64_t)blockIdx.x * NLL_BLOCK + threadIdx.x; i < n; i += (int64_t)gridDim.x * NLL_BLOCK) {
-    double2 v[KC];
-#pragma unroll
-    for (int k = 0; k < KC; ++k) v[k] = __ldcs(a + k * ld + i);
-    double ti = __ldcs(t + i);
-    double2 A, Ab;
-    amplitude_sums<KC>(R, v, A, Ab);
-    double B = bracket<SMALL>(A, Ab, yG * ti, xG * ti);
-    la.add(B);
-    if (PROB) prob_out[i] = exp(-R.Gamma * ti) * B / s_norm;
-  }
-  nll_finish<NLL_BLOCK>(R, n, sum_t, la.value(), (double)la.bad, norm0, partials, ticket, result, red, &last);
-}
-
-// Call after a mass or width moved: steps 2+3 for every column from the step-1 caches, columns written back for the
-// coupling-only calls that follow, and steps 4+5+7 in the same pass (the fresh columns never leave registers).
-constexpr int CNLL_BLOCK = NLL_BLOCK;   // same block size and grid as nll_kernel: the two paths then add the same
-                                        // per-thread terms in the same order and return bit-identical NLLs
-template <int KC, bool SMALL>
-__global__ void __launch_bounds__(CNLL_BLOCK, KC <= 8 ? 4 : 1)
-columns_nll_kernel(const __grid_constant__ ModelTab M, const __grid_constant__ LineParams LP,
-                   const double *__restrict__ s, const double *__restrict__ g, const double *__restrict__ f, int64_t ld,
-                   const double *__restrict__ t, int64_t n, double2 *__restrict__ a,
-                   const __grid_constant__ RateParams R, const double *__restrict__ G, double inv_n_norm, double sum_t,
-                   double *__restrict__ partials, unsigned int *ticket, double *__restrict__ result) {
-  extern __shared__ double2 sT[];                        // [n_inst][CNLL_BLOCK]
-  __shared__ double red[CNLL_BLOCK / 32];
-  __shared__ bool last;
-  double norm0 = 0.0;
-  if (blockIdx.x == 0) norm0 = norm_from_gram<CNLL_BLOCK>(R, G, KC, inv_n_norm, red);
-  LogAcc la;
-  const double yG = R.y * R.Gamma, xG = R.x * R.Gamma;
-  for (int64_t i = (int64_t)blockIdx.x * CNLL_BLOCK + threadIdx.x; i < n; i += (int64_t)gridDim.x * CNLL_BLOCK) {
-    double2 v[KC];
-    event_columns<KC, CNLL_BLOCK>(M, LP, s, g, f, ld, i, sT, threadIdx.x, v);
-    double ti = __ldcs(t + i);
-#pragma unroll
-    for (int k = 0; k < KC; ++k) a[k * ld + i] = v[k];
-    double2 A, Ab;
-    amplitude_sums<KC>(R, v, A, Ab);
-    la.add(bracket<SMALL>(A, Ab, yG * ti, xG * ti));
-  }
-  nll_finish<CNLL_BLOCK>(R, n, sum_t, la.value(), (double)la.bad, norm0, partials, ticket, result, red, &last);
-}
-
 // deterministic sum and max |.| of a vector (decay times at load): one block, fixed order
 __global__ void __launch_bounds__(1024) stat_kernel(const double *__restrict__ v, int64_t n, double *out /* [2] */) {
   __shared__ double red[32];
@@ -454,6 +201,10 @@ __global__ void __launch_bounds__(1024) stat_kernel(const double *__restrict__ v
     out[1] = mx;
   }
 }
+
+}  // namespace tddp4k
+#include "stream_kernels.cuh"
+namespace tddp4k {
 
 // ------------------------------------------------------------------------------------------------
 // G1-G4: candidate generation and rate on the fly (no caches).  One thread per candidate.

@@ -29,7 +29,7 @@ struct EventSet {
   double2 *a = nullptr;                              // coupling columns [K_c][ld]
   double *t = nullptr, *sigma_t = nullptr, *w = nullptr;
   double sum_t = 0.0, t_max = 0.0;                   // sum and max |t| of the decay times (fixed-order kernel)
-  uint32_t dirty_cols = 0;                           // columns to recompute before next use
+  bool cols_dirty = true;                            // coupling columns stale (a mass or width moved since they were built)
   bool loaded = false;
 };
 
@@ -51,7 +51,6 @@ struct tddp4 {
   LineParams LP{};
   RateParams RP{};
   std::vector<double> mass, width;
-  uint32_t col_of_inst[MAX_INST] = {0};   // columns fed by each instance
   EventSet set[2];
   // normalisation
   double *G = nullptr;               // device [K_c][K_c][2] sums
@@ -82,6 +81,7 @@ struct tddp4 {
   int64_t prof_n[TDDP4_K_COUNT] = {0};
   int64_t launches = 0;
   int sm_count = 148;
+  int tile = 256;                    // events per tile of the streaming kernels (128 for very large models)
   std::string err;
 };
 
@@ -201,63 +201,53 @@ void free_set(EventSet &e) {
   e = EventSet{};
 }
 
-uint32_t all_cols(const tddp4 *h) { return h->M.n_kc >= 32 ? 0xffffffffu : ((1u << h->M.n_kc) - 1u); }
+// rows of one tile for the kernels that start from the step-1 caches: s rows in use, g rows, f rows [, extra]
+RowList static_rows(const tddp4 *h, const EventSet &e, const double *extra) {
+  const ModelTab &M = h->M;
+  RowList r{};
+  r.arr[0] = reinterpret_cast<const char *>(e.s);
+  r.arr[1] = reinterpret_cast<const char *>(e.g);
+  r.arr[2] = reinterpret_cast<const char *>(e.f);
+  r.arr[3] = reinterpret_cast<const char *>(extra);
+  for (int i = 0; i < M.n_su; ++i) r.add(0, M.su_sys[i], 8);
+  for (int j = 0; j < M.n_inst; ++j) r.add(1, j, 8);
+  for (int k = 0; k < M.n_terms; ++k) r.add(2, k, 8);
+  if (extra) r.add(3, 0, 8);
+  return r;
+}
+// rows of one tile for the coupling-only kernel: K_c columns (16-byte elements), then t
+RowList column_rows(const tddp4 *h, const EventSet &e) {
+  RowList r{};
+  r.arr[0] = reinterpret_cast<const char *>(e.a);
+  r.arr[1] = reinterpret_cast<const char *>(e.t);
+  for (int k = 0; k < h->M.n_kc; ++k) r.add(0, k, 16);
+  r.add(1, 0, 8);
+  return r;
+}
 
-// steps 2+3 on one event set for the columns in its dirty mask
-int run_columns(tddp4 *h, EventSet &e) {
-  if (!e.dirty_cols || e.n == 0) { e.dirty_cols = 0; return TDDP4_OK; }
-  uint32_t inst_mask = 0;
-  for (int j = 0; j < h->M.n_inst; ++j)
-    if (h->col_of_inst[j] & e.dirty_cols) inst_mask |= 1u << j;
-  int grid = (int)((e.n + COL_BLOCK - 1) / COL_BLOCK);
-  size_t smem = (size_t)std::max(1, h->M.n_inst) * COL_BLOCK * sizeof(double2);
-  // algorithmic bytes: s rows and g rows of the dirty instances, f rows of the dirty columns' terms, columns written
-  unsigned sys_seen = 0;
-  int rows = 0;
-  for (int j = 0; j < h->M.n_inst; ++j)
-    if (inst_mask & (1u << j)) { ++rows; if (!(sys_seen & (1u << h->M.inst[j].sys))) { sys_seen |= 1u << h->M.inst[j].sys; ++rows; } }
-  int ncol = 0;
-  for (int kap = 0; kap < h->M.n_kc; ++kap)
-    if (e.dirty_cols & (1u << kap)) { ++ncol; rows += h->M.col_begin[kap + 1] - h->M.col_begin[kap]; }
-  {
-    Prof p(h, TDDP4_K_COLUMNS, (double)e.n * (8.0 * rows + 16.0 * ncol));
-    columns_kernel<<<grid, COL_BLOCK, smem, h->stream>>>(h->M, h->LP, inst_mask, e.dirty_cols, e.s, e.g, e.f, e.ld,
-                                                         e.n, e.a);
-  }
-  CU(cudaGetLastError());
-  e.dirty_cols = 0;
+int stream_grid(const tddp4 *h, int64_t n, int tile) {
+  return (int)std::max<int64_t>(1, std::min<int64_t>((n + tile - 1) / tile, (int64_t)h->sm_count));
+}
+
+template <class K>
+int set_smem(tddp4 *h, K kernel, size_t bytes) {
+  CU(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
   return TDDP4_OK;
 }
 
-// number of distinct s rows the lineshape instances read
-int used_sys_rows(const ModelTab &M) {
-  unsigned seen = 0;
-  int rows = 0;
-  for (int j = 0; j < M.n_inst; ++j)
-    if (!(seen & (1u << M.inst[j].sys))) { seen |= 1u << M.inst[j].sys; ++rows; }
-  return rows;
-}
-
-// persistent grid: one wave of resident blocks (or fewer if the sample is small)
-template <class K>
-int one_wave(tddp4 *h, K kernel, int block, size_t smem, int64_t n_items_per_block_unit) {
-  int per_sm = 1;
-  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, kernel, block, smem) != cudaSuccess || per_sm < 1) per_sm = 1;
-  int64_t need = (n_items_per_block_unit + block - 1) / block;
-  return (int)std::max<int64_t>(1, std::min<int64_t>(need, (int64_t)h->sm_count * per_sm));
-}
-
-template <int NB>
+template <int NB, int TILE>
 int launch_gram(tddp4 *h, const EventSet &e) {
-  size_t smem = gram_smem_bytes(NB, h->M.n_inst);
-  cudaFuncSetAttribute(gram_fused_kernel<NB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  int grid = one_wave(h, gram_fused_kernel<NB>, GRAM_BLOCK, smem, e.n);
-  int rc = ensure_partials(h, (size_t)grid * 64 * NB * NB + 16);
-  if (rc) return rc;
   const ModelTab &M = h->M;
-  Prof p(h, TDDP4_K_GRAM, (double)e.n * 8.0 * (used_sys_rows(M) + M.n_inst + M.n_terms + (e.w ? 1 : 0)));
-  gram_fused_kernel<NB><<<grid, GRAM_BLOCK, smem, h->stream>>>(M, h->LP, e.s, e.g, e.f, e.ld, e.w, e.n, h->partials,
-                                                              h->ticket, h->G);
+  RowList rows = static_rows(h, e, e.w);
+  size_t smem = gram_smem_bytes<TILE>(NB, rows.bytes_per_event, M.n_inst);
+  int rc = set_smem(h, gram_stream_kernel<NB, TILE>, smem);
+  if (rc) return rc;
+  int grid = stream_grid(h, e.n, TILE);
+  rc = ensure_partials(h, (size_t)grid * 64 * NB * NB + 16);
+  if (rc) return rc;
+  Prof p(h, TDDP4_K_GRAM, (double)e.n * rows.bytes_per_event);
+  gram_stream_kernel<NB, TILE><<<grid, TILE, smem, h->stream>>>(M, h->LP, rows, e.ld, e.n, e.w ? 1 : 0, h->partials,
+                                                                h->ticket, h->G);
   return TDDP4_OK;
 }
 
@@ -267,10 +257,11 @@ int ensure_gram(tddp4 *h) {
   EventSet &e = h->set[1];
   if (!e.loaded) return fail(h, TDDP4_ERR_STATE, "normalisation sample not loaded");
   int KC = h->M.n_kc, rc;
-  if (KC <= 4) rc = launch_gram<1>(h, e);
-  else if (KC <= 8) rc = launch_gram<2>(h, e);
-  else if (KC <= 12) rc = launch_gram<3>(h, e);
-  else rc = launch_gram<4>(h, e);
+  bool big = h->tile == 256;
+  if (KC <= 4) rc = big ? launch_gram<1, 256>(h, e) : launch_gram<1, 128>(h, e);
+  else if (KC <= 8) rc = big ? launch_gram<2, 256>(h, e) : launch_gram<2, 128>(h, e);
+  else if (KC <= 12) rc = big ? launch_gram<3, 256>(h, e) : launch_gram<3, 128>(h, e);
+  else rc = big ? launch_gram<4, 256>(h, e) : launch_gram<4, 128>(h, e);
   if (rc) return rc;
   CU(cudaGetLastError());
   h->gram_valid = true;
@@ -279,48 +270,73 @@ int ensure_gram(tddp4 *h) {
   return TDDP4_OK;
 }
 
-// One grid policy for nll_kernel and columns_nll_kernel (both NLL_BLOCK threads, launch bounds of 4 resident blocks
-// per SM up to K_c = 8, 1 above): the same events meet the same threads on either path, so the fixed-order
-// reduction returns the same bits whether the columns were cached or rebuilt in the call.
-int nll_grid(const tddp4 *h, int64_t n) {
-  int per_sm = h->M.n_kc <= 8 ? 4 : 1;
-  return (int)std::max<int64_t>(1, std::min<int64_t>((n + NLL_BLOCK - 1) / NLL_BLOCK, (int64_t)h->sm_count * per_sm));
-}
-
-template <int KC, bool PROB, bool SMALL>
+template <int KC, bool PROB, bool SMALL, int TILE>
 int launch_nll_t(tddp4 *h, const EventSet &e, double inv_n, double *result, double *prob) {
-  int grid = nll_grid(h, e.n);
-  int rc = ensure_partials(h, (size_t)2 * grid + 16);
+  RowList rows = column_rows(h, e);
+  size_t smem = nll_smem_bytes<TILE>(KC);
+  int rc = set_smem(h, nll_stream_kernel<KC, PROB, SMALL, TILE>, smem);
   if (rc) return rc;
-  Prof p(h, TDDP4_K_NLL, (double)e.n * (16.0 * KC + 8.0 + (PROB ? 8.0 : 0.0)));
-  nll_kernel<KC, PROB, SMALL><<<grid, NLL_BLOCK, 0, h->stream>>>(e.a, e.ld, e.t, e.n, h->RP, h->G, inv_n, e.sum_t,
-                                                                 h->partials, h->ticket, result, prob);
+  int grid = stream_grid(h, e.n, TILE);
+  rc = ensure_partials(h, (size_t)2 * grid + 16);
+  if (rc) return rc;
+  Prof p(h, TDDP4_K_NLL, (double)e.n * (rows.bytes_per_event + (PROB ? 8.0 : 0.0)));
+  nll_stream_kernel<KC, PROB, SMALL, TILE><<<grid, TILE, smem, h->stream>>>(rows, e.ld, e.n, h->RP, h->G, inv_n, e.sum_t,
+                                                                            h->partials, h->ticket, result, prob);
   return TDDP4_OK;
 }
 template <int KC>
 int launch_nll(tddp4 *h, const EventSet &e, double inv_n, double *result, double *prob, bool small) {
-  if (prob) return small ? launch_nll_t<KC, true, true>(h, e, inv_n, result, prob) : launch_nll_t<KC, true, false>(h, e, inv_n, result, prob);
-  return small ? launch_nll_t<KC, false, true>(h, e, inv_n, result, prob) : launch_nll_t<KC, false, false>(h, e, inv_n, result, prob);
+#define GO(P, S) (h->tile == 256 ? launch_nll_t<KC, P, S, 256>(h, e, inv_n, result, prob) : launch_nll_t<KC, P, S, 128>(h, e, inv_n, result, prob))
+  if (prob) return small ? GO(true, true) : GO(true, false);
+  return small ? GO(false, true) : GO(false, false);
+#undef GO
 }
 
-template <int KC, bool SMALL>
+template <int KC, bool SMALL, int TILE>
 int launch_colnll_t(tddp4 *h, const EventSet &e, double inv_n, double *result) {
   const ModelTab &M = h->M;
-  size_t smem = (size_t)std::max(1, M.n_inst) * CNLL_BLOCK * sizeof(double2);
-  cudaFuncSetAttribute(columns_nll_kernel<KC, SMALL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
-  int grid = nll_grid(h, e.n);
-  int rc = ensure_partials(h, (size_t)2 * grid + 16);
+  RowList rows = static_rows(h, e, e.t);
+  size_t smem = colnll_smem_bytes<TILE>(rows.bytes_per_event, M.n_inst);
+  int rc = set_smem(h, colnll_stream_kernel<KC, SMALL, TILE>, smem);
   if (rc) return rc;
-  Prof p(h, TDDP4_K_COLNLL, (double)e.n * (8.0 * (used_sys_rows(M) + M.n_inst + M.n_terms + 1) + 16.0 * KC));
-  columns_nll_kernel<KC, SMALL><<<grid, CNLL_BLOCK, smem, h->stream>>>(M, h->LP, e.s, e.g, e.f, e.ld, e.t, e.n, e.a, h->RP,
-                                                                       h->G, inv_n, e.sum_t, h->partials, h->ticket, result);
+  int grid = stream_grid(h, e.n, TILE);
+  rc = ensure_partials(h, (size_t)2 * grid + 16);
+  if (rc) return rc;
+  Prof p(h, TDDP4_K_COLNLL, (double)e.n * (rows.bytes_per_event + 16.0 * KC));
+  colnll_stream_kernel<KC, SMALL, TILE><<<grid, TILE, smem, h->stream>>>(M, h->LP, rows, e.ld, e.n, e.a, h->RP, h->G, inv_n,
+                                                                         e.sum_t, h->partials, h->ticket, result);
   return TDDP4_OK;
 }
 template <int KC>
 int launch_colnll(tddp4 *h, const EventSet &e, double inv_n, double *result, bool small) {
-  return small ? launch_colnll_t<KC, true>(h, e, inv_n, result) : launch_colnll_t<KC, false>(h, e, inv_n, result);
+  if (h->tile == 256) return small ? launch_colnll_t<KC, true, 256>(h, e, inv_n, result) : launch_colnll_t<KC, false, 256>(h, e, inv_n, result);
+  return small ? launch_colnll_t<KC, true, 128>(h, e, inv_n, result) : launch_colnll_t<KC, false, 128>(h, e, inv_n, result);
 }
 
+int dispatch_nll(tddp4 *h, EventSet &d, bool fused, double inv_n, double *result, double *prob, bool small) {
+  int rc;
+  switch (h->M.n_kc) {
+#define CASE(k) case k: rc = fused ? launch_colnll<k>(h, d, inv_n, result, small) : launch_nll<k>(h, d, inv_n, result, prob, small); break;
+    CASE(1) CASE(2) CASE(3) CASE(4) CASE(5) CASE(6) CASE(7) CASE(8) CASE(9) CASE(10) CASE(11) CASE(12)
+    CASE(13) CASE(14) CASE(15) CASE(16)
+#undef CASE
+    default: return fail(h, TDDP4_ERR_ARG, "unsupported number of couplings %d", h->M.n_kc);
+  }
+  if (rc) return rc;
+  CU(cudaGetLastError());
+  return TDDP4_OK;
+}
+
+// inspection path: coupling columns of the data set for the current masses/widths, no normalisation needed
+int enqueue_columns_only(tddp4 *h) {
+  EventSet &d = h->set[0];
+  int rc = dispatch_nll(h, d, true, 0.0, h->results + (size_t)N_SLOTS * SLOT_DOUBLES, nullptr, false);
+  if (rc) return rc;
+  d.cols_dirty = false;
+  return TDDP4_OK;
+}
+
+// steps 2..7 for the current parameters; result: device [SLOT_DOUBLES]; prob: device [n] or NULL
 int enqueue_nll(tddp4 *h, double *result, double *prob) {
   if (!h->have_params) return fail(h, TDDP4_ERR_STATE, "tddp4_set_params has not been called");
   EventSet &d = h->set[0];
@@ -328,27 +344,19 @@ int enqueue_nll(tddp4 *h, double *result, double *prob) {
   if (h->use_resolution) return fail(h, TDDP4_ERR_ARG, "use_resolution = 1 is not implemented yet");
   int rc = ensure_gram(h);
   if (rc) return rc;
-  int KC = h->M.n_kc;
   double inv_n = h->gram_n > 0 ? 1.0 / (double)h->gram_n : 0.0;
   // Taylor forms of the four time functions are valid when both mixing phases stay below 1/4 on this sample
   const RateParams &R = h->RP;
   bool small = std::fabs(R.y) * R.Gamma * d.t_max < 0.25 && std::fabs(R.x) * R.Gamma * d.t_max < 0.25;
-  bool fused = !prob && d.dirty_cols != 0 && d.n > 0;
-  if (!fused) {
-    rc = run_columns(h, d);
+  if (d.cols_dirty && d.n > 0) {
+    // columns stale: the fused kernel rebuilds them and finishes the NLL in the same pass; with prob_out a second,
+    // column-reading pass follows (same value bit for bit, plus the per-event probabilities)
+    rc = dispatch_nll(h, d, true, inv_n, result, nullptr, small);
     if (rc) return rc;
+    d.cols_dirty = false;
+    if (!prob) return TDDP4_OK;
   }
-  switch (KC) {
-#define CASE(k) case k: rc = fused ? launch_colnll<k>(h, d, inv_n, result, small) : launch_nll<k>(h, d, inv_n, result, prob, small); break;
-    CASE(1) CASE(2) CASE(3) CASE(4) CASE(5) CASE(6) CASE(7) CASE(8) CASE(9) CASE(10) CASE(11) CASE(12)
-    CASE(13) CASE(14) CASE(15) CASE(16)
-#undef CASE
-    default: return fail(h, TDDP4_ERR_ARG, "unsupported number of couplings %d", KC);
-  }
-  if (rc) return rc;
-  CU(cudaGetLastError());
-  if (fused) d.dirty_cols = 0;
-  return TDDP4_OK;
+  return dispatch_nll(h, d, false, inv_n, result, prob, small);
 }
 
 int enqueue_nll_slot(tddp4 *h, int slot, double *prob) {
@@ -444,11 +452,11 @@ int tddp4_create(const tddp4_model_desc *desc, tddp4 **out) {
     if (ia < 0 || ib < 0) return bail(fail(h, TDDP4_ERR_ARG, "too many lineshape instances"));
     tm.inst0 = (int8_t)ia; tm.inst1 = (int8_t)ib;
   }
-  for (int kap = 0; kap < M.n_kc; ++kap)
-    for (int k = M.col_begin[kap]; k < M.col_begin[kap + 1]; ++k) {
-      if (M.term[k].inst0 >= 0) h->col_of_inst[M.term[k].inst0] |= 1u << kap;
-      if (M.term[k].inst1 >= 0) h->col_of_inst[M.term[k].inst1] |= 1u << kap;
-    }
+  // the s rows some lineshape reads, in system order: these are the rows the per-call kernels stage
+  for (int i = 0; i < MAX_SYS; ++i) M.sys_slot[i] = -1;
+  for (int j = 0; j < M.n_inst; ++j) M.sys_slot[M.inst[j].sys] = 0;
+  for (int i = 0; i < M.n_sys; ++i)
+    if (M.sys_slot[i] == 0) { M.sys_slot[i] = (int8_t)M.n_su; M.su_sys[M.n_su++] = (int8_t)i; }
   h->mass.assign(desc->n_res, 0.0);
   h->width.assign(desc->n_res, 0.0);
 
@@ -464,7 +472,7 @@ int tddp4_create(const tddp4_model_desc *desc, tddp4 **out) {
   int KC = M.n_kc;
   bool ok = cudaMalloc(&h->G, sizeof(double) * 2 * KC * KC) == cudaSuccess &&
             cudaMalloc(&h->ticket, sizeof(unsigned int)) == cudaSuccess &&
-            cudaMalloc(&h->results, sizeof(double) * N_SLOTS * SLOT_DOUBLES) == cudaSuccess &&
+            cudaMalloc(&h->results, sizeof(double) * (N_SLOTS + 1) * SLOT_DOUBLES) == cudaSuccess &&
             cudaMallocHost(&h->results_host, sizeof(double) * N_SLOTS * SLOT_DOUBLES) == cudaSuccess &&
             cudaMalloc(&h->gen_scalars, sizeof(unsigned long long) * 2) == cudaSuccess &&
             cudaMemset(h->ticket, 0, sizeof(unsigned int)) == cudaSuccess &&
@@ -473,7 +481,14 @@ int tddp4_create(const tddp4_model_desc *desc, tddp4 **out) {
   if (!ok) return bail(fail(h, TDDP4_ERR_CUDA, "allocation failed: %s", cudaGetErrorString(cudaGetLastError())));
   // kernels that need more than 48 KB of dynamic shared memory
   cudaFuncSetAttribute(gen_ratio_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gen_smem_bytes(MAX_SYS, MAX_INST));
-  cudaFuncSetAttribute(columns_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(MAX_INST * COL_BLOCK * sizeof(double2)));
+  {   // tile size of the streaming kernels: 256 events unless this model's stages would not fit in shared memory
+    int bpe = 8 * (M.n_su + M.n_inst + M.n_terms + 1), NB = (KC + 3) / 4;
+    size_t limit = prop.sharedMemPerBlockOptin - 1024;
+    auto fits = [&](size_t a, size_t b, size_t c) { return a <= limit && b <= limit && c <= limit; };
+    if (fits(colnll_smem_bytes<256>(bpe, M.n_inst), gram_smem_bytes<256>(NB, bpe, M.n_inst), nll_smem_bytes<256>(KC))) h->tile = 256;
+    else if (fits(colnll_smem_bytes<128>(bpe, M.n_inst), gram_smem_bytes<128>(NB, bpe, M.n_inst), nll_smem_bytes<128>(KC))) h->tile = 128;
+    else return bail(fail(h, TDDP4_ERR_ARG, "model too large for the shared-memory stages of the streaming kernels"));
+  }
   cudaFuncSetAttribute(terms_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(MAX_INST * COL_BLOCK * sizeof(double2)));
   *out = h;
   return TDDP4_OK;
@@ -560,7 +575,7 @@ int tddp4_load_events(tddp4 *h, int which, int64_t n, int64_t ld_in, const doubl
     CU(cudaStreamSynchronize(h->stream));
     if (staging) cudaFree(staging);
   }
-  e.dirty_cols = all_cols(h);
+  e.cols_dirty = true;
   e.loaded = true;
   if (which == 1) { h->gram_valid = false; h->gram_overridden = false; }
   return TDDP4_OK;
@@ -585,10 +600,9 @@ int tddp4_set_params(tddp4 *h, const double *c, const double *cbar, const double
     lp.m0sq[j] = m0 * m0;
     lp.gam[j] = m0 * m0 * g0 / (std::pow(q0, 2 * in.L + 1) * host_barrier2(in.L, z0));
   }
-  uint32_t dirty = 0;
+  bool dirty = !h->have_params;                       // any lineshape constant moved: columns and Gram are stale
   for (int j = 0; j < M.n_inst; ++j)
-    if (!h->have_params || lp.m0sq[j] != h->LP.m0sq[j] || lp.gam[j] != h->LP.gam[j]) dirty |= h->col_of_inst[j];
-  if (!h->have_params) dirty = all_cols(h);
+    if (lp.m0sq[j] != h->LP.m0sq[j] || lp.gam[j] != h->LP.gam[j]) dirty = true;
   h->LP = lp;
   for (int r = 0; r < nres; ++r) { h->mass[r] = mass_width[2 * r]; h->width[r] = mass_width[2 * r + 1]; }
   RateParams &R = h->RP;
@@ -600,8 +614,7 @@ int tddp4_set_params(tddp4 *h, const double *c, const double *cbar, const double
   R.t_lo = h->t_lo; R.t_hi = h->t_hi; R.use_resolution = h->use_resolution;
   time_integrals(x, y, R.Gamma, h->t_lo, h->t_hi, R.T);
   if (dirty) {
-    h->set[0].dirty_cols |= dirty;
-    h->set[1].dirty_cols |= dirty;
+    h->set[0].cols_dirty = true;
     h->gram_valid = false;
     h->gram_overridden = false;
   }
@@ -865,8 +878,10 @@ int tddp4_get(tddp4 *h, int which, int what, double *out) {
     case TDDP4_GET_COLUMNS: {
       if (which != 0) return fail(h, TDDP4_ERR_ARG, "the normalisation sample keeps no coupling columns");
       if (!h->have_params) return fail(h, TDDP4_ERR_STATE, "tddp4_set_params has not been called");
-      int rc = run_columns(h, e);
-      if (rc) return rc;
+      if (e.cols_dirty && e.n > 0) {                   // rebuild through the fused kernel; its NLL goes to a scratch slot
+        int rc = enqueue_columns_only(h);
+        if (rc) return rc;
+      }
       return rows(reinterpret_cast<const double *>(e.a), M.n_kc, sizeof(double2));
     }
     case TDDP4_GET_TERMS: {
