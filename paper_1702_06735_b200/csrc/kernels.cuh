@@ -75,111 +75,6 @@ terms_kernel(const __grid_constant__ ModelTab M, const __grid_constant__ LinePar
 }
 
 // ------------------------------------------------------------------------------------------------
-// steps 4+5+7: amplitude sums (eq. 2), mixing rate (eq. 1), -log reduction.
-// result slot layout (doubles): [0] sum log B, [1] sum t, [2] N, [3] NLL, [4] #bad events
-
-// N from the Gram matrix in force: N = T1 (nAA + nBB) + T2 (nAA - nBB) - 2 T3 Re X - 2 T4 Im X,
-// nAA = c^T G conj(c), nBB likewise for cbar, X = sum_kl c_k conj(cbar_l) G_kl   (O-8, step 6).
-// One (k,l) pair per thread, fixed-order block reduction; every thread of the block must call; valid in thread 0.
-template <int BLOCK>
-__device__ __forceinline__ double norm_from_gram(const RateParams &R, const double *__restrict__ G, int KC,
-                                                 double inv_n, double *red) {
-  double nAA = 0.0, nBB = 0.0, xr = 0.0, xi = 0.0;
-  for (int q = threadIdx.x; q < KC * KC; q += BLOCK) {
-    int k = q / KC, l = q % KC;
-    double gr = __ldcg(G + q * 2) * inv_n, gi = __ldcg(G + q * 2 + 1) * inv_n;
-    double pr = R.c[k][0] * R.c[l][0] + R.c[k][1] * R.c[l][1], pi = R.c[k][1] * R.c[l][0] - R.c[k][0] * R.c[l][1];
-    nAA += pr * gr - pi * gi;
-    pr = R.cbar[k][0] * R.cbar[l][0] + R.cbar[k][1] * R.cbar[l][1];
-    pi = R.cbar[k][1] * R.cbar[l][0] - R.cbar[k][0] * R.cbar[l][1];
-    nBB += pr * gr - pi * gi;
-    pr = R.c[k][0] * R.cbar[l][0] + R.c[k][1] * R.cbar[l][1];
-    pi = R.c[k][1] * R.cbar[l][0] - R.c[k][0] * R.cbar[l][1];
-    xr += pr * gr - pi * gi;
-    xi += pr * gi + pi * gr;
-  }
-  nAA = block_sum<BLOCK>(nAA, red);
-  nBB = block_sum<BLOCK>(nBB, red);
-  xr = block_sum<BLOCK>(xr, red);
-  xi = block_sum<BLOCK>(xi, red);
-  return R.T[0] * (nAA + nBB) + R.T[1] * (nAA - nBB) - 2.0 * R.T[2] * xr - 2.0 * R.T[3] * xi;
-}
-
-// sum_i log B_i without a log per event: B = m 2^e with m in [1,2); the mantissas are multiplied up, the exponents
-// added as integers, and one log is taken per thread at the end:  sum log B = log(prod m) + ln2 * sum e.
-struct LogAcc {
-  double prod = 1.0;
-  long long esum = 0;
-  int bad = 0, since = 0;
-  __device__ __forceinline__ void add(double B) {
-    long long bits = __double_as_longlong(B);
-    int e = (int)((bits >> 52) & 0x7ff);
-    if (bits <= 0 || e == 0x7ff) { ++bad; return; }              // B <= 0 (sign bit or zero), inf, nan
-    if (e == 0) {                                                 // subnormal: rescale first
-      bits = __double_as_longlong(B * 0x1.0p64);
-      e = (int)((bits >> 52) & 0x7ff) - 64;
-    }
-    esum += e - 1023;
-    prod *= __longlong_as_double((bits & 0x000fffffffffffffLL) | 0x3ff0000000000000LL);
-    if (++since == 512) renorm();
-  }
-  __device__ __forceinline__ void renorm() {
-    long long bits = __double_as_longlong(prod);
-    esum += (int)((bits >> 52) & 0x7ff) - 1023;
-    prod = __longlong_as_double((bits & 0x000fffffffffffffLL) | 0x3ff0000000000000LL);
-    since = 0;
-  }
-  __device__ __forceinline__ double value() const { return log(prod) + 0.693147180559945309417 * (double)esum; }
-};
-
-// A, Abar from the K_c columns of one event (eq. 2)
-template <int KC>
-__device__ __forceinline__ void amplitude_sums(const RateParams &R, const double2 v[KC], double2 &A, double2 &Ab) {
-  A = make_double2(0.0, 0.0);
-  Ab = make_double2(0.0, 0.0);
-#pragma unroll
-  for (int k = 0; k < KC; ++k) {
-    A.x += R.c[k][0] * v[k].x - R.c[k][1] * v[k].y;
-    A.y += R.c[k][0] * v[k].y + R.c[k][1] * v[k].x;
-    Ab.x += R.cbar[k][0] * v[k].x - R.cbar[k][1] * v[k].y;
-    Ab.y += R.cbar[k][0] * v[k].y + R.cbar[k][1] * v[k].x;
-  }
-}
-
-// common tail of the two NLL kernels: block partials, last block adds them in index order and finishes the NLL
-template <int BLOCK>
-__device__ __forceinline__ void nll_finish(const RateParams &R, int64_t n, double sum_t, double acc, double bad,
-                                           double norm_block0, double *__restrict__ partials, unsigned int *ticket,
-                                           double *__restrict__ result, double *red, bool *last) {
-  double r = block_sum<BLOCK>(acc, red);
-  double rb = block_sum<BLOCK>(bad, red);
-  if (threadIdx.x == 0) {
-    partials[2 * blockIdx.x] = r;
-    partials[2 * blockIdx.x + 1] = rb;
-    if (blockIdx.x == 0) partials[2 * gridDim.x] = norm_block0;
-  }
-  __threadfence();
-  if (threadIdx.x == 0) *last = atomicAdd(ticket, 1u) == gridDim.x - 1;
-  __syncthreads();
-  if (!*last) return;
-  __threadfence();
-  double s0 = 0.0, s1 = 0.0;
-  for (unsigned b = threadIdx.x; b < gridDim.x; b += BLOCK) {
-    s0 += __ldcg(partials + 2 * b);
-    s1 += __ldcg(partials + 2 * b + 1);
-  }
-  s0 = block_sum<BLOCK>(s0, red);
-  s1 = block_sum<BLOCK>(s1, red);
-  if (threadIdx.x == 0) {
-    double norm = __ldcg(partials + 2 * gridDim.x);
-    // -sum log(e^{-Gamma t} B / N) = Gamma sum t - sum log B + n log N
-    double nll = R.Gamma * sum_t - s0 + (double)n * log(norm);
-    if (s1 > 0.0 || !(norm > 0.0)) nll = INFINITY;
-    result[0] = s0; result[1] = sum_t; result[2] = norm; result[3] = nll; result[4] = s1;
-    *ticket = 0;
-  }
-}
-
 // deterministic sum and max |.| of a vector (decay times at load): one block, fixed order
 __global__ void __launch_bounds__(1024) stat_kernel(const double *__restrict__ v, int64_t n, double *out /* [2] */) {
   __shared__ double red[32];

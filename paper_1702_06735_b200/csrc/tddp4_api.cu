@@ -81,7 +81,6 @@ struct tddp4 {
   int64_t prof_n[TDDP4_K_COUNT] = {0};
   int64_t launches = 0;
   int sm_count = 148;
-  int tile = 256;                    // events per tile of the streaming kernels (128 for very large models)
   std::string err;
 };
 
@@ -201,53 +200,23 @@ void free_set(EventSet &e) {
   e = EventSet{};
 }
 
-// rows of one tile for the kernels that start from the step-1 caches: s rows in use, g rows, f rows [, extra]
-RowList static_rows(const tddp4 *h, const EventSet &e, const double *extra) {
-  const ModelTab &M = h->M;
-  RowList r{};
-  r.arr[0] = reinterpret_cast<const char *>(e.s);
-  r.arr[1] = reinterpret_cast<const char *>(e.g);
-  r.arr[2] = reinterpret_cast<const char *>(e.f);
-  r.arr[3] = reinterpret_cast<const char *>(extra);
-  for (int i = 0; i < M.n_su; ++i) r.add(0, M.su_sys[i], 8);
-  for (int j = 0; j < M.n_inst; ++j) r.add(1, j, 8);
-  for (int k = 0; k < M.n_terms; ++k) r.add(2, k, 8);
-  if (extra) r.add(3, 0, 8);
-  return r;
-}
-// rows of one tile for the coupling-only kernel: K_c columns (16-byte elements), then t
-RowList column_rows(const tddp4 *h, const EventSet &e) {
-  RowList r{};
-  r.arr[0] = reinterpret_cast<const char *>(e.a);
-  r.arr[1] = reinterpret_cast<const char *>(e.t);
-  for (int k = 0; k < h->M.n_kc; ++k) r.add(0, k, 16);
-  r.add(1, 0, 8);
-  return r;
+int stream_grid(const tddp4 *h, int64_t n) {
+  return (int)std::max<int64_t>(1, std::min<int64_t>((n + STREAM_BLOCK - 1) / STREAM_BLOCK,
+                                                     (int64_t)h->sm_count * STREAM_BLOCKS_PER_SM));
 }
 
-int stream_grid(const tddp4 *h, int64_t n, int tile) {
-  return (int)std::max<int64_t>(1, std::min<int64_t>((n + tile - 1) / tile, (int64_t)h->sm_count));
-}
+// algorithmic bytes per event of the step-1 caches a dirty call has to read: s rows in use, g rows, f rows
+double static_bytes_per_event(const tddp4 *h) { return 8.0 * (h->M.n_su + h->M.n_inst + h->M.n_terms); }
 
-template <class K>
-int set_smem(tddp4 *h, K kernel, size_t bytes) {
-  CU(cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
-  return TDDP4_OK;
-}
-
-template <int NB, int TILE>
+template <int NB>
 int launch_gram(tddp4 *h, const EventSet &e) {
   const ModelTab &M = h->M;
-  RowList rows = static_rows(h, e, e.w);
-  size_t smem = gram_smem_bytes<TILE>(NB, rows.bytes_per_event, M.n_inst);
-  int rc = set_smem(h, gram_stream_kernel<NB, TILE>, smem);
+  int grid = stream_grid(h, e.n);
+  int rc = ensure_partials(h, (size_t)grid * 64 * NB * NB + 16);
   if (rc) return rc;
-  int grid = stream_grid(h, e.n, TILE);
-  rc = ensure_partials(h, (size_t)grid * 64 * NB * NB + 16);
-  if (rc) return rc;
-  Prof p(h, TDDP4_K_GRAM, (double)e.n * rows.bytes_per_event);
-  gram_stream_kernel<NB, TILE><<<grid, TILE, smem, h->stream>>>(M, h->LP, rows, e.ld, e.n, e.w ? 1 : 0, h->partials,
-                                                                h->ticket, h->G);
+  Prof p(h, TDDP4_K_GRAM, (double)e.n * (static_bytes_per_event(h) + (e.w ? 8.0 : 0.0)));
+  gram_stream_kernel<NB><<<grid, STREAM_BLOCK, gram_smem_bytes(NB, M.n_inst), h->stream>>>(M, h->LP, e.s, e.g, e.f, e.w, e.ld, e.n,
+                                                                                      h->partials, h->ticket, h->G);
   return TDDP4_OK;
 }
 
@@ -257,11 +226,10 @@ int ensure_gram(tddp4 *h) {
   EventSet &e = h->set[1];
   if (!e.loaded) return fail(h, TDDP4_ERR_STATE, "normalisation sample not loaded");
   int KC = h->M.n_kc, rc;
-  bool big = h->tile == 256;
-  if (KC <= 4) rc = big ? launch_gram<1, 256>(h, e) : launch_gram<1, 128>(h, e);
-  else if (KC <= 8) rc = big ? launch_gram<2, 256>(h, e) : launch_gram<2, 128>(h, e);
-  else if (KC <= 12) rc = big ? launch_gram<3, 256>(h, e) : launch_gram<3, 128>(h, e);
-  else rc = big ? launch_gram<4, 256>(h, e) : launch_gram<4, 128>(h, e);
+  if (KC <= 4) rc = launch_gram<1>(h, e);
+  else if (KC <= 8) rc = launch_gram<2>(h, e);
+  else if (KC <= 12) rc = launch_gram<3>(h, e);
+  else rc = launch_gram<4>(h, e);
   if (rc) return rc;
   CU(cudaGetLastError());
   h->gram_valid = true;
@@ -270,57 +238,49 @@ int ensure_gram(tddp4 *h) {
   return TDDP4_OK;
 }
 
-template <int KC, bool PROB, bool SMALL, int TILE>
-int launch_nll_t(tddp4 *h, const EventSet &e, double inv_n, double *result, double *prob) {
-  RowList rows = column_rows(h, e);
-  size_t smem = nll_smem_bytes<TILE>(KC);
-  int rc = set_smem(h, nll_stream_kernel<KC, PROB, SMALL, TILE>, smem);
-  if (rc) return rc;
-  int grid = stream_grid(h, e.n, TILE);
-  rc = ensure_partials(h, (size_t)2 * grid + 16);
-  if (rc) return rc;
-  Prof p(h, TDDP4_K_NLL, (double)e.n * (rows.bytes_per_event + (PROB ? 8.0 : 0.0)));
-  nll_stream_kernel<KC, PROB, SMALL, TILE><<<grid, TILE, smem, h->stream>>>(rows, e.ld, e.n, h->RP, h->G, inv_n, e.sum_t,
-                                                                            h->partials, h->ticket, result, prob);
-  return TDDP4_OK;
-}
 template <int KC>
-int launch_nll(tddp4 *h, const EventSet &e, double inv_n, double *result, double *prob, bool small) {
-#define GO(P, S) (h->tile == 256 ? launch_nll_t<KC, P, S, 256>(h, e, inv_n, result, prob) : launch_nll_t<KC, P, S, 128>(h, e, inv_n, result, prob))
-  if (prob) return small ? GO(true, true) : GO(true, false);
-  return small ? GO(false, true) : GO(false, false);
-#undef GO
+int launch_nll(tddp4 *h, const EventSet &e, double inv_n, double *result, bool small) {
+  int grid = stream_grid(h, e.n);
+  int rc = ensure_partials(h, (size_t)3 * grid + 16);
+  if (rc) return rc;
+  Prof p(h, TDDP4_K_NLL, (double)e.n * (16.0 * KC + 8.0));
+  if (small)
+    nll_stream_kernel<KC, true><<<grid, STREAM_BLOCK, 0, h->stream>>>(e.a, e.t, e.ld, e.n, h->RP, h->G, inv_n, e.sum_t, h->partials,
+                                                                     h->ticket, result);
+  else
+    nll_stream_kernel<KC, false><<<grid, STREAM_BLOCK, 0, h->stream>>>(e.a, e.t, e.ld, e.n, h->RP, h->G, inv_n, e.sum_t, h->partials,
+                                                                      h->ticket, result);
+  return TDDP4_OK;
 }
 
-template <int KC, bool SMALL, int TILE>
-int launch_colnll_t(tddp4 *h, const EventSet &e, double inv_n, double *result) {
-  const ModelTab &M = h->M;
-  RowList rows = static_rows(h, e, e.t);
-  size_t smem = colnll_smem_bytes<TILE>(rows.bytes_per_event, M.n_inst);
-  int rc = set_smem(h, colnll_stream_kernel<KC, SMALL, TILE>, smem);
-  if (rc) return rc;
-  int grid = stream_grid(h, e.n, TILE);
-  rc = ensure_partials(h, (size_t)2 * grid + 16);
-  if (rc) return rc;
-  Prof p(h, TDDP4_K_COLNLL, (double)e.n * (rows.bytes_per_event + 16.0 * KC));
-  colnll_stream_kernel<KC, SMALL, TILE><<<grid, TILE, smem, h->stream>>>(M, h->LP, rows, e.ld, e.n, e.a, h->RP, h->G, inv_n,
-                                                                         e.sum_t, h->partials, h->ticket, result);
-  return TDDP4_OK;
-}
-template <int KC>
 int launch_colnll(tddp4 *h, const EventSet &e, double inv_n, double *result, bool small) {
-  if (h->tile == 256) return small ? launch_colnll_t<KC, true, 256>(h, e, inv_n, result) : launch_colnll_t<KC, false, 256>(h, e, inv_n, result);
-  return small ? launch_colnll_t<KC, true, 128>(h, e, inv_n, result) : launch_colnll_t<KC, false, 128>(h, e, inv_n, result);
+  const ModelTab &M = h->M;
+  int grid = stream_grid(h, e.n);
+  int rc = ensure_partials(h, (size_t)3 * grid + 16);
+  if (rc) return rc;
+  size_t smem = colnll_smem_bytes(M.n_inst);
+  Prof p(h, TDDP4_K_COLNLL, (double)e.n * (static_bytes_per_event(h) + 8.0 + 16.0 * M.n_kc));
+  if (small)
+    colnll_stream_kernel<true><<<grid, STREAM_BLOCK, smem, h->stream>>>(M, h->LP, e.s, e.g, e.f, e.t, e.ld, e.n, e.a, h->RP, h->G,
+                                                                       inv_n, e.sum_t, h->partials, h->ticket, result);
+  else
+    colnll_stream_kernel<false><<<grid, STREAM_BLOCK, smem, h->stream>>>(M, h->LP, e.s, e.g, e.f, e.t, e.ld, e.n, e.a, h->RP, h->G,
+                                                                        inv_n, e.sum_t, h->partials, h->ticket, result);
+  return TDDP4_OK;
 }
 
-int dispatch_nll(tddp4 *h, EventSet &d, bool fused, double inv_n, double *result, double *prob, bool small) {
+int dispatch_nll(tddp4 *h, EventSet &d, bool fused, double inv_n, double *result, bool small) {
   int rc;
-  switch (h->M.n_kc) {
-#define CASE(k) case k: rc = fused ? launch_colnll<k>(h, d, inv_n, result, small) : launch_nll<k>(h, d, inv_n, result, prob, small); break;
-    CASE(1) CASE(2) CASE(3) CASE(4) CASE(5) CASE(6) CASE(7) CASE(8) CASE(9) CASE(10) CASE(11) CASE(12)
-    CASE(13) CASE(14) CASE(15) CASE(16)
+  if (fused) {
+    rc = launch_colnll(h, d, inv_n, result, small);
+  } else {
+    switch (h->M.n_kc) {
+#define CASE(k) case k: rc = launch_nll<k>(h, d, inv_n, result, small); break;
+      CASE(1) CASE(2) CASE(3) CASE(4) CASE(5) CASE(6) CASE(7) CASE(8) CASE(9) CASE(10) CASE(11) CASE(12)
+      CASE(13) CASE(14) CASE(15) CASE(16)
 #undef CASE
-    default: return fail(h, TDDP4_ERR_ARG, "unsupported number of couplings %d", h->M.n_kc);
+      default: return fail(h, TDDP4_ERR_ARG, "unsupported number of couplings %d", h->M.n_kc);
+    }
   }
   if (rc) return rc;
   CU(cudaGetLastError());
@@ -330,7 +290,7 @@ int dispatch_nll(tddp4 *h, EventSet &d, bool fused, double inv_n, double *result
 // inspection path: coupling columns of the data set for the current masses/widths, no normalisation needed
 int enqueue_columns_only(tddp4 *h) {
   EventSet &d = h->set[0];
-  int rc = dispatch_nll(h, d, true, 0.0, h->results + (size_t)N_SLOTS * SLOT_DOUBLES, nullptr, false);
+  int rc = dispatch_nll(h, d, true, 0.0, h->results + (size_t)N_SLOTS * SLOT_DOUBLES, false);
   if (rc) return rc;
   d.cols_dirty = false;
   return TDDP4_OK;
@@ -349,14 +309,22 @@ int enqueue_nll(tddp4 *h, double *result, double *prob) {
   const RateParams &R = h->RP;
   bool small = std::fabs(R.y) * R.Gamma * d.t_max < 0.25 && std::fabs(R.x) * R.Gamma * d.t_max < 0.25;
   if (d.cols_dirty && d.n > 0) {
-    // columns stale: the fused kernel rebuilds them and finishes the NLL in the same pass; with prob_out a second,
-    // column-reading pass follows (same value bit for bit, plus the per-event probabilities)
-    rc = dispatch_nll(h, d, true, inv_n, result, nullptr, small);
+    // columns stale: the fused kernel rebuilds them and finishes the NLL in the same pass
+    rc = dispatch_nll(h, d, true, inv_n, result, small);
     if (rc) return rc;
     d.cols_dirty = false;
-    if (!prob) return TDDP4_OK;
+  } else {
+    rc = dispatch_nll(h, d, false, inv_n, result, small);
+    if (rc) return rc;
   }
-  return dispatch_nll(h, d, false, inv_n, result, prob, small);
+  if (prob && d.n > 0) {   // per-event probabilities from the columns and the N the NLL kernel has just written
+    int grid = (int)((d.n + STREAM_BLOCK - 1) / STREAM_BLOCK);
+    ++h->launches;
+    if (small) prob_kernel<true><<<grid, STREAM_BLOCK, 0, h->stream>>>(d.a, d.t, d.ld, d.n, h->M.n_kc, h->RP, result, prob);
+    else prob_kernel<false><<<grid, STREAM_BLOCK, 0, h->stream>>>(d.a, d.t, d.ld, d.n, h->M.n_kc, h->RP, result, prob);
+    CU(cudaGetLastError());
+  }
+  return TDDP4_OK;
 }
 
 int enqueue_nll_slot(tddp4 *h, int slot, double *prob) {
@@ -481,13 +449,16 @@ int tddp4_create(const tddp4_model_desc *desc, tddp4 **out) {
   if (!ok) return bail(fail(h, TDDP4_ERR_CUDA, "allocation failed: %s", cudaGetErrorString(cudaGetLastError())));
   // kernels that need more than 48 KB of dynamic shared memory
   cudaFuncSetAttribute(gen_ratio_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gen_smem_bytes(MAX_SYS, MAX_INST));
-  {   // tile size of the streaming kernels: 256 events unless this model's stages would not fit in shared memory
-    int bpe = 8 * (M.n_su + M.n_inst + M.n_terms + 1), NB = (KC + 3) / 4;
-    size_t limit = prop.sharedMemPerBlockOptin - 1024;
-    auto fits = [&](size_t a, size_t b, size_t c) { return a <= limit && b <= limit && c <= limit; };
-    if (fits(colnll_smem_bytes<256>(bpe, M.n_inst), gram_smem_bytes<256>(NB, bpe, M.n_inst), nll_smem_bytes<256>(KC))) h->tile = 256;
-    else if (fits(colnll_smem_bytes<128>(bpe, M.n_inst), gram_smem_bytes<128>(NB, bpe, M.n_inst), nll_smem_bytes<128>(KC))) h->tile = 128;
-    else return bail(fail(h, TDDP4_ERR_ARG, "model too large for the shared-memory stages of the streaming kernels"));
+  {   // shared memory of the per-call kernels: per-warp lineshape scratch (+ the X tile of the Gram kernel)
+    int NB = (KC + 3) / 4;
+    size_t limit = prop.sharedMemPerBlockOptin - 1024, sc = colnll_smem_bytes(M.n_inst), sg = gram_smem_bytes(NB, M.n_inst);
+    if (sc > limit || sg > limit) return bail(fail(h, TDDP4_ERR_ARG, "model too large for the shared-memory scratch of the streaming kernels"));
+    cudaFuncSetAttribute(colnll_stream_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sc);
+    cudaFuncSetAttribute(colnll_stream_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sc);
+    if (NB == 1) cudaFuncSetAttribute(gram_stream_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sg);
+    else if (NB == 2) cudaFuncSetAttribute(gram_stream_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sg);
+    else if (NB == 3) cudaFuncSetAttribute(gram_stream_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sg);
+    else cudaFuncSetAttribute(gram_stream_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sg);
   }
   cudaFuncSetAttribute(terms_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(MAX_INST * COL_BLOCK * sizeof(double2)));
   *out = h;
