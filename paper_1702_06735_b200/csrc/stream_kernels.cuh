@@ -219,58 +219,58 @@ prob_kernel(const double2 *__restrict__ a, const double *__restrict__ t, int64_t
 }
 
 // ------------------------------------------------------------------------------------------------
-// steps 2+3 of ONE event from the step-1 caches in global memory.
-// Lineshapes: T_R of every de-duplicated instance goes to the thread's own slots sT[instance * 32 + lane] of
-// its warp's scratch (chains index it through the model tables, so it cannot live in registers).  Loads are issued
-// in batches of 4 instances (8 loads in flight); the s rows are shared by several instances and stay in L1.
-__device__ __forceinline__ void lineshapes_to_scratch(const ModelTab &M, const LineParams &LP, const double *__restrict__ s,
-                                                      const double *__restrict__ g, int64_t ld, int64_t i,
-                                                      double2 *sT, int lane) {
-  for (int j0 = 0; j0 < M.n_inst; j0 += 4) {
-    double sv[4], gv[4];
+// steps 2+3 of ONE event from the step-1 caches in global memory.  Both loops are unrolled to the table maxima with
+// warp-uniform guards, so every table entry and lineshape constant is an immediate-indexed constant-bank operand.
+// Lineshapes: T_R of every de-duplicated instance goes to the thread's own slots sTl[instance * 32] of its
+// warp's scratch (chains index it through the model tables, so it cannot live in registers).  Loads are issued in
+// batches of 8 instances (16 loads in flight); the s rows are shared by several instances and stay in L1.
+// s_i, g_i, f_i: the row-0 addresses of this thread's event.
+__device__ __forceinline__ void lineshapes_to_scratch(const StreamTab &S, const LineParams &LP, const double *__restrict__ s_i,
+                                                      const double *__restrict__ g_i, int64_t ld, double2 *sTl) {
 #pragma unroll
-    for (int u = 0; u < 4; ++u)
-      if (j0 + u < M.n_inst) {
-        sv[u] = __ldg(s + (int64_t)M.inst[j0 + u].sys * ld + i);
-        gv[u] = ldg_stream1(g + (int64_t)(j0 + u) * ld + i);
-      }
+  for (int j0 = 0; j0 < MAX_INST; j0 += 8) {
+    if (j0 < S.n_inst) {
+      double sv[8], gv[8];
 #pragma unroll
-    for (int u = 0; u < 4; ++u)
-      if (j0 + u < M.n_inst) sT[(j0 + u) * 32 + lane] = breit_wigner(LP.m0sq[j0 + u], LP.gam[j0 + u], sv[u], gv[u]);
+      for (int u = 0; u < 8; ++u)
+        if (j0 + u < S.n_inst) {
+          sv[u] = __ldg(s_i + S.inst_srow[j0 + u] * ld);
+          gv[u] = ldg_stream1(g_i + (j0 + u) * ld);
+        }
+#pragma unroll
+      for (int u = 0; u < 8; ++u)
+        if (j0 + u < S.n_inst) sTl[(j0 + u) * 32] = breit_wigner(LP.m0sq[j0 + u], LP.gam[j0 + u], sv[u], gv[u]);
+    }
   }
 }
 // Component products summed into coupling columns: a_kappa = sum_{k in kappa} f_k T_{R1(k)} T_{R2(k)} (terms are sorted
-// by coupling).  flush(kappa, a_kappa) is called once per column, kappa = 0 .. K_c-1 in order.  8 f loads in flight.
+// by coupling).  flush(kappa, a_kappa) is called once per non-empty column, in order.  8 f loads in flight.
 template <class Flush>
-__device__ __forceinline__ void columns_from_scratch(const ModelTab &M, const double *__restrict__ f, int64_t ld, int64_t i,
-                                                     const double2 *sT, int lane, Flush &&flush) {
+__device__ __forceinline__ void columns_from_scratch(const StreamTab &S, const double *__restrict__ f_i, int64_t ld,
+                                                     const double2 *sTl, Flush &&flush) {
   double2 acc = make_double2(0.0, 0.0);
-  int kap = 0;
-  for (int k0 = 0; k0 < M.n_terms; k0 += 8) {
-    double fv[8];
 #pragma unroll
-    for (int u = 0; u < 8; ++u)
-      if (k0 + u < M.n_terms) fv[u] = ldg_stream1(f + (int64_t)(k0 + u) * ld + i);
+  for (int k0 = 0; k0 < MAX_TERMS; k0 += 8) {
+    if (k0 < S.n_terms) {
+      double fv[8];
 #pragma unroll
-    for (int u = 0; u < 8; ++u) {
-      const int k = k0 + u;
-      if (k < M.n_terms) {
-        while (k >= M.col_begin[kap + 1]) {
-          flush(kap, acc);
-          acc = make_double2(0.0, 0.0);
-          ++kap;
+      for (int u = 0; u < 8; ++u)
+        if (k0 + u < S.n_terms) fv[u] = ldg_stream1(f_i + (k0 + u) * ld);
+#pragma unroll
+      for (int u = 0; u < 8; ++u) {
+        const int k = k0 + u;
+        if (k < S.n_terms) {
+          double2 T = make_double2(1.0, 0.0);
+          if (S.term_t0[k] != 0xFFFF) T = cmul(sTl[S.term_t0[k]], sTl[S.term_t1[k]]);
+          acc.x = fma(fv[u], T.x, acc.x);
+          acc.y = fma(fv[u], T.y, acc.y);
+          if (S.term_last[k]) {
+            flush((int)S.term_col[k], acc);
+            acc = make_double2(0.0, 0.0);
+          }
         }
-        const TermTab &tm = M.term[k];
-        double2 T = make_double2(1.0, 0.0);
-        if (tm.inst0 >= 0) T = cmul(sT[tm.inst0 * 32 + lane], sT[tm.inst1 * 32 + lane]);
-        acc.x = fma(fv[u], T.x, acc.x);
-        acc.y = fma(fv[u], T.y, acc.y);
       }
     }
-  }
-  for (; kap < M.n_kc; ++kap) {
-    flush(kap, acc);
-    acc = make_double2(0.0, 0.0);
   }
 }
 __host__ __device__ inline size_t lineshape_scratch_bytes(int n_inst) { return (size_t)(n_inst > 0 ? n_inst : 1) * 32 * sizeof(double2); }
@@ -282,29 +282,29 @@ inline size_t colnll_smem_bytes(int n_inst) { return STREAM_WARPS * lineshape_sc
 
 template <bool SMALL>
 __global__ void __launch_bounds__(STREAM_BLOCK, STREAM_BLOCKS_PER_SM)
-colnll_stream_kernel(const __grid_constant__ ModelTab M, const __grid_constant__ LineParams LP,
+colnll_stream_kernel(const __grid_constant__ StreamTab S, const __grid_constant__ LineParams LP,
                      const double *__restrict__ s, const double *__restrict__ g, const double *__restrict__ f,
                      const double *__restrict__ t, int64_t ld, int64_t n, double2 *__restrict__ a,
                      const __grid_constant__ RateParams R, const double *__restrict__ G, double inv_n_norm, double sum_t,
                      double *__restrict__ partials, unsigned int *ticket, double *__restrict__ result) {
   extern __shared__ __align__(16) char smem_raw[];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  double2 *sT = reinterpret_cast<double2 *>(smem_raw + (size_t)warp * lineshape_scratch_bytes(M.n_inst));
+  double2 *sTl = reinterpret_cast<double2 *>(smem_raw + (size_t)warp * lineshape_scratch_bytes(S.n_inst)) + lane;
   MantAcc la;
   const double yG = R.y * R.Gamma, xG = R.x * R.Gamma;
   const int64_t stride = (int64_t)gridDim.x * STREAM_BLOCK;
 #pragma unroll 1
   for (int64_t i = (int64_t)blockIdx.x * STREAM_BLOCK + threadIdx.x; i < n; i += stride) {
     double ti = ldg_stream1(t + i);
-    lineshapes_to_scratch(M, LP, s, g, ld, i, sT, lane);
+    lineshapes_to_scratch(S, LP, s + i, g + i, ld, sTl);
     double2 A = make_double2(0.0, 0.0), Ab = make_double2(0.0, 0.0);
-    columns_from_scratch(M, f, ld, i, sT, lane, [&](int kap, double2 col) {
+    columns_from_scratch(S, f + i, ld, sTl, [&](int kap, double2 col) {
       a[(int64_t)kap * ld + i] = col;
       amp_add(A, Ab, R.c[kap][0], R.c[kap][1], R.cbar[kap][0], R.cbar[kap][1], col);
     });
     la.add(bracket<SMALL>(A, Ab, yG * ti, xG * ti));
   }
-  nll_finish(R, M.n_kc, n, sum_t, la, G, inv_n_norm, partials, ticket, result);
+  nll_finish(R, S.n_kc, n, sum_t, la, G, inv_n_norm, partials, ticket, result);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -333,7 +333,7 @@ __device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double
 
 template <int NB>
 __global__ void __launch_bounds__(STREAM_BLOCK, STREAM_BLOCKS_PER_SM)
-gram_stream_kernel(const __grid_constant__ ModelTab M, const __grid_constant__ LineParams LP,
+gram_stream_kernel(const __grid_constant__ StreamTab S, const __grid_constant__ LineParams LP,
                    const double *__restrict__ s, const double *__restrict__ g, const double *__restrict__ f,
                    const double *__restrict__ w /* or NULL */, int64_t ld, int64_t n,
                    double *__restrict__ partials /* [grid][64 NB NB] */, unsigned int *ticket,
@@ -342,11 +342,11 @@ gram_stream_kernel(const __grid_constant__ ModelTab M, const __grid_constant__ L
   extern __shared__ __align__(16) char smem_raw[];
   __shared__ bool last;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int KC = M.n_kc;
-  const size_t t_bytes = align_up(lineshape_scratch_bytes(M.n_inst), 128);
+  const int KC = S.n_kc;
+  const size_t t_bytes = align_up(lineshape_scratch_bytes(S.n_inst), 128);
   const size_t x_bytes = align_up((size_t)32 * STRIDE * sizeof(double), 128);
   char *scratch = smem_raw + (size_t)warp * (t_bytes + x_bytes);
-  double2 *sT = reinterpret_cast<double2 *>(scratch);          // [n_inst][32]
+  double2 *sTl = reinterpret_cast<double2 *>(scratch) + lane;  // [n_inst][32], this lane's slots
   double *Xs = reinterpret_cast<double *>(scratch + t_bytes);  // [32][STRIDE]: row = event, F features + weight
   double *row = Xs + lane * STRIDE;
 #pragma unroll
@@ -361,8 +361,8 @@ gram_stream_kernel(const __grid_constant__ ModelTab M, const __grid_constant__ L
     const int64_t i = i0 + lane;
     if (i < n) {
       double wj = w ? ldg_stream1(w + i) : 1.0;
-      lineshapes_to_scratch(M, LP, s, g, ld, i, sT, lane);
-      columns_from_scratch(M, f, ld, i, sT, lane, [&](int kap, double2 col) { *reinterpret_cast<double2 *>(row + 2 * kap) = col; });
+      lineshapes_to_scratch(S, LP, s + i, g + i, ld, sTl);
+      columns_from_scratch(S, f + i, ld, sTl, [&](int kap, double2 col) { *reinterpret_cast<double2 *>(row + 2 * kap) = col; });
       row[F] = wj;
     } else {
       for (int c = 0; c < 2 * KC; ++c) row[c] = 0.0;

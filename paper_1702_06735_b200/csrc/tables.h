@@ -47,6 +47,15 @@ struct ModelTab {
   double r_res2, r_parent2;        // radii squared, GeV^-2
 };
 
+struct StreamTab {                 // the per-call kernels' view of the model: flat, indexable with immediates
+  int n_inst, n_terms, n_kc;
+  uint8_t inst_srow[MAX_INST];     // s row (system index) of lineshape instance j
+  uint16_t term_t0[MAX_TERMS];     // element offset (instance * 32) of T_R1 in the warp's lineshape scratch; 0xFFFF: none
+  uint16_t term_t1[MAX_TERMS];     // ... of T_R2
+  uint8_t term_col[MAX_TERMS];     // coupling column of term k (terms are sorted by coupling)
+  uint8_t term_last[MAX_TERMS];    // 1: term k closes its column
+};
+
 struct LineParams {                // per set_params: T = 1 / (m0sq - s - i gam g(s)),  O-6
   double m0sq[MAX_INST];
   double gam[MAX_INST];            // m0^2 Gamma0 / (q0^(2L+1) F_L(z0)^2)

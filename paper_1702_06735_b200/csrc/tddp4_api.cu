@@ -42,6 +42,7 @@ struct tddp4 {
   cudaStream_t stream = nullptr;
   bool own_stream = false;
   ModelTab M{};
+  StreamTab S{};                     // the same model, flattened for the per-call kernels
   std::vector<tddp4_res> res;
   std::vector<tddp4_term> terms;   // caller's order
   double t_lo = 0.0, t_hi = INFINITY;
@@ -215,7 +216,7 @@ int launch_gram(tddp4 *h, const EventSet &e) {
   int rc = ensure_partials(h, (size_t)grid * 64 * NB * NB + 16);
   if (rc) return rc;
   Prof p(h, TDDP4_K_GRAM, (double)e.n * (static_bytes_per_event(h) + (e.w ? 8.0 : 0.0)));
-  gram_stream_kernel<NB><<<grid, STREAM_BLOCK, gram_smem_bytes(NB, M.n_inst), h->stream>>>(M, h->LP, e.s, e.g, e.f, e.w, e.ld, e.n,
+  gram_stream_kernel<NB><<<grid, STREAM_BLOCK, gram_smem_bytes(NB, M.n_inst), h->stream>>>(h->S, h->LP, e.s, e.g, e.f, e.w, e.ld, e.n,
                                                                                       h->partials, h->ticket, h->G);
   return TDDP4_OK;
 }
@@ -261,10 +262,10 @@ int launch_colnll(tddp4 *h, const EventSet &e, double inv_n, double *result, boo
   size_t smem = colnll_smem_bytes(M.n_inst);
   Prof p(h, TDDP4_K_COLNLL, (double)e.n * (static_bytes_per_event(h) + 8.0 + 16.0 * M.n_kc));
   if (small)
-    colnll_stream_kernel<true><<<grid, STREAM_BLOCK, smem, h->stream>>>(M, h->LP, e.s, e.g, e.f, e.t, e.ld, e.n, e.a, h->RP, h->G,
+    colnll_stream_kernel<true><<<grid, STREAM_BLOCK, smem, h->stream>>>(h->S, h->LP, e.s, e.g, e.f, e.t, e.ld, e.n, e.a, h->RP, h->G,
                                                                        inv_n, e.sum_t, h->partials, h->ticket, result);
   else
-    colnll_stream_kernel<false><<<grid, STREAM_BLOCK, smem, h->stream>>>(M, h->LP, e.s, e.g, e.f, e.t, e.ld, e.n, e.a, h->RP, h->G,
+    colnll_stream_kernel<false><<<grid, STREAM_BLOCK, smem, h->stream>>>(h->S, h->LP, e.s, e.g, e.f, e.t, e.ld, e.n, e.a, h->RP, h->G,
                                                                         inv_n, e.sum_t, h->partials, h->ticket, result);
   return TDDP4_OK;
 }
@@ -425,6 +426,20 @@ int tddp4_create(const tddp4_model_desc *desc, tddp4 **out) {
   for (int j = 0; j < M.n_inst; ++j) M.sys_slot[M.inst[j].sys] = 0;
   for (int i = 0; i < M.n_sys; ++i)
     if (M.sys_slot[i] == 0) { M.sys_slot[i] = (int8_t)M.n_su; M.su_sys[M.n_su++] = (int8_t)i; }
+  {   // flat tables of the per-call kernels
+    StreamTab &S = h->S;
+    memset(&S, 0, sizeof S);
+    S.n_inst = M.n_inst; S.n_terms = M.n_terms; S.n_kc = M.n_kc;
+    for (int j = 0; j < M.n_inst; ++j) S.inst_srow[j] = (uint8_t)M.inst[j].sys;
+    for (int kap = 0; kap < M.n_kc; ++kap)
+      for (int k = M.col_begin[kap]; k < M.col_begin[kap + 1]; ++k) {
+        const TermTab &tm = M.term[k];
+        S.term_t0[k] = tm.inst0 >= 0 ? (uint16_t)(tm.inst0 * 32) : (uint16_t)0xFFFF;
+        S.term_t1[k] = tm.inst1 >= 0 ? (uint16_t)(tm.inst1 * 32) : (uint16_t)0xFFFF;
+        S.term_col[k] = (uint8_t)kap;
+        S.term_last[k] = k == M.col_begin[kap + 1] - 1;
+      }
+  }
   h->mass.assign(desc->n_res, 0.0);
   h->width.assign(desc->n_res, 0.0);
 
@@ -505,7 +520,10 @@ int tddp4_load_events(tddp4 *h, int which, int64_t n, int64_t ld_in, const doubl
   CU(cudaMalloc(&e.s, sizeof(double) * M.n_sys * e.ld));
   CU(cudaMalloc(&e.g, sizeof(double) * std::max(1, M.n_inst) * e.ld));
   CU(cudaMalloc(&e.f, sizeof(double) * M.n_terms * e.ld));
-  if (which == 0) CU(cudaMalloc(&e.a, sizeof(double2) * M.n_kc * e.ld));   // the normalisation sample keeps no columns
+  if (which == 0) {   // the normalisation sample keeps no columns; a coupling without chains keeps its zero column
+    CU(cudaMalloc(&e.a, sizeof(double2) * M.n_kc * e.ld));
+    CU(cudaMemsetAsync(e.a, 0, sizeof(double2) * M.n_kc * e.ld, h->stream));
+  }
   cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
   auto copy_vec = [&](double **dst, const double *src) -> cudaError_t {
     if (!src || n == 0) return cudaSuccess;
