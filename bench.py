@@ -242,13 +242,14 @@ def run_ours(args):
     roof = {"kernel": dominant, "bound": "hbm", "achieved": ktab[dominant]["achieved_GBs"], "peak": hbm, "unit": "GB/s",
             "frac": ktab[dominant]["frac"], "peak_source": which, "traffic": None,
             "alg_bytes_per_launch": ktab[dominant]["alg_MB_per_launch"] * 1e6, "us_per_launch": ktab[dominant]["us_per_launch"]}
-    traffic_file = os.path.join(ROOT, "profiles", "traffic.json")
+    traffic_file = os.path.join(ROOT, "profiles", "traffic.csv")   # from the committed ncu --set full capture
     if os.path.exists(traffic_file):
+        import csv
         with open(traffic_file) as f:
-            tr = json.load(f)
-        roof["traffic"] = tr.get(dominant, {}).get("dram_bytes_per_launch")
+            tr = {r["kernel"]: float(r["dram_bytes_per_launch"]) for r in csv.DictReader(f)}
+        roof["traffic"] = tr.get(dominant)
         for k in ktab:
-            ktab[k]["traffic"] = tr.get(k, {}).get("dram_bytes_per_launch")
+            ktab[k]["traffic"] = tr.get(k)
 
     cpu = cpu_baseline(mdl, p0, p4, t, p4n)
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
