@@ -146,6 +146,10 @@ class Tddp4:
             raise Tddp4Error(rc, text)
         self.n = [0, 0]
 
+    @property
+    def n_data(self):
+        return self.n[0]
+
     # -- plumbing ---------------------------------------------------------------------------------
     def _check(self, rc, allow=()):
         if rc != OK and rc not in allow:

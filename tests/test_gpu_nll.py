@@ -341,3 +341,24 @@ def test_more_than_eight_couplings(B, chains):
     h.set_params(step)
     ref = oracle.nll(mdl, step, p4, t, p4n)
     assert nll_close(h.nll(), ref[0], np.log(ref[2]))
+
+
+def test_sharded_wrapper_on_one_rank(B):
+    """sharded.ShardedNLL around the CUDA handle, world size 1: same value as the handle's own NLL to rounding of the
+    recombination (Gamma sum t - sum log B + n log N is formed on the host here, on the device there)."""
+    from paper_1702_06735_b200 import sharded
+    mdl = samples.model_of(("C", 2))
+    par = W.initial_params(mdl)
+    p4, t, _ = samples.data_sample(("C", 2), 2_049)
+    p4n, _ = samples.flat_sample(10_001)
+    h = B.Tddp4(mdl)
+    h.load_events(0, p4, t); h.load_events(1, p4n)
+    h.set_params(par)
+    direct = h.nll()
+    sh = sharded.ShardedNLL(h)
+    sh.set_params(par)
+    assert abs(sh.nll() - direct) <= 1e-13 * abs(direct)
+    p2 = par.copy(); p2.mass[1] *= 1.0005
+    h.set_params(p2); direct2 = h.nll()
+    sh.set_params(p2)
+    assert abs(sh.nll() - direct2) <= 1e-13 * abs(direct2)
