@@ -239,7 +239,7 @@ def config(i: int) -> Config:
     if i == 3:
         return Config("C3", build_model(range(1, 9), bose=True), 1_000_000, 4_000_000, 1000, "minuit")
     if i == 4:
-        return Config("C4", build_model(range(1, 9)), 0, 0, 1, "coupling_only", n_candidates=10_000_000)
+        return Config("C4", build_model([1, 2, 3]), 0, 0, 1, "coupling_only", n_candidates=10_000_000)
     if i == 5:
         return Config("C5", build_model(range(1, 9), bose=True, t_lo=0.0, t_hi=4.0, use_resolution=1),
                       10_000_000, 10_000_000, 100, "minuit", sigma_t=(0.03, 0.08), efficiency=(0.5, 1.0))
