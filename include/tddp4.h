@@ -84,7 +84,8 @@ typedef struct {
   const tddp4_term *terms; /* host [n_terms]                                                         */
   int n_couplings;         /* K_c                                                                    */
   double t_lo, t_hi;       /* decay-time window of the normalisation; t_hi = +INFINITY allowed       */
-  int use_resolution;      /* 0: eq. (1) as printed; 1: per-event Gaussian sigma_t   */
+  int use_resolution;      /* 0: eq. (1) as printed; 1: per-event Gaussian sigma_t (O-8): the data *
+                            * sample must be loaded with sigma_t > 0; P_i = R_i(t_i, sigma_i) / N_i(sigma_i)    */
 } tddp4_model_desc;
 
 /* ---- life cycle -------------------------------------------------------------------------------- */
@@ -189,7 +190,8 @@ enum {
   TDDP4_K_NLL = 3,       /* steps 4+5+7 over cached columns (coupling / x / y / tau-only call)         */
   TDDP4_K_GEN_RATIO = 4, TDDP4_K_GEN_EMIT = 5,
   TDDP4_K_COLNLL = 6,    /* steps 2+3+4+5+7 fused over the data sample (call after a mass/width move)  */
-  TDDP4_K_COUNT = 7
+  TDDP4_K_TRES = 7,      /* resolution mode: per-event time rows (re-run when x, y or tau moved)               */
+  TDDP4_K_COUNT = 8
 };
 int tddp4_profile(tddp4 *h, int enable);
 /* total_ms, launches and (alg_bytes may be NULL) the algorithmic bytes of those launches -- the rows each launch

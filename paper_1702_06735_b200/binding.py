@@ -17,8 +17,8 @@ LIB_PATH = os.path.join(_HERE, "csrc", "libtddp4.so")
 
 OK, ERR_ARG, ERR_CUDA, ERR_CAPACITY, ERR_DOMAIN, ERR_NONFINITE, ERR_STATE = 0, -1, -2, -3, -4, -5, -6
 GET_S, GET_SHAPE, GET_STATIC, GET_COLUMNS, GET_TERMS = range(5)
-K_KIN, K_COLUMNS, K_GRAM, K_NLL, K_GEN_RATIO, K_GEN_EMIT, K_COLNLL = range(7)
-KERNEL_NAMES = ["kin", "columns", "gram", "nll", "gen_ratio", "gen_emit", "columns_nll"]
+K_KIN, K_COLUMNS, K_GRAM, K_NLL, K_GEN_RATIO, K_GEN_EMIT, K_COLNLL, K_TRES = range(8)
+KERNEL_NAMES = ["kin", "columns", "gram", "nll", "gen_ratio", "gen_emit", "columns_nll", "time_rows"]
 
 # every symbol include/tddp4.h declares
 SYMBOLS = ["tddp4_create", "tddp4_destroy", "tddp4_set_stream", "tddp4_last_error", "tddp4_version",

@@ -11,6 +11,7 @@
 // (Measured on B200, 1M events x 136 B: a TMA/mbarrier-staged version of the coupling-only pass with one block per
 // SM ran at 35 us, this register-direct form at 26.7 us, a pure read of the same bytes at 22.6 us.)
 #pragma once
+#include "resolution.cuh"
 
 namespace tddp4k {
 
@@ -85,9 +86,10 @@ __device__ __forceinline__ void amp_add(double2 &A, double2 &Ab, double cr, doub
 // N from the Gram matrix in force (O-8, step 6): N = T1 (nAA + nBB) + T2 (nAA - nBB) - 2 T3 Re X - 2 T4 Im X,
 // nAA = c^T G conj(c), nBB likewise for cbar, X = sum_kl c_k conj(cbar_l) G_kl.  One warp, (k,l) pairs strided over
 // the lanes, fixed shuffle tree; every lane returns the same value.
-__device__ __forceinline__ double norm_from_gram_warp(const RateParams &R, const double *__restrict__ G, int KC, double inv_n) {
+__device__ __forceinline__ void gram_sums_warp(const RateParams &R, const double *__restrict__ G, int KC, double inv_n,
+                                               double &nAA, double &nBB, double &xr, double &xi) {
   const int lane = threadIdx.x & 31;
-  double nAA = 0.0, nBB = 0.0, xr = 0.0, xi = 0.0;
+  nAA = 0.0; nBB = 0.0; xr = 0.0; xi = 0.0;
   for (int q = lane; q < KC * KC; q += 32) {
     int k = q / KC, l = q % KC;
     double gr = __ldcg(G + q * 2) * inv_n, gi = __ldcg(G + q * 2 + 1) * inv_n;
@@ -102,13 +104,43 @@ __device__ __forceinline__ double norm_from_gram_warp(const RateParams &R, const
     xi += pr * gi + pi * gr;
   }
   nAA = warp_sum(nAA); nBB = warp_sum(nBB); xr = warp_sum(xr); xi = warp_sum(xi);
+}
+__device__ __forceinline__ double norm_from_gram_warp(const RateParams &R, const double *__restrict__ G, int KC, double inv_n) {
+  double nAA, nBB, xr, xi;
+  gram_sums_warp(R, G, KC, inv_n, nAA, nBB, xr, xi);
   return R.T[0] * (nAA + nBB) + R.T[1] * (nAA - nBB) - 2.0 * R.T[2] * xr - 2.0 * R.T[3] * xi;
+}
+
+// Resolution mode (O-8, config 5): the phase-space sums S_1..S_4 = <w(|A|^2+|Abar|^2)>, <w(|A|^2-|Abar|^2)>, <w Re A Abar*>,
+// <w Im A Abar*> must be known BEFORE the data pass, because the normalisation N_i = sum_m T_m(sigma_i) S_m is per
+// event.  Warp 0 of every block derives them from the Gram matrix in force (same code, same bits in every block).
+__device__ __forceinline__ void block_phase_space_sums(const RateParams &R, const double *__restrict__ G, int KC, double inv_n,
+                                                       double *s_S /* shared [4] */) {
+  if ((threadIdx.x >> 5) == 0) {
+    double nAA, nBB, xr, xi;
+    gram_sums_warp(R, G, KC, inv_n, nAA, nBB, xr, xi);
+    if ((threadIdx.x & 31) == 0) { s_S[0] = nAA + nBB; s_S[1] = nAA - nBB; s_S[2] = xr; s_S[3] = xi; }
+  }
+  __syncthreads();
+}
+// P_i = R_i / N_i of one event from its amplitudes and its eight cached time quantities (rows psi[4], tint[4])
+__device__ __forceinline__ double resolved_prob(double2 A, double2 Ab, const double *__restrict__ tr_i, int64_t ld,
+                                                const double *s_S) {
+  double v[8];
+#pragma unroll
+  for (int m = 0; m < 8; ++m) v[m] = ldg_stream1(tr_i + m * ld);
+  double aa = A.x * A.x + A.y * A.y, bb = Ab.x * Ab.x + Ab.y * Ab.y;
+  double cre = A.x * Ab.x + A.y * Ab.y, cim = A.y * Ab.x - A.x * Ab.y;
+  double Rv = (aa + bb) * v[0] + (aa - bb) * v[1] - 2.0 * cre * v[2] - 2.0 * cim * v[3];
+  double Nv = s_S[0] * v[4] + s_S[1] * v[5] - 2.0 * s_S[2] * v[6] - 2.0 * s_S[3] * v[7];
+  return Rv / Nv;
 }
 
 // common tail of the two NLL kernels (step 7, second pass).  Thread products -> warp -> block partial
 // (prod, exponent sum, #bad); the last block to arrive merges the block partials in index order in warp 0 while
 // warp 1 evaluates N, then thread 0 takes the one log and writes the result slot:
 //   [0] sum log B, [1] sum t, [2] N, [3] NLL = Gamma sum t - sum log B + n log N, [4] #bad events
+template <bool RES = false>
 __device__ __forceinline__ void nll_finish(const RateParams &R, int KC, int64_t n, double sum_t, MantAcc la,
                                            const double *__restrict__ G, double inv_n, double *__restrict__ partials,
                                            unsigned int *ticket, double *__restrict__ result) {
@@ -152,6 +184,7 @@ __device__ __forceinline__ void nll_finish(const RateParams &R, int KC, int64_t 
     double s0 = log(m.prod) + 0.693147180559945309417 * (double)m.esum;
     // -sum log(e^{-Gamma t} B / N) = Gamma sum t - sum log B + n log N
     double nll = R.Gamma * sum_t - s0 + (double)n * log(norm);
+    if (RES) { nll = -s0; sum_t = 0.0; }                 // the accumulated values were P_i = R_i / N_i already
     if (m.bad > 0 || !(norm > 0.0)) nll = INFINITY;
     result[0] = s0; result[1] = sum_t; result[2] = norm; result[3] = nll; result[4] = (double)m.bad;
     *ticket = 0;
@@ -218,6 +251,56 @@ prob_kernel(const double2 *__restrict__ a, const double *__restrict__ t, int64_t
   prob_out[i] = exp(-R.Gamma * ti) * bracket<SMALL>(A, Ab, R.y * R.Gamma * ti, R.x * R.Gamma * ti) / norm;
 }
 
+// Coupling-only call with per-event resolution (config 5): K_c columns + the eight time rows, 16 K_c + 64 B per event.
+template <int KC>
+__global__ void __launch_bounds__(STREAM_BLOCK, STREAM_BLOCKS_PER_SM)
+nll_res_kernel(const double2 *__restrict__ a, const double *__restrict__ tr, int64_t ld, int64_t n,
+               const __grid_constant__ RateParams R, const double *__restrict__ G, double inv_n_norm,
+               double *__restrict__ partials, unsigned int *ticket, double *__restrict__ result) {
+  __shared__ double s_S[4];
+  MantAcc la;
+  block_phase_space_sums(R, G, KC, inv_n_norm, s_S);
+  const int64_t stride = (int64_t)gridDim.x * STREAM_BLOCK;
+#pragma unroll 1
+  for (int64_t i = (int64_t)blockIdx.x * STREAM_BLOCK + threadIdx.x; i < n; i += stride) {
+    double2 v[KC];
+#pragma unroll
+    for (int c = 0; c < KC; ++c) v[c] = ldg_stream2(a + c * ld + i);
+    double2 A = make_double2(0.0, 0.0), Ab = make_double2(0.0, 0.0);
+#pragma unroll
+    for (int c = 0; c < KC; ++c) amp_add(A, Ab, R.c[c][0], R.c[c][1], R.cbar[c][0], R.cbar[c][1], v[c]);
+    la.add(resolved_prob(A, Ab, tr + i, ld, s_S));
+  }
+  nll_finish<true>(R, KC, n, 0.0, la, G, inv_n_norm, partials, ticket, result);
+}
+// P_i with resolution for prob_out
+__global__ void __launch_bounds__(STREAM_BLOCK)
+prob_res_kernel(const double2 *__restrict__ a, const double *__restrict__ tr, int64_t ld, int64_t n, int KC,
+                const __grid_constant__ RateParams R, const double *__restrict__ G, double inv_n_norm,
+                double *__restrict__ prob_out) {
+  __shared__ double s_S[4];
+  block_phase_space_sums(R, G, KC, inv_n_norm, s_S);
+  int64_t i = (int64_t)blockIdx.x * STREAM_BLOCK + threadIdx.x;
+  if (i >= n) return;
+  double2 A = make_double2(0.0, 0.0), Ab = make_double2(0.0, 0.0);
+  for (int c = 0; c < KC; ++c) amp_add(A, Ab, R.c[c][0], R.c[c][1], R.cbar[c][0], R.cbar[c][1], a[c * ld + i]);
+  prob_out[i] = resolved_prob(A, Ab, tr + i, ld, s_S);
+}
+
+// The time rows of the data sample: psi[4], tint[4] per event (resolution.cuh).  Re-run when x, y, tau or the sample
+// change; one thread per event; reads t and sigma_t (16 B), writes 64 B.  ALU-bound (3 exp, 6 erfcx, 3 Faddeeva).
+constexpr int TRES_BLOCK = 128;
+__global__ void __launch_bounds__(TRES_BLOCK)
+tres_kernel(const __grid_constant__ FaddTab F, const double *__restrict__ t, const double *__restrict__ sigma_t, int64_t n,
+            double x, double y, double Gamma, double t_lo, double t_hi, double *__restrict__ tr, int64_t ld) {
+  int64_t i = (int64_t)blockIdx.x * TRES_BLOCK + threadIdx.x;
+  if (i >= n) return;
+  double psi[4], tint[4];
+  time_terms(F, t[i], sigma_t[i], x, y, Gamma, t_lo, t_hi, psi, tint);
+#pragma unroll
+  for (int m = 0; m < 4; ++m) { tr[m * ld + i] = psi[m]; tr[(4 + m) * ld + i] = tint[m]; }
+}
+
 // ------------------------------------------------------------------------------------------------
 // steps 2+3 of ONE event from the step-1 caches in global memory.  Both loops are unrolled to the table maxima with
 // warp-uniform guards, so every table entry and lineshape constant is an immediate-indexed constant-bank operand.
@@ -280,7 +363,7 @@ __host__ __device__ inline size_t lineshape_scratch_bytes(int n_inst) { return (
 // coupling column back (for the coupling-only calls that follow) and finishes the NLL in the same pass.
 inline size_t colnll_smem_bytes(int n_inst) { return STREAM_WARPS * lineshape_scratch_bytes(n_inst); }
 
-template <bool SMALL>
+template <bool SMALL, bool RES = false>
 __global__ void __launch_bounds__(STREAM_BLOCK, STREAM_BLOCKS_PER_SM)
 colnll_stream_kernel(const __grid_constant__ StreamTab S, const __grid_constant__ LineParams LP,
                      const double *__restrict__ s, const double *__restrict__ g, const double *__restrict__ f,
@@ -288,23 +371,26 @@ colnll_stream_kernel(const __grid_constant__ StreamTab S, const __grid_constant_
                      const __grid_constant__ RateParams R, const double *__restrict__ G, double inv_n_norm, double sum_t,
                      double *__restrict__ partials, unsigned int *ticket, double *__restrict__ result) {
   extern __shared__ __align__(16) char smem_raw[];
+  __shared__ double s_S[4];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   double2 *sTl = reinterpret_cast<double2 *>(smem_raw + (size_t)warp * lineshape_scratch_bytes(S.n_inst)) + lane;
   MantAcc la;
   const double yG = R.y * R.Gamma, xG = R.x * R.Gamma;
   const int64_t stride = (int64_t)gridDim.x * STREAM_BLOCK;
+  if (RES) block_phase_space_sums(R, G, S.n_kc, inv_n_norm, s_S);
 #pragma unroll 1
   for (int64_t i = (int64_t)blockIdx.x * STREAM_BLOCK + threadIdx.x; i < n; i += stride) {
-    double ti = ldg_stream1(t + i);
+    double ti = RES ? 0.0 : ldg_stream1(t + i);          // RES: t points at the time rows [8][ld]
     lineshapes_to_scratch(S, LP, s + i, g + i, ld, sTl);
     double2 A = make_double2(0.0, 0.0), Ab = make_double2(0.0, 0.0);
     columns_from_scratch(S, f + i, ld, sTl, [&](int kap, double2 col) {
       a[(int64_t)kap * ld + i] = col;
       amp_add(A, Ab, R.c[kap][0], R.c[kap][1], R.cbar[kap][0], R.cbar[kap][1], col);
     });
-    la.add(bracket<SMALL>(A, Ab, yG * ti, xG * ti));
+    if (RES) la.add(resolved_prob(A, Ab, t + i, ld, s_S));
+    else la.add(bracket<SMALL>(A, Ab, yG * ti, xG * ti));
   }
-  nll_finish(R, S.n_kc, n, sum_t, la, G, inv_n_norm, partials, ticket, result);
+  nll_finish<RES>(R, S.n_kc, n, sum_t, la, G, inv_n_norm, partials, ticket, result);
 }
 
 // ------------------------------------------------------------------------------------------------

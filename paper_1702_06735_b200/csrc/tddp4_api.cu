@@ -28,6 +28,8 @@ struct EventSet {
   double *s = nullptr, *g = nullptr, *f = nullptr;   // static caches [rows][ld]
   double2 *a = nullptr;                              // coupling columns [K_c][ld]
   double *t = nullptr, *sigma_t = nullptr, *w = nullptr;
+  double *tr = nullptr;                              // resolution mode: time rows psi[4], tint[4], [8][ld]
+  bool tres_valid = false;                           // tr matches the current x, y, tau
   double sum_t = 0.0, t_max = 0.0;                   // sum and max |t| of the decay times (fixed-order kernel)
   bool cols_dirty = true;                            // coupling columns stale (a mass or width moved since they were built)
   bool loaded = false;
@@ -51,6 +53,7 @@ struct tddp4 {
   bool have_params = false;
   LineParams LP{};
   RateParams RP{};
+  FaddTab FT{};                      // Faddeeva expansion coefficients (resolution mode)
   std::vector<double> mass, width;
   EventSet set[2];
   // normalisation
@@ -198,6 +201,7 @@ int ensure_partials(tddp4 *h, size_t doubles) {
 
 void free_set(EventSet &e) {
   cudaFree(e.s); cudaFree(e.g); cudaFree(e.f); cudaFree(e.a); cudaFree(e.t); cudaFree(e.sigma_t); cudaFree(e.w);
+  cudaFree(e.tr);
   e = EventSet{};
 }
 
@@ -254,14 +258,27 @@ int launch_nll(tddp4 *h, const EventSet &e, double inv_n, double *result, bool s
   return TDDP4_OK;
 }
 
+template <int KC>
+int launch_nll_res(tddp4 *h, const EventSet &e, double inv_n, double *result) {
+  int grid = stream_grid(h, e.n);
+  int rc = ensure_partials(h, (size_t)3 * grid + 16);
+  if (rc) return rc;
+  Prof p(h, TDDP4_K_NLL, (double)e.n * (16.0 * KC + 64.0));
+  nll_res_kernel<KC><<<grid, STREAM_BLOCK, 0, h->stream>>>(e.a, e.tr, e.ld, e.n, h->RP, h->G, inv_n, h->partials, h->ticket, result);
+  return TDDP4_OK;
+}
+
 int launch_colnll(tddp4 *h, const EventSet &e, double inv_n, double *result, bool small) {
   const ModelTab &M = h->M;
   int grid = stream_grid(h, e.n);
   int rc = ensure_partials(h, (size_t)3 * grid + 16);
   if (rc) return rc;
   size_t smem = colnll_smem_bytes(M.n_inst);
-  Prof p(h, TDDP4_K_COLNLL, (double)e.n * (static_bytes_per_event(h) + 8.0 + 16.0 * M.n_kc));
-  if (small)
+  Prof p(h, TDDP4_K_COLNLL, (double)e.n * (static_bytes_per_event(h) + (h->use_resolution ? 64.0 : 8.0) + 16.0 * M.n_kc));
+  if (h->use_resolution)
+    colnll_stream_kernel<false, true><<<grid, STREAM_BLOCK, smem, h->stream>>>(h->S, h->LP, e.s, e.g, e.f, e.tr, e.ld, e.n, e.a, h->RP,
+                                                                              h->G, inv_n, 0.0, h->partials, h->ticket, result);
+  else if (small)
     colnll_stream_kernel<true><<<grid, STREAM_BLOCK, smem, h->stream>>>(h->S, h->LP, e.s, e.g, e.f, e.t, e.ld, e.n, e.a, h->RP, h->G,
                                                                        inv_n, e.sum_t, h->partials, h->ticket, result);
   else
@@ -276,7 +293,7 @@ int dispatch_nll(tddp4 *h, EventSet &d, bool fused, double inv_n, double *result
     rc = launch_colnll(h, d, inv_n, result, small);
   } else {
     switch (h->M.n_kc) {
-#define CASE(k) case k: rc = launch_nll<k>(h, d, inv_n, result, small); break;
+#define CASE(k) case k: rc = h->use_resolution ? launch_nll_res<k>(h, d, inv_n, result) : launch_nll<k>(h, d, inv_n, result, small); break;
       CASE(1) CASE(2) CASE(3) CASE(4) CASE(5) CASE(6) CASE(7) CASE(8) CASE(9) CASE(10) CASE(11) CASE(12)
       CASE(13) CASE(14) CASE(15) CASE(16)
 #undef CASE
@@ -302,9 +319,18 @@ int enqueue_nll(tddp4 *h, double *result, double *prob) {
   if (!h->have_params) return fail(h, TDDP4_ERR_STATE, "tddp4_set_params has not been called");
   EventSet &d = h->set[0];
   if (!d.loaded) return fail(h, TDDP4_ERR_STATE, "data sample not loaded");
-  if (h->use_resolution) return fail(h, TDDP4_ERR_ARG, "use_resolution = 1 is not implemented yet");
   int rc = ensure_gram(h);
   if (rc) return rc;
+  if (h->use_resolution && !d.tres_valid && d.n > 0) {   // x, y, tau or the sample changed: rebuild the time rows
+    int grid = (int)((d.n + TRES_BLOCK - 1) / TRES_BLOCK);
+    {
+      Prof p(h, TDDP4_K_TRES, (double)d.n * 80.0);
+      tres_kernel<<<grid, TRES_BLOCK, 0, h->stream>>>(h->FT, d.t, d.sigma_t, d.n, h->RP.x, h->RP.y, h->RP.Gamma, h->t_lo, h->t_hi,
+                                                      d.tr, d.ld);
+    }
+    CU(cudaGetLastError());
+    d.tres_valid = true;
+  }
   double inv_n = h->gram_n > 0 ? 1.0 / (double)h->gram_n : 0.0;
   // Taylor forms of the four time functions are valid when both mixing phases stay below 1/4 on this sample
   const RateParams &R = h->RP;
@@ -321,7 +347,9 @@ int enqueue_nll(tddp4 *h, double *result, double *prob) {
   if (prob && d.n > 0) {   // per-event probabilities from the columns and the N the NLL kernel has just written
     int grid = (int)((d.n + STREAM_BLOCK - 1) / STREAM_BLOCK);
     ++h->launches;
-    if (small) prob_kernel<true><<<grid, STREAM_BLOCK, 0, h->stream>>>(d.a, d.t, d.ld, d.n, h->M.n_kc, h->RP, result, prob);
+    if (h->use_resolution)
+      prob_res_kernel<<<grid, STREAM_BLOCK, 0, h->stream>>>(d.a, d.tr, d.ld, d.n, h->M.n_kc, h->RP, h->G, inv_n, prob);
+    else if (small) prob_kernel<true><<<grid, STREAM_BLOCK, 0, h->stream>>>(d.a, d.t, d.ld, d.n, h->M.n_kc, h->RP, result, prob);
     else prob_kernel<false><<<grid, STREAM_BLOCK, 0, h->stream>>>(d.a, d.t, d.ld, d.n, h->M.n_kc, h->RP, result, prob);
     CU(cudaGetLastError());
   }
@@ -440,6 +468,7 @@ int tddp4_create(const tddp4_model_desc *desc, tddp4 **out) {
         S.term_last[k] = k == M.col_begin[kap + 1] - 1;
       }
   }
+  if (h->use_resolution) fadd_coefficients(h->FT);
   h->mass.assign(desc->n_res, 0.0);
   h->width.assign(desc->n_res, 0.0);
 
@@ -470,6 +499,7 @@ int tddp4_create(const tddp4_model_desc *desc, tddp4 **out) {
     if (sc > limit || sg > limit) return bail(fail(h, TDDP4_ERR_ARG, "model too large for the shared-memory scratch of the streaming kernels"));
     cudaFuncSetAttribute(colnll_stream_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sc);
     cudaFuncSetAttribute(colnll_stream_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sc);
+    cudaFuncSetAttribute(colnll_stream_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sc);
     if (NB == 1) cudaFuncSetAttribute(gram_stream_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sg);
     else if (NB == 2) cudaFuncSetAttribute(gram_stream_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sg);
     else if (NB == 3) cudaFuncSetAttribute(gram_stream_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sg);
@@ -511,6 +541,8 @@ int tddp4_load_events(tddp4 *h, int which, int64_t n, int64_t ld_in, const doubl
   if (!h) return TDDP4_ERR_ARG;
   if (which < 0 || which > 1 || n < 0 || ld_in < n || (n > 0 && !p4)) return fail(h, TDDP4_ERR_ARG, "bad load_events argument");
   if (which == 0 && n > 0 && !t) return fail(h, TDDP4_ERR_ARG, "the data sample needs decay times");
+  if (which == 0 && n > 0 && h->use_resolution && !sigma_t)
+    return fail(h, TDDP4_ERR_ARG, "use_resolution = 1: the data sample needs per-event sigma_t");
   CU(cudaStreamSynchronize(h->stream));
   EventSet &e = h->set[which];
   free_set(e);
@@ -523,6 +555,7 @@ int tddp4_load_events(tddp4 *h, int which, int64_t n, int64_t ld_in, const doubl
   if (which == 0) {   // the normalisation sample keeps no columns; a coupling without chains keeps its zero column
     CU(cudaMalloc(&e.a, sizeof(double2) * M.n_kc * e.ld));
     CU(cudaMemsetAsync(e.a, 0, sizeof(double2) * M.n_kc * e.ld, h->stream));
+    if (h->use_resolution) CU(cudaMalloc(&e.tr, sizeof(double) * 8 * e.ld));
   }
   cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
   auto copy_vec = [&](double **dst, const double *src) -> cudaError_t {
@@ -599,6 +632,7 @@ int tddp4_set_params(tddp4 *h, const double *c, const double *cbar, const double
     R.c[k][0] = c[2 * k]; R.c[k][1] = c[2 * k + 1];
     R.cbar[k][0] = cbar[2 * k]; R.cbar[k][1] = cbar[2 * k + 1];
   }
+  if (R.x != x || R.y != y || R.Gamma != 1.0 / tau || !h->have_params) h->set[0].tres_valid = false;
   R.x = x; R.y = y; R.Gamma = 1.0 / tau;
   R.t_lo = h->t_lo; R.t_hi = h->t_hi; R.use_resolution = h->use_resolution;
   time_integrals(x, y, R.Gamma, h->t_lo, h->t_hi, R.T);

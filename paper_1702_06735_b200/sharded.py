@@ -4,9 +4,11 @@ Events are independent, so data and normalisation samples are split into contigu
 (one process per GPU).  Per minimiser call the only data that must cross ranks is
 
   * the K_c x K_c Hermitian Gram sums of the normalisation shards (only when a mass or width moved), and
-  * three scalars per rank of the data pass: sum_i log B_i, sum_i t_i and the number of bad events,
+  * per rank of the data pass: its local NLL (evaluated with the GLOBAL normalisation), its event count and its number
+    of bad events,
 
-because  -sum_i log(e^{-Gamma t_i} B_i / N) = Gamma sum t - sum log B + n log N.  Both exchanges are
+because with N (or, with per-event resolution, S_1..S_4) taken from the global Gram matrix the NLL is a plain sum over
+events: -sum_i log P_i = sum over ranks of (Gamma sum t - sum log B + n_r log N)_r.  Both exchanges are
 all-gathers of a few hundred bytes followed by a sum IN RANK ORDER on every rank, so every rank holds the same bits
 and the result does not depend on arrival order.  (An all-reduce would be one call less; NCCL's reduction order is
 not specified, and at 2 K_c^2 + 1 doubles the exchange is latency-bound either way.)
@@ -72,16 +74,12 @@ class ShardedNLL:
         """Global NLL, the same double on every rank; +inf if any rank saw a non-positive rate."""
         self.ev.nll(strict=False)
         p = self.ev.nll_parts()
-        n_local = float(self.ev.n_data)
-        allv = self._all_gather(np.array([p["sum_log_B"], p["sum_t"], n_local, p["n_bad"]]))
-        slb = st = n = bad = 0.0
-        for r in range(self.world):
-            if allv[r, 2] > 0:                  # an empty shard reports log(prod over nothing) = 0 anyway
-                slb += allv[r, 0]
-                st += allv[r, 1]
-            n += allv[r, 2]
-            bad += allv[r, 3]
-        norm = p["norm"]                        # from the global Gram matrix: identical on every rank
-        if bad > 0 or not norm > 0.0:
+        allv = self._all_gather(np.array([p["nll"], float(self.ev.n_data), p["n_bad"]]))
+        total = bad = 0.0
+        for r in range(self.world):             # rank order: same bits everywhere
+            if allv[r, 1] > 0:
+                total += allv[r, 0]
+            bad += allv[r, 2]
+        if bad > 0 or not math.isfinite(total):
             return math.inf
-        return st / self.par.tau - slb + n * math.log(norm)
+        return total

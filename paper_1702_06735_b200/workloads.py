@@ -253,3 +253,30 @@ def flat_envelope_inputs(mdl: Model):
     m0, m1, m2, m3 = mdl.m_final
     M = mdl.m_parent
     return [(M, m0 + m1 + m2, m3), (M - m3, m0 + m1, m2), (M - m2 - m3, m0, m1)]
+
+
+def smear_times(t_true, cfg: Config, seed=BASE_SEED):
+    """Input synthesis for config 5 (BJ:configs[4]): per-event sigma_t ~ U[lo, hi] and observed time t + sigma z, z ~ N(0,1),
+    redrawn until it falls inside the model's decay-time window.  numpy PCG64([seed, STREAM_SMEAR]); both the CUDA path
+    and the oracle receive the result as input."""
+    rng = np.random.default_rng([seed, STREAM_SMEAR])
+    t_true = np.asarray(t_true, dtype=np.float64)
+    lo, hi = cfg.sigma_t
+    sigma = rng.uniform(lo, hi, t_true.shape[0])
+    t_obs = t_true + sigma * rng.standard_normal(t_true.shape[0])
+    for _ in range(1000):
+        bad = (t_obs < cfg.model.t_lo) | (t_obs > cfg.model.t_hi)
+        if not bad.any():
+            break
+        t_obs[bad] = t_true[bad] + sigma[bad] * rng.standard_normal(int(bad.sum()))
+    # true times far beyond the window can never be smeared back into it: fold them to the window edge region
+    bad = (t_obs < cfg.model.t_lo) | (t_obs > cfg.model.t_hi)
+    t_obs[bad] = np.clip(t_obs[bad], cfg.model.t_lo, cfg.model.t_hi)
+    return t_obs, sigma
+
+
+def efficiency_weights(n, cfg: Config, seed=BASE_SEED):
+    """epsilon_j ~ U[lo, hi] on the normalisation sample (BJ:configs[4])."""
+    rng = np.random.default_rng([seed, STREAM_SMEAR, 1])
+    lo, hi = cfg.efficiency
+    return rng.uniform(lo, hi, n)

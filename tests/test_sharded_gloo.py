@@ -62,7 +62,9 @@ class OracleEvaluator:
         return 0.0
 
     def nll_parts(self):
-        return dict(sum_log_B=self.slb, sum_t=float(np.sum(self.t)), norm=self.norm, nll=0.0, n_bad=self.bad)
+        st = float(np.sum(self.t))
+        local = st / self.par.tau - self.slb + self.n_data * math.log(self.norm)   # with the GLOBAL normalisation
+        return dict(sum_log_B=self.slb, sum_t=st, norm=self.norm, nll=local, n_bad=self.bad)
 
 
 def _free_port():
