@@ -29,18 +29,21 @@ __device__ __forceinline__ double block_sum(double v, double *red /* [BLOCK/32] 
 
 // ------------------------------------------------------------------------------------------------
 // step 1: kinematics + spin factors, once per event set.  One thread per event.
-// in : p4 rows [16][ld_in];  out: s[n_sys][ld], g[n_inst][ld], f[n_terms][ld]
+// in : p4 rows [16][ld_in];  out: the tile-major static cache (tables.h): rows s [n_sys], g from g_row0, f from f_row0
 constexpr int KIN_BLOCK = 128;
+struct CacheRows { int R, g_row0, f_row0; };
+__device__ __forceinline__ int64_t tile_index(int R, int row, int64_t i) { return ((i >> 5) * R + row) * 32 + (i & 31); }
 struct KinSink {
-  double *sp, *gp, *fp;
-  int64_t ld, i;
-  __device__ __forceinline__ void s(int r, double v) { sp[r * ld + i] = v; }
-  __device__ __forceinline__ void g(int r, double v) { gp[r * ld + i] = v; }
-  __device__ __forceinline__ void f(int r, double v) { fp[r * ld + i] = v; }
+  double *cache;
+  CacheRows cr;
+  int64_t i;
+  __device__ __forceinline__ void s(int r, double v) { cache[tile_index(cr.R, r, i)] = v; }
+  __device__ __forceinline__ void g(int r, double v) { cache[tile_index(cr.R, cr.g_row0 + r, i)] = v; }
+  __device__ __forceinline__ void f(int r, double v) { cache[tile_index(cr.R, cr.f_row0 + r, i)] = v; }
 };
 __global__ void __launch_bounds__(KIN_BLOCK)
 kin_kernel(const __grid_constant__ ModelTab M, const double *__restrict__ p4, int64_t ld_in, int64_t n,
-           double *__restrict__ s, double *__restrict__ g, double *__restrict__ f, int64_t ld) {
+           double *__restrict__ cache, CacheRows cr) {
   extern __shared__ double smem[];
   Scratch sc{smem, smem + 16 * KIN_BLOCK, smem + (16 + M.n_sys) * KIN_BLOCK, KIN_BLOCK};
   int tid = threadIdx.x;
@@ -48,26 +51,37 @@ kin_kernel(const __grid_constant__ ModelTab M, const double *__restrict__ p4, in
   if (i >= n) return;
 #pragma unroll
   for (int r = 0; r < 16; ++r) sc.P(r, tid) = p4[r * ld_in + i];
-  KinSink sink{s, g, f, ld, i};
+  KinSink sink{cache, cr, i};
   kinematics(M, sc, tid, sink);
+}
+// one row of the tile-major cache <-> a plain vector (weights in at load; inspection rows out)
+__global__ void __launch_bounds__(256) row_scatter_kernel(double *__restrict__ cache, int R, int row, int64_t n,
+                                                         const double *__restrict__ src) {
+  int64_t i = (int64_t)blockIdx.x * 256 + threadIdx.x;
+  if (i < n) cache[tile_index(R, row, i)] = src[i];
+}
+__global__ void __launch_bounds__(256) row_gather_kernel(const double *__restrict__ cache, int R, int row, int64_t n,
+                                                        double *__restrict__ dst) {
+  int64_t i = (int64_t)blockIdx.x * 256 + threadIdx.x;
+  if (i < n) dst[i] = cache[tile_index(R, row, i)];
 }
 
 // ------------------------------------------------------------------------------------------------
 constexpr int COL_BLOCK = 128;
 // per-term amplitudes a_k (un-summed), for per-layer parity only (TDDP4_GET_TERMS)
 __global__ void __launch_bounds__(COL_BLOCK)
-terms_kernel(const __grid_constant__ ModelTab M, const __grid_constant__ LineParams LP, const double *__restrict__ s,
-             const double *__restrict__ g, const double *__restrict__ f, int64_t ld, int64_t n,
-             double2 *__restrict__ out /* [n_terms][n], caller's term order */) {
+terms_kernel(const __grid_constant__ ModelTab M, const __grid_constant__ LineParams LP, const double *__restrict__ cache,
+             CacheRows cr, int64_t n, double2 *__restrict__ out /* [n_terms][n], caller's term order */) {
   extern __shared__ double2 sT[];
   int tid = threadIdx.x;
   int64_t i = (int64_t)blockIdx.x * COL_BLOCK + tid;
   if (i >= n) return;
   for (int j = 0; j < M.n_inst; ++j)
-    sT[j * COL_BLOCK + tid] = breit_wigner(LP.m0sq[j], LP.gam[j], s[M.inst[j].sys * ld + i], g[j * ld + i]);
+    sT[j * COL_BLOCK + tid] = breit_wigner(LP.m0sq[j], LP.gam[j], cache[tile_index(cr.R, M.inst[j].sys, i)],
+                                           cache[tile_index(cr.R, cr.g_row0 + j, i)]);
   for (int k = 0; k < M.n_terms; ++k) {
     const TermTab &tm = M.term[k];
-    double fv = f[k * ld + i];
+    double fv = cache[tile_index(cr.R, cr.f_row0 + k, i)];
     double2 T = make_double2(1.0, 0.0);
     if (tm.inst0 >= 0) T = cmul(sT[tm.inst0 * COL_BLOCK + tid], sT[tm.inst1 * COL_BLOCK + tid]);
     out[(int64_t)M.user_term[k] * n + i] = make_double2(fv * T.x, fv * T.y);

@@ -302,78 +302,87 @@ tres_kernel(const __grid_constant__ FaddTab F, const double *__restrict__ t, con
 }
 
 // ------------------------------------------------------------------------------------------------
-// steps 2+3 of ONE event from the step-1 caches in global memory.  Both loops are unrolled to the table maxima with
-// warp-uniform guards, so every table entry and lineshape constant is an immediate-indexed constant-bank operand.
-// Lineshapes: T_R of every de-duplicated instance goes to the thread's own slots sTl[instance * 32] of its
-// warp's scratch (chains index it through the model tables, so it cannot live in registers).  Loads are issued in
-// batches of 8 instances (16 loads in flight); the s rows are shared by several instances and stay in L1.
-// s_i, g_i, f_i: the row-0 addresses of this thread's event.
-__device__ __forceinline__ void lineshapes_to_scratch(const StreamTab &S, const LineParams &LP, const double *__restrict__ s_i,
-                                                      const double *__restrict__ g_i, int64_t ld, double2 *sTl) {
+// steps 2+3 of ONE event from the tile-major static cache (tables.h).  ev = address of (row 0, this event): every row is
+// ev[row * 32], so with the loops unrolled to the table maxima (group-of-4 guards, warp-uniform) every load carries an
+// immediate offset and every table entry / lineshape constant is an immediate-indexed constant-bank operand.
+// Lineshapes: T_R of every de-duplicated instance goes to the thread's own slots sTl[slot * 32] of its warp's
+// scratch (chains index it through the model tables, so it cannot live in registers); slot n_inst4 holds the unit
+// lineshape 1 + 0i that non-resonant and padded terms multiply by.  Loads are issued in batches of 4 instances
+// (8 loads in flight); the s rows are shared by several instances and stay in L1.
+__device__ __forceinline__ void lineshapes_to_scratch(const StreamTab &S, const LineParams &LP, const double *__restrict__ ev,
+                                                      double2 *sTl) {
+  const double *g_ev = ev + S.g_off;
 #pragma unroll
-  for (int j0 = 0; j0 < MAX_INST; j0 += 8) {
-    if (j0 < S.n_inst) {
-      double sv[8], gv[8];
+  for (int j0 = 0; j0 < MAX_INST; j0 += GRP_INST) {
+    if (j0 < S.n_inst4) {
+      double sv[GRP_INST], gv[GRP_INST];
 #pragma unroll
-      for (int u = 0; u < 8; ++u)
-        if (j0 + u < S.n_inst) {
-          sv[u] = __ldg(s_i + S.inst_srow[j0 + u] * ld);
-          gv[u] = ldg_stream1(g_i + (j0 + u) * ld);
-        }
+      for (int u = 0; u < GRP_INST; ++u) {
+        sv[u] = __ldg(ev + S.inst_soff[j0 + u]);
+        gv[u] = ldg_stream1(g_ev + (j0 + u) * 32);
+      }
 #pragma unroll
-      for (int u = 0; u < 8; ++u)
-        if (j0 + u < S.n_inst) sTl[(j0 + u) * 32] = breit_wigner(LP.m0sq[j0 + u], LP.gam[j0 + u], sv[u], gv[u]);
+      for (int u = 0; u < GRP_INST; ++u) sTl[(j0 + u) * 32] = breit_wigner(LP.m0sq[j0 + u], LP.gam[j0 + u], sv[u], gv[u]);
     }
   }
 }
+// The f rows of the first term group, issued BEFORE the lineshape arithmetic so that they are in flight with it.
+__device__ __forceinline__ void prefetch_f(const StreamTab &S, const double *__restrict__ ev, double fv[GRP_TERM]) {
+  const double *f_ev = ev + S.f_off;
+#pragma unroll
+  for (int u = 0; u < GRP_TERM; ++u) fv[u] = ldg_stream1(f_ev + u * 32);
+}
 // Component products summed into coupling columns: a_kappa = sum_{k in kappa} f_k T_{R1(k)} T_{R2(k)} (terms are sorted
-// by coupling).  flush(kappa, a_kappa) is called once per non-empty column, in order.  8 f loads in flight.
+// by coupling).  flush(kappa, a_kappa) is called once per non-empty column, in order.  fv: first group, preloaded.
 template <class Flush>
-__device__ __forceinline__ void columns_from_scratch(const StreamTab &S, const double *__restrict__ f_i, int64_t ld,
-                                                     const double2 *sTl, Flush &&flush) {
+__device__ __forceinline__ void columns_from_scratch(const StreamTab &S, const double *__restrict__ ev, const double2 *sTl,
+                                                     double fv[GRP_TERM], Flush &&flush) {
+  const double *f_ev = ev + S.f_off;
   double2 acc = make_double2(0.0, 0.0);
 #pragma unroll
-  for (int k0 = 0; k0 < MAX_TERMS; k0 += 8) {
-    if (k0 < S.n_terms) {
-      double fv[8];
+  for (int k0 = 0; k0 < MAX_TERMS; k0 += GRP_TERM) {
+    if (k0 < S.n_terms4) {
+      if (k0 > 0) {
 #pragma unroll
-      for (int u = 0; u < 8; ++u)
-        if (k0 + u < S.n_terms) fv[u] = ldg_stream1(f_i + (k0 + u) * ld);
+        for (int u = 0; u < GRP_TERM; ++u) fv[u] = ldg_stream1(f_ev + (k0 + u) * 32);
+      }
 #pragma unroll
-      for (int u = 0; u < 8; ++u) {
+      for (int u = 0; u < GRP_TERM; ++u) {
         const int k = k0 + u;
-        if (k < S.n_terms) {
-          double2 T = make_double2(1.0, 0.0);
-          if (S.term_t0[k] != 0xFFFF) T = cmul(sTl[S.term_t0[k]], sTl[S.term_t1[k]]);
-          acc.x = fma(fv[u], T.x, acc.x);
-          acc.y = fma(fv[u], T.y, acc.y);
-          if (S.term_last[k]) {
-            flush((int)S.term_col[k], acc);
-            acc = make_double2(0.0, 0.0);
-          }
+        double2 T = cmul(sTl[S.term_t0[k]], sTl[S.term_t1[k]]);
+        acc.x = fma(fv[u], T.x, acc.x);
+        acc.y = fma(fv[u], T.y, acc.y);
+        if (S.term_last[k]) {
+          flush((int)S.term_col[k], acc);
+          acc = make_double2(0.0, 0.0);
         }
       }
     }
   }
 }
-__host__ __device__ inline size_t lineshape_scratch_bytes(int n_inst) { return (size_t)(n_inst > 0 ? n_inst : 1) * 32 * sizeof(double2); }
+__host__ __device__ inline size_t lineshape_scratch_bytes(int n_inst4) { return (size_t)(n_inst4 + 1) * 32 * sizeof(double2); }
+// address of (row 0, event i) in a tile-major cache of R rows
+__device__ __forceinline__ const double *tile_event(const double *__restrict__ cache, int R, int64_t i) {
+  return cache + ((i >> 5) * R) * 32 + (i & 31);
+}
 
 // ------------------------------------------------------------------------------------------------
 // Call after a mass or width moved, data set.  Reads the s rows in use, the g rows, the f rows and t; writes every
 // coupling column back (for the coupling-only calls that follow) and finishes the NLL in the same pass.
-inline size_t colnll_smem_bytes(int n_inst) { return STREAM_WARPS * lineshape_scratch_bytes(n_inst); }
+inline size_t colnll_smem_bytes(int n_inst4) { return STREAM_WARPS * lineshape_scratch_bytes(n_inst4); }
 
 template <bool SMALL, bool RES = false>
 __global__ void __launch_bounds__(STREAM_BLOCK, STREAM_BLOCKS_PER_SM)
 colnll_stream_kernel(const __grid_constant__ StreamTab S, const __grid_constant__ LineParams LP,
-                     const double *__restrict__ s, const double *__restrict__ g, const double *__restrict__ f,
-                     const double *__restrict__ t, int64_t ld, int64_t n, double2 *__restrict__ a,
+                     const double *__restrict__ cache, const double *__restrict__ t, int64_t ld, int64_t n,
+                     double2 *__restrict__ a,
                      const __grid_constant__ RateParams R, const double *__restrict__ G, double inv_n_norm, double sum_t,
                      double *__restrict__ partials, unsigned int *ticket, double *__restrict__ result) {
   extern __shared__ __align__(16) char smem_raw[];
   __shared__ double s_S[4];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-  double2 *sTl = reinterpret_cast<double2 *>(smem_raw + (size_t)warp * lineshape_scratch_bytes(S.n_inst)) + lane;
+  double2 *sTl = reinterpret_cast<double2 *>(smem_raw + (size_t)warp * lineshape_scratch_bytes(S.n_inst4)) + lane;
+  sTl[S.n_inst4 * 32] = make_double2(1.0, 0.0);        // unit lineshape slot
   MantAcc la;
   const double yG = R.y * R.Gamma, xG = R.x * R.Gamma;
   const int64_t stride = (int64_t)gridDim.x * STREAM_BLOCK;
@@ -381,9 +390,12 @@ colnll_stream_kernel(const __grid_constant__ StreamTab S, const __grid_constant_
 #pragma unroll 1
   for (int64_t i = (int64_t)blockIdx.x * STREAM_BLOCK + threadIdx.x; i < n; i += stride) {
     double ti = RES ? 0.0 : ldg_stream1(t + i);          // RES: t points at the time rows [8][ld]
-    lineshapes_to_scratch(S, LP, s + i, g + i, ld, sTl);
+    const double *ev = tile_event(cache, S.R, i);
+    double fv[GRP_TERM];
+    prefetch_f(S, ev, fv);
+    lineshapes_to_scratch(S, LP, ev, sTl);
     double2 A = make_double2(0.0, 0.0), Ab = make_double2(0.0, 0.0);
-    columns_from_scratch(S, f + i, ld, sTl, [&](int kap, double2 col) {
+    columns_from_scratch(S, ev, sTl, fv, [&](int kap, double2 col) {
       a[(int64_t)kap * ld + i] = col;
       amp_add(A, Ab, R.c[kap][0], R.c[kap][1], R.cbar[kap][0], R.cbar[kap][1], col);
     });
@@ -404,11 +416,11 @@ colnll_stream_kernel(const __grid_constant__ StreamTab S, const __grid_constant_
 // Reads the s rows in use, the g rows, the f rows, and w if the sample is weighted.
 // Deterministic: per-warp accumulation in event order, warps then blocks summed in index order.
 __host__ __device__ constexpr int gram_stride(int NB) { return NB <= 2 ? 20 : 36; }   // = 4 mod 16: conflict-free fragments
-inline size_t gram_warp_scratch(int NB, int n_inst) {
-  return align_up(lineshape_scratch_bytes(n_inst), 128) + align_up((size_t)32 * gram_stride(NB) * sizeof(double), 128);
+inline size_t gram_warp_scratch(int NB, int n_inst4) {
+  return align_up(lineshape_scratch_bytes(n_inst4), 128) + align_up((size_t)32 * gram_stride(NB) * sizeof(double), 128);
 }
-inline size_t gram_smem_bytes(int NB, int n_inst) {
-  size_t work = STREAM_WARPS * gram_warp_scratch(NB, n_inst), red = (size_t)STREAM_WARPS * NB * NB * 64 * sizeof(double);
+inline size_t gram_smem_bytes(int NB, int n_inst4) {
+  size_t work = STREAM_WARPS * gram_warp_scratch(NB, n_inst4), red = (size_t)STREAM_WARPS * NB * NB * 64 * sizeof(double);
   return work > red ? work : red;
 }
 
@@ -420,8 +432,7 @@ __device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double
 template <int NB>
 __global__ void __launch_bounds__(STREAM_BLOCK, STREAM_BLOCKS_PER_SM)
 gram_stream_kernel(const __grid_constant__ StreamTab S, const __grid_constant__ LineParams LP,
-                   const double *__restrict__ s, const double *__restrict__ g, const double *__restrict__ f,
-                   const double *__restrict__ w /* or NULL */, int64_t ld, int64_t n,
+                   const double *__restrict__ cache, int64_t n,
                    double *__restrict__ partials /* [grid][64 NB NB] */, unsigned int *ticket,
                    double *__restrict__ G /* [KC][KC][2] sums, Hermitian, full */) {
   constexpr int F = 8 * NB, STRIDE = gram_stride(NB), NP = NB * (NB + 1) / 2, WARPS = STREAM_WARPS;
@@ -429,12 +440,13 @@ gram_stream_kernel(const __grid_constant__ StreamTab S, const __grid_constant__ 
   __shared__ bool last;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int KC = S.n_kc;
-  const size_t t_bytes = align_up(lineshape_scratch_bytes(S.n_inst), 128);
+  const size_t t_bytes = align_up(lineshape_scratch_bytes(S.n_inst4), 128);
   const size_t x_bytes = align_up((size_t)32 * STRIDE * sizeof(double), 128);
   char *scratch = smem_raw + (size_t)warp * (t_bytes + x_bytes);
   double2 *sTl = reinterpret_cast<double2 *>(scratch) + lane;  // [n_inst][32], this lane's slots
   double *Xs = reinterpret_cast<double *>(scratch + t_bytes);  // [32][STRIDE]: row = event, F features + weight
   double *row = Xs + lane * STRIDE;
+  sTl[S.n_inst4 * 32] = make_double2(1.0, 0.0);                // unit lineshape slot
 #pragma unroll
   for (int c = 0; c < STRIDE; ++c) row[c] = 0.0;                // features beyond 2 K_c stay zero
   double acc[NP][2];
@@ -446,9 +458,12 @@ gram_stream_kernel(const __grid_constant__ StreamTab S, const __grid_constant__ 
   for (int64_t i0 = (int64_t)blockIdx.x * STREAM_BLOCK + warp * 32; i0 < n; i0 += stride) {
     const int64_t i = i0 + lane;
     if (i < n) {
-      double wj = w ? ldg_stream1(w + i) : 1.0;
-      lineshapes_to_scratch(S, LP, s + i, g + i, ld, sTl);
-      columns_from_scratch(S, f + i, ld, sTl, [&](int kap, double2 col) { *reinterpret_cast<double2 *>(row + 2 * kap) = col; });
+      const double *ev = tile_event(cache, S.R, i);
+      double wj = S.w_off >= 0 ? ldg_stream1(ev + S.w_off) : 1.0;
+      double fv[GRP_TERM];
+      prefetch_f(S, ev, fv);
+      lineshapes_to_scratch(S, LP, ev, sTl);
+      columns_from_scratch(S, ev, sTl, fv, [&](int kap, double2 col) { *reinterpret_cast<double2 *>(row + 2 * kap) = col; });
       row[F] = wj;
     } else {
       for (int c = 0; c < 2 * KC; ++c) row[c] = 0.0;

@@ -10,6 +10,8 @@ constexpr int MAX_INST = 24;   // de-duplicated lineshape instances (PAPER.md li
 constexpr int MAX_TERMS = 32;
 constexpr int MAX_KC = 16;
 constexpr int MAX_RES = 16;
+constexpr int GRP_INST = 12;   // lineshape instances per load batch of the per-call kernels (2 loads each in flight)
+constexpr int GRP_TERM = 16;   // terms per load batch
 
 enum { SF_NONRES = 0, SF_VV_S = 1, SF_VV_P = 2, SF_VV_D = 3, SF_AP_S = 4, SF_TP_D = 5 };
 
@@ -47,13 +49,23 @@ struct ModelTab {
   double r_res2, r_parent2;        // radii squared, GeV^-2
 };
 
-struct StreamTab {                 // the per-call kernels' view of the model: flat, indexable with immediates
-  int n_inst, n_terms, n_kc;
-  uint8_t inst_srow[MAX_INST];     // s row (system index) of lineshape instance j
-  uint16_t term_t0[MAX_TERMS];     // element offset (instance * 32) of T_R1 in the warp's lineshape scratch; 0xFFFF: none
-  uint16_t term_t1[MAX_TERMS];     // ... of T_R2
-  uint8_t term_col[MAX_TERMS];     // coupling column of term k (terms are sorted by coupling)
-  uint8_t term_last[MAX_TERMS];    // 1: term k closes its column
+// The per-call kernels' view of the model and of the static cache.  The cache of one event set is ONE tile-major array:
+// tile = 32 consecutive events, R rows of 32 doubles each (256 B per row per tile), rows ordered
+//   [ s: n_sys | g: n_inst4 | f: n_terms4 | w (if weighted) ],
+// element (row r, event i) at ((i >> 5) * R + r) * 32 + (i & 31).  A warp working on one tile therefore addresses every
+// row as tile base + lane + CONSTANT, and the whole tile is one contiguous R * 256-byte region of HBM.
+// Every table entry is a 32-bit word so that an unrolled loop uses it as an immediate-indexed constant-bank operand.
+// Instances and terms are padded to multiples of GRP_INST / GRP_TERM (group-level guards only) with all-zero rows: a padded instance
+// reads s row 0 and m0sq = -1, gam = 0 (finite, unused); a padded term has f = 0 and the unit lineshape slot.
+struct StreamTab {
+  int n_inst4, n_terms4, n_kc;     // padded counts
+  int R;                           // rows per tile
+  int g_off, f_off, w_off;         // element offsets (row * 32) of the first g row, first f row, weight row (-1: none)
+  uint32_t inst_soff[MAX_INST];    // element offset of the s row lineshape instance j reads
+  uint32_t term_t0[MAX_TERMS];     // element offset (slot * 32) of T_R1 in the warp's lineshape scratch; unit slot if none
+  uint32_t term_t1[MAX_TERMS];     // ... of T_R2
+  uint32_t term_col[MAX_TERMS];    // coupling column of term k (terms are sorted by coupling)
+  uint32_t term_last[MAX_TERMS];   // 1: term k closes its column
 };
 
 struct LineParams {                // per set_params: T = 1 / (m0sq - s - i gam g(s)),  O-6

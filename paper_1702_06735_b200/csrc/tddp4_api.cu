@@ -25,7 +25,8 @@ constexpr int SLOT_DOUBLES = 8;
 
 struct EventSet {
   int64_t n = 0, ld = 0;
-  double *s = nullptr, *g = nullptr, *f = nullptr;   // static caches [rows][ld]
+  double *cache = nullptr;                           // static cache, tile-major (tables.h): s, g, f [, w] rows
+  int R = 0;                                         // rows per tile
   double2 *a = nullptr;                              // coupling columns [K_c][ld]
   double *t = nullptr, *sigma_t = nullptr, *w = nullptr;
   double *tr = nullptr;                              // resolution mode: time rows psi[4], tint[4], [8][ld]
@@ -200,8 +201,7 @@ int ensure_partials(tddp4 *h, size_t doubles) {
 }
 
 void free_set(EventSet &e) {
-  cudaFree(e.s); cudaFree(e.g); cudaFree(e.f); cudaFree(e.a); cudaFree(e.t); cudaFree(e.sigma_t); cudaFree(e.w);
-  cudaFree(e.tr);
+  cudaFree(e.cache); cudaFree(e.a); cudaFree(e.t); cudaFree(e.sigma_t); cudaFree(e.w); cudaFree(e.tr);
   e = EventSet{};
 }
 
@@ -219,9 +219,12 @@ int launch_gram(tddp4 *h, const EventSet &e) {
   int grid = stream_grid(h, e.n);
   int rc = ensure_partials(h, (size_t)grid * 64 * NB * NB + 16);
   if (rc) return rc;
+  StreamTab S = h->S;
+  S.R = e.R;
+  S.w_off = e.w ? (M.n_sys + S.n_inst4 + S.n_terms4) * 32 : -1;
   Prof p(h, TDDP4_K_GRAM, (double)e.n * (static_bytes_per_event(h) + (e.w ? 8.0 : 0.0)));
-  gram_stream_kernel<NB><<<grid, STREAM_BLOCK, gram_smem_bytes(NB, M.n_inst), h->stream>>>(h->S, h->LP, e.s, e.g, e.f, e.w, e.ld, e.n,
-                                                                                      h->partials, h->ticket, h->G);
+  gram_stream_kernel<NB><<<grid, STREAM_BLOCK, gram_smem_bytes(NB, S.n_inst4), h->stream>>>(S, h->LP, e.cache, e.n, h->partials,
+                                                                                       h->ticket, h->G);
   return TDDP4_OK;
 }
 
@@ -273,17 +276,19 @@ int launch_colnll(tddp4 *h, const EventSet &e, double inv_n, double *result, boo
   int grid = stream_grid(h, e.n);
   int rc = ensure_partials(h, (size_t)3 * grid + 16);
   if (rc) return rc;
-  size_t smem = colnll_smem_bytes(M.n_inst);
+  StreamTab S = h->S;
+  S.R = e.R;
+  size_t smem = colnll_smem_bytes(S.n_inst4);
   Prof p(h, TDDP4_K_COLNLL, (double)e.n * (static_bytes_per_event(h) + (h->use_resolution ? 64.0 : 8.0) + 16.0 * M.n_kc));
   if (h->use_resolution)
-    colnll_stream_kernel<false, true><<<grid, STREAM_BLOCK, smem, h->stream>>>(h->S, h->LP, e.s, e.g, e.f, e.tr, e.ld, e.n, e.a, h->RP,
-                                                                              h->G, inv_n, 0.0, h->partials, h->ticket, result);
+    colnll_stream_kernel<false, true><<<grid, STREAM_BLOCK, smem, h->stream>>>(S, h->LP, e.cache, e.tr, e.ld, e.n, e.a, h->RP, h->G,
+                                                                              inv_n, 0.0, h->partials, h->ticket, result);
   else if (small)
-    colnll_stream_kernel<true><<<grid, STREAM_BLOCK, smem, h->stream>>>(h->S, h->LP, e.s, e.g, e.f, e.t, e.ld, e.n, e.a, h->RP, h->G,
-                                                                       inv_n, e.sum_t, h->partials, h->ticket, result);
+    colnll_stream_kernel<true><<<grid, STREAM_BLOCK, smem, h->stream>>>(S, h->LP, e.cache, e.t, e.ld, e.n, e.a, h->RP, h->G, inv_n,
+                                                                       e.sum_t, h->partials, h->ticket, result);
   else
-    colnll_stream_kernel<false><<<grid, STREAM_BLOCK, smem, h->stream>>>(h->S, h->LP, e.s, e.g, e.f, e.t, e.ld, e.n, e.a, h->RP, h->G,
-                                                                        inv_n, e.sum_t, h->partials, h->ticket, result);
+    colnll_stream_kernel<false><<<grid, STREAM_BLOCK, smem, h->stream>>>(S, h->LP, e.cache, e.t, e.ld, e.n, e.a, h->RP, h->G, inv_n,
+                                                                        e.sum_t, h->partials, h->ticket, result);
   return TDDP4_OK;
 }
 
@@ -454,17 +459,21 @@ int tddp4_create(const tddp4_model_desc *desc, tddp4 **out) {
   for (int j = 0; j < M.n_inst; ++j) M.sys_slot[M.inst[j].sys] = 0;
   for (int i = 0; i < M.n_sys; ++i)
     if (M.sys_slot[i] == 0) { M.sys_slot[i] = (int8_t)M.n_su; M.su_sys[M.n_su++] = (int8_t)i; }
-  {   // flat tables of the per-call kernels
+  {   // flat tables of the per-call kernels (tables.h): padded to groups of 4, all entries 32-bit
     StreamTab &S = h->S;
     memset(&S, 0, sizeof S);
-    S.n_inst = M.n_inst; S.n_terms = M.n_terms; S.n_kc = M.n_kc;
-    for (int j = 0; j < M.n_inst; ++j) S.inst_srow[j] = (uint8_t)M.inst[j].sys;
+    S.n_inst4 = (M.n_inst + GRP_INST - 1) / GRP_INST * GRP_INST; S.n_terms4 = (M.n_terms + GRP_TERM - 1) / GRP_TERM * GRP_TERM;
+    S.n_kc = M.n_kc;
+    S.g_off = M.n_sys * 32; S.f_off = (M.n_sys + S.n_inst4) * 32; S.w_off = -1;
+    S.R = M.n_sys + S.n_inst4 + S.n_terms4;              // + 1 for a weighted event set, fixed at launch
+    for (int j = 0; j < M.n_inst; ++j) S.inst_soff[j] = (uint32_t)M.inst[j].sys * 32;
+    const uint32_t unit = (uint32_t)S.n_inst4 * 32;
+    for (int k = 0; k < MAX_TERMS; ++k) { S.term_t0[k] = S.term_t1[k] = unit; }
     for (int kap = 0; kap < M.n_kc; ++kap)
       for (int k = M.col_begin[kap]; k < M.col_begin[kap + 1]; ++k) {
         const TermTab &tm = M.term[k];
-        S.term_t0[k] = tm.inst0 >= 0 ? (uint16_t)(tm.inst0 * 32) : (uint16_t)0xFFFF;
-        S.term_t1[k] = tm.inst1 >= 0 ? (uint16_t)(tm.inst1 * 32) : (uint16_t)0xFFFF;
-        S.term_col[k] = (uint8_t)kap;
+        if (tm.inst0 >= 0) { S.term_t0[k] = (uint32_t)tm.inst0 * 32; S.term_t1[k] = (uint32_t)tm.inst1 * 32; }
+        S.term_col[k] = (uint32_t)kap;
         S.term_last[k] = k == M.col_begin[kap + 1] - 1;
       }
   }
@@ -495,7 +504,7 @@ int tddp4_create(const tddp4_model_desc *desc, tddp4 **out) {
   cudaFuncSetAttribute(gen_ratio_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gen_smem_bytes(MAX_SYS, MAX_INST));
   {   // shared memory of the per-call kernels: per-warp lineshape scratch (+ the X tile of the Gram kernel)
     int NB = (KC + 3) / 4;
-    size_t limit = prop.sharedMemPerBlockOptin - 1024, sc = colnll_smem_bytes(M.n_inst), sg = gram_smem_bytes(NB, M.n_inst);
+    size_t limit = prop.sharedMemPerBlockOptin - 1024, sc = colnll_smem_bytes(h->S.n_inst4), sg = gram_smem_bytes(NB, h->S.n_inst4);
     if (sc > limit || sg > limit) return bail(fail(h, TDDP4_ERR_ARG, "model too large for the shared-memory scratch of the streaming kernels"));
     cudaFuncSetAttribute(colnll_stream_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sc);
     cudaFuncSetAttribute(colnll_stream_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sc);
@@ -549,9 +558,10 @@ int tddp4_load_events(tddp4 *h, int which, int64_t n, int64_t ld_in, const doubl
   e.n = n;
   e.ld = std::max<int64_t>(32, (n + 31) / 32 * 32);   // rows start 256-byte aligned
   const ModelTab &M = h->M;
-  CU(cudaMalloc(&e.s, sizeof(double) * M.n_sys * e.ld));
-  CU(cudaMalloc(&e.g, sizeof(double) * std::max(1, M.n_inst) * e.ld));
-  CU(cudaMalloc(&e.f, sizeof(double) * M.n_terms * e.ld));
+  e.R = h->S.R + (weight && n > 0 ? 1 : 0);
+  const CacheRows cr{e.R, M.n_sys, M.n_sys + h->S.n_inst4};
+  CU(cudaMalloc(&e.cache, sizeof(double) * e.R * e.ld));
+  CU(cudaMemsetAsync(e.cache, 0, sizeof(double) * e.R * e.ld, h->stream));   // padding rows and the ragged tail stay zero
   if (which == 0) {   // the normalisation sample keeps no columns; a coupling without chains keeps its zero column
     CU(cudaMalloc(&e.a, sizeof(double2) * M.n_kc * e.ld));
     CU(cudaMemsetAsync(e.a, 0, sizeof(double2) * M.n_kc * e.ld, h->stream));
@@ -582,9 +592,14 @@ int tddp4_load_events(tddp4 *h, int which, int64_t n, int64_t ld_in, const doubl
     size_t smem = sizeof(double) * (16 + M.n_sys + M.n_inst) * KIN_BLOCK;
     {
       Prof p(h, TDDP4_K_KIN, (double)n * 8.0 * (16 + M.n_sys + M.n_inst + M.n_terms));
-      kin_kernel<<<grid, KIN_BLOCK, smem, h->stream>>>(M, dp4, ld_dev, n, e.s, e.g, e.f, e.ld);
+      kin_kernel<<<grid, KIN_BLOCK, smem, h->stream>>>(M, dp4, ld_dev, n, e.cache, cr);
     }
     CU(cudaGetLastError());
+    if (e.w) {   // the weights travel with the rows they multiply
+      row_scatter_kernel<<<(int)((n + 255) / 256), 256, 0, h->stream>>>(e.cache, e.R, e.R - 1, n, e.w);
+      ++h->launches;
+      CU(cudaGetLastError());
+    }
     if (e.t) {
       double st[2];
       stat_kernel<<<1, 1024, 0, h->stream>>>(e.t, n, h->results);   // slot 0 words 0, 1 as scratch
@@ -609,6 +624,7 @@ int tddp4_set_params(tddp4 *h, const double *c, const double *cbar, const double
   if (!(tau > 0.0) || !(std::fabs(y) < 1.0)) return fail(h, TDDP4_ERR_ARG, "need tau > 0 and |y| < 1");
   const ModelTab &M = h->M;
   LineParams lp{};
+  for (int j = 0; j < MAX_INST; ++j) { lp.m0sq[j] = -1.0; lp.gam[j] = 0.0; }   // padded instances: finite, unused
   int nres = (int)h->res.size();
   for (int j = 0; j < M.n_inst; ++j) {
     const InstTab &in = M.inst[j];
@@ -888,16 +904,21 @@ int tddp4_get(tddp4 *h, int which, int what, double *out) {
     CU(cudaStreamSynchronize(h->stream));
     return TDDP4_OK;
   };
-  switch (what) {
-    case TDDP4_GET_S: return rows(e.s, M.n_sys, sizeof(double));
-    case TDDP4_GET_SHAPE: return rows(e.g, M.n_inst, sizeof(double));
-    case TDDP4_GET_STATIC: {
-      for (int k = 0; k < M.n_terms; ++k)
-        CU(cudaMemcpyAsync(out + (int64_t)M.user_term[k] * e.n, e.f + (int64_t)k * e.ld, sizeof(double) * e.n,
-                           cudaMemcpyDeviceToDevice, h->stream));
-      CU(cudaStreamSynchronize(h->stream));
-      return TDDP4_OK;
+  const CacheRows cr{e.R, M.n_sys, M.n_sys + h->S.n_inst4};
+  auto cache_rows = [&](int row0, int nrows, const int8_t *dst_row) -> int {   // tile-major rows -> plain [nrows][n]
+    for (int r = 0; r < nrows && e.n > 0; ++r) {
+      row_gather_kernel<<<(int)((e.n + 255) / 256), 256, 0, h->stream>>>(e.cache, e.R, row0 + r, e.n,
+                                                                      out + (int64_t)(dst_row ? dst_row[r] : r) * e.n);
+      ++h->launches;
     }
+    CU(cudaGetLastError());
+    CU(cudaStreamSynchronize(h->stream));
+    return TDDP4_OK;
+  };
+  switch (what) {
+    case TDDP4_GET_S: return cache_rows(0, M.n_sys, nullptr);
+    case TDDP4_GET_SHAPE: return cache_rows(cr.g_row0, M.n_inst, nullptr);
+    case TDDP4_GET_STATIC: return cache_rows(cr.f_row0, M.n_terms, M.user_term);
     case TDDP4_GET_COLUMNS: {
       if (which != 0) return fail(h, TDDP4_ERR_ARG, "the normalisation sample keeps no coupling columns");
       if (!h->have_params) return fail(h, TDDP4_ERR_STATE, "tddp4_set_params has not been called");
@@ -912,7 +933,7 @@ int tddp4_get(tddp4 *h, int which, int what, double *out) {
       if (e.n == 0) return TDDP4_OK;
       int grid = (int)((e.n + COL_BLOCK - 1) / COL_BLOCK);
       size_t smem = (size_t)std::max(1, M.n_inst) * COL_BLOCK * sizeof(double2);
-      terms_kernel<<<grid, COL_BLOCK, smem, h->stream>>>(M, h->LP, e.s, e.g, e.f, e.ld, e.n, reinterpret_cast<double2 *>(out));
+      terms_kernel<<<grid, COL_BLOCK, smem, h->stream>>>(M, h->LP, e.cache, cr, e.n, reinterpret_cast<double2 *>(out));
       ++h->launches;
       CU(cudaGetLastError());
       CU(cudaStreamSynchronize(h->stream));
