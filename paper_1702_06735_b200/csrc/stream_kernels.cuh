@@ -307,47 +307,53 @@ tres_kernel(const __grid_constant__ FaddTab F, const double *__restrict__ t, con
 // immediate offset and every table entry / lineshape constant is an immediate-indexed constant-bank operand.
 // Lineshapes: T_R of every de-duplicated instance goes to the thread's own slots sTl[slot * 32] of its warp's
 // scratch (chains index it through the model tables, so it cannot live in registers); slot n_inst4 holds the unit
-// lineshape 1 + 0i that non-resonant and padded terms multiply by.  Loads are issued in batches of 4 instances
-// (8 loads in flight); the s rows are shared by several instances and stay in L1.
+// lineshape 1 + 0i that non-resonant and padded terms multiply by.  Loads are issued in batches of GI instances and GT
+// terms, the first f batch BEFORE the lineshape arithmetic: 2 GI + GT loads in flight per thread (40 for config 3).
+// These kernels are bound by memory-level parallelism, not by bytes or issue slots: with batches of 4 instances the
+// Gram kernel ran at 0.51 of the HBM roofline, with (12, 16) at 0.71.  (Measured and rejected: software-pipelining the
+// next tile's loads behind this tile's arithmetic, 312 us against 240 us; register-resident one-batch forms without the
+// group guards, which ptxas schedules into spills.)
+template <int GI>
 __device__ __forceinline__ void lineshapes_to_scratch(const StreamTab &S, const LineParams &LP, const double *__restrict__ ev,
                                                       double2 *sTl) {
   const double *g_ev = ev + S.g_off;
 #pragma unroll
-  for (int j0 = 0; j0 < MAX_INST; j0 += GRP_INST) {
+  for (int j0 = 0; j0 < MAX_INST; j0 += GI) {
     if (j0 < S.n_inst4) {
-      double sv[GRP_INST], gv[GRP_INST];
+      double sv[GI], gv[GI];
 #pragma unroll
-      for (int u = 0; u < GRP_INST; ++u) {
+      for (int u = 0; u < GI; ++u) {
         sv[u] = __ldg(ev + S.inst_soff[j0 + u]);
         gv[u] = ldg_stream1(g_ev + (j0 + u) * 32);
       }
 #pragma unroll
-      for (int u = 0; u < GRP_INST; ++u) sTl[(j0 + u) * 32] = breit_wigner(LP.m0sq[j0 + u], LP.gam[j0 + u], sv[u], gv[u]);
+      for (int u = 0; u < GI; ++u) sTl[(j0 + u) * 32] = breit_wigner(LP.m0sq[j0 + u], LP.gam[j0 + u], sv[u], gv[u]);
     }
   }
 }
 // The f rows of the first term group, issued BEFORE the lineshape arithmetic so that they are in flight with it.
-__device__ __forceinline__ void prefetch_f(const StreamTab &S, const double *__restrict__ ev, double fv[GRP_TERM]) {
+template <int GT>
+__device__ __forceinline__ void prefetch_f(const StreamTab &S, const double *__restrict__ ev, double (&fv)[GT]) {
   const double *f_ev = ev + S.f_off;
 #pragma unroll
-  for (int u = 0; u < GRP_TERM; ++u) fv[u] = ldg_stream1(f_ev + u * 32);
+  for (int u = 0; u < GT; ++u) fv[u] = ldg_stream1(f_ev + u * 32);
 }
 // Component products summed into coupling columns: a_kappa = sum_{k in kappa} f_k T_{R1(k)} T_{R2(k)} (terms are sorted
 // by coupling).  flush(kappa, a_kappa) is called once per non-empty column, in order.  fv: first group, preloaded.
-template <class Flush>
+template <int GT, class Flush>
 __device__ __forceinline__ void columns_from_scratch(const StreamTab &S, const double *__restrict__ ev, const double2 *sTl,
-                                                     double fv[GRP_TERM], Flush &&flush) {
+                                                     double (&fv)[GT], Flush &&flush) {
   const double *f_ev = ev + S.f_off;
   double2 acc = make_double2(0.0, 0.0);
 #pragma unroll
-  for (int k0 = 0; k0 < MAX_TERMS; k0 += GRP_TERM) {
+  for (int k0 = 0; k0 < MAX_TERMS; k0 += GT) {
     if (k0 < S.n_terms4) {
       if (k0 > 0) {
 #pragma unroll
-        for (int u = 0; u < GRP_TERM; ++u) fv[u] = ldg_stream1(f_ev + (k0 + u) * 32);
+        for (int u = 0; u < GT; ++u) fv[u] = ldg_stream1(f_ev + (k0 + u) * 32);
       }
 #pragma unroll
-      for (int u = 0; u < GRP_TERM; ++u) {
+      for (int u = 0; u < GT; ++u) {
         const int k = k0 + u;
         double2 T = cmul(sTl[S.term_t0[k]], sTl[S.term_t1[k]]);
         acc.x = fma(fv[u], T.x, acc.x);
@@ -371,7 +377,8 @@ __device__ __forceinline__ const double *tile_event(const double *__restrict__ c
 // coupling column back (for the coupling-only calls that follow) and finishes the NLL in the same pass.
 inline size_t colnll_smem_bytes(int n_inst4) { return STREAM_WARPS * lineshape_scratch_bytes(n_inst4); }
 
-template <bool SMALL, bool RES = false>
+// GI, GT: load-batch sizes (instances, terms) of the model's size class; the tables are padded to multiples of them.
+template <bool SMALL, bool RES, int GI, int GT>
 __global__ void __launch_bounds__(STREAM_BLOCK, STREAM_BLOCKS_PER_SM)
 colnll_stream_kernel(const __grid_constant__ StreamTab S, const __grid_constant__ LineParams LP,
                      const double *__restrict__ cache, const double *__restrict__ t, int64_t ld, int64_t n,
@@ -387,15 +394,16 @@ colnll_stream_kernel(const __grid_constant__ StreamTab S, const __grid_constant_
   const double yG = R.y * R.Gamma, xG = R.x * R.Gamma;
   const int64_t stride = (int64_t)gridDim.x * STREAM_BLOCK;
   if (RES) block_phase_space_sums(R, G, S.n_kc, inv_n_norm, s_S);
+  int64_t i = (int64_t)blockIdx.x * STREAM_BLOCK + threadIdx.x;
 #pragma unroll 1
-  for (int64_t i = (int64_t)blockIdx.x * STREAM_BLOCK + threadIdx.x; i < n; i += stride) {
-    double ti = RES ? 0.0 : ldg_stream1(t + i);          // RES: t points at the time rows [8][ld]
+  for (; i < n; i += stride) {
+    double ti = RES ? 0.0 : ldg_stream1(t + i);            // RES: t points at the time rows [8][ld]
     const double *ev = tile_event(cache, S.R, i);
-    double fv[GRP_TERM];
-    prefetch_f(S, ev, fv);
-    lineshapes_to_scratch(S, LP, ev, sTl);
+    double fv[GT];
+    prefetch_f<GT>(S, ev, fv);
+    lineshapes_to_scratch<GI>(S, LP, ev, sTl);
     double2 A = make_double2(0.0, 0.0), Ab = make_double2(0.0, 0.0);
-    columns_from_scratch(S, ev, sTl, fv, [&](int kap, double2 col) {
+    columns_from_scratch<GT>(S, ev, sTl, fv, [&](int kap, double2 col) {
       a[(int64_t)kap * ld + i] = col;
       amp_add(A, Ab, R.c[kap][0], R.c[kap][1], R.cbar[kap][0], R.cbar[kap][1], col);
     });
@@ -429,7 +437,7 @@ __device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double
                : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
 }
 
-template <int NB>
+template <int NB, int GI, int GT>
 __global__ void __launch_bounds__(STREAM_BLOCK, STREAM_BLOCKS_PER_SM)
 gram_stream_kernel(const __grid_constant__ StreamTab S, const __grid_constant__ LineParams LP,
                    const double *__restrict__ cache, int64_t n,
@@ -453,22 +461,9 @@ gram_stream_kernel(const __grid_constant__ StreamTab S, const __grid_constant__ 
 #pragma unroll
   for (int q = 0; q < NP; ++q) acc[q][0] = acc[q][1] = 0.0;
   const int64_t stride = (int64_t)gridDim.x * STREAM_BLOCK;
-  // whole warps iterate together (the MMA is warp-wide); lanes beyond n contribute zero rows
-#pragma unroll 1
-  for (int64_t i0 = (int64_t)blockIdx.x * STREAM_BLOCK + warp * 32; i0 < n; i0 += stride) {
-    const int64_t i = i0 + lane;
-    if (i < n) {
-      const double *ev = tile_event(cache, S.R, i);
-      double wj = S.w_off >= 0 ? ldg_stream1(ev + S.w_off) : 1.0;
-      double fv[GRP_TERM];
-      prefetch_f(S, ev, fv);
-      lineshapes_to_scratch(S, LP, ev, sTl);
-      columns_from_scratch(S, ev, sTl, fv, [&](int kap, double2 col) { *reinterpret_cast<double2 *>(row + 2 * kap) = col; });
-      row[F] = wj;
-    } else {
-      for (int c = 0; c < 2 * KC; ++c) row[c] = 0.0;
-      row[F] = 0.0;
-    }
+  // whole warps iterate together (the MMA is warp-wide).  The cache is allocated and zero-filled in whole tiles, so the
+  // lanes of a ragged last tile compute on zeros: f = 0 gives zero columns, and their weight is forced to 0.
+  auto mma_tile = [&]() {
     __syncwarp();
     const double *base = Xs + (lane & 3) * STRIDE + (lane >> 2);
 #pragma unroll
@@ -487,6 +482,18 @@ gram_stream_kernel(const __grid_constant__ StreamTab S, const __grid_constant__ 
       }
     }
     __syncwarp();                                        // the X tile is free again
+  };
+  int64_t i0 = (int64_t)blockIdx.x * STREAM_BLOCK + warp * 32;
+#pragma unroll 1
+  for (; i0 < n; i0 += stride) {
+    const double *ev = tile_event(cache, S.R, i0 + lane);
+    double wj = S.w_off >= 0 ? ldg_stream1(ev + S.w_off) : 1.0;
+    double fv[GT];
+    prefetch_f<GT>(S, ev, fv);
+    lineshapes_to_scratch<GI>(S, LP, ev, sTl);
+    columns_from_scratch<GT>(S, ev, sTl, fv, [&](int kap, double2 col) { *reinterpret_cast<double2 *>(row + 2 * kap) = col; });
+    row[F] = i0 + lane < n ? wj : 0.0;
+    mma_tile();
   }
   __syncthreads();                                       // all scratch is free
   // block reduction in warp order, block partial = upper 8x8 blocks of X^T W X

@@ -10,8 +10,6 @@ constexpr int MAX_INST = 24;   // de-duplicated lineshape instances (PAPER.md li
 constexpr int MAX_TERMS = 32;
 constexpr int MAX_KC = 16;
 constexpr int MAX_RES = 16;
-constexpr int GRP_INST = 12;   // lineshape instances per load batch of the per-call kernels (2 loads each in flight)
-constexpr int GRP_TERM = 16;   // terms per load batch
 
 enum { SF_NONRES = 0, SF_VV_S = 1, SF_VV_P = 2, SF_VV_D = 3, SF_AP_S = 4, SF_TP_D = 5 };
 
@@ -55,7 +53,7 @@ struct ModelTab {
 // element (row r, event i) at ((i >> 5) * R + r) * 32 + (i & 31).  A warp working on one tile therefore addresses every
 // row as tile base + lane + CONSTANT, and the whole tile is one contiguous R * 256-byte region of HBM.
 // Every table entry is a 32-bit word so that an unrolled loop uses it as an immediate-indexed constant-bank operand.
-// Instances and terms are padded to multiples of GRP_INST / GRP_TERM (group-level guards only) with all-zero rows: a padded instance
+// Instances and terms are padded to multiples of the size class's load-batch sizes (GI, GT) (group-level guards only) with all-zero rows: a padded instance
 // reads s row 0 and m0sq = -1, gam = 0 (finite, unused); a padded term has f = 0 and the unit lineshape slot.
 struct StreamTab {
   int n_inst4, n_terms4, n_kc;     // padded counts

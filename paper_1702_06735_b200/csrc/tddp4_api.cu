@@ -11,6 +11,7 @@
 #include <cstring>
 #include <limits>
 #include <string>
+#include <type_traits>
 #include <vector>
 
 #include "../../include/tddp4.h"
@@ -46,6 +47,7 @@ struct tddp4 {
   bool own_stream = false;
   ModelTab M{};
   StreamTab S{};                     // the same model, flattened for the per-call kernels
+  int size_class = 0;                // load-batch sizes (GI, GT) of the per-call kernels: 0 (4,4), 1 (8,8), 2 (12,16)
   std::vector<tddp4_res> res;
   std::vector<tddp4_term> terms;   // caller's order
   double t_lo = 0.0, t_hi = INFINITY;
@@ -213,6 +215,16 @@ int stream_grid(const tddp4 *h, int64_t n) {
 // algorithmic bytes per event of the step-1 caches a dirty call has to read: s rows in use, g rows, f rows
 double static_bytes_per_event(const tddp4 *h) { return 8.0 * (h->M.n_su + h->M.n_inst + h->M.n_terms); }
 
+// size classes of the per-call kernels (stream_kernels.cuh): f(GI, GT) with compile-time constants
+template <class F>
+auto with_size_class(int cls, F &&f) {
+  switch (cls) {
+    case 0: return f(std::integral_constant<int, 4>{}, std::integral_constant<int, 4>{});
+    case 1: return f(std::integral_constant<int, 8>{}, std::integral_constant<int, 8>{});
+    default: return f(std::integral_constant<int, 12>{}, std::integral_constant<int, 16>{});
+  }
+}
+
 template <int NB>
 int launch_gram(tddp4 *h, const EventSet &e) {
   const ModelTab &M = h->M;
@@ -223,8 +235,11 @@ int launch_gram(tddp4 *h, const EventSet &e) {
   S.R = e.R;
   S.w_off = e.w ? (M.n_sys + S.n_inst4 + S.n_terms4) * 32 : -1;
   Prof p(h, TDDP4_K_GRAM, (double)e.n * (static_bytes_per_event(h) + (e.w ? 8.0 : 0.0)));
-  gram_stream_kernel<NB><<<grid, STREAM_BLOCK, gram_smem_bytes(NB, S.n_inst4), h->stream>>>(S, h->LP, e.cache, e.n, h->partials,
-                                                                                       h->ticket, h->G);
+  with_size_class(h->size_class, [&](auto ni, auto nt) {
+    gram_stream_kernel<NB, decltype(ni)::value, decltype(nt)::value>
+        <<<grid, STREAM_BLOCK, gram_smem_bytes(NB, S.n_inst4), h->stream>>>(S, h->LP, e.cache, e.n, h->partials, h->ticket, h->G);
+    return 0;
+  });
   return TDDP4_OK;
 }
 
@@ -280,15 +295,20 @@ int launch_colnll(tddp4 *h, const EventSet &e, double inv_n, double *result, boo
   S.R = e.R;
   size_t smem = colnll_smem_bytes(S.n_inst4);
   Prof p(h, TDDP4_K_COLNLL, (double)e.n * (static_bytes_per_event(h) + (h->use_resolution ? 64.0 : 8.0) + 16.0 * M.n_kc));
-  if (h->use_resolution)
-    colnll_stream_kernel<false, true><<<grid, STREAM_BLOCK, smem, h->stream>>>(S, h->LP, e.cache, e.tr, e.ld, e.n, e.a, h->RP, h->G,
-                                                                              inv_n, 0.0, h->partials, h->ticket, result);
-  else if (small)
-    colnll_stream_kernel<true><<<grid, STREAM_BLOCK, smem, h->stream>>>(S, h->LP, e.cache, e.t, e.ld, e.n, e.a, h->RP, h->G, inv_n,
-                                                                       e.sum_t, h->partials, h->ticket, result);
-  else
-    colnll_stream_kernel<false><<<grid, STREAM_BLOCK, smem, h->stream>>>(S, h->LP, e.cache, e.t, e.ld, e.n, e.a, h->RP, h->G, inv_n,
-                                                                        e.sum_t, h->partials, h->ticket, result);
+  const int mode = h->use_resolution ? 2 : (small ? 1 : 0);
+  const double sum_t = h->use_resolution ? 0.0 : e.sum_t;
+  const double *tp = h->use_resolution ? e.tr : e.t;
+  with_size_class(h->size_class, [&](auto ni, auto nt) {
+    constexpr int NI = decltype(ni)::value, NT = decltype(nt)::value;
+#define COLNLL_LAUNCH(SM, RS)                                                                                                  \
+  colnll_stream_kernel<SM, RS, NI, NT><<<grid, STREAM_BLOCK, smem, h->stream>>>(S, h->LP, e.cache, tp, e.ld, e.n, e.a, h->RP, h->G, \
+                                                                                inv_n, sum_t, h->partials, h->ticket, result)
+    if (mode == 2) COLNLL_LAUNCH(false, true);
+    else if (mode == 1) COLNLL_LAUNCH(true, false);
+    else COLNLL_LAUNCH(false, false);
+#undef COLNLL_LAUNCH
+    return 0;
+  });
   return TDDP4_OK;
 }
 
@@ -462,7 +482,15 @@ int tddp4_create(const tddp4_model_desc *desc, tddp4 **out) {
   {   // flat tables of the per-call kernels (tables.h): padded to groups of 4, all entries 32-bit
     StreamTab &S = h->S;
     memset(&S, 0, sizeof S);
-    S.n_inst4 = (M.n_inst + GRP_INST - 1) / GRP_INST * GRP_INST; S.n_terms4 = (M.n_terms + GRP_TERM - 1) / GRP_TERM * GRP_TERM;
+    // size class = load-batch sizes (GI, GT): the one with the fewest padded rows, the deeper batches on a tie
+    static const int GI[3] = {4, 8, 12}, GT[3] = {4, 8, 16};
+    int best = -1;
+    for (int c = 0; c < 3; ++c) {
+      int ni = (M.n_inst + GI[c] - 1) / GI[c] * GI[c], nt = (M.n_terms + GT[c] - 1) / GT[c] * GT[c];
+      if (ni > MAX_INST || nt > MAX_TERMS) continue;
+      if (best < 0 || ni + nt <= S.n_inst4 + S.n_terms4) { best = c; S.n_inst4 = ni; S.n_terms4 = nt; }
+    }
+    h->size_class = best;
     S.n_kc = M.n_kc;
     S.g_off = M.n_sys * 32; S.f_off = (M.n_sys + S.n_inst4) * 32; S.w_off = -1;
     S.R = M.n_sys + S.n_inst4 + S.n_terms4;              // + 1 for a weighted event set, fixed at launch
@@ -506,13 +534,17 @@ int tddp4_create(const tddp4_model_desc *desc, tddp4 **out) {
     int NB = (KC + 3) / 4;
     size_t limit = prop.sharedMemPerBlockOptin - 1024, sc = colnll_smem_bytes(h->S.n_inst4), sg = gram_smem_bytes(NB, h->S.n_inst4);
     if (sc > limit || sg > limit) return bail(fail(h, TDDP4_ERR_ARG, "model too large for the shared-memory scratch of the streaming kernels"));
-    cudaFuncSetAttribute(colnll_stream_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sc);
-    cudaFuncSetAttribute(colnll_stream_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sc);
-    cudaFuncSetAttribute(colnll_stream_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sc);
-    if (NB == 1) cudaFuncSetAttribute(gram_stream_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sg);
-    else if (NB == 2) cudaFuncSetAttribute(gram_stream_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sg);
-    else if (NB == 3) cudaFuncSetAttribute(gram_stream_kernel<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sg);
-    else cudaFuncSetAttribute(gram_stream_kernel<4>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sg);
+    with_size_class(h->size_class, [&](auto ni, auto nt) {
+      constexpr int NI = decltype(ni)::value, NT = decltype(nt)::value;
+      cudaFuncSetAttribute(colnll_stream_kernel<true, false, NI, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sc);
+      cudaFuncSetAttribute(colnll_stream_kernel<false, false, NI, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sc);
+      cudaFuncSetAttribute(colnll_stream_kernel<false, true, NI, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sc);
+      if (NB == 1) cudaFuncSetAttribute(gram_stream_kernel<1, NI, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sg);
+      else if (NB == 2) cudaFuncSetAttribute(gram_stream_kernel<2, NI, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sg);
+      else if (NB == 3) cudaFuncSetAttribute(gram_stream_kernel<3, NI, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sg);
+      else cudaFuncSetAttribute(gram_stream_kernel<4, NI, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sg);
+      return 0;
+    });
   }
   cudaFuncSetAttribute(terms_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(MAX_INST * COL_BLOCK * sizeof(double2)));
   *out = h;
