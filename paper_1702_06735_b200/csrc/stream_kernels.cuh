@@ -33,6 +33,12 @@ __device__ __forceinline__ double ldg_stream1(const double *p) {
   return v;
 }
 
+// One lane asks the memory system to bring a whole contiguous region into L2 (no destination, no register, no scoreboard):
+// the tile-major cache makes the NEXT tile of a warp one such region, so its loads later hit L2 instead of HBM.
+__device__ __forceinline__ void prefetch_l2_bulk(const void *p, uint32_t bytes) {
+  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
+}
+
 // ------------------------------------------------------------------------------------------------
 // sum_i log B_i without a log per event: B = m 2^e with m in [1,2); the mantissas are multiplied up and the
 // exponents added as integers.  Partial results are merged by multiplication too (thread -> warp -> block -> grid,
@@ -397,6 +403,7 @@ colnll_stream_kernel(const __grid_constant__ StreamTab S, const __grid_constant_
   int64_t i = (int64_t)blockIdx.x * STREAM_BLOCK + threadIdx.x;
 #pragma unroll 1
   for (; i < n; i += stride) {
+    if (lane == 0 && i + stride < n) prefetch_l2_bulk(tile_event(cache, S.R, i + stride), (uint32_t)S.R * 256u);
     double ti = RES ? 0.0 : ldg_stream1(t + i);            // RES: t points at the time rows [8][ld]
     const double *ev = tile_event(cache, S.R, i);
     double fv[GT];
@@ -486,6 +493,7 @@ gram_stream_kernel(const __grid_constant__ StreamTab S, const __grid_constant__ 
   int64_t i0 = (int64_t)blockIdx.x * STREAM_BLOCK + warp * 32;
 #pragma unroll 1
   for (; i0 < n; i0 += stride) {
+    if (lane == 0 && i0 + stride < n) prefetch_l2_bulk(tile_event(cache, S.R, i0 + stride), (uint32_t)S.R * 256u);
     const double *ev = tile_event(cache, S.R, i0 + lane);
     double wj = S.w_off >= 0 ? ldg_stream1(ev + S.w_off) : 1.0;
     double fv[GT];
