@@ -70,7 +70,9 @@ __device__ __forceinline__ double conv_exp_real(double t, double lam, double sig
   double ts = t / sigma;
   double g0 = exp(-0.5 * ts * ts);
   if (u >= 0.0) return 0.5 * g0 * erfcx(u);
-  return exp(0.5 * lam * lam * sigma * sigma - lam * t) - 0.5 * g0 * erfcx(-u);
+  double E = exp(0.5 * lam * lam * sigma * sigma - lam * t);
+  if (g0 < 1e-18 * E) return E;                               // correction below half an ulp (erfcx <= 1): same bits
+  return E - 0.5 * g0 * erfcx(-u);
 }
 
 // h for complex lambda = (lr, li)
@@ -83,11 +85,12 @@ __device__ __forceinline__ double2 conv_exp_complex(const FaddTab &F, double t, 
     double2 w = faddeeva_upper(F, make_double2(-ui, ur));     // i u
     return make_double2(0.5 * g0 * w.x, 0.5 * g0 * w.y);
   }
-  double2 w = faddeeva_upper(F, make_double2(ui, -ur));       // -i u
   double s2 = sigma * sigma;
   double ere = 0.5 * (lr * lr - li * li) * s2 - lr * t, eim = lr * li * s2 - li * t;
   double mag = exp(ere), sn, cs;
   sincos(eim, &sn, &cs);
+  if (g0 < 1e-18 * mag * fmin(fabs(cs), fabs(sn))) return make_double2(mag * cs, mag * sn);   // |w| <= 1: below half an ulp
+  double2 w = faddeeva_upper(F, make_double2(ui, -ur));       // -i u
   return make_double2(mag * cs - 0.5 * g0 * w.x, mag * sn - 0.5 * g0 * w.y);
 }
 

@@ -173,18 +173,43 @@ __device__ __forceinline__ void nll_finish(const RateParams &R, int KC, int64_t 
   __syncthreads();
   if (!last) return;
   __threadfence();
+  // last block: every thread takes the block partials b = tid, tid + 256, ... (loads independent, issued together), warps
+  // merge by butterfly, thread 0 merges the warps in order; warp 7 also evaluates N.  Fixed order: same bits every run.
   MantAcc m;
-  if (warp == 0) {
-    for (unsigned b = lane; b < gridDim.x; b += 32) {
+  {
+    constexpr int PER = 8;                                // up to 8 * 256 = 2048 blocks
+    double pp[PER], pe[PER], pb[PER];
+#pragma unroll
+    for (int r = 0; r < PER; ++r) {
+      unsigned b = threadIdx.x + r * STREAM_BLOCK;
+      bool ok = b < gridDim.x;
+      pp[r] = ok ? __ldcg(partials + 3 * b) : 1.0;
+      pe[r] = ok ? __ldcg(partials + 3 * b + 1) : 0.0;
+      pb[r] = ok ? __ldcg(partials + 3 * b + 2) : 0.0;
+    }
+#pragma unroll
+    for (int r = 0; r < PER; ++r) {
+      m.merge(pp[r], (long long)pe[r], (int)pb[r]);
+      m.renorm();
+    }
+    for (unsigned b = threadIdx.x + PER * STREAM_BLOCK; b < gridDim.x; b += STREAM_BLOCK) {   // larger grids: the slow way
       m.merge(__ldcg(partials + 3 * b), (long long)__ldcg(partials + 3 * b + 1), (int)__ldcg(partials + 3 * b + 2));
       m.renorm();
     }
-    warp_merge(m);
-  } else if (warp == 1) {
+  }
+  warp_merge(m);
+  __syncthreads();                                        // s_p .. s_b of the first stage are free
+  if (lane == 0) { s_p[warp] = m.prod; s_e[warp] = m.esum; s_b[warp] = m.bad; }
+  if (warp == STREAM_WARPS - 1) {
     double nv = norm_from_gram_warp(R, G, KC, inv_n);
     if (lane == 0) s_norm = nv;
   }
   __syncthreads();
+  if (threadIdx.x == 0) {
+    m = MantAcc();
+#pragma unroll
+    for (int w = 0; w < STREAM_WARPS; ++w) { m.merge(s_p[w], s_e[w], s_b[w]); m.renorm(); }
+  }
   if (threadIdx.x == 0) {
     double norm = s_norm;
     double s0 = log(m.prod) + 0.693147180559945309417 * (double)m.esum;
@@ -537,8 +562,22 @@ gram_stream_kernel(const __grid_constant__ StreamTab S, const __grid_constant__ 
   for (int e = tid; e < NB * NB * 64; e += STREAM_BLOCK) {
     int bi = e / (NB * 64), bj = (e / 64) % NB;
     if (bi > bj) continue;
+    // 16 independent chains (block b goes to chain b mod 16), chains added in index order: a fixed summation tree with
+    // 16 loads in flight instead of gridDim.x dependent L2 round trips at the tail of the kernel
+    double part[16];
+#pragma unroll
+    for (int c = 0; c < 16; ++c) part[c] = 0.0;
+    unsigned b = 0;
+    for (; b + 16 <= gridDim.x; b += 16) {
+#pragma unroll
+      for (int c = 0; c < 16; ++c) part[c] += __ldcg(partials + (int64_t)(b + c) * NB * NB * 64 + e);
+    }
+#pragma unroll
+    for (int c = 0; c < 16; ++c)
+      if (b + c < gridDim.x) part[c] += __ldcg(partials + (int64_t)(b + c) * NB * NB * 64 + e);
     double sum = 0.0;
-    for (unsigned b = 0; b < gridDim.x; ++b) sum += __ldcg(partials + (int64_t)b * NB * NB * 64 + e);
+#pragma unroll
+    for (int c = 0; c < 16; ++c) sum += part[c];
     XtX[e] = sum;
   }
   __syncthreads();
