@@ -33,6 +33,14 @@ __device__ __forceinline__ double ldg_stream1(const double *p) {
   return v;
 }
 
+// Programmatic dependent launch (the host launches the per-call kernels with programmatic stream serialization): a kernel
+// lets its successor's blocks become resident as soon as its own blocks exit, so the successor's launch latency, ramp-up
+// and read-only streaming overlap this kernel's tail and final reduction.  pdl_wait() blocks until the predecessor grid
+// has completed and its memory is visible; it sits in front of the first access to anything the predecessor may read or
+// write (partials, ticket, G, result slots; the columns when the predecessor or this kernel writes them).
+__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;"); }
+__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+
 // One lane asks the memory system to bring a whole contiguous region into L2 (no destination, no register, no scoreboard):
 // the tile-major cache makes the NEXT tile of a warp one such region, so its loads later hit L2 instead of HBM.
 __device__ __forceinline__ void prefetch_l2_bulk(const void *p, uint32_t bytes) {
@@ -229,8 +237,10 @@ template <int KC, bool SMALL>
 __global__ void __launch_bounds__(STREAM_BLOCK, STREAM_BLOCKS_PER_SM)
 nll_stream_kernel(const double2 *__restrict__ a, const double *__restrict__ t, int64_t ld, int64_t n,
                   const __grid_constant__ RateParams R, const double *__restrict__ G, double inv_n_norm, double sum_t,
-                  double *__restrict__ partials, unsigned int *ticket, double *__restrict__ result) {
+                  double *__restrict__ partials, unsigned int *ticket, double *__restrict__ result, int early_wait) {
   constexpr int UNR = KC <= 8 ? 2 : 1;   // wider models: one event per iteration, or the columns spill
+  pdl_launch_dependents();
+  if (early_wait) pdl_wait();            // the predecessor wrote the columns
   MantAcc la;
   const double yG = R.y * R.Gamma, xG = R.x * R.Gamma;
   const int64_t stride = (int64_t)gridDim.x * STREAM_BLOCK;
@@ -264,6 +274,7 @@ nll_stream_kernel(const double2 *__restrict__ a, const double *__restrict__ t, i
     for (int c = 0; c < KC; ++c) amp_add(A, Ab, R.c[c][0], R.c[c][1], R.cbar[c][0], R.cbar[c][1], v[c]);
     la.add(bracket<SMALL>(A, Ab, yG * ti, xG * ti));
   }
+  if (!early_wait) pdl_wait();
   nll_finish(R, KC, n, sum_t, la, G, inv_n_norm, partials, ticket, result);
 }
 
@@ -290,6 +301,8 @@ nll_res_kernel(const double2 *__restrict__ a, const double *__restrict__ tr, int
                double *__restrict__ partials, unsigned int *ticket, double *__restrict__ result) {
   __shared__ double s_S[4];
   MantAcc la;
+  pdl_launch_dependents();
+  pdl_wait();                              // G is read first thing
   block_phase_space_sums(R, G, KC, inv_n_norm, s_S);
   const int64_t stride = (int64_t)gridDim.x * STREAM_BLOCK;
 #pragma unroll 1
@@ -415,9 +428,11 @@ colnll_stream_kernel(const __grid_constant__ StreamTab S, const __grid_constant_
                      const double *__restrict__ cache, const double *__restrict__ t, int64_t ld, int64_t n,
                      double2 *__restrict__ a,
                      const __grid_constant__ RateParams R, const double *__restrict__ G, double inv_n_norm, double sum_t,
-                     double *__restrict__ partials, unsigned int *ticket, double *__restrict__ result) {
+                     double *__restrict__ partials, unsigned int *ticket, double *__restrict__ result, int early_wait) {
   extern __shared__ __align__(16) char smem_raw[];
   __shared__ double s_S[4];
+  pdl_launch_dependents();
+  if (RES || early_wait) pdl_wait();       // the predecessor reads the columns this kernel rewrites (or RES: G first)
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   double2 *sTl = reinterpret_cast<double2 *>(smem_raw + (size_t)warp * lineshape_scratch_bytes(S.n_inst4)) + lane;
   sTl[S.n_inst4 * 32] = make_double2(1.0, 0.0);        // unit lineshape slot
@@ -442,6 +457,7 @@ colnll_stream_kernel(const __grid_constant__ StreamTab S, const __grid_constant_
     if (RES) la.add(resolved_prob(A, Ab, t + i, ld, s_S));
     else la.add(bracket<SMALL>(A, Ab, yG * ti, xG * ti));
   }
+  if (!(RES || early_wait)) pdl_wait();
   nll_finish<RES>(R, S.n_kc, n, sum_t, la, G, inv_n_norm, partials, ticket, result);
 }
 
@@ -480,6 +496,7 @@ gram_stream_kernel(const __grid_constant__ StreamTab S, const __grid_constant__ 
   __shared__ bool last;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int KC = S.n_kc;
+  pdl_launch_dependents();                 // this kernel reads only the static cache until its final reduction
   const size_t t_bytes = align_up(lineshape_scratch_bytes(S.n_inst4), 128);
   const size_t x_bytes = align_up((size_t)32 * STRIDE * sizeof(double), 128);
   char *scratch = smem_raw + (size_t)warp * (t_bytes + x_bytes);
@@ -543,6 +560,7 @@ gram_stream_kernel(const __grid_constant__ StreamTab S, const __grid_constant__ 
       }
   }
   __syncthreads();
+  pdl_wait();                              // partials, ticket and G may still be in use by the predecessor
   for (int e = tid; e < NB * NB * 64; e += STREAM_BLOCK) {
     int bi = e / (NB * 64), bj = (e / 64) % NB;
     if (bi > bj) continue;

@@ -47,6 +47,7 @@ struct tddp4 {
   bool own_stream = false;
   ModelTab M{};
   StreamTab S{};                     // the same model, flattened for the per-call kernels
+  int prev_kind = 0;                 // last per-call kernel enqueued with nothing after it: 0 none/other, 1 NLL, 2 COLNLL, 3 GRAM
   int size_class = 0;                // load-batch sizes (GI, GT) of the per-call kernels: 0 (4,4), 1 (8,8), 2 (12,16)
   std::vector<tddp4_res> res;
   std::vector<tddp4_term> terms;   // caller's order
@@ -225,6 +226,24 @@ auto with_size_class(int cls, F &&f) {
   }
 }
 
+// launch with programmatic stream serialization (stream_kernels.cuh, pdl_*): the kernel may become resident while its
+// predecessor in the stream drains; it synchronises with it through griddepcontrol.wait
+template <class... KArgs, class... Args>
+void launch_pdl(void (*kernel)(KArgs...), int grid, int block, size_t smem, cudaStream_t stream, Args &&...args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)grid);
+  cfg.blockDim = dim3((unsigned)block);
+  cfg.dynamicSmemBytes = smem;
+  cfg.stream = stream;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = at;
+  cfg.numAttrs = 1;
+  cudaLaunchKernelEx(&cfg, kernel, std::forward<Args>(args)...);
+}
+enum { PREV_NONE = 0, PREV_NLL = 1, PREV_COLNLL = 2, PREV_GRAM = 3 };
+
 template <int NB>
 int launch_gram(tddp4 *h, const EventSet &e) {
   const ModelTab &M = h->M;
@@ -236,10 +255,11 @@ int launch_gram(tddp4 *h, const EventSet &e) {
   S.w_off = e.w ? (M.n_sys + S.n_inst4 + S.n_terms4) * 32 : -1;
   Prof p(h, TDDP4_K_GRAM, (double)e.n * (static_bytes_per_event(h) + (e.w ? 8.0 : 0.0)));
   with_size_class(h->size_class, [&](auto ni, auto nt) {
-    gram_stream_kernel<NB, decltype(ni)::value, decltype(nt)::value>
-        <<<grid, STREAM_BLOCK, gram_smem_bytes(NB, S.n_inst4), h->stream>>>(S, h->LP, e.cache, e.n, h->partials, h->ticket, h->G);
+    launch_pdl(gram_stream_kernel<NB, decltype(ni)::value, decltype(nt)::value>, grid, STREAM_BLOCK,
+               gram_smem_bytes(NB, S.n_inst4), h->stream, S, h->LP, (const double *)e.cache, e.n, h->partials, h->ticket, h->G);
     return 0;
   });
+  h->prev_kind = PREV_GRAM;
   return TDDP4_OK;
 }
 
@@ -267,12 +287,15 @@ int launch_nll(tddp4 *h, const EventSet &e, double inv_n, double *result, bool s
   int rc = ensure_partials(h, (size_t)3 * grid + 16);
   if (rc) return rc;
   Prof p(h, TDDP4_K_NLL, (double)e.n * (16.0 * KC + 8.0));
+  // the columns and t are untouched by a preceding NLL or Gram kernel: only the final reduction has to wait for it
+  const int early = !(h->prev_kind == PREV_NLL || h->prev_kind == PREV_GRAM);
   if (small)
-    nll_stream_kernel<KC, true><<<grid, STREAM_BLOCK, 0, h->stream>>>(e.a, e.t, e.ld, e.n, h->RP, h->G, inv_n, e.sum_t, h->partials,
-                                                                     h->ticket, result);
+    launch_pdl(nll_stream_kernel<KC, true>, grid, STREAM_BLOCK, 0, h->stream, (const double2 *)e.a, (const double *)e.t, e.ld, e.n, h->RP,
+               (const double *)h->G, inv_n, e.sum_t, h->partials, h->ticket, result, early);
   else
-    nll_stream_kernel<KC, false><<<grid, STREAM_BLOCK, 0, h->stream>>>(e.a, e.t, e.ld, e.n, h->RP, h->G, inv_n, e.sum_t, h->partials,
-                                                                      h->ticket, result);
+    launch_pdl(nll_stream_kernel<KC, false>, grid, STREAM_BLOCK, 0, h->stream, (const double2 *)e.a, (const double *)e.t, e.ld, e.n, h->RP,
+               (const double *)h->G, inv_n, e.sum_t, h->partials, h->ticket, result, early);
+  h->prev_kind = PREV_NLL;
   return TDDP4_OK;
 }
 
@@ -282,7 +305,9 @@ int launch_nll_res(tddp4 *h, const EventSet &e, double inv_n, double *result) {
   int rc = ensure_partials(h, (size_t)3 * grid + 16);
   if (rc) return rc;
   Prof p(h, TDDP4_K_NLL, (double)e.n * (16.0 * KC + 64.0));
-  nll_res_kernel<KC><<<grid, STREAM_BLOCK, 0, h->stream>>>(e.a, e.tr, e.ld, e.n, h->RP, h->G, inv_n, h->partials, h->ticket, result);
+  launch_pdl(nll_res_kernel<KC>, grid, STREAM_BLOCK, 0, h->stream, (const double2 *)e.a, (const double *)e.tr, e.ld, e.n, h->RP,
+             (const double *)h->G, inv_n, h->partials, h->ticket, result);
+  h->prev_kind = PREV_NLL;
   return TDDP4_OK;
 }
 
@@ -296,19 +321,21 @@ int launch_colnll(tddp4 *h, const EventSet &e, double inv_n, double *result, boo
   size_t smem = colnll_smem_bytes(S.n_inst4);
   Prof p(h, TDDP4_K_COLNLL, (double)e.n * (static_bytes_per_event(h) + (h->use_resolution ? 64.0 : 8.0) + 16.0 * M.n_kc));
   const int mode = h->use_resolution ? 2 : (small ? 1 : 0);
+  const int early = h->prev_kind != PREV_GRAM;   // a Gram kernel neither reads nor writes the columns this kernel rewrites
   const double sum_t = h->use_resolution ? 0.0 : e.sum_t;
   const double *tp = h->use_resolution ? e.tr : e.t;
   with_size_class(h->size_class, [&](auto ni, auto nt) {
     constexpr int NI = decltype(ni)::value, NT = decltype(nt)::value;
 #define COLNLL_LAUNCH(SM, RS)                                                                                                  \
-  colnll_stream_kernel<SM, RS, NI, NT><<<grid, STREAM_BLOCK, smem, h->stream>>>(S, h->LP, e.cache, tp, e.ld, e.n, e.a, h->RP, h->G, \
-                                                                                inv_n, sum_t, h->partials, h->ticket, result)
+  launch_pdl(colnll_stream_kernel<SM, RS, NI, NT>, grid, STREAM_BLOCK, smem, h->stream, S, h->LP, (const double *)e.cache, tp, e.ld, e.n, \
+             e.a, h->RP, (const double *)h->G, inv_n, sum_t, h->partials, h->ticket, result, early)
     if (mode == 2) COLNLL_LAUNCH(false, true);
     else if (mode == 1) COLNLL_LAUNCH(true, false);
     else COLNLL_LAUNCH(false, false);
 #undef COLNLL_LAUNCH
     return 0;
   });
+  h->prev_kind = PREV_COLNLL;
   return TDDP4_OK;
 }
 
@@ -574,6 +601,7 @@ int tddp4_set_stream(tddp4 *h, void *cuda_stream) {
   if (h->stream) CU(cudaStreamSynchronize(h->stream));
   if (h->own_stream) { cudaStreamDestroy(h->stream); h->own_stream = false; }
   h->stream = (cudaStream_t)cuda_stream;
+  h->prev_kind = PREV_NONE;
   return TDDP4_OK;
 }
 
@@ -585,6 +613,7 @@ int tddp4_load_events(tddp4 *h, int which, int64_t n, int64_t ld_in, const doubl
   if (which == 0 && n > 0 && h->use_resolution && !sigma_t)
     return fail(h, TDDP4_ERR_ARG, "use_resolution = 1: the data sample needs per-event sigma_t");
   CU(cudaStreamSynchronize(h->stream));
+  h->prev_kind = PREV_NONE;
   EventSet &e = h->set[which];
   free_set(e);
   e.n = n;
