@@ -70,7 +70,8 @@ struct tddp4 {
   size_t partials_cap = 0;
   unsigned int *ticket = nullptr;
   double *results = nullptr;         // device [N_SLOTS][SLOT_DOUBLES]
-  double *results_host = nullptr;    // pinned mirror
+  double *results_host = nullptr;    // pinned host slots; the NLL kernels write them directly (zero-copy) ...
+  double *results_host_dev = nullptr; // ... through this device alias
   cudaEvent_t slot_event[N_SLOTS] = {nullptr};
   bool slot_used[N_SLOTS] = {false};
   double *batch_res = nullptr;       // device [batch_cap][SLOT_DOUBLES]
@@ -409,11 +410,16 @@ int enqueue_nll(tddp4 *h, double *result, double *prob) {
 }
 
 int enqueue_nll_slot(tddp4 *h, int slot, double *prob) {
-  double *result = h->results + (size_t)slot * SLOT_DOUBLES;
+  // without prob_out the last block writes its five doubles straight into the pinned host slot: no copy on the
+  // critical path of a synchronous call.  With prob_out the probability kernel reads N back from the slot, so the slot
+  // stays in device memory and is copied.
+  const bool direct = prob == nullptr;
+  double *result = (direct ? h->results_host_dev : h->results) + (size_t)slot * SLOT_DOUBLES;
   int rc = enqueue_nll(h, result, prob);
   if (rc) return rc;
-  CU(cudaMemcpyAsync(h->results_host + (size_t)slot * SLOT_DOUBLES, result, SLOT_DOUBLES * sizeof(double),
-                     cudaMemcpyDeviceToHost, h->stream));
+  if (!direct)
+    CU(cudaMemcpyAsync(h->results_host + (size_t)slot * SLOT_DOUBLES, result, SLOT_DOUBLES * sizeof(double),
+                       cudaMemcpyDeviceToHost, h->stream));
   CU(cudaEventRecord(h->slot_event[slot], h->stream));
   h->slot_used[slot] = true;
   return TDDP4_OK;
@@ -549,7 +555,8 @@ int tddp4_create(const tddp4_model_desc *desc, tddp4 **out) {
   bool ok = cudaMalloc(&h->G, sizeof(double) * 2 * KC * KC) == cudaSuccess &&
             cudaMalloc(&h->ticket, sizeof(unsigned int)) == cudaSuccess &&
             cudaMalloc(&h->results, sizeof(double) * (N_SLOTS + 1) * SLOT_DOUBLES) == cudaSuccess &&
-            cudaMallocHost(&h->results_host, sizeof(double) * N_SLOTS * SLOT_DOUBLES) == cudaSuccess &&
+            cudaHostAlloc(&h->results_host, sizeof(double) * N_SLOTS * SLOT_DOUBLES, cudaHostAllocMapped) == cudaSuccess &&
+            cudaHostGetDevicePointer((void **)&h->results_host_dev, h->results_host, 0) == cudaSuccess &&
             cudaMalloc(&h->gen_scalars, sizeof(unsigned long long) * 2) == cudaSuccess &&
             cudaMemset(h->ticket, 0, sizeof(unsigned int)) == cudaSuccess &&
             cudaMemset(h->G, 0, sizeof(double) * 2 * KC * KC) == cudaSuccess;
