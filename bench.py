@@ -262,6 +262,22 @@ def run_ours(args):
         for k in ktab:
             ktab[k]["traffic"] = tr.get(k)
 
+    # ---- analytic gradient: one pass against the 2 (4 K_c + 2) NLL calls of a numerical gradient ----
+    grad = {}
+    try:
+        h.set_params(p0)
+        h.nll_grad()
+        h.profile(True)
+        h.profile_reset()
+        for _ in range(20):
+            h.nll_grad()
+        gms, gn, gby = h.profile_read()["nll_grad"]
+        h.profile(False)
+        grad = {"us_per_call": round(1e3 * gms / gn, 3), "alg_MB_per_call": gby / gn / 1e6,
+                "frac": round(gby / (gms * 1e-3) / 1e9 / peaks()[0], 4), "n_derivatives": 4 * KC + 2,
+                "numerical_gradient_us": round(2 * (4 * KC + 2) * 1e3 * sub["coupling_only"]["ms_per_step"], 1)}
+    except Exception as e:
+        grad = {"error": repr(e)}
     cpu = cpu_baseline(mdl, p0, p4, t, p4n)
     h.close()
     others = other_configs(binding, device) if world == 1 and not args.headline_only else {}
@@ -275,7 +291,7 @@ def run_ours(args):
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roof, "kernels": ktab,
             "ms_per_step_with_kernel_events": ms_prof / args.steps,
             "coupling_only": sub["coupling_only"], "all_dirty": sub["all"], "cpu_baseline": cpu,
-            "nll_first_last": [float(nll_vals[0]), float(nll_vals[-1])], "other_configs": others}
+            "nll_first_last": [float(nll_vals[0]), float(nll_vals[-1])], "gradient": grad, "other_configs": others}
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()

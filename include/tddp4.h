@@ -127,6 +127,15 @@ int tddp4_nll_result(tddp4 *h, int slot, double *nll_out);
  * of events with non-positive / non-finite rate.                                                     */
 int tddp4_nll_parts(tddp4 *h, int slot, double out[5]);
 
+/* NLL and its analytic gradient in one pass over the data sample (derived from eq. (1) and
+ * eq. (2)).  grad_out: host [4 K_c + 2]:
+ *   [2k], [2k+1]             d NLL / d Re c_k, d NLL / d Im c_k            (k < K_c)
+ *   [2 K_c + 2k], [.. + 1]   d NLL / d Re cbar_k, d NLL / d Im cbar_k
+ *   [4 K_c], [4 K_c + 1]     d NLL / dx, d NLL / dy
+ * Masses, widths and tau are not differentiated.  Stale columns / Gram matrix are refreshed first.  Synchronous.
+ * Not available with use_resolution = 1 (TDDP4_ERR_ARG).                                               */
+int tddp4_nll_grad(tddp4 *h, double *nll_out, double *grad_out);
+
 /* Batched form for independent parameter points (the 2 n_par points of a numerical gradient, a scan, a
  * replayed minimiser trajectory): equivalent to tddp4_set_params + tddp4_nll for each point in order, with all
  * evaluations enqueued back to back and ONE synchronisation at the end.  params: host [n_points][stride],
@@ -191,7 +200,8 @@ enum {
   TDDP4_K_GEN_RATIO = 4, TDDP4_K_GEN_EMIT = 5,
   TDDP4_K_COLNLL = 6,    /* steps 2+3+4+5+7 fused over the data sample (call after a mass/width move)  */
   TDDP4_K_TRES = 7,      /* resolution mode: per-event time rows (re-run when x, y or tau moved)               */
-  TDDP4_K_COUNT = 8
+  TDDP4_K_GRAD = 8,      /* steps 4+5+7 and the analytic gradient in one pass over cached columns (tddp4_nll_grad) */
+  TDDP4_K_COUNT = 9
 };
 int tddp4_profile(tddp4 *h, int enable);
 /* total_ms, launches and (alg_bytes may be NULL) the algorithmic bytes of those launches -- the rows each launch

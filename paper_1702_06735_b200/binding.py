@@ -17,13 +17,13 @@ LIB_PATH = os.path.join(_HERE, "csrc", "libtddp4.so")
 
 OK, ERR_ARG, ERR_CUDA, ERR_CAPACITY, ERR_DOMAIN, ERR_NONFINITE, ERR_STATE = 0, -1, -2, -3, -4, -5, -6
 GET_S, GET_SHAPE, GET_STATIC, GET_COLUMNS, GET_TERMS = range(5)
-K_KIN, K_COLUMNS, K_GRAM, K_NLL, K_GEN_RATIO, K_GEN_EMIT, K_COLNLL, K_TRES = range(8)
-KERNEL_NAMES = ["kin", "columns", "gram", "nll", "gen_ratio", "gen_emit", "columns_nll", "time_rows"]
+K_KIN, K_COLUMNS, K_GRAM, K_NLL, K_GEN_RATIO, K_GEN_EMIT, K_COLNLL, K_TRES, K_GRAD = range(9)
+KERNEL_NAMES = ["kin", "columns", "gram", "nll", "gen_ratio", "gen_emit", "columns_nll", "time_rows", "nll_grad"]
 
 # every symbol include/tddp4.h declares
 SYMBOLS = ["tddp4_create", "tddp4_destroy", "tddp4_set_stream", "tddp4_last_error", "tddp4_version",
            "tddp4_load_events", "tddp4_set_params", "tddp4_nll", "tddp4_nll_async", "tddp4_nll_result",
-           "tddp4_nll_parts", "tddp4_param_stride", "tddp4_nll_batch", "tddp4_gram", "tddp4_gram_override", "tddp4_norm", "tddp4_generate", "tddp4_weight_bound",
+           "tddp4_nll_parts", "tddp4_nll_grad", "tddp4_param_stride", "tddp4_nll_batch", "tddp4_gram", "tddp4_gram_override", "tddp4_norm", "tddp4_generate", "tddp4_weight_bound",
            "tddp4_candidates", "tddp4_get", "tddp4_layout", "tddp4_profile", "tddp4_profile_read",
            "tddp4_profile_reset", "tddp4_launch_count"]
 
@@ -71,6 +71,7 @@ def load_library():
     L.tddp4_load_events.argtypes = [vp, C.c_int, i64, i64, vp, vp, vp, vp, C.c_int]
     L.tddp4_set_params.argtypes = [vp, vp, vp, vp, dbl, dbl, dbl]
     L.tddp4_nll.argtypes = [vp, dp, vp]
+    L.tddp4_nll_grad.argtypes = [vp, dp, vp]
     L.tddp4_nll_async.argtypes = [vp, C.c_int]
     L.tddp4_nll_result.argtypes = [vp, C.c_int, dp]
     L.tddp4_nll_parts.argtypes = [vp, C.c_int, dp]
@@ -212,6 +213,13 @@ class Tddp4:
         rc = self._check(self.lib.tddp4_nll(self._h, C.byref(out), _ptr(prob_out)),
                          allow=() if strict else (ERR_NONFINITE,))
         return out.value if rc == OK else math.inf
+
+    def nll_grad(self):
+        """(NLL, gradient[4 K_c + 2]) for the current parameters; layout as tddp4_nll_grad."""
+        out = C.c_double()
+        g = np.empty(4 * self.kc + 2)
+        self._check(self.lib.tddp4_nll_grad(self._h, C.byref(out), g.ctypes.data))
+        return out.value, g
 
     def nll_async(self, slot):
         self._check(self.lib.tddp4_nll_async(self._h, slot))

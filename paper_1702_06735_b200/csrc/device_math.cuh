@@ -216,12 +216,9 @@ __device__ __forceinline__ void rl_candidate(const ModelTab &M, double tau, uint
 // eq. (1): bracket B from A, Abar and the mixing phases u = y Gamma t, v = x Gamma t.
 // SMALL (|u|, |v| < 1/4, guaranteed by the host): cosh, sinh, cos, sin as Taylor polynomials up to u^12 / u^13;
 // the first omitted term is below 4e-20 of the leading one.
+// the four time functions of eq. (1) at mixing phases u = y Gamma t, v = x Gamma t
 template <bool SMALL>
-__device__ __forceinline__ double bracket(double2 A, double2 Ab, double u, double v) {
-  double aa = A.x * A.x + A.y * A.y, bb = Ab.x * Ab.x + Ab.y * Ab.y;
-  double cre = A.x * Ab.x + A.y * Ab.y;   // Re(A conj(Abar))
-  double cim = A.y * Ab.x - A.x * Ab.y;   // Im(A conj(Abar))
-  double ch, sh, sn, cs;
+__device__ __forceinline__ void mixing_functions(double u, double v, double &ch, double &sh, double &cs, double &sn) {
   if (SMALL) {
     const double c2 = 1.0 / 2, c4 = 1.0 / 24, c6 = 1.0 / 720, c8 = 1.0 / 40320, c10 = 1.0 / 3628800, c12 = 1.0 / 479001600;
     const double s3 = 1.0 / 6, s5 = 1.0 / 120, s7 = 1.0 / 5040, s9 = 1.0 / 362880, s11 = 1.0 / 39916800, s13 = 1.0 / 6227020800.0;
@@ -236,6 +233,14 @@ __device__ __forceinline__ double bracket(double2 A, double2 Ab, double u, doubl
     sh = 0.5 * (e - ei);
     sincos(v, &sn, &cs);
   }
+}
+template <bool SMALL>
+__device__ __forceinline__ double bracket(double2 A, double2 Ab, double u, double v) {
+  double aa = A.x * A.x + A.y * A.y, bb = Ab.x * Ab.x + Ab.y * Ab.y;
+  double cre = A.x * Ab.x + A.y * Ab.y;   // Re(A conj(Abar))
+  double cim = A.y * Ab.x - A.x * Ab.y;   // Im(A conj(Abar))
+  double ch, sh, sn, cs;
+  mixing_functions<SMALL>(u, v, ch, sh, cs, sn);
   return (aa + bb) * ch + (aa - bb) * cs - 2.0 * cre * sh - 2.0 * cim * sn;
 }
 

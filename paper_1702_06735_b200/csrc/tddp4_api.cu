@@ -16,6 +16,7 @@
 
 #include "../../include/tddp4.h"
 #include "kernels.cuh"
+#include "grad_kernels.cuh"
 
 using namespace tddp4k;
 
@@ -74,6 +75,7 @@ struct tddp4 {
   double *results_host_dev = nullptr; // ... through this device alias
   cudaEvent_t slot_event[N_SLOTS] = {nullptr};
   bool slot_used[N_SLOTS] = {false};
+  double *grad_host = nullptr, *grad_host_dev = nullptr;   // mapped pinned result of tddp4_nll_grad: [GRAD_OFFSET + 4 K_c + 2]
   double *batch_res = nullptr;       // device [batch_cap][SLOT_DOUBLES]
   double *batch_res_host = nullptr;  // pinned mirror
   int64_t batch_cap = 0;
@@ -192,6 +194,27 @@ void time_integrals(double x, double y, double Gamma, double lo, double hi, doub
   T[1] = Ix.real();
   T[2] = 0.5 * (Im.real() - Ip.real());
   T[3] = Ix.imag();
+}
+
+// d/dx and d/dy of those integrals: dI/dlambda = (-lo e^{-lambda lo} + hi e^{-lambda hi}) / lambda - I / lambda,
+// d lambda-+ / dy = -+Gamma, d lambda_x / dx = -i Gamma
+GradParams time_integral_derivatives(double x, double y, double Gamma, double lo, double hi) {
+  using cd = std::complex<double>;
+  auto dI = [&](cd lam) {
+    cd a = std::exp(-lam * lo);
+    cd b = std::isinf(hi) ? cd(0.0, 0.0) : std::exp(-lam * hi);
+    cd hb = std::isinf(hi) ? cd(0.0, 0.0) : hi * b;
+    cd I = (a - b) / lam;
+    return (-lo * a + hb) / lam - I / lam;
+  };
+  cd dm = dI(cd(Gamma * (1.0 - y), 0.0)), dp = dI(cd(Gamma * (1.0 + y), 0.0)), dx = dI(cd(Gamma, -Gamma * x));
+  cd ddx = cd(0.0, -Gamma) * dx;
+  GradParams g;
+  g.dT1dx = ddx.real();
+  g.dT3dx = ddx.imag();
+  g.dT0dy = 0.5 * (-Gamma * dm.real() + Gamma * dp.real());
+  g.dT2dy = 0.5 * (-Gamma * dm.real() - Gamma * dp.real());
+  return g;
 }
 
 int ensure_partials(tddp4 *h, size_t doubles) {
@@ -425,6 +448,22 @@ int enqueue_nll_slot(tddp4 *h, int slot, double *prob) {
   return TDDP4_OK;
 }
 
+template <int KC>
+int launch_nll_grad(tddp4 *h, const EventSet &e, double inv_n, bool small) {
+  int grid = (int)std::max<int64_t>(1, std::min<int64_t>((e.n + STREAM_BLOCK - 1) / STREAM_BLOCK, (int64_t)h->sm_count));
+  int rc = ensure_partials(h, (size_t)grid * (4 * KC + 5) + 16);
+  if (rc) return rc;
+  GradParams gp = time_integral_derivatives(h->RP.x, h->RP.y, h->RP.Gamma, h->t_lo, h->t_hi);
+  Prof p(h, TDDP4_K_GRAD, (double)e.n * (16.0 * KC + 8.0));
+  if (small)
+    nll_grad_kernel<KC, true><<<grid, STREAM_BLOCK, 0, h->stream>>>(e.a, e.t, e.ld, e.n, h->RP, gp, h->G, inv_n, e.sum_t, h->partials,
+                                                                   h->ticket, h->grad_host_dev);
+  else
+    nll_grad_kernel<KC, false><<<grid, STREAM_BLOCK, 0, h->stream>>>(e.a, e.t, e.ld, e.n, h->RP, gp, h->G, inv_n, e.sum_t, h->partials,
+                                                                    h->ticket, h->grad_host_dev);
+  return TDDP4_OK;
+}
+
 }  // namespace
 
 // =====================================================================================================
@@ -557,6 +596,8 @@ int tddp4_create(const tddp4_model_desc *desc, tddp4 **out) {
             cudaMalloc(&h->results, sizeof(double) * (N_SLOTS + 1) * SLOT_DOUBLES) == cudaSuccess &&
             cudaHostAlloc(&h->results_host, sizeof(double) * N_SLOTS * SLOT_DOUBLES, cudaHostAllocMapped) == cudaSuccess &&
             cudaHostGetDevicePointer((void **)&h->results_host_dev, h->results_host, 0) == cudaSuccess &&
+            cudaHostAlloc(&h->grad_host, sizeof(double) * (GRAD_OFFSET + 4 * MAX_KC + 2), cudaHostAllocMapped) == cudaSuccess &&
+            cudaHostGetDevicePointer((void **)&h->grad_host_dev, h->grad_host, 0) == cudaSuccess &&
             cudaMalloc(&h->gen_scalars, sizeof(unsigned long long) * 2) == cudaSuccess &&
             cudaMemset(h->ticket, 0, sizeof(unsigned int)) == cudaSuccess &&
             cudaMemset(h->G, 0, sizeof(double) * 2 * KC * KC) == cudaSuccess;
@@ -595,6 +636,7 @@ int tddp4_destroy(tddp4 *h) {
   cudaFree(h->G); cudaFree(h->partials); cudaFree(h->ticket); cudaFree(h->results); cudaFree(h->batch_res);
   if (h->batch_res_host) cudaFreeHost(h->batch_res_host);
   if (h->results_host) cudaFreeHost(h->results_host);
+  if (h->grad_host) cudaFreeHost(h->grad_host);
   cudaFree(h->gen_flags); cudaFree(h->gen_counts); cudaFree(h->gen_offs); cudaFree(h->gen_scalars);
   for (int s = 0; s < N_SLOTS; ++s)
     if (h->slot_event[s]) cudaEventDestroy(h->slot_event[s]);
@@ -752,6 +794,42 @@ int tddp4_nll(tddp4 *h, double *nll_out, double *prob_out) {
   int rc = enqueue_nll_slot(h, 0, prob_out);
   if (rc) return rc;
   return tddp4_nll_result(h, 0, nll_out);
+}
+
+int tddp4_nll_grad(tddp4 *h, double *nll_out, double *grad_out) {
+  if (!h || !nll_out || !grad_out) return fail(h, TDDP4_ERR_ARG, "null argument");
+  if (!h->have_params) return fail(h, TDDP4_ERR_STATE, "tddp4_set_params has not been called");
+  if (h->use_resolution) return fail(h, TDDP4_ERR_ARG, "tddp4_nll_grad: resolution mode is not supported");
+  EventSet &d = h->set[0];
+  if (!d.loaded) return fail(h, TDDP4_ERR_STATE, "data sample not loaded");
+  int rc;
+  if (d.cols_dirty || !h->gram_valid) {   // bring the columns and the Gram matrix up to date (scratch slot)
+    rc = enqueue_nll(h, h->results + (size_t)N_SLOTS * SLOT_DOUBLES, nullptr);
+    if (rc) return rc;
+  }
+  double inv_n = h->gram_n > 0 ? 1.0 / (double)h->gram_n : 0.0;
+  const RateParams &R = h->RP;
+  bool small = std::fabs(R.y) * R.Gamma * d.t_max < 0.25 && std::fabs(R.x) * R.Gamma * d.t_max < 0.25;
+  switch (h->M.n_kc) {
+#define CASE(k) case k: rc = launch_nll_grad<k>(h, d, inv_n, small); break;
+    CASE(1) CASE(2) CASE(3) CASE(4) CASE(5) CASE(6) CASE(7) CASE(8) CASE(9) CASE(10) CASE(11) CASE(12)
+    CASE(13) CASE(14) CASE(15) CASE(16)
+#undef CASE
+    default: return fail(h, TDDP4_ERR_ARG, "unsupported number of couplings %d", h->M.n_kc);
+  }
+  if (rc) return rc;
+  CU(cudaGetLastError());
+  h->prev_kind = PREV_NONE;
+  CU(cudaStreamSynchronize(h->stream));
+  const double *r = h->grad_host;
+  const int na = 4 * h->M.n_kc + 2;
+  memcpy(grad_out, r + GRAD_OFFSET, sizeof(double) * na);
+  *nll_out = r[3];
+  if (r[4] > 0.0 || !std::isfinite(r[3])) {
+    *nll_out = INFINITY;
+    return fail(h, TDDP4_ERR_NONFINITE, "%g events with non-positive or non-finite rate (N = %g)", r[4], r[2]);
+  }
+  return TDDP4_OK;
 }
 
 int tddp4_nll_parts(tddp4 *h, int slot, double out[5]) {
