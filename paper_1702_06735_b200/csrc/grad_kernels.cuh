@@ -23,7 +23,7 @@ struct GradParams {
 constexpr int GRAD_OFFSET = 8;
 
 template <int KC, bool SMALL>
-__global__ void __launch_bounds__(STREAM_BLOCK, 1)
+__global__ void __launch_bounds__(STREAM_BLOCK, KC <= 8 ? 2 : 1)
 nll_grad_kernel(const double2 *__restrict__ a, const double *__restrict__ t, int64_t ld, int64_t n,
                 const __grid_constant__ RateParams R, const __grid_constant__ GradParams GP, const double *__restrict__ G,
                 double inv_n_norm, double sum_t, double *__restrict__ partials /* [grid][NA + 3] */, unsigned int *ticket,

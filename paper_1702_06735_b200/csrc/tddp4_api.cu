@@ -450,7 +450,7 @@ int enqueue_nll_slot(tddp4 *h, int slot, double *prob) {
 
 template <int KC>
 int launch_nll_grad(tddp4 *h, const EventSet &e, double inv_n, bool small) {
-  int grid = (int)std::max<int64_t>(1, std::min<int64_t>((e.n + STREAM_BLOCK - 1) / STREAM_BLOCK, (int64_t)h->sm_count));
+  int grid = (int)std::max<int64_t>(1, std::min<int64_t>((e.n + STREAM_BLOCK - 1) / STREAM_BLOCK, (int64_t)h->sm_count * (KC <= 8 ? 2 : 1)));
   int rc = ensure_partials(h, (size_t)grid * (4 * KC + 5) + 16);
   if (rc) return rc;
   GradParams gp = time_integral_derivatives(h->RP.x, h->RP.y, h->RP.Gamma, h->t_lo, h->t_hi);
