@@ -278,7 +278,7 @@ def run_ours(args):
                 "numerical_gradient_us": round(2 * (4 * KC + 2) * 1e3 * sub["coupling_only"]["ms_per_step"], 1)}
     except Exception as e:
         grad = {"error": repr(e)}
-    cpu = cpu_baseline(mdl, p0, p4, t, p4n)
+    cpu = cpu_baseline(mdl, p0, p4, t, p4n) if world == 1 else None      # the oracle is timed at N = 1 only
     h.close()
     others = other_configs(binding, device) if world == 1 and not args.headline_only else {}
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,

@@ -362,3 +362,24 @@ def test_sharded_wrapper_on_one_rank(B):
     h.set_params(p2); direct2 = h.nll()
     sh.set_params(p2)
     assert abs(sh.nll() - direct2) <= 1e-13 * abs(direct2)
+
+
+def test_maximum_model_size(B):
+    """The limits of include/tddp4.h: 16 couplings, 32 terms (all eight chains twice, both Bose orderings), and a model
+    whose instance/term counts fall between the load-batch size classes (5 instances, 5 terms -> padded rows)."""
+    mdl = W.build_model(list(range(1, 9)) * 2, bose=True)
+    assert mdl.n_couplings == 16 and mdl.n_terms == 32
+    par = W.initial_params(mdl)
+    p4, t, _ = samples.data_sample(("C", 3), 777)
+    p4n, _ = samples.flat_sample(2_222)
+    w = np.random.default_rng(5).uniform(0.5, 1.0, 2_222)
+    h = check_against_oracle(B, mdl, par, p4, t, p4n, w)
+    from oracle import gradient as OG
+    ref, _ = OG.nll_gradient(mdl, par, p4, t, p4n, w)
+    _, g = h.nll_grad()
+    assert np.max(np.abs(g - ref)) <= 1e-10 * np.abs(ref).max()
+    odd = W.build_model([1, 2, 3, 8, 4], bose=False)             # 5 couplings, 5 terms, 6 lineshape instances
+    par = W.initial_params(odd)
+    check_against_oracle(B, odd, par, p4, t, p4n, w)
+    with pytest.raises(B.Tddp4Error):
+        B.Tddp4(W.build_model(list(range(1, 9)) * 2 + [1], bose=True))   # 17 couplings / 34 terms: refused at create
