@@ -181,7 +181,7 @@ __device__ __forceinline__ void two_body(double m_first, double m_second, double
   double ct = 2.0 * u_cos - 1.0;
   double st = sqrt(1.0 - ct * ct);
   double sphi, cphi;
-  sincos(6.283185307179586476925 * u_phi, &sphi, &cphi);
+  sincospi(2.0 * u_phi, &sphi, &cphi);   // phi = 2 pi u: exact argument reduction, no multiple-of-pi rounding
   double nx = st * cphi, ny = st * sphi, nz = ct;
   first = {sqrt(m_first * m_first + ps * ps), ps * nx, ps * ny, ps * nz};
   second = {sqrt(m_second * m_second + ps * ps), -ps * nx, -ps * ny, -ps * nz};

@@ -165,7 +165,7 @@ __device__ __forceinline__ double candidate_ratio(const ModelTab &M, const LineP
 }
 
 // mode 0: raw candidate dump (parity); mode 1: pilot maximum (G5); mode 2: accept flags + block counts (G6)
-__global__ void __launch_bounds__(GEN_BLOCK)
+__global__ void __launch_bounds__(GEN_BLOCK, 4)
 gen_ratio_kernel(const __grid_constant__ ModelTab M, const __grid_constant__ LineParams LP,
                  const __grid_constant__ RateParams R, double tau, uint64_t seed, uint32_t stream, uint64_t first,
                  int64_t n, int mode, double envelope,
