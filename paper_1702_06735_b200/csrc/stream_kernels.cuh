@@ -443,7 +443,7 @@ colnll_stream_kernel(const __grid_constant__ StreamTab S, const __grid_constant_
   int64_t i = (int64_t)blockIdx.x * STREAM_BLOCK + threadIdx.x;
 #pragma unroll 1
   for (; i < n; i += stride) {
-    if (lane == 0 && i + stride < n) prefetch_l2_bulk(tile_event(cache, S.R, i + stride), (uint32_t)S.R * 256u);
+    if (lane == 0 && i + stride < n) prefetch_l2_bulk(tile_event(cache, S.R, i + stride) + S.skip, (uint32_t)(S.R * 32 - S.skip) * 8u);
     double ti = RES ? 0.0 : ldg_stream1(t + i);            // RES: t points at the time rows [8][ld]
     const double *ev = tile_event(cache, S.R, i);
     double fv[GT];
@@ -535,7 +535,7 @@ gram_stream_kernel(const __grid_constant__ StreamTab S, const __grid_constant__ 
   int64_t i0 = (int64_t)blockIdx.x * STREAM_BLOCK + warp * 32;
 #pragma unroll 1
   for (; i0 < n; i0 += stride) {
-    if (lane == 0 && i0 + stride < n) prefetch_l2_bulk(tile_event(cache, S.R, i0 + stride), (uint32_t)S.R * 256u);
+    if (lane == 0 && i0 + stride < n) prefetch_l2_bulk(tile_event(cache, S.R, i0 + stride) + S.skip, (uint32_t)(S.R * 32 - S.skip) * 8u);
     const double *ev = tile_event(cache, S.R, i0 + lane);
     double wj = S.w_off >= 0 ? ldg_stream1(ev + S.w_off) : 1.0;
     double fv[GT];

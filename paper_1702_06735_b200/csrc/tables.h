@@ -59,6 +59,7 @@ struct StreamTab {
   int n_inst4, n_terms4, n_kc;     // padded counts
   int R;                           // rows per tile
   int g_off, f_off, w_off;         // element offsets (row * 32) of the first g row, first f row, weight row (-1: none)
+  int skip;                        // element offset of the first row the kernels read (unused s rows come first)
   uint32_t inst_soff[MAX_INST];    // element offset of the s row lineshape instance j reads
   uint32_t term_t0[MAX_TERMS];     // element offset (slot * 32) of T_R1 in the warp's lineshape scratch; unit slot if none
   uint32_t term_t1[MAX_TERMS];     // ... of T_R2

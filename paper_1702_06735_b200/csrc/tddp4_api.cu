@@ -546,6 +546,24 @@ int tddp4_create(const tddp4_model_desc *desc, tddp4 **out) {
     if (ia < 0 || ib < 0) return bail(fail(h, TDDP4_ERR_ARG, "too many lineshape instances"));
     tm.inst0 = (int8_t)ia; tm.inst1 = (int8_t)ib;
   }
+  // renumber the particle systems so that those no lineshape reads (the four-body system, ...) come FIRST: the rows
+  // the per-call kernels stream are then one contiguous range of every tile, and the bulk L2 prefetch can skip the rest
+  {
+    bool used[MAX_SYS] = {false};
+    for (int j = 0; j < M.n_inst; ++j) used[M.inst[j].sys] = true;
+    int remap[MAX_SYS], next = 0;
+    for (int pass = 0; pass < 2; ++pass)
+      for (int i = 0; i < M.n_sys; ++i)
+        if (used[i] == (pass == 1)) remap[i] = next++;
+    uint8_t mask[MAX_SYS];
+    for (int i = 0; i < M.n_sys; ++i) mask[remap[i]] = M.sys_mask[i];
+    for (int i = 0; i < M.n_sys; ++i) M.sys_mask[i] = mask[i];
+    M.sysD = remap[M.sysD];
+    for (int j = 0; j < M.n_inst; ++j) {
+      M.inst[j].sys = (int8_t)remap[M.inst[j].sys];
+      if (M.inst[j].sub >= 0) M.inst[j].sub = (int8_t)remap[M.inst[j].sub];
+    }
+  }
   // the s rows some lineshape reads, in system order: these are the rows the per-call kernels stage
   for (int i = 0; i < MAX_SYS; ++i) M.sys_slot[i] = -1;
   for (int j = 0; j < M.n_inst; ++j) M.sys_slot[M.inst[j].sys] = 0;
@@ -565,6 +583,7 @@ int tddp4_create(const tddp4_model_desc *desc, tddp4 **out) {
     h->size_class = best;
     S.n_kc = M.n_kc;
     S.g_off = M.n_sys * 32; S.f_off = (M.n_sys + S.n_inst4) * 32; S.w_off = -1;
+    S.skip = (M.n_sys - M.n_su) * 32;                    // leading rows nobody streams
     S.R = M.n_sys + S.n_inst4 + S.n_terms4;              // + 1 for a weighted event set, fixed at launch
     for (int j = 0; j < M.n_inst; ++j) S.inst_soff[j] = (uint32_t)M.inst[j].sys * 32;
     const uint32_t unit = (uint32_t)S.n_inst4 * 32;
