@@ -194,7 +194,7 @@ int tddp4_layout(const tddp4 *h, int *n_sys, int *sys_mask, int *n_inst, int *in
 /* Per-kernel CUDA-event timing on the handle's stream.  kernel ids: */
 enum {
   TDDP4_K_KIN = 0,       /* step 1 at load                                                            */
-  TDDP4_K_COLUMNS = 1,   /* steps 2+3 alone (only on the prob_out / inspection paths)                  */
+  TDDP4_K_COLUMNS = 1,   /* reserved (steps 2+3 alone are never launched: they are fused into COLNLL / GRAM)   */
   TDDP4_K_GRAM = 2,      /* steps 2+3+6 fused over the normalisation sample (fp64 tensor-core Gram)    */
   TDDP4_K_NLL = 3,       /* steps 4+5+7 over cached columns (coupling / x / y / tau-only call)         */
   TDDP4_K_GEN_RATIO = 4, TDDP4_K_GEN_EMIT = 5,

@@ -12,7 +12,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(CSRC, "libtddp4.so")
 SOURCES = ["tddp4_api.cu"]
-HEADERS = ["kernels.cuh", "stream_kernels.cuh", "device_math.cuh", "resolution.cuh", "tables.h", os.path.join("..", "..", "include", "tddp4.h")]
+HEADERS = ["kernels.cuh", "stream_kernels.cuh", "device_math.cuh", "resolution.cuh", "grad_kernels.cuh", "tables.h", os.path.join("..", "..", "include", "tddp4.h")]
 
 
 def nvcc_path() -> str:

@@ -1,15 +1,17 @@
-// stream_kernels.cuh -- the three per-call kernels of the NLL path:
-//   nll_stream_kernel     steps 4+5+7   over cached coupling columns            (coupling / x / y / tau-only call)
-//   colnll_stream_kernel  steps 2..5+7  over the step-1 caches of the data set  (call after a mass or width moved)
-//   gram_stream_kernel    steps 2+3+6   over the step-1 caches of the normalisation set (fp64 tensor-core Gram)
-// All three are HBM streams: every row is read exactly once per call with coalesced loads straight into registers
-// (256-byte warp segments of 8-byte rows, 512-byte segments of the 16-byte columns), batched so that each thread has
-// 8-18 loads in flight, from STREAM_BLOCK-thread persistent blocks, two per SM.  Event i always belongs to thread
-// (i mod stride) of the grid-stride decomposition, stride = gridDim.x * STREAM_BLOCK, and every thread visits its
-// events in increasing order; nll_stream and colnll_stream are launched with the same grid, so the fixed-order
-// reduction returns bit-identical NLLs whether the columns were cached or rebuilt in the call.
-// (Measured on B200, 1M events x 136 B: a TMA/mbarrier-staged version of the coupling-only pass with one block per
-// SM ran at 35 us, this register-direct form at 26.7 us, a pure read of the same bytes at 22.6 us.)
+// stream_kernels.cuh -- the per-call kernels of the NLL path:
+//   nll_stream_kernel     steps 4+5+7   over cached coupling columns             (coupling / x / y / tau-only call)
+//   colnll_stream_kernel  steps 2..5+7  over the static cache of the data set    (call after a mass or width moved)
+//   gram_stream_kernel    steps 2+3+6   over the static cache of the normalisation set (fp64 tensor-core Gram)
+//   nll_res_kernel, tres_kernel, prob_*  resolution mode (config 5) and per-event probabilities
+// All are HBM streams: every row is read exactly once per call with coalesced loads straight into registers (256-byte
+// warp segments of 8-byte rows, 512-byte segments of the 16-byte columns), every load of an event requested before any
+// arithmetic (17-40 loads in flight per thread), from STREAM_BLOCK-thread persistent blocks, two per SM.  Event i always
+// belongs to thread (i mod stride) of the grid-stride decomposition, stride = gridDim.x * STREAM_BLOCK, and every thread
+// visits its events in increasing order; nll_stream and colnll_stream are launched with the same grid, so the fixed-order
+// reduction returns bit-identical NLLs whether the columns were cached or rebuilt in the call.  Consecutive kernels
+// overlap through programmatic dependent launch (pdl_* below).
+// (Measured on B200, 1M events x 136 B: a cp.async.bulk/mbarrier-staged version of the coupling-only pass with one block
+// per SM ran at 35 us, this register-direct form at 26.7 us, a pure read of the same bytes at 22.6 us.)
 #pragma once
 #include "resolution.cuh"
 
@@ -347,7 +349,7 @@ tres_kernel(const __grid_constant__ FaddTab F, const double *__restrict__ t, con
 
 // ------------------------------------------------------------------------------------------------
 // steps 2+3 of ONE event from the tile-major static cache (tables.h).  ev = address of (row 0, this event): every row is
-// ev[row * 32], so with the loops unrolled to the table maxima (group-of-4 guards, warp-uniform) every load carries an
+// ev[row * 32], so with the loops unrolled to the table maxima (one warp-uniform guard per load batch) every load carries an
 // immediate offset and every table entry / lineshape constant is an immediate-indexed constant-bank operand.
 // Lineshapes: T_R of every de-duplicated instance goes to the thread's own slots sTl[slot * 32] of its warp's
 // scratch (chains index it through the model tables, so it cannot live in registers); slot n_inst4 holds the unit

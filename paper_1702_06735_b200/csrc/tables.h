@@ -35,9 +35,7 @@ struct ModelTab {
   int n_sys, n_inst, n_terms, n_kc;
   int sysD;                        // index of the four-body system
   uint8_t sys_mask[MAX_SYS];
-  int n_su;                        // systems whose s some lineshape instance reads (the staged s rows)
-  int8_t su_sys[MAX_SYS];          // staged slot -> system index
-  int8_t sys_slot[MAX_SYS];        // system index -> staged slot, -1 if no instance reads it
+  int n_su;                        // systems whose s some lineshape instance reads (they are numbered last)
   int8_t col_begin[MAX_KC + 1];    // terms (sorted by coupling) of column kappa: [col_begin[k], col_begin[k+1])
   int8_t user_term[MAX_TERMS];     // sorted position -> caller's term index
   InstTab inst[MAX_INST];

@@ -555,6 +555,8 @@ int tddp4_create(const tddp4_model_desc *desc, tddp4 **out) {
     for (int pass = 0; pass < 2; ++pass)
       for (int i = 0; i < M.n_sys; ++i)
         if (used[i] == (pass == 1)) remap[i] = next++;
+    M.n_su = 0;
+    for (int i = 0; i < M.n_sys; ++i) M.n_su += used[i] ? 1 : 0;
     uint8_t mask[MAX_SYS];
     for (int i = 0; i < M.n_sys; ++i) mask[remap[i]] = M.sys_mask[i];
     for (int i = 0; i < M.n_sys; ++i) M.sys_mask[i] = mask[i];
@@ -564,11 +566,6 @@ int tddp4_create(const tddp4_model_desc *desc, tddp4 **out) {
       if (M.inst[j].sub >= 0) M.inst[j].sub = (int8_t)remap[M.inst[j].sub];
     }
   }
-  // the s rows some lineshape reads, in system order: these are the rows the per-call kernels stage
-  for (int i = 0; i < MAX_SYS; ++i) M.sys_slot[i] = -1;
-  for (int j = 0; j < M.n_inst; ++j) M.sys_slot[M.inst[j].sys] = 0;
-  for (int i = 0; i < M.n_sys; ++i)
-    if (M.sys_slot[i] == 0) { M.sys_slot[i] = (int8_t)M.n_su; M.su_sys[M.n_su++] = (int8_t)i; }
   {   // flat tables of the per-call kernels (tables.h): padded to groups of 4, all entries 32-bit
     StreamTab &S = h->S;
     memset(&S, 0, sizeof S);
