@@ -146,6 +146,12 @@ class Tddp4:
             self._h = None
             raise Tddp4Error(rc, text)
         self.n = [0, 0]
+        c, cb = np.empty(self.kc, np.complex128), np.empty(self.kc, np.complex128)
+        mw = np.zeros((max(1, self.n_res), 2))
+        self._pbuf = (c, cb, mw, c.ctypes.data, cb.ctypes.data, mw.ctypes.data)
+        self.h2d_bytes_per_call = c.nbytes + cb.nbytes + (mw.nbytes if self.n_res else 0) + 24
+        self._nll_out = C.c_double()
+        self._nll_ref = C.byref(self._nll_out)
 
     @property
     def n_data(self):
@@ -199,20 +205,20 @@ class Tddp4:
     # -- tddp4_set_params -------------------------------------------------------------------------
     def set_params(self, par):
         """par: workloads.Params-like (c, cbar complex arrays; mass, width; x, y, tau)."""
-        c = np.ascontiguousarray(np.asarray(par.c, dtype=np.complex128)).view(np.float64)
-        cb = np.ascontiguousarray(np.asarray(par.cbar, dtype=np.complex128)).view(np.float64)
-        mw = np.ascontiguousarray(np.stack([np.asarray(par.mass, float), np.asarray(par.width, float)], axis=1)) \
-            if self.n_res else np.zeros(2)
-        self._check(self.lib.tddp4_set_params(self._h, c.ctypes.data, cb.ctypes.data, mw.ctypes.data,
-                                              float(par.x), float(par.y), float(par.tau)))
-        self.h2d_bytes_per_call = c.nbytes + cb.nbytes + (mw.nbytes if self.n_res else 0) + 24
+        b = self._pbuf                                   # preallocated marshalling buffers: no allocation per call
+        b[0][:] = par.c
+        b[1][:] = par.cbar
+        if self.n_res:
+            b[2][:, 0] = par.mass
+            b[2][:, 1] = par.width
+        self._check(self.lib.tddp4_set_params(self._h, b[3], b[4], b[5], par.x, par.y, par.tau))
 
     # -- tddp4_nll and friends --------------------------------------------------------------------
     def nll(self, prob_out=None, strict=True):
-        out = C.c_double()
-        rc = self._check(self.lib.tddp4_nll(self._h, C.byref(out), _ptr(prob_out)),
-                         allow=() if strict else (ERR_NONFINITE,))
-        return out.value if rc == OK else math.inf
+        rc = self.lib.tddp4_nll(self._h, self._nll_ref, None if prob_out is None else _ptr(prob_out))
+        if rc != OK and (strict or rc != ERR_NONFINITE):
+            self._check(rc)
+        return self._nll_out.value if rc == OK else math.inf
 
     def nll_grad(self):
         """(NLL, gradient[4 K_c + 2]) for the current parameters; layout as tddp4_nll_grad."""
