@@ -63,12 +63,18 @@ __device__ __forceinline__ double2 faddeeva_upper(const FaddTab &F, double2 z) {
   return make_double2(fma(2.0, r.x, RSPI * inv.x), fma(2.0, r.y, RSPI * inv.y));
 }
 
+// g0 = exp(-t^2 / (2 sigma^2)) with the two exact shortcuts of the window edges: 1 at t = 0, 0 once it underflows
+__device__ __forceinline__ double gauss0(double t, double sigma) {
+  if (t == 0.0) return 1.0;
+  double ts = t / sigma, a = 0.5 * ts * ts;
+  return a > 746.0 ? 0.0 : exp(-a);
+}
+
 // h for real lambda
 __device__ __forceinline__ double conv_exp_real(double t, double lam, double sigma) {
   const double RS2 = 0.70710678118654752440;
   double u = (lam * sigma * sigma - t) * (RS2 / sigma);
-  double ts = t / sigma;
-  double g0 = exp(-0.5 * ts * ts);
+  double g0 = gauss0(t, sigma);
   if (u >= 0.0) return 0.5 * g0 * erfcx(u);
   double E = exp(0.5 * lam * lam * sigma * sigma - lam * t);
   if (g0 < 1e-18 * E) return E;                               // correction below half an ulp (erfcx <= 1): same bits
@@ -79,8 +85,7 @@ __device__ __forceinline__ double conv_exp_real(double t, double lam, double sig
 __device__ __forceinline__ double2 conv_exp_complex(const FaddTab &F, double t, double lr, double li, double sigma) {
   const double RS2 = 0.70710678118654752440;
   double ur = (lr * sigma * sigma - t) * (RS2 / sigma), ui = li * sigma * RS2;
-  double ts = t / sigma;
-  double g0 = exp(-0.5 * ts * ts);
+  double g0 = gauss0(t, sigma);
   if (ur >= 0.0) {
     double2 w = faddeeva_upper(F, make_double2(-ui, ur));     // i u
     return make_double2(0.5 * g0 * w.x, 0.5 * g0 * w.y);
@@ -96,18 +101,22 @@ __device__ __forceinline__ double2 conv_exp_complex(const FaddTab &F, double t, 
 
 // window integrals int_{lo}^{hi} h dt; hi may be +inf, lo may be -inf
 __device__ __forceinline__ double erf_scaled(double t, double sigma) {
-  if (isinf(t)) return t > 0.0 ? 1.0 : -1.0;
-  return erf(t * 0.70710678118654752440 / sigma);
+  if (t == 0.0) return 0.0;
+  double a = t * 0.70710678118654752440 / sigma;
+  if (fabs(a) > 6.0) return a > 0.0 ? 1.0 : -1.0;            // erf(6) = 1 - 2e-17: rounds to 1 (also t = +-inf)
+  return erf(a);
 }
-__device__ __forceinline__ double window_real(double lo, double hi, double lam, double sigma) {
+// derf = erf(hi / (sqrt2 sigma)) - erf(lo / (sqrt2 sigma)), the same for all three lambdas of an event
+__device__ __forceinline__ double window_real(double lo, double hi, double lam, double sigma, double derf) {
   double hl = isinf(lo) ? 0.0 : conv_exp_real(lo, lam, sigma);
   double hh = isinf(hi) ? 0.0 : conv_exp_real(hi, lam, sigma);
-  return (erf_scaled(hi, sigma) - erf_scaled(lo, sigma) - 2.0 * (hh - hl)) / (2.0 * lam);
+  return (derf - 2.0 * (hh - hl)) / (2.0 * lam);
 }
-__device__ __forceinline__ double2 window_complex(const FaddTab &F, double lo, double hi, double lr, double li, double sigma) {
+__device__ __forceinline__ double2 window_complex(const FaddTab &F, double lo, double hi, double lr, double li, double sigma,
+                                                  double derf) {
   double2 hl = isinf(lo) ? make_double2(0.0, 0.0) : conv_exp_complex(F, lo, lr, li, sigma);
   double2 hh = isinf(hi) ? make_double2(0.0, 0.0) : conv_exp_complex(F, hi, lr, li, sigma);
-  double2 num = make_double2(erf_scaled(hi, sigma) - erf_scaled(lo, sigma) - 2.0 * (hh.x - hl.x), -2.0 * (hh.y - hl.y));
+  double2 num = make_double2(derf - 2.0 * (hh.x - hl.x), -2.0 * (hh.y - hl.y));
   return cdiv(num, make_double2(2.0 * lr, 2.0 * li));
 }
 
@@ -119,8 +128,9 @@ __device__ __forceinline__ void time_terms(const FaddTab &F, double t, double si
   double hm = conv_exp_real(t, lm, sigma), hp = conv_exp_real(t, lp, sigma);
   double2 hx = conv_exp_complex(F, t, lxr, lxi, sigma);
   psi[0] = 0.5 * (hm + hp); psi[1] = hx.x; psi[2] = 0.5 * (hm - hp); psi[3] = hx.y;
-  double Im = window_real(t_lo, t_hi, lm, sigma), Ip = window_real(t_lo, t_hi, lp, sigma);
-  double2 Ix = window_complex(F, t_lo, t_hi, lxr, lxi, sigma);
+  const double derf = erf_scaled(t_hi, sigma) - erf_scaled(t_lo, sigma);
+  double Im = window_real(t_lo, t_hi, lm, sigma, derf), Ip = window_real(t_lo, t_hi, lp, sigma, derf);
+  double2 Ix = window_complex(F, t_lo, t_hi, lxr, lxi, sigma, derf);
   tint[0] = 0.5 * (Im + Ip); tint[1] = Ix.x; tint[2] = 0.5 * (Im - Ip); tint[3] = Ix.y;
 }
 #endif  // __CUDACC__
