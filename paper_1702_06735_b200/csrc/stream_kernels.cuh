@@ -430,7 +430,8 @@ colnll_stream_kernel(const __grid_constant__ StreamTab S, const __grid_constant_
                      const double *__restrict__ cache, const double *__restrict__ t, int64_t ld, int64_t n,
                      double2 *__restrict__ a,
                      const __grid_constant__ RateParams R, const double *__restrict__ G, double inv_n_norm, double sum_t,
-                     double *__restrict__ partials, unsigned int *ticket, double *__restrict__ result, int early_wait) {
+                     double *__restrict__ partials, unsigned int *ticket, double *__restrict__ result, int early_wait,
+                     uint32_t store_mask /* bit kappa: the stored column kappa is stale and is rewritten */) {
   extern __shared__ __align__(16) char smem_raw[];
   __shared__ double s_S[4];
   pdl_launch_dependents();
@@ -453,7 +454,8 @@ colnll_stream_kernel(const __grid_constant__ StreamTab S, const __grid_constant_
     lineshapes_to_scratch<GI>(S, LP, ev, sTl);
     double2 A = make_double2(0.0, 0.0), Ab = make_double2(0.0, 0.0);
     columns_from_scratch<GT>(S, ev, sTl, fv, [&](int kap, double2 col) {
-      a[(int64_t)kap * ld + i] = col;
+      // a column none of whose lineshapes moved is recomputed to the bits already stored: skip its 16-byte store
+      if ((store_mask >> kap) & 1u) a[(int64_t)kap * ld + i] = col;
       amp_add(A, Ab, R.c[kap][0], R.c[kap][1], R.cbar[kap][0], R.cbar[kap][1], col);
     });
     if (RES) la.add(resolved_prob(A, Ab, t + i, ld, s_S));

@@ -48,6 +48,7 @@ struct tddp4 {
   bool own_stream = false;
   ModelTab M{};
   StreamTab S{};                     // the same model, flattened for the per-call kernels
+  uint32_t store_mask = 0xFFFFFFFFu; // coupling columns of the data sample whose stored values are stale (bit = column)
   int prev_kind = 0;                 // last per-call kernel enqueued with nothing after it: 0 none/other, 1 NLL, 2 COLNLL, 3 GRAM
   int size_class = 0;                // load-batch sizes (GI, GT) of the per-call kernels: 0 (4,4), 1 (8,8), 2 (12,16)
   std::vector<tddp4_res> res;
@@ -343,7 +344,9 @@ int launch_colnll(tddp4 *h, const EventSet &e, double inv_n, double *result, boo
   StreamTab S = h->S;
   S.R = e.R;
   size_t smem = colnll_smem_bytes(S.n_inst4);
-  Prof p(h, TDDP4_K_COLNLL, (double)e.n * (static_bytes_per_event(h) + (h->use_resolution ? 64.0 : 8.0) + 16.0 * M.n_kc));
+  int n_stored = 0;                      // columns actually rewritten by this launch
+  for (int kap = 0; kap < M.n_kc; ++kap) n_stored += (h->store_mask >> kap) & 1u;
+  Prof p(h, TDDP4_K_COLNLL, (double)e.n * (static_bytes_per_event(h) + (h->use_resolution ? 64.0 : 8.0) + 16.0 * n_stored));
   const int mode = h->use_resolution ? 2 : (small ? 1 : 0);
   const int early = h->prev_kind != PREV_GRAM;   // a Gram kernel neither reads nor writes the columns this kernel rewrites
   const double sum_t = h->use_resolution ? 0.0 : e.sum_t;
@@ -352,7 +355,7 @@ int launch_colnll(tddp4 *h, const EventSet &e, double inv_n, double *result, boo
     constexpr int NI = decltype(ni)::value, NT = decltype(nt)::value;
 #define COLNLL_LAUNCH(SM, RS)                                                                                                  \
   launch_pdl(colnll_stream_kernel<SM, RS, NI, NT>, grid, STREAM_BLOCK, smem, h->stream, S, h->LP, (const double *)e.cache, tp, e.ld, e.n, \
-             e.a, h->RP, (const double *)h->G, inv_n, sum_t, h->partials, h->ticket, result, early)
+             e.a, h->RP, (const double *)h->G, inv_n, sum_t, h->partials, h->ticket, result, early, h->store_mask)
     if (mode == 2) COLNLL_LAUNCH(false, true);
     else if (mode == 1) COLNLL_LAUNCH(true, false);
     else COLNLL_LAUNCH(false, false);
@@ -360,6 +363,7 @@ int launch_colnll(tddp4 *h, const EventSet &e, double inv_n, double *result, boo
     return 0;
   });
   h->prev_kind = PREV_COLNLL;
+  h->store_mask = 0;
   return TDDP4_OK;
 }
 
@@ -679,6 +683,7 @@ int tddp4_load_events(tddp4 *h, int which, int64_t n, int64_t ld_in, const doubl
     return fail(h, TDDP4_ERR_ARG, "use_resolution = 1: the data sample needs per-event sigma_t");
   CU(cudaStreamSynchronize(h->stream));
   h->prev_kind = PREV_NONE;
+  if (which == 0) h->store_mask = 0xFFFFFFFFu;
   EventSet &e = h->set[which];
   free_set(e);
   e.n = n;
@@ -765,8 +770,13 @@ int tddp4_set_params(tddp4 *h, const double *c, const double *cbar, const double
     lp.gam[j] = m0 * m0 * g0 / (std::pow(q0, 2 * in.L + 1) * host_barrier2(in.L, z0));
   }
   bool dirty = !h->have_params;                       // any lineshape constant moved: columns and Gram are stale
+  bool moved[MAX_INST] = {false};
   for (int j = 0; j < M.n_inst; ++j)
-    if (lp.m0sq[j] != h->LP.m0sq[j] || lp.gam[j] != h->LP.gam[j]) dirty = true;
+    if (lp.m0sq[j] != h->LP.m0sq[j] || lp.gam[j] != h->LP.gam[j]) dirty = moved[j] = true;
+  if (!h->have_params) h->store_mask = 0xFFFFFFFFu;
+  for (int kap = 0; kap < M.n_kc; ++kap)              // which stored columns that makes stale (accumulates until rebuilt)
+    for (int k = M.col_begin[kap]; k < M.col_begin[kap + 1]; ++k)
+      if (M.term[k].inst0 >= 0 && (moved[M.term[k].inst0] || moved[M.term[k].inst1])) h->store_mask |= 1u << kap;
   h->LP = lp;
   for (int r = 0; r < nres; ++r) { h->mass[r] = mass_width[2 * r]; h->width[r] = mass_width[2 * r + 1]; }
   RateParams &R = h->RP;

@@ -383,3 +383,53 @@ def test_maximum_model_size(B):
     check_against_oracle(B, odd, par, p4, t, p4n, w)
     with pytest.raises(B.Tddp4Error):
         B.Tddp4(W.build_model(list(range(1, 9)) * 2 + [1], bose=True))   # 17 couplings / 34 terms: refused at create
+
+
+def test_stale_column_tracking(B):
+    """Only the stored columns whose lineshapes moved are rewritten after a mass/width step (nothing is recomputed
+    that did not change -- here: nothing is re-stored).  After single-resonance moves, several moves without an
+    evaluation in between, and a move back, the stored columns equal the oracle's and the NLL equals, bit for bit,
+    that of a fresh handle."""
+    mdl = samples.model_of(("C", 3))
+    par = W.initial_params(mdl)
+    p4, t, _ = samples.data_sample(("C", 3), 1_537)
+    p4n, _ = samples.flat_sample(4_001)
+    h = B.Tddp4(mdl)
+    h.load_events(0, p4, t); h.load_events(1, p4n)
+    h.set_params(par); h.nll()
+    names = mdl.res_names
+
+    def columns_ok(p):
+        _, _, a = oracle.terms(mdl, p, p4)
+        ref = np.zeros((mdl.n_couplings, p4.shape[1]), complex)
+        for k, kap in enumerate(mdl.term_coupling):
+            ref[kap] += a[k]
+        col = h.get(0, B.GET_COLUMNS).cpu().numpy()
+        scale = np.abs(ref).max(axis=1, keepdims=True)
+        assert np.max(np.abs(col - ref) / scale) < TOL_LAYER
+
+    def fresh(p):
+        g = B.Tddp4(mdl)
+        g.load_events(0, p4, t); g.load_events(1, p4n)
+        g.set_params(p)
+        return g.nll()
+
+    cur = par.copy()
+    for res, what in [("a1(1260)", "mass"), ("K*(892)0", "width"), ("K2*(1430)", "mass"), ("rho(770)0", "mass")]:
+        r = names.index(res)
+        if what == "mass":
+            cur.mass[r] *= 1.002
+        else:
+            cur.width[r] *= 0.99
+        h.set_params(cur)
+        assert h.nll() == fresh(cur)
+        columns_ok(cur)
+    two = cur.copy(); two.mass[names.index("K1(1270)")] *= 1.001
+    h.set_params(two)                                            # no evaluation: the stale set must accumulate
+    three = two.copy(); three.width[names.index("K1(1400)")] *= 1.01
+    h.set_params(three)
+    assert h.nll() == fresh(three)
+    columns_ok(three)
+    h.set_params(par)                                            # all the way back
+    assert h.nll() == fresh(par)
+    columns_ok(par)
