@@ -92,12 +92,13 @@ def build_workload(binding, cfg, device, seed):
     flat = W.flat_model()
     hf = binding.Tddp4(flat, device)
     hf.set_params(W.flat_params(flat))
-    p4n, _, _, _ = hf.generate_n(seed, W.STREAM_NORM, cfg.n_norm, 0, 2.0 * hf.weight_bound(), chunk=1 << 24)
+    p4n, _, idxn, _ = hf.generate_n(seed, W.STREAM_NORM, cfg.n_norm, 0, 2.0 * hf.weight_bound(), chunk=1 << 24, want_index=True)
     hf.close()
     hg = binding.Tddp4(cfg.model, device)
     hg.set_params(W.initial_params(cfg.model))
-    p4, t, _, info = hg.generate_n(seed, W.STREAM_DATA, cfg.n_data, cfg.n_pilot, cfg.envelope_scale, chunk=1 << 24)
+    p4, t, idx, info = hg.generate_n(seed, W.STREAM_DATA, cfg.n_data, cfg.n_pilot, cfg.envelope_scale, chunk=1 << 24, want_index=True)
     hg.close()
+    info["index"], info["index_norm"], info["seed"] = idx, idxn, seed      # candidate indices: the oracle regenerates from them
     return p4, t, p4n, info
 
 
@@ -278,7 +279,7 @@ def run_ours(args):
                 "numerical_gradient_us": round(2 * (4 * KC + 2) * 1e3 * sub["coupling_only"]["ms_per_step"], 1)}
     except Exception as e:
         grad = {"error": repr(e)}
-    cpu = cpu_baseline(mdl, p0, p4, t, p4n) if world == 1 else None      # the oracle is timed at N = 1 only
+    cpu = cpu_baseline(mdl, p0, ginfo) if world == 1 else None      # the oracle is timed at N = 1 only
     h.close()
     others = other_configs(binding, device) if world == 1 and not args.headline_only else {}
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
@@ -411,12 +412,14 @@ def other_configs(binding, device, steps_c5=100):
     return out
 
 
-def cpu_baseline(mdl, par, p4, t, p4n, n_data=100_000):
-    """The oracle as it stands, timed on this box's host cores on a bounded sample of the same workload."""
+def cpu_baseline(mdl, par, ginfo, n_data=100_000):
+    """The oracle as it stands, timed on this box's host cores on a bounded sample of the same workload: the first events
+    of both samples, which the oracle regenerates itself from their candidate indices (it is handed no CUDA output)."""
     import oracle
     n_norm = 4 * n_data
-    a, b, c = p4[:, :n_data].cpu().numpy(), t[:n_data].cpu().numpy(), p4n[:, :n_norm].cpu().numpy()
-    a, c = np.ascontiguousarray(a), np.ascontiguousarray(c)
+    flat = W.flat_model()
+    a, b, _, _ = oracle.candidates_at(mdl, par.tau, ginfo["seed"], W.STREAM_DATA, ginfo["index"][:n_data].cpu().numpy())
+    c, _, _, _ = oracle.candidates_at(flat, W.TAU_D0, ginfo["seed"], W.STREAM_NORM, ginfo["index_norm"][:n_norm].cpu().numpy())
     best = float("inf")
     for _ in range(3):
         t0 = time.perf_counter()
