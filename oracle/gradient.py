@@ -118,3 +118,52 @@ def nll_gradient(mdl, par, p4, t, p4_norm, w_norm=None):
 
     nll = G * np.sum(t) - np.sum(np.log(B)) + n * np.log(N)
     return grad, float(nll)
+
+
+def nll_gradient_resolution(mdl, par, p4, t, sigma_t, p4_norm, w_norm=None):
+    """The same gradient with per-event Gaussian decay-time resolution (O-8, config 5):
+    NLL = -sum_i log(R_i / N_i), R_i the quadratic form with the convolved time functions psi_m(t_i, sigma_i),
+    N_i = T_0i S_1 + T_1i S_2 - 2 T_2i S_3 - 2 T_3i S_4 with the per-event window integrals T_mi and the phase-space
+    averages S_m (direct sums over the normalisation sample).  Returns (grad[4 K_c + 2], nll)."""
+    from oracle import resolution as R
+    kc = mdl.n_couplings
+    c, cb = np.asarray(par.c, complex), np.asarray(par.cbar, complex)
+    grad = np.zeros(4 * kc + 2)
+    col = _columns(mdl, par, p4)
+    A, Ab = c @ col, cb @ col
+    z = np.stack([A.real, A.imag, Ab.real, Ab.imag])
+    psi = R.time_functions(t, sigma_t, par.x, par.y, par.tau)
+    dpsi_dx, dpsi_dy = R.time_function_derivatives(t, sigma_t, par.x, par.y, par.tau)
+    T = R.time_integrals(sigma_t, par.x, par.y, par.tau, mdl.t_lo, mdl.t_hi)
+    dT_dx, dT_dy = R.time_integral_derivatives(sigma_t, par.x, par.y, par.tau, mdl.t_lo, mdl.t_hi)
+
+    def form_m(zz, f):            # quadratic form with (cosh, cos, sinh, sin)-type coefficients f[0..3]
+        return _form(zz, f[0] + f[1], f[0] - f[1], f[2], f[3])
+
+    Rv = form_m(z, psi)
+    dRdz = _form_grad_z(z, psi[0] + psi[1], psi[0] - psi[1], psi[2], psi[3])
+    # phase-space averages and their z-gradients on the normalisation sample, one per time coefficient
+    coln = _columns(mdl, par, p4_norm)
+    w = np.ones(p4_norm.shape[1]) if w_norm is None else np.asarray(w_norm, float)
+    An, Abn = c @ coln, cb @ coln
+    zn = np.stack([An.real, An.imag, Abn.real, Abn.imag])
+    nn = p4_norm.shape[1]
+    unit = np.eye(4)
+    S = np.array([np.sum(w * form_m(zn, unit[m])) / nn for m in range(4)])        # coefficient of T_m in N_i
+    Nv = T[0] * S[0] + T[1] * S[1] + T[2] * S[2] + T[3] * S[3]
+    Wm = np.array([np.sum(T[m] / Nv) for m in range(4)])                          # sum_i T_mi / N_i
+    dSdz = [(_form_grad_z(zn, unit[m][0] + unit[m][1], unit[m][0] - unit[m][1], unit[m][2], unit[m][3]) * w) for m in range(4)]
+    for k in range(kc):
+        ar, ai = col[k].real, col[k].imag
+        nr, ni = coln[k].real, coln[k].imag
+        for off, (i0, i1) in ((0, (0, 1)), (2 * kc, (2, 3))):
+            grad[off + 2 * k] -= np.sum((dRdz[i0] * ar + dRdz[i1] * ai) / Rv)
+            grad[off + 2 * k + 1] -= np.sum((-dRdz[i0] * ai + dRdz[i1] * ar) / Rv)
+            for m in range(4):
+                grad[off + 2 * k] += Wm[m] * np.sum(dSdz[m][i0] * nr + dSdz[m][i1] * ni) / nn
+                grad[off + 2 * k + 1] += Wm[m] * np.sum(-dSdz[m][i0] * ni + dSdz[m][i1] * nr) / nn
+    for j, (dpsi, dT) in enumerate(((dpsi_dx, dT_dx), (dpsi_dy, dT_dy))):
+        dN = dT[0] * S[0] + dT[1] * S[1] + dT[2] * S[2] + dT[3] * S[3]
+        grad[4 * kc + j] = -np.sum(form_m(z, dpsi) / Rv) + np.sum(dN / Nv)
+    nll = -np.sum(np.log(Rv / Nv))
+    return grad, float(nll)

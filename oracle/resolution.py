@@ -85,3 +85,44 @@ def nll(mdl, par, p4, t, sigma_t, p4_norm, w_norm=None):
     if not np.all(np.isfinite(P)) or np.any(P <= 0.0):
         return math.inf, P, 2
     return -math.fsum(np.log(P)), P, 0
+
+
+# ---- derivatives with respect to the mixing parameters (for the gradient oracle) ---------------------------------------
+def dh_dlam(t, lam, sigma):
+    """d h / d lambda, the derivative of the definition: with g0 = exp(-t^2 / (2 sigma^2)),
+    d/dlambda [1/2 exp(lambda^2 sigma^2/2 - lambda t) erfc(u)] = (lambda sigma^2 - t) h - sigma g0 / sqrt(2 pi)
+    (d erfc(u)/du = -2 e^{-u^2}/sqrt(pi), du/dlambda = sigma/sqrt2, and exp(lambda^2 sigma^2/2 - lambda t) e^{-u^2} = g0)."""
+    t = np.asarray(t, dtype=np.float64)
+    sigma = np.asarray(sigma, dtype=np.float64)
+    g0 = np.exp(-t * t / (2.0 * sigma * sigma))
+    return (lam * sigma * sigma - t) * h(t, lam, sigma) - sigma * g0 / math.sqrt(2.0 * math.pi)
+
+
+def dH_dlam(t, lam, sigma):
+    """d H / d lambda of H = [erf(t/(sqrt2 sigma)) - 2 h] / (2 lambda):  -H/lambda - (dh/dlambda)/lambda."""
+    sigma = np.asarray(sigma, dtype=np.float64)
+    if np.isscalar(t) and math.isinf(t):
+        return -H(t, lam, sigma) / lam
+    return -H(t, lam, sigma) / lam - dh_dlam(t, lam, sigma) / lam
+
+
+def time_function_derivatives(t, sigma, x, y, tau):
+    """(d psi_m / dx, d psi_m / dy), each [4][n]: d lambda_-+ / dy = -+Gamma, d lambda_x / dx = -i Gamma."""
+    G = 1.0 / tau
+    lm, lp, lx = lambdas(x, y, tau)
+    dm, dp, dx = dh_dlam(t, lm, sigma), dh_dlam(t, lp, sigma), -1j * G * dh_dlam(t, lx, sigma)
+    z = np.zeros_like(np.asarray(t, dtype=np.float64))
+    return (np.stack([z, dx.real, z, dx.imag]),
+            np.stack([0.5 * (-G * dm + G * dp).real, z, 0.5 * (-G * dm - G * dp).real, z]))
+
+
+def time_integral_derivatives(sigma, x, y, tau, t_lo, t_hi):
+    """(d T_m / dx, d T_m / dy) of the per-event window integrals, each [4][n]."""
+    G = 1.0 / tau
+    lm, lp, lx = lambdas(x, y, tau)
+    dm = dH_dlam(t_hi, lm, sigma) - dH_dlam(t_lo, lm, sigma)
+    dp = dH_dlam(t_hi, lp, sigma) - dH_dlam(t_lo, lp, sigma)
+    dx = -1j * G * (dH_dlam(t_hi, lx, sigma) - dH_dlam(t_lo, lx, sigma))
+    z = np.zeros_like(np.asarray(sigma, dtype=np.float64))
+    return (np.stack([z, dx.real, z, dx.imag]),
+            np.stack([0.5 * (-G * dm + G * dp).real, z, 0.5 * (-G * dm - G * dp).real, z]))

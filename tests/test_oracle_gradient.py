@@ -124,3 +124,56 @@ def test_gradient_brute_force_mpmath():
         order = tuple(1 if i == j else 0 for i in range(len(th)))
         d = mp.diff(nll_mp, tuple(th), order)
         assert abs(float(d) - g[j]) < 1e-10 * max(abs(float(d)), 1e-3 * np.abs(g).max()), (j, float(d), g[j])
+
+
+# ---- resolution mode -------------------------------------------------------------------------------------------------------
+def test_resolution_lambda_derivatives_mpmath():
+    """d h / d lambda and d H / d lambda against 30-digit numerical differentiation of the mpmath definitions."""
+    from oracle import resolution as R
+
+    def h_mp(t, lam, s):
+        return mp.mpf(1) / 2 * mp.exp(lam * lam * s * s / 2 - lam * t) * mp.erfc((lam * s * s - t) / (mp.sqrt(2) * s))
+
+    def H_mp(t, lam, s):
+        return (mp.erf(t / (mp.sqrt(2) * s)) - 2 * h_mp(t, lam, s)) / (2 * lam)
+    for lam in (complex(2.4, 0.0), complex(2.45, -0.012), complex(1.9, -2.2)):
+        for t, s in ((0.0, 0.05), (0.03, 0.08), (0.7, 0.03), (4.0, 0.06)):
+            want = complex(mp.diff(lambda l: h_mp(mp.mpf(t), l, mp.mpf(s)), mp.mpc(lam)))
+            got = complex(R.dh_dlam(np.array([t]), lam, np.array([s]))[0])
+            assert abs(got - want) <= 1e-12 * max(abs(want), 1e-6), (lam, t, s)
+            want = complex(mp.diff(lambda l: H_mp(mp.mpf(t), l, mp.mpf(s)), mp.mpc(lam)))
+            got = complex(R.dH_dlam(t, lam, np.array([s]))[0])
+            assert abs(got - want) <= 1e-12 * abs(want), (lam, t, s)
+        got = complex(R.dH_dlam(np.inf, lam, np.array([0.05]))[0])
+        assert abs(got + 1.0 / (2 * lam * lam)) < 1e-15
+
+
+@pytest.mark.parametrize("x,y", [(W.X_MIX, W.Y_MIX), (0.6, 0.25)])
+def test_resolution_gradient_is_the_derivative_of_the_oracle_nll(x, y):
+    from oracle import resolution as R
+    cfg = W.config(5)
+    mdl = cfg.model
+    par = W.initial_params(mdl)
+    par.x, par.y = x, y
+    kc = mdl.n_couplings
+    p4, t_true, _ = samples.data_sample(("C", 5), 80)
+    t, sig = W.smear_times(t_true, cfg)
+    p4n, _ = samples.flat_sample(500)
+    w = W.efficiency_weights(500, cfg)
+    g, nll = OG.nll_gradient_resolution(mdl, par, p4, t, sig, p4n, w)
+    ref = R.nll(mdl, par, p4, t, sig, p4n, w)[0]
+    assert abs(nll - ref) < 1e-11 * abs(ref)
+    th = theta_get(par, kc)
+    for j in list(range(0, 4 * kc, 5)) + [4 * kc, 4 * kc + 1]:
+        h = 1e-5 * max(abs(th[j]), 1e-2)
+        vals = []
+        for s in (+1, -1, +2, -2):
+            tj = th.copy(); tj[j] += s * h
+            vals.append(R.nll(mdl, theta_set(par, tj, kc), p4, t, sig, p4n, w)[0])
+        fd = (8 * (vals[0] - vals[1]) - (vals[2] - vals[3])) / (12 * h)
+        assert abs(g[j] - fd) < 1e-6 * abs(fd) + 1e-12 * abs(ref) / h, (j, g[j], fd)
+    gc = g[:4 * kc].view(complex)
+    cc = np.concatenate([par.c, par.cbar])
+    size = np.sum(np.abs(cc) * np.abs(gc))
+    assert abs(np.sum(cc.real * gc.real + cc.imag * gc.imag)) < 1e-11 * size      # common scale
+    assert abs(np.sum(-cc.imag * gc.real + cc.real * gc.imag)) < 1e-11 * size     # common phase
