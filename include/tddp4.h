@@ -132,8 +132,8 @@ int tddp4_nll_parts(tddp4 *h, int slot, double out[5]);
  *   [2k], [2k+1]             d NLL / d Re c_k, d NLL / d Im c_k            (k < K_c)
  *   [2 K_c + 2k], [.. + 1]   d NLL / d Re cbar_k, d NLL / d Im cbar_k
  *   [4 K_c], [4 K_c + 1]     d NLL / dx, d NLL / dy
- * Masses, widths and tau are not differentiated.  Stale columns / Gram matrix are refreshed first.  Synchronous.
- * Not available with use_resolution = 1 (TDDP4_ERR_ARG).                                               */
+ * Masses, widths and tau are not differentiated.  Stale columns / Gram matrix / time rows are refreshed first.
+ * Works in both modes (use_resolution = 0 and 1).  Synchronous.                                         */
 int tddp4_nll_grad(tddp4 *h, double *nll_out, double *grad_out);
 
 /* Batched form for independent parameter points (the 2 n_par points of a numerical gradient, a scan, a

@@ -133,6 +133,45 @@ __device__ __forceinline__ void time_terms(const FaddTab &F, double t, double si
   double2 Ix = window_complex(F, t_lo, t_hi, lxr, lxi, sigma, derf);
   tint[0] = 0.5 * (Im + Ip); tint[1] = Ix.x; tint[2] = 0.5 * (Im - Ip); tint[3] = Ix.y;
 }
+
+// Derivatives with respect to the mixing parameters (tddp4_nll_grad in resolution mode).  From the definition,
+//   dh/dlambda = (lambda sigma^2 - t) h - sigma g0 / sqrt(2 pi),      dH/dlambda = -H/lambda - (dh/dlambda)/lambda,
+// and d lambda_-+ / dy = -+Gamma, d lambda_x / dx = -i Gamma.  out[0..3] = d psi_1/dx, d psi_3/dx, d psi_0/dy, d psi_2/dy;
+// out[4..7] = d T_1/dx, d T_3/dx, d T_0/dy, d T_2/dy (the other derivatives vanish).
+__device__ __forceinline__ double dconv_real(double t, double lam, double sigma, double h) {
+  return (lam * sigma * sigma - t) * h - sigma * gauss0(t, sigma) * 0.39894228040143267794;   // 1/sqrt(2 pi)
+}
+__device__ __forceinline__ double2 dconv_complex(double t, double lr, double li, double sigma, double2 h) {
+  double ar = lr * sigma * sigma - t, ai = li * sigma * sigma;
+  return make_double2(ar * h.x - ai * h.y - sigma * gauss0(t, sigma) * 0.39894228040143267794, ar * h.y + ai * h.x);
+}
+__device__ __forceinline__ void time_term_derivatives(const FaddTab &F, double t, double sigma, double x, double y, double Gamma,
+                                                      double t_lo, double t_hi, double out[8]) {
+  const double lm = Gamma * (1.0 - y), lp = Gamma * (1.0 + y), lxr = Gamma, lxi = -Gamma * x;
+  // at the observed time
+  double dm = dconv_real(t, lm, sigma, conv_exp_real(t, lm, sigma));
+  double dp = dconv_real(t, lp, sigma, conv_exp_real(t, lp, sigma));
+  double2 dx = dconv_complex(t, lxr, lxi, sigma, conv_exp_complex(F, t, lxr, lxi, sigma));
+  out[0] = Gamma * dx.y;  out[1] = -Gamma * dx.x;              // -i Gamma (a + i b) = Gamma b - i Gamma a
+  out[2] = 0.5 * Gamma * (dp - dm);  out[3] = -0.5 * Gamma * (dp + dm);
+  // window integrals: dI/dlambda = -I/lambda - (dh(hi) - dh(lo))/lambda
+  const double derf = erf_scaled(t_hi, sigma) - erf_scaled(t_lo, sigma);
+  auto edge_real = [&](double lam) {
+    double hl = isinf(t_lo) ? 0.0 : conv_exp_real(t_lo, lam, sigma), hh = isinf(t_hi) ? 0.0 : conv_exp_real(t_hi, lam, sigma);
+    double I = (derf - 2.0 * (hh - hl)) / (2.0 * lam);
+    double dl = isinf(t_lo) ? 0.0 : dconv_real(t_lo, lam, sigma, hl), dh = isinf(t_hi) ? 0.0 : dconv_real(t_hi, lam, sigma, hh);
+    return -(I + (dh - dl)) / lam;
+  };
+  double Dm = edge_real(lm), Dp = edge_real(lp);
+  double2 hl = isinf(t_lo) ? make_double2(0.0, 0.0) : conv_exp_complex(F, t_lo, lxr, lxi, sigma);
+  double2 hh = isinf(t_hi) ? make_double2(0.0, 0.0) : conv_exp_complex(F, t_hi, lxr, lxi, sigma);
+  double2 I = cdiv(make_double2(derf - 2.0 * (hh.x - hl.x), -2.0 * (hh.y - hl.y)), make_double2(2.0 * lxr, 2.0 * lxi));
+  double2 dl = isinf(t_lo) ? make_double2(0.0, 0.0) : dconv_complex(t_lo, lxr, lxi, sigma, hl);
+  double2 dh = isinf(t_hi) ? make_double2(0.0, 0.0) : dconv_complex(t_hi, lxr, lxi, sigma, hh);
+  double2 Dx = cdiv(make_double2(-(I.x + dh.x - dl.x), -(I.y + dh.y - dl.y)), make_double2(lxr, lxi));
+  out[4] = Gamma * Dx.y;  out[5] = -Gamma * Dx.x;
+  out[6] = 0.5 * Gamma * (Dp - Dm);  out[7] = -0.5 * Gamma * (Dp + Dm);
+}
 #endif  // __CUDACC__
 
 }  // namespace tddp4k

@@ -347,6 +347,18 @@ tres_kernel(const __grid_constant__ FaddTab F, const double *__restrict__ t, con
   for (int m = 0; m < 4; ++m) { tr[m * ld + i] = psi[m]; tr[(4 + m) * ld + i] = tint[m]; }
 }
 
+// The derivative rows of the data sample for the gradient in resolution mode (resolution.cuh): 8 rows per event.
+__global__ void __launch_bounds__(TRES_BLOCK)
+tres_grad_kernel(const __grid_constant__ FaddTab F, const double *__restrict__ t, const double *__restrict__ sigma_t, int64_t n,
+                 double x, double y, double Gamma, double t_lo, double t_hi, double *__restrict__ trg, int64_t ld) {
+  int64_t i = (int64_t)blockIdx.x * TRES_BLOCK + threadIdx.x;
+  if (i >= n) return;
+  double d[8];
+  time_term_derivatives(F, t[i], sigma_t[i], x, y, Gamma, t_lo, t_hi, d);
+#pragma unroll
+  for (int m = 0; m < 8; ++m) trg[m * ld + i] = d[m];
+}
+
 // ------------------------------------------------------------------------------------------------
 // steps 2+3 of ONE event from the tile-major static cache (tables.h).  ev = address of (row 0, this event): every row is
 // ev[row * 32], so with the loops unrolled to the table maxima (one warp-uniform guard per load batch) every load carries an

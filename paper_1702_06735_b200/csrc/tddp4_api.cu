@@ -33,6 +33,8 @@ struct EventSet {
   double *t = nullptr, *sigma_t = nullptr, *w = nullptr;
   double *tr = nullptr;                              // resolution mode: time rows psi[4], tint[4], [8][ld]
   bool tres_valid = false;                           // tr matches the current x, y, tau
+  double *trg = nullptr;                             // derivative rows of the gradient in resolution mode, [8][ld] (on demand)
+  bool tresg_valid = false;
   double sum_t = 0.0, t_max = 0.0;                   // sum and max |t| of the decay times (fixed-order kernel)
   bool cols_dirty = true;                            // coupling columns stale (a mass or width moved since they were built)
   bool loaded = false;
@@ -229,7 +231,7 @@ int ensure_partials(tddp4 *h, size_t doubles) {
 }
 
 void free_set(EventSet &e) {
-  cudaFree(e.cache); cudaFree(e.a); cudaFree(e.t); cudaFree(e.sigma_t); cudaFree(e.w); cudaFree(e.tr);
+  cudaFree(e.cache); cudaFree(e.a); cudaFree(e.t); cudaFree(e.sigma_t); cudaFree(e.w); cudaFree(e.tr); cudaFree(e.trg);
   e = EventSet{};
 }
 
@@ -449,6 +451,17 @@ int enqueue_nll_slot(tddp4 *h, int slot, double *prob) {
                        cudaMemcpyDeviceToHost, h->stream));
   CU(cudaEventRecord(h->slot_event[slot], h->stream));
   h->slot_used[slot] = true;
+  return TDDP4_OK;
+}
+
+template <int KC>
+int launch_nll_grad_res(tddp4 *h, const EventSet &e, double inv_n) {
+  int grid = (int)std::max<int64_t>(1, std::min<int64_t>((e.n + STREAM_BLOCK - 1) / STREAM_BLOCK, (int64_t)h->sm_count));
+  int rc = ensure_partials(h, (size_t)grid * (4 * KC + 9) + 16);
+  if (rc) return rc;
+  Prof p(h, TDDP4_K_GRAD, (double)e.n * (16.0 * KC + 128.0));
+  nll_grad_res_kernel<KC><<<grid, STREAM_BLOCK, 0, h->stream>>>(e.a, e.tr, e.trg, e.ld, e.n, h->RP, h->G, inv_n, h->partials, h->ticket,
+                                                              h->grad_host_dev);
   return TDDP4_OK;
 }
 
@@ -784,7 +797,7 @@ int tddp4_set_params(tddp4 *h, const double *c, const double *cbar, const double
     R.c[k][0] = c[2 * k]; R.c[k][1] = c[2 * k + 1];
     R.cbar[k][0] = cbar[2 * k]; R.cbar[k][1] = cbar[2 * k + 1];
   }
-  if (R.x != x || R.y != y || R.Gamma != 1.0 / tau || !h->have_params) h->set[0].tres_valid = false;
+  if (R.x != x || R.y != y || R.Gamma != 1.0 / tau || !h->have_params) h->set[0].tres_valid = h->set[0].tresg_valid = false;
   R.x = x; R.y = y; R.Gamma = 1.0 / tau;
   R.t_lo = h->t_lo; R.t_hi = h->t_hi; R.use_resolution = h->use_resolution;
   time_integrals(x, y, R.Gamma, h->t_lo, h->t_hi, R.T);
@@ -825,19 +838,28 @@ int tddp4_nll(tddp4 *h, double *nll_out, double *prob_out) {
 int tddp4_nll_grad(tddp4 *h, double *nll_out, double *grad_out) {
   if (!h || !nll_out || !grad_out) return fail(h, TDDP4_ERR_ARG, "null argument");
   if (!h->have_params) return fail(h, TDDP4_ERR_STATE, "tddp4_set_params has not been called");
-  if (h->use_resolution) return fail(h, TDDP4_ERR_ARG, "tddp4_nll_grad: resolution mode is not supported");
   EventSet &d = h->set[0];
   if (!d.loaded) return fail(h, TDDP4_ERR_STATE, "data sample not loaded");
   int rc;
-  if (d.cols_dirty || !h->gram_valid) {   // bring the columns and the Gram matrix up to date (scratch slot)
+  if (d.cols_dirty || !h->gram_valid || (h->use_resolution && !d.tres_valid)) {   // columns, Gram matrix, time rows up to date
     rc = enqueue_nll(h, h->results + (size_t)N_SLOTS * SLOT_DOUBLES, nullptr);
     if (rc) return rc;
   }
   double inv_n = h->gram_n > 0 ? 1.0 / (double)h->gram_n : 0.0;
   const RateParams &R = h->RP;
   bool small = std::fabs(R.y) * R.Gamma * d.t_max < 0.25 && std::fabs(R.x) * R.Gamma * d.t_max < 0.25;
+  if (h->use_resolution && !d.tresg_valid && d.n > 0) {   // derivative rows: rebuilt when x, y, tau or the sample changed
+    if (!d.trg) CU(cudaMalloc(&d.trg, sizeof(double) * 8 * d.ld));
+    int grid = (int)((d.n + TRES_BLOCK - 1) / TRES_BLOCK);
+    {
+      Prof p(h, TDDP4_K_TRES, (double)d.n * 80.0);
+      tres_grad_kernel<<<grid, TRES_BLOCK, 0, h->stream>>>(h->FT, d.t, d.sigma_t, d.n, R.x, R.y, R.Gamma, h->t_lo, h->t_hi, d.trg, d.ld);
+    }
+    CU(cudaGetLastError());
+    d.tresg_valid = true;
+  }
   switch (h->M.n_kc) {
-#define CASE(k) case k: rc = launch_nll_grad<k>(h, d, inv_n, small); break;
+#define CASE(k) case k: rc = h->use_resolution ? launch_nll_grad_res<k>(h, d, inv_n) : launch_nll_grad<k>(h, d, inv_n, small); break;
     CASE(1) CASE(2) CASE(3) CASE(4) CASE(5) CASE(6) CASE(7) CASE(8) CASE(9) CASE(10) CASE(11) CASE(12)
     CASE(13) CASE(14) CASE(15) CASE(16)
 #undef CASE

@@ -94,3 +94,32 @@ def test_gradient_matches_finite_differences_of_the_gpu_nll(B):
     vals, _ = h.nll_batch(h.pack_params(pts))
     fd = (vals[0::2] - vals[1::2]) / (2 * np.array(hs))
     assert np.max(np.abs(fd - g)) < 1e-5 * np.abs(g).max()
+
+
+@pytest.mark.parametrize("x,y,t_hi", [(W.X_MIX, W.Y_MIX, 4.0), (0.7, -0.3, 4.0), (0.05, 0.02, float("inf"))])
+def test_gradient_with_resolution(B, x, y, t_hi):
+    """Resolution mode (config 5 model): columns, time rows and their x/y derivative rows in one pass."""
+    cfg = W.config(5)
+    mdl = W.build_model(range(1, 9), bose=True, t_lo=0.0, t_hi=t_hi, use_resolution=1)
+    p4, t_true, _ = samples.data_sample(("C", 5), 1_200)
+    t, sig = W.smear_times(t_true, cfg)
+    t[:30] = np.linspace(0.0, 0.02, 30)                          # both erfc branches
+    p4n, _ = samples.flat_sample(6_000)
+    w = W.efficiency_weights(6_000, cfg)
+    h = B.Tddp4(mdl)
+    h.load_events(0, p4, t, sigma_t=sig)
+    h.load_events(1, p4n, None, weight=w)
+    par = W.initial_params(mdl)
+    par.x, par.y = x, y
+    for step in range(3):
+        ref, ref_nll = OG.nll_gradient_resolution(mdl, par, p4, t, sig, p4n, w)
+        h.set_params(par)
+        nll, g = h.nll_grad()
+        assert abs(nll - ref_nll) <= 1e-11 * abs(ref_nll)
+        assert abs(nll - h.nll()) <= 1e-13 * abs(nll)
+        assert np.max(np.abs(g - ref)) <= 1e-10 * np.abs(ref).max()
+        par = par.copy()
+        if step == 0:
+            par.c[2] *= 1.03; par.mass[1] *= 1.0005               # stale columns + Gram
+        else:
+            par.x *= 1.2; par.y *= 0.9                           # stale time rows and derivative rows
