@@ -40,6 +40,12 @@ __device__ __forceinline__ double ldg_stream1(const double *p) {
 // and read-only streaming overlap this kernel's tail and final reduction.  pdl_wait() blocks until the predecessor grid
 // has completed and its memory is visible; it sits in front of the first access to anything the predecessor may read or
 // write (partials, ticket, G, result slots; the columns when the predecessor or this kernel writes them).
+// Ordering rule: a successor may become resident as soon as every block of this kernel has executed
+// launch_dependents -- possibly while this kernel's own predecessor is still running.  A successor that skips its early
+// wait must therefore never conflict with that older kernel: (i) a kernel that has an early wait triggers only after it,
+// (ii) the Gram kernel, after which the column-writing kernel skips its early wait, triggers only after its late wait,
+// (iii) an NLL kernel without early wait may trigger at once: whatever follows it either waits early or only reads what
+// no kernel before it writes.
 __device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;"); }
 __device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
 
@@ -241,8 +247,8 @@ nll_stream_kernel(const double2 *__restrict__ a, const double *__restrict__ t, i
                   const __grid_constant__ RateParams R, const double *__restrict__ G, double inv_n_norm, double sum_t,
                   double *__restrict__ partials, unsigned int *ticket, double *__restrict__ result, int early_wait) {
   constexpr int UNR = KC <= 8 ? 2 : 1;   // wider models: one event per iteration, or the columns spill
-  pdl_launch_dependents();
   if (early_wait) pdl_wait();            // the predecessor wrote the columns
+  pdl_launch_dependents();               // only after this kernel's own early wait: see the ordering note at pdl_wait()
   MantAcc la;
   const double yG = R.y * R.Gamma, xG = R.x * R.Gamma;
   const int64_t stride = (int64_t)gridDim.x * STREAM_BLOCK;
@@ -303,8 +309,8 @@ nll_res_kernel(const double2 *__restrict__ a, const double *__restrict__ tr, int
                double *__restrict__ partials, unsigned int *ticket, double *__restrict__ result) {
   __shared__ double s_S[4];
   MantAcc la;
-  pdl_launch_dependents();
   pdl_wait();                              // G is read first thing
+  pdl_launch_dependents();
   block_phase_space_sums(R, G, KC, inv_n_norm, s_S);
   const int64_t stride = (int64_t)gridDim.x * STREAM_BLOCK;
 #pragma unroll 1
@@ -446,8 +452,8 @@ colnll_stream_kernel(const __grid_constant__ StreamTab S, const __grid_constant_
                      uint32_t store_mask /* bit kappa: the stored column kappa is stale and is rewritten */) {
   extern __shared__ __align__(16) char smem_raw[];
   __shared__ double s_S[4];
-  pdl_launch_dependents();
   if (RES || early_wait) pdl_wait();       // the predecessor reads the columns this kernel rewrites (or RES: G first)
+  pdl_launch_dependents();
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   double2 *sTl = reinterpret_cast<double2 *>(smem_raw + (size_t)warp * lineshape_scratch_bytes(S.n_inst4)) + lane;
   sTl[S.n_inst4 * 32] = make_double2(1.0, 0.0);        // unit lineshape slot
@@ -512,7 +518,6 @@ gram_stream_kernel(const __grid_constant__ StreamTab S, const __grid_constant__ 
   __shared__ bool last;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int KC = S.n_kc;
-  pdl_launch_dependents();                 // this kernel reads only the static cache until its final reduction
   const size_t t_bytes = align_up(lineshape_scratch_bytes(S.n_inst4), 128);
   const size_t x_bytes = align_up((size_t)32 * STRIDE * sizeof(double), 128);
   char *scratch = smem_raw + (size_t)warp * (t_bytes + x_bytes);
@@ -577,6 +582,8 @@ gram_stream_kernel(const __grid_constant__ StreamTab S, const __grid_constant__ 
   }
   __syncthreads();
   pdl_wait();                              // partials, ticket and G may still be in use by the predecessor
+  pdl_launch_dependents();                 // not earlier: a successor that skips its early wait relies on this kernel's
+                                           // predecessors being complete once it becomes resident
   for (int e = tid; e < NB * NB * 64; e += STREAM_BLOCK) {
     int bi = e / (NB * 64), bj = (e / 64) % NB;
     if (bi > bj) continue;

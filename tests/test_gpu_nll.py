@@ -433,3 +433,33 @@ def test_stale_column_tracking(B):
     h.set_params(par)                                            # all the way back
     assert h.nll() == fresh(par)
     columns_ok(par)
+
+
+@pytest.mark.parametrize("n,nn", [(300, 900), (70_000, 150_000)])
+def test_overlapped_launches_match_synchronous_calls(B, n, nn):
+    """The per-call kernels overlap through programmatic dependent launch (a successor becomes resident while its
+    predecessors drain).  A batched minuit-like trajectory (kernels back to back, every ordering of NLL / Gram / fused
+    kernels) must give, bit for bit, what one synchronous call per point gives -- on a grid that leaves SMs free for
+    early successors (small n) and on one that fills the GPU."""
+    mdl = samples.model_of(("C", 3))
+    par = W.initial_params(mdl)
+    if n <= 1000:
+        p4, t, _ = samples.data_sample(("C", 3), n)
+        p4n, _ = samples.flat_sample(nn)
+    else:                                                        # any physical events will do: raw candidates
+        p4, t, _, _ = oracle.candidates(mdl, par.tau, 7, 0, 0, n)
+        p4n, _, _, _ = oracle.candidates(mdl, par.tau, 7, 2, 0, nn)
+    traj = W.trajectory(mdl, par, 150, "minuit")
+    hb, hs = B.Tddp4(mdl), B.Tddp4(mdl)
+    for h in (hb, hs):
+        h.load_events(0, p4, t); h.load_events(1, p4n)
+    for rep in range(3):
+        vals, st = hb.nll_batch(hb.pack_params(traj))
+        assert not st.any()
+        if rep == 0:
+            ref = []
+            for p in traj:
+                hs.set_params(p)
+                ref.append(hs.nll())
+            ref = np.array(ref)
+        assert np.array_equal(vals, ref)
