@@ -85,7 +85,9 @@ typedef struct {
   int n_couplings;         /* K_c                                                                    */
   double t_lo, t_hi;       /* decay-time window of the normalisation; t_hi = +INFINITY allowed       */
   int use_resolution;      /* 0: eq. (1) as printed; 1: per-event Gaussian sigma_t (O-8): the data *
-                            * sample must be loaded with sigma_t > 0; P_i = R_i(t_i, sigma_i) / N_i(sigma_i)    */
+                            * sample must be loaded with sigma_t > 0; P_i = R_i(t_i, sigma_i) / N_i(sigma_i);   *
+                            * 2: time-integrated (decay time not measured): P_i = int_window R(p_i, t) dt / N,  *
+                            * the data sample is loaded without t and sigma_t                                    */
 } tddp4_model_desc;
 
 /* ---- life cycle -------------------------------------------------------------------------------- */

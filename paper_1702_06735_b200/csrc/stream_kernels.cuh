@@ -353,6 +353,17 @@ tres_kernel(const __grid_constant__ FaddTab F, const double *__restrict__ t, con
   for (int m = 0; m < 4; ++m) { tr[m * ld + i] = psi[m]; tr[(4 + m) * ld + i] = tint[m]; }
 }
 
+// Time-integrated mode (use_resolution = 2): every event has the same eight "time quantities", the window integrals
+// T_m themselves (psi_m = T_m: the rate integrated over the window; N_i = sum_m T_m S_m = N), so the resolution-mode
+// kernels evaluate P_i = F(p_i) / N unchanged.  vals: the eight row constants.
+struct Row8 { double v[8]; };
+__global__ void __launch_bounds__(256) fill_rows_kernel(double *__restrict__ rows, int64_t ld, int64_t n, Row8 vals) {
+  int64_t i = (int64_t)blockIdx.x * 256 + threadIdx.x;
+  if (i >= n) return;
+#pragma unroll
+  for (int m = 0; m < 8; ++m) rows[m * ld + i] = vals.v[m];
+}
+
 // The derivative rows of the data sample for the gradient in resolution mode (resolution.cuh): 8 rows per event.
 __global__ void __launch_bounds__(TRES_BLOCK)
 tres_grad_kernel(const __grid_constant__ FaddTab F, const double *__restrict__ t, const double *__restrict__ sigma_t, int64_t n,

@@ -405,7 +405,12 @@ int enqueue_nll(tddp4 *h, double *result, double *prob) {
   if (rc) return rc;
   if (h->use_resolution && !d.tres_valid && d.n > 0) {   // x, y, tau or the sample changed: rebuild the time rows
     int grid = (int)((d.n + TRES_BLOCK - 1) / TRES_BLOCK);
-    {
+    if (h->use_resolution == 2) {          // time-integrated: the rows are the window integrals, the same for every event
+      Row8 v;
+      for (int m = 0; m < 4; ++m) v.v[m] = v.v[4 + m] = h->RP.T[m];
+      Prof p(h, TDDP4_K_TRES, (double)d.n * 64.0);
+      fill_rows_kernel<<<(int)((d.n + 255) / 256), 256, 0, h->stream>>>(d.tr, d.ld, d.n, v);
+    } else {
       Prof p(h, TDDP4_K_TRES, (double)d.n * 80.0);
       tres_kernel<<<grid, TRES_BLOCK, 0, h->stream>>>(h->FT, d.t, d.sigma_t, d.n, h->RP.x, h->RP.y, h->RP.Gamma, h->t_lo, h->t_hi,
                                                       d.tr, d.ld);
@@ -499,6 +504,7 @@ int tddp4_create(const tddp4_model_desc *desc, tddp4 **out) {
       desc->n_couplings < 1 || desc->n_couplings > TDDP4_MAX_COUPLINGS)
     return bail(fail(h, TDDP4_ERR_ARG, "model size out of range"));
   if (!(desc->t_hi > desc->t_lo)) return bail(fail(h, TDDP4_ERR_ARG, "empty decay-time window"));
+  if (desc->use_resolution < 0 || desc->use_resolution > 2) return bail(fail(h, TDDP4_ERR_ARG, "use_resolution must be 0, 1 or 2"));
   h->res.assign(desc->res, desc->res + desc->n_res);
   h->terms.assign(desc->terms, desc->terms + desc->n_terms);
   h->t_lo = desc->t_lo; h->t_hi = desc->t_hi; h->use_resolution = desc->use_resolution;
@@ -691,8 +697,8 @@ int tddp4_load_events(tddp4 *h, int which, int64_t n, int64_t ld_in, const doubl
                       const double *sigma_t, const double *weight, int on_device) {
   if (!h) return TDDP4_ERR_ARG;
   if (which < 0 || which > 1 || n < 0 || ld_in < n || (n > 0 && !p4)) return fail(h, TDDP4_ERR_ARG, "bad load_events argument");
-  if (which == 0 && n > 0 && !t) return fail(h, TDDP4_ERR_ARG, "the data sample needs decay times");
-  if (which == 0 && n > 0 && h->use_resolution && !sigma_t)
+  if (which == 0 && n > 0 && !t && h->use_resolution != 2) return fail(h, TDDP4_ERR_ARG, "the data sample needs decay times");
+  if (which == 0 && n > 0 && h->use_resolution == 1 && !sigma_t)
     return fail(h, TDDP4_ERR_ARG, "use_resolution = 1: the data sample needs per-event sigma_t");
   CU(cudaStreamSynchronize(h->stream));
   h->prev_kind = PREV_NONE;
@@ -851,7 +857,13 @@ int tddp4_nll_grad(tddp4 *h, double *nll_out, double *grad_out) {
   if (h->use_resolution && !d.tresg_valid && d.n > 0) {   // derivative rows: rebuilt when x, y, tau or the sample changed
     if (!d.trg) CU(cudaMalloc(&d.trg, sizeof(double) * 8 * d.ld));
     int grid = (int)((d.n + TRES_BLOCK - 1) / TRES_BLOCK);
-    {
+    if (h->use_resolution == 2) {          // time-integrated: constant derivative rows (dT1/dx, dT3/dx, dT0/dy, dT2/dy) twice
+      GradParams gp = time_integral_derivatives(R.x, R.y, R.Gamma, h->t_lo, h->t_hi);
+      Row8 v;
+      v.v[0] = v.v[4] = gp.dT1dx; v.v[1] = v.v[5] = gp.dT3dx; v.v[2] = v.v[6] = gp.dT0dy; v.v[3] = v.v[7] = gp.dT2dy;
+      Prof p(h, TDDP4_K_TRES, (double)d.n * 64.0);
+      fill_rows_kernel<<<(int)((d.n + 255) / 256), 256, 0, h->stream>>>(d.trg, d.ld, d.n, v);
+    } else {
       Prof p(h, TDDP4_K_TRES, (double)d.n * 80.0);
       tres_grad_kernel<<<grid, TRES_BLOCK, 0, h->stream>>>(h->FT, d.t, d.sigma_t, d.n, R.x, R.y, R.Gamma, h->t_lo, h->t_hi, d.trg, d.ld);
     }

@@ -68,7 +68,7 @@ class Model:
     r_parent: float = 1.5
     t_lo: float = 0.0
     t_hi: float = math.inf
-    use_resolution: int = 0
+    use_resolution: int = 0      # 0: eq. (1); 1: per-event Gaussian decay-time resolution; 2: time-integrated (no t)
     res_names: list = field(default_factory=list)
     res_L: list = field(default_factory=list)
     res_mass: list = field(default_factory=list)    # nominal m0 (initial parameter values)
