@@ -203,11 +203,13 @@ class Tddp4:
         self.n[which] = n
 
     # -- tddp4_set_params -------------------------------------------------------------------------
-    def set_params(self, par):
-        """par: workloads.Params-like (c, cbar complex arrays; mass, width; x, y, tau)."""
+    def set_params(self, par, dbar=False):
+        """par: workloads.Params-like (c, cbar complex arrays; mass, width; x, y, tau).  dbar: this handle holds a
+        D0bar-tagged sample, for which the two amplitudes of eq. (1) exchange their roles: the coupling vectors are
+        handed over in the opposite order (marshalling only)."""
         b = self._pbuf                                   # preallocated marshalling buffers: no allocation per call
-        b[0][:] = par.c
-        b[1][:] = par.cbar
+        b[0][:] = par.cbar if dbar else par.c
+        b[1][:] = par.c if dbar else par.cbar
         if self.n_res:
             b[2][:, 0] = par.mass
             b[2][:, 1] = par.width

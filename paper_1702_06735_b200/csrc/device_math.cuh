@@ -234,14 +234,27 @@ __device__ __forceinline__ void mixing_functions(double u, double v, double &ch,
     sincos(v, &sn, &cs);
   }
 }
+// |A|^2, |Abar|^2, Re(A conj(Abar)), Im(A conj(Abar)) and the bracket itself with every contraction written out
+// (fma / __dmul_rn): the NLL, column-rebuilding and gradient kernels must produce the same bits for the same event, and
+// nvcc's default -fmad=true would otherwise be free to contract the sums differently per template instantiation.
+struct Bilinears { double aa, bb, cre, cim; };
+__device__ __forceinline__ Bilinears bilinears(double2 A, double2 Ab) {
+  Bilinears q;
+  q.aa = fma(A.x, A.x, __dmul_rn(A.y, A.y));
+  q.bb = fma(Ab.x, Ab.x, __dmul_rn(Ab.y, Ab.y));
+  q.cre = fma(A.x, Ab.x, __dmul_rn(A.y, Ab.y));
+  q.cim = fma(A.y, Ab.x, -__dmul_rn(A.x, Ab.y));
+  return q;
+}
+// (aa + bb) f0 + (aa - bb) f1 - 2 cre f2 - 2 cim f3: eq. (1) with f = (cosh, cos, sinh, sin), or its convolved / integrated forms
+__device__ __forceinline__ double rate_form(const Bilinears &q, double f0, double f1, double f2, double f3) {
+  return fma(__dadd_rn(q.aa, q.bb), f0, fma(__dsub_rn(q.aa, q.bb), f1, fma(-2.0 * q.cre, f2, __dmul_rn(-2.0 * q.cim, f3))));
+}
 template <bool SMALL>
 __device__ __forceinline__ double bracket(double2 A, double2 Ab, double u, double v) {
-  double aa = A.x * A.x + A.y * A.y, bb = Ab.x * Ab.x + Ab.y * Ab.y;
-  double cre = A.x * Ab.x + A.y * Ab.y;   // Re(A conj(Abar))
-  double cim = A.y * Ab.x - A.x * Ab.y;   // Im(A conj(Abar))
   double ch, sh, sn, cs;
   mixing_functions<SMALL>(u, v, ch, sh, cs, sn);
-  return (aa + bb) * ch + (aa - bb) * cs - 2.0 * cre * sh - 2.0 * cim * sn;
+  return rate_form(bilinears(A, Ab), ch, cs, sh, sn);
 }
 
 }  // namespace tddp4k

@@ -55,9 +55,9 @@ nll_grad_kernel(const double2 *__restrict__ a, const double *__restrict__ t, int
     for (int c = 0; c < KC; ++c) amp_add(A, Ab, R.c[c][0], R.c[c][1], R.cbar[c][0], R.cbar[c][1], v[c]);
     double ch, sh, cs, sn;
     mixing_functions<SMALL>(yG * ti, xG * ti, ch, sh, cs, sn);
-    const double aa = A.x * A.x + A.y * A.y, bb = Ab.x * Ab.x + Ab.y * Ab.y;
-    const double cre = A.x * Ab.x + A.y * Ab.y, cim = A.y * Ab.x - A.x * Ab.y;
-    const double B = (aa + bb) * ch + (aa - bb) * cs - 2.0 * cre * sh - 2.0 * cim * sn;   // same expression as bracket()
+    const Bilinears q = bilinears(A, Ab);
+    const double aa = q.aa, bb = q.bb, cre = q.cre, cim = q.cim;
+    const double B = rate_form(q, ch, cs, sh, sn);                                        // the bits of bracket()
     la.add(B);
     const double inv = 1.0 / B;
     const double gx = ((ch + cs) * A.x - (sh * Ab.x - sn * Ab.y)) * inv, gy = ((ch + cs) * A.y - (sh * Ab.y + sn * Ab.x)) * inv;
@@ -209,11 +209,11 @@ nll_grad_res_kernel(const double2 *__restrict__ a, const double *__restrict__ tr
     double2 A = make_double2(0.0, 0.0), Ab = make_double2(0.0, 0.0);
 #pragma unroll
     for (int c = 0; c < KC; ++c) amp_add(A, Ab, R.c[c][0], R.c[c][1], R.cbar[c][0], R.cbar[c][1], v[c]);
-    const double aa = A.x * A.x + A.y * A.y, bb = Ab.x * Ab.x + Ab.y * Ab.y;
-    const double cre = A.x * Ab.x + A.y * Ab.y, cim = A.y * Ab.x - A.x * Ab.y;
-    const double Rv = (aa + bb) * w[0] + (aa - bb) * w[1] - 2.0 * cre * w[2] - 2.0 * cim * w[3];   // as resolved_prob()
-    const double Nv = S1 * w[4] + S2 * w[5] - 2.0 * S3 * w[6] - 2.0 * S4 * w[7];
-    la.add(Rv / Nv);
+    const Bilinears q = bilinears(A, Ab);
+    const double aa = q.aa, bb = q.bb, cre = q.cre, cim = q.cim;
+    const double Rv = rate_form(q, w[0], w[1], w[2], w[3]);                                        // the bits of resolved_prob()
+    const double Nv = fma(S1, w[4], fma(S2, w[5], fma(-2.0 * S3, w[6], __dmul_rn(-2.0 * S4, w[7]))));
+    la.add(__ddiv_rn(Rv, Nv));
     const double invR = 1.0 / Rv, invN = 1.0 / Nv;
     const double gx = ((w[0] + w[1]) * A.x - (w[2] * Ab.x - w[3] * Ab.y)) * invR, gy = ((w[0] + w[1]) * A.y - (w[2] * Ab.y + w[3] * Ab.x)) * invR;
     const double hx = ((w[0] - w[1]) * Ab.x - (w[2] * A.x + w[3] * A.y)) * invR, hy = ((w[0] - w[1]) * Ab.y - (w[2] * A.y - w[3] * A.x)) * invR;

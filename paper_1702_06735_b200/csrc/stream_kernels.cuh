@@ -151,11 +151,9 @@ __device__ __forceinline__ double resolved_prob(double2 A, double2 Ab, const dou
   double v[8];
 #pragma unroll
   for (int m = 0; m < 8; ++m) v[m] = ldg_stream1(tr_i + m * ld);
-  double aa = A.x * A.x + A.y * A.y, bb = Ab.x * Ab.x + Ab.y * Ab.y;
-  double cre = A.x * Ab.x + A.y * Ab.y, cim = A.y * Ab.x - A.x * Ab.y;
-  double Rv = (aa + bb) * v[0] + (aa - bb) * v[1] - 2.0 * cre * v[2] - 2.0 * cim * v[3];
-  double Nv = s_S[0] * v[4] + s_S[1] * v[5] - 2.0 * s_S[2] * v[6] - 2.0 * s_S[3] * v[7];
-  return Rv / Nv;
+  double Rv = rate_form(bilinears(A, Ab), v[0], v[1], v[2], v[3]);
+  double Nv = fma(s_S[0], v[4], fma(s_S[1], v[5], fma(-2.0 * s_S[2], v[6], __dmul_rn(-2.0 * s_S[3], v[7]))));
+  return __ddiv_rn(Rv, Nv);
 }
 
 // common tail of the two NLL kernels (step 7, second pass).  Thread products -> warp -> block partial

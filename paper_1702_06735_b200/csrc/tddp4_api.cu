@@ -256,7 +256,7 @@ auto with_size_class(int cls, F &&f) {
 // launch with programmatic stream serialization (stream_kernels.cuh, pdl_*): the kernel may become resident while its
 // predecessor in the stream drains; it synchronises with it through griddepcontrol.wait
 template <class... KArgs, class... Args>
-void launch_pdl(void (*kernel)(KArgs...), int grid, int block, size_t smem, cudaStream_t stream, Args &&...args) {
+cudaError_t launch_pdl(void (*kernel)(KArgs...), int grid, int block, size_t smem, cudaStream_t stream, Args &&...args) {
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3((unsigned)grid);
   cfg.blockDim = dim3((unsigned)block);
@@ -267,8 +267,14 @@ void launch_pdl(void (*kernel)(KArgs...), int grid, int block, size_t smem, cuda
   at[0].val.programmaticStreamSerializationAllowed = 1;
   cfg.attrs = at;
   cfg.numAttrs = 1;
-  cudaLaunchKernelEx(&cfg, kernel, std::forward<Args>(args)...);
+  return cudaLaunchKernelEx(&cfg, kernel, std::forward<Args>(args)...);
 }
+// a failed launch leaves the handle's bookkeeping untouched (nothing was enqueued): the caller may retry
+#define CU_LAUNCH(expr)                                                                              \
+  do {                                                                                               \
+    cudaError_t e_ = (expr);                                                                         \
+    if (e_ != cudaSuccess) return fail(h, TDDP4_ERR_CUDA, "kernel launch: %s", cudaGetErrorString(e_)); \
+  } while (0)
 enum { PREV_NONE = 0, PREV_NLL = 1, PREV_COLNLL = 2, PREV_GRAM = 3 };
 
 template <int NB>
@@ -281,11 +287,10 @@ int launch_gram(tddp4 *h, const EventSet &e) {
   S.R = e.R;
   S.w_off = e.w ? (M.n_sys + S.n_inst4 + S.n_terms4) * 32 : -1;
   Prof p(h, TDDP4_K_GRAM, (double)e.n * (static_bytes_per_event(h) + (e.w ? 8.0 : 0.0)));
-  with_size_class(h->size_class, [&](auto ni, auto nt) {
-    launch_pdl(gram_stream_kernel<NB, decltype(ni)::value, decltype(nt)::value>, grid, STREAM_BLOCK,
-               gram_smem_bytes(NB, S.n_inst4), h->stream, S, h->LP, (const double *)e.cache, e.n, h->partials, h->ticket, h->G);
-    return 0;
-  });
+  CU_LAUNCH(with_size_class(h->size_class, [&](auto ni, auto nt) {
+    return launch_pdl(gram_stream_kernel<NB, decltype(ni)::value, decltype(nt)::value>, grid, STREAM_BLOCK,
+                      gram_smem_bytes(NB, S.n_inst4), h->stream, S, h->LP, (const double *)e.cache, e.n, h->partials, h->ticket, h->G);
+  }));
   h->prev_kind = PREV_GRAM;
   return TDDP4_OK;
 }
@@ -317,11 +322,11 @@ int launch_nll(tddp4 *h, const EventSet &e, double inv_n, double *result, bool s
   // the columns and t are untouched by a preceding NLL or Gram kernel: only the final reduction has to wait for it
   const int early = !(h->prev_kind == PREV_NLL || h->prev_kind == PREV_GRAM);
   if (small)
-    launch_pdl(nll_stream_kernel<KC, true>, grid, STREAM_BLOCK, 0, h->stream, (const double2 *)e.a, (const double *)e.t, e.ld, e.n, h->RP,
-               (const double *)h->G, inv_n, e.sum_t, h->partials, h->ticket, result, early);
+    CU_LAUNCH(launch_pdl(nll_stream_kernel<KC, true>, grid, STREAM_BLOCK, 0, h->stream, (const double2 *)e.a, (const double *)e.t, e.ld, e.n, h->RP,
+                         (const double *)h->G, inv_n, e.sum_t, h->partials, h->ticket, result, early));
   else
-    launch_pdl(nll_stream_kernel<KC, false>, grid, STREAM_BLOCK, 0, h->stream, (const double2 *)e.a, (const double *)e.t, e.ld, e.n, h->RP,
-               (const double *)h->G, inv_n, e.sum_t, h->partials, h->ticket, result, early);
+    CU_LAUNCH(launch_pdl(nll_stream_kernel<KC, false>, grid, STREAM_BLOCK, 0, h->stream, (const double2 *)e.a, (const double *)e.t, e.ld, e.n, h->RP,
+                         (const double *)h->G, inv_n, e.sum_t, h->partials, h->ticket, result, early));
   h->prev_kind = PREV_NLL;
   return TDDP4_OK;
 }
@@ -332,8 +337,8 @@ int launch_nll_res(tddp4 *h, const EventSet &e, double inv_n, double *result) {
   int rc = ensure_partials(h, (size_t)3 * grid + 16);
   if (rc) return rc;
   Prof p(h, TDDP4_K_NLL, (double)e.n * (16.0 * KC + 64.0));
-  launch_pdl(nll_res_kernel<KC>, grid, STREAM_BLOCK, 0, h->stream, (const double2 *)e.a, (const double *)e.tr, e.ld, e.n, h->RP,
-             (const double *)h->G, inv_n, h->partials, h->ticket, result);
+  CU_LAUNCH(launch_pdl(nll_res_kernel<KC>, grid, STREAM_BLOCK, 0, h->stream, (const double2 *)e.a, (const double *)e.tr, e.ld, e.n, h->RP,
+                       (const double *)h->G, inv_n, h->partials, h->ticket, result));
   h->prev_kind = PREV_NLL;
   return TDDP4_OK;
 }
@@ -353,18 +358,18 @@ int launch_colnll(tddp4 *h, const EventSet &e, double inv_n, double *result, boo
   const int early = h->prev_kind != PREV_GRAM;   // a Gram kernel neither reads nor writes the columns this kernel rewrites
   const double sum_t = h->use_resolution ? 0.0 : e.sum_t;
   const double *tp = h->use_resolution ? e.tr : e.t;
-  with_size_class(h->size_class, [&](auto ni, auto nt) {
-    constexpr int NI = decltype(ni)::value, NT = decltype(nt)::value;
 #define COLNLL_LAUNCH(SM, RS)                                                                                                  \
   launch_pdl(colnll_stream_kernel<SM, RS, NI, NT>, grid, STREAM_BLOCK, smem, h->stream, S, h->LP, (const double *)e.cache, tp, e.ld, e.n, \
              e.a, h->RP, (const double *)h->G, inv_n, sum_t, h->partials, h->ticket, result, early, h->store_mask)
-    if (mode == 2) COLNLL_LAUNCH(false, true);
-    else if (mode == 1) COLNLL_LAUNCH(true, false);
-    else COLNLL_LAUNCH(false, false);
-#undef COLNLL_LAUNCH
-    return 0;
+  cudaError_t launched = with_size_class(h->size_class, [&](auto ni, auto nt) {
+    constexpr int NI = decltype(ni)::value, NT = decltype(nt)::value;
+    if (mode == 2) return COLNLL_LAUNCH(false, true);
+    if (mode == 1) return COLNLL_LAUNCH(true, false);
+    return COLNLL_LAUNCH(false, false);
   });
-  h->prev_kind = PREV_COLNLL;
+#undef COLNLL_LAUNCH
+  CU_LAUNCH(launched);
+  h->prev_kind = PREV_COLNLL;   // committed only after the launch succeeded: a failed launch keeps the stale-column set
   h->store_mask = 0;
   return TDDP4_OK;
 }
@@ -644,6 +649,7 @@ int tddp4_create(const tddp4_model_desc *desc, tddp4 **out) {
   if (!ok) return bail(fail(h, TDDP4_ERR_CUDA, "allocation failed: %s", cudaGetErrorString(cudaGetLastError())));
   // kernels that need more than 48 KB of dynamic shared memory
   cudaFuncSetAttribute(gen_ratio_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)gen_smem_bytes(MAX_SYS, MAX_INST));
+  cudaFuncSetAttribute(kin_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(sizeof(double) * (16 + MAX_SYS + MAX_INST) * KIN_BLOCK));
   {   // shared memory of the per-call kernels: per-warp lineshape scratch (+ the X tile of the Gram kernel)
     int NB = (KC + 3) / 4;
     size_t limit = prop.sharedMemPerBlockOptin - 1024, sc = colnll_smem_bytes(h->S.n_inst4), sg = gram_smem_bytes(NB, h->S.n_inst4);

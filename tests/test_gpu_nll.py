@@ -309,6 +309,32 @@ def test_sharded_evaluation_adds_up(B):
     assert abs(nll - full) < 1e-12 * abs(full)
 
 
+def test_dbar_tagged_sample(B):
+    """SURVEY.md 8(f) NEXT-2, D0bar-tagged sample: a handle holding the D0bar-tagged events is fed the two coupling vectors
+    exchanged (binding: set_params(par, dbar=True)); the oracle writes the D0bar rate and its normalisation out
+    explicitly (oracle/tagged.py).  Both tags share one normalisation sample and one parameter point."""
+    from oracle import tagged as OT
+    mdl = samples.model_of(("C", 2))
+    par = W.initial_params(mdl)
+    par.x, par.y = 0.21, 0.13                       # large mixing: the cos and sin terms, which change sign, matter
+    p4, t, _ = samples.data_sample(("C", 2), 4_133)
+    p4n, _ = samples.flat_sample(20_011)
+    tag = np.where(np.random.default_rng(9).uniform(size=p4.shape[1]) < 0.5, 1, -1)
+    ref_nll, ref_P = OT.nll_tagged(mdl, par, p4, t, tag, p4n)
+    total, P = 0.0, np.empty(p4.shape[1])
+    for sign in (1, -1):
+        sel = np.nonzero(tag == sign)[0]
+        h = B.Tddp4(mdl)
+        h.load_events(0, np.ascontiguousarray(p4[:, sel]), t[sel].copy())
+        h.load_events(1, p4n)
+        h.set_params(par, dbar=sign < 0)
+        prob = h.empty(len(sel))
+        total += h.nll(prob)
+        P[sel] = prob.cpu().numpy()
+    assert samples.rel_err(P, ref_P) < TOL_P
+    assert nll_close(total, ref_nll, np.log(ref_P))
+
+
 def test_large_mixing_phases_use_the_full_range_functions(B):
     """x, y far from the small-phase regime: the kernels switch from Taylor polynomials to exp / sincos."""
     mdl = samples.model_of(("C", 2))
@@ -383,6 +409,39 @@ def test_maximum_model_size(B):
     check_against_oracle(B, odd, par, p4, t, p4n, w)
     with pytest.raises(B.Tddp4Error):
         B.Tddp4(W.build_model(list(range(1, 9)) * 2 + [1], bose=True))   # 17 couplings / 34 terms: refused at create
+
+
+def many_instance_model():
+    """24 de-duplicated lineshape instances on 10 particle systems (the limits of the tables are 24 and 12): two copies of
+    the resonance list under different names, the second copy's K* rho chain on the systems (0,2), (1,3)."""
+    mdl = W.Model()
+    for copy in (0, 1):
+        for nm, (m0, g0, L) in W.RESONANCES.items():
+            mdl.res_names.append(f"{nm}#{copy}"); mdl.res_L.append(L)
+            mdl.res_mass.append(m0 * (1.0 + 0.01 * copy)); mdl.res_width.append(g0 * (1.0 + 0.1 * copy))
+    names = list(W.RESONANCES)
+    for copy, chains in ((0, (1, 2, 3, 4, 5)), (1, (1, 2, 3, 4))):
+        for cid in chains:
+            sf, res, perm = W.CHAINS[cid]
+            if copy == 1 and cid == 1:
+                perm = (0, 2, 1, 3)
+            idx = tuple(names.index(r) + 6 * copy for r in res)
+            for pm in (perm, W._swap13(perm)):
+                mdl.term_sf.append(sf); mdl.term_res.append(idx); mdl.term_perm.append(tuple(pm))
+                mdl.term_coupling.append(mdl.n_couplings)
+            mdl.n_couplings += 1
+    return mdl
+
+
+def test_many_lineshape_instances(B):
+    """n_sys + n_inst = 34: the kinematics kernel needs more than 48 KB of dynamic shared memory (opt-in attribute)."""
+    mdl = many_instance_model()
+    par = W.initial_params(mdl)
+    p4, t, _ = samples.data_sample(("C", 3), 515)
+    p4n, _ = samples.flat_sample(1_301)
+    h = check_against_oracle(B, mdl, par, p4, t, p4n)
+    lay = h.layout()
+    assert len(lay["inst_res"]) == 24 and len(lay["sys_mask"]) == 10
 
 
 def test_stale_column_tracking(B):
