@@ -158,6 +158,26 @@ int tddp4_gram_override(tddp4 *h, const double *G_sum, int64_t n_norm);
 /* N for the current parameters from the Gram matrix in force; host out.                              */
 int tddp4_norm(tddp4 *h, double *norm_out);
 
+/* ---- event-sharded evaluation: the same exchange without a host round trip --------
+ * One process per GPU holds a contiguous block of both samples.  Per call each rank enqueues
+ *   tddp4_gram_enqueue   (only when a mass or width moved)  -> all-gather of 2 K_c^2 + 1 doubles -> tddp4_gram_reduce
+ *   tddp4_nll_enqueue                                        -> all-gather of 8 doubles           -> sum in rank order
+ * on the handle's stream; the collective (NCCL, the caller's) runs on that same stream between them, so nothing
+ * synchronises until the gathered result words are read.
+ * tddp4_gram_enqueue: G_dev device [2 K_c^2 + 1] receives this rank's Gram sums ([K_c][K_c][2]) followed by its
+ *   normalisation event count as a double (refreshed first if stale; an override in force is dropped).
+ * tddp4_gram_reduce: gathered_dev device [world][2 K_c^2 + 1]; the handle's Gram matrix becomes the sum over ranks,
+ *   added in rank order by one kernel (same bits on every rank), normalised by n_norm_total.  Stays in force
+ *   until the masses/widths change or the normalisation sample is reloaded.
+ * tddp4_nll_enqueue: result_dev device [8]: words 0..4 as tddp4_nll_parts ([3] = this rank's NLL term
+ *   Gamma sum t - sum log B + n log N with the Gram matrix in force), [5] = sequence stamp, [6..7] unused.
+ * tddp4_gram_state: *valid = the matrix in force matches the current masses/widths; *overridden = it came from
+ *   tddp4_gram_override / tddp4_gram_reduce.                                                           */
+int tddp4_gram_enqueue(tddp4 *h, double *G_dev);
+int tddp4_gram_reduce(tddp4 *h, const double *gathered_dev, int world, int64_t n_norm_total);
+int tddp4_nll_enqueue(tddp4 *h, double *result_dev);
+int tddp4_gram_state(const tddp4 *h, int *valid, int *overridden);
+
 /* ---- companion path: generation (G1-G6) ---------------------------------------------------------- */
 /* Candidates first .. first+n_candidates-1 of Philox stream (seed, stream_id) are generated by
  * Raubold-Lynch with t ~ Exp(tau), weighted by w B (eq. 1 with the current parameters) and accepted
@@ -213,6 +233,10 @@ int tddp4_profile_read(tddp4 *h, int kernel_id, double *total_ms, int64_t *launc
 int tddp4_profile_reset(tddp4 *h);
 /* Number of kernels this handle has launched since creation (all kinds).                            */
 int64_t tddp4_launch_count(const tddp4 *h);
+/* Measured fp64 issue rate of this GPU: a dependent-free chain of DFMA instructions on every SM (the
+ * denominator of the "alu"-bound fractions of the generator, kinematics and time-row kernels).  Host out:
+ * fp64 instructions per second (one per lane; an FMA counts once).  Synchronous, ~1 ms.              */
+int tddp4_fp64_peak(tddp4 *h, double *inst_per_s);
 
 #ifdef __cplusplus
 }

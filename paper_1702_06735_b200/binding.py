@@ -25,7 +25,8 @@ SYMBOLS = ["tddp4_create", "tddp4_destroy", "tddp4_set_stream", "tddp4_last_erro
            "tddp4_load_events", "tddp4_set_params", "tddp4_nll", "tddp4_nll_async", "tddp4_nll_result",
            "tddp4_nll_parts", "tddp4_nll_grad", "tddp4_param_stride", "tddp4_nll_batch", "tddp4_gram", "tddp4_gram_override", "tddp4_norm", "tddp4_generate", "tddp4_weight_bound",
            "tddp4_candidates", "tddp4_get", "tddp4_layout", "tddp4_profile", "tddp4_profile_read",
-           "tddp4_profile_reset", "tddp4_launch_count"]
+           "tddp4_profile_reset", "tddp4_launch_count", "tddp4_gram_enqueue", "tddp4_gram_reduce", "tddp4_nll_enqueue",
+           "tddp4_gram_state", "tddp4_fp64_peak"]
 
 
 class Tddp4Error(RuntimeError):
@@ -91,6 +92,11 @@ def load_library():
     L.tddp4_profile_reset.argtypes = [vp]
     L.tddp4_launch_count.argtypes = [vp]
     L.tddp4_launch_count.restype = i64
+    L.tddp4_gram_enqueue.argtypes = [vp, vp]
+    L.tddp4_gram_reduce.argtypes = [vp, vp, C.c_int, i64]
+    L.tddp4_nll_enqueue.argtypes = [vp, vp]
+    L.tddp4_gram_state.argtypes = [vp, C.POINTER(C.c_int), C.POINTER(C.c_int)]
+    L.tddp4_fp64_peak.argtypes = [vp, dp]
     _lib = L
     return L
 
@@ -146,6 +152,7 @@ class Tddp4:
             self._h = None
             raise Tddp4Error(rc, text)
         self.n = [0, 0]
+        self.stream = None
         c, cb = np.empty(self.kc, np.complex128), np.empty(self.kc, np.complex128)
         mw = np.zeros((max(1, self.n_res), 2))
         self._pbuf = (c, cb, mw, c.ctypes.data, cb.ctypes.data, mw.ctypes.data)
@@ -177,6 +184,7 @@ class Tddp4:
     def set_stream(self, stream):
         """stream: torch.cuda.Stream (or None for the legacy default stream)."""
         self._check(self.lib.tddp4_set_stream(self._h, stream.cuda_stream if stream is not None else None))
+        self.stream = stream
 
     def empty(self, *shape, dtype=None):
         return self._torch.empty(*shape, dtype=dtype or self._torch.float64, device=self.device)
@@ -275,6 +283,29 @@ class Tddp4:
     def gram_override(self, G_sum, n_norm):
         G = np.ascontiguousarray(np.stack([np.real(G_sum), np.imag(G_sum)], axis=-1), dtype=np.float64)
         self._check(self.lib.tddp4_gram_override(self._h, G.ctypes.data, int(n_norm)))
+
+    # -- event-sharded evaluation: everything stays on the handle's stream --------------------------------
+    def gram_enqueue(self, G_dev):
+        """G_dev: CUDA tensor [2 K_c^2 + 1] <- this rank's Gram sums and its normalisation event count."""
+        self._check(self.lib.tddp4_gram_enqueue(self._h, _ptr(G_dev)))
+
+    def gram_reduce(self, gathered_dev, world, n_norm_total):
+        """gathered_dev: CUDA tensor [world][2 K_c^2 + 1]; the rank-ordered sum becomes the Gram matrix in force."""
+        self._check(self.lib.tddp4_gram_reduce(self._h, _ptr(gathered_dev), int(world), int(n_norm_total)))
+
+    def nll_enqueue(self, result_dev):
+        """result_dev: CUDA tensor [8] <- (sum log B, sum t, N, NLL term, #bad, stamp, -, -) of this rank."""
+        self._check(self.lib.tddp4_nll_enqueue(self._h, _ptr(result_dev)))
+
+    def gram_state(self):
+        v, o = C.c_int(), C.c_int()
+        self._check(self.lib.tddp4_gram_state(self._h, C.byref(v), C.byref(o)))
+        return bool(v.value), bool(o.value)
+
+    def fp64_peak(self):
+        out = C.c_double()
+        self._check(self.lib.tddp4_fp64_peak(self._h, C.byref(out)))
+        return out.value
 
     def norm(self):
         out = C.c_double()

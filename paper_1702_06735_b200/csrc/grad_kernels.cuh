@@ -11,6 +11,13 @@
 // ubar = cbar^T G / n):   dN/dc_k* = (T0+T1) u_k - (T2 + i T3) ubar_k,   dN/dcbar_k* = (T0-T1) ubar_k - (T2 - i T3) u_k,
 //     dN/dx = T1' (nAA - nBB) - 2 T3' Im X,   dN/dy = T0' (nAA + nBB) - 2 T2' Re X,
 // and writes  grad = -(data part) + n (dN/dtheta) / N.   Deterministic: fixed-order block and grid reductions.
+//
+// The 4 K_c coupling sums are ONE dense contraction over events, D = W^T X with W_i = (Re gA, Im gA, Re gAbar, Im gAbar)_i / B_i
+// and X_i = (Re a_i0, Im a_i0, Re a_i1, ...): it runs on the fp64 tensor cores (mma.sync m8n8k4, SASS DMMA), 4 events per
+// instruction, from per-warp shared-memory tiles laid out as in the Gram kernel (conflict-free stores and fragment loads).
+// A thread then carries 2 NB accumulator registers instead of 4 K_c + 2 (the scalar form held 34 accumulators next to the
+// 8 columns of its event and spilled: 31 STL / 26 LDL in the loop at 128 registers, 58.7 us per 1 M events, 0.35 of the
+// HBM roofline).
 #pragma once
 
 namespace tddp4k {
@@ -22,72 +29,65 @@ struct GradParams {
 // result layout: [0..4] as the NLL kernels (sum log B, sum t, N, NLL, #bad), [8 ...] the 4 K_c + 2 gradient entries
 constexpr int GRAD_OFFSET = 8;
 
-template <int KC, bool SMALL>
-__global__ void __launch_bounds__(STREAM_BLOCK, KC <= 8 ? 2 : 1)
-nll_grad_kernel(const double2 *__restrict__ a, const double *__restrict__ t, int64_t ld, int64_t n,
-                const __grid_constant__ RateParams R, const __grid_constant__ GradParams GP, const double *__restrict__ G,
-                double inv_n_norm, double sum_t, double *__restrict__ partials /* [grid][NA + 3] */, unsigned int *ticket,
-                double *__restrict__ result) {
-  constexpr int NA = 4 * KC + 2, PS = NA + 3;
-  __shared__ double s_red[STREAM_WARPS][NA];
-  __shared__ double s_sum[NA];
-  __shared__ double s_p[STREAM_WARPS];
-  __shared__ long long s_e[STREAM_WARPS];
-  __shared__ int s_b[STREAM_WARPS];
-  __shared__ double s_n[4];
-  __shared__ double2 s_u[KC], s_ub[KC];
-  __shared__ bool last;
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  MantAcc la;
-  double acc[NA];
+// shared-memory tiles of one warp: X [32][gram_stride(NB)] (event-major, as the Gram kernel), W [32][GRAD_WS] (rows 4..7 zero)
+constexpr int GRAD_WS = 10;
+// resident blocks per SM (the kernel is latency-bound on its 9 loads per event: 24 warps per SM where the registers allow it)
+template <int KC> __host__ __device__ constexpr int grad_bps() { return KC <= 8 ? 3 : 2; }
+template <int KC> __host__ __device__ constexpr int grad_nb() { return (KC + 3) / 4; }
+template <int KC> __host__ __device__ constexpr size_t grad_warp_bytes() {
+  return align_up((size_t)32 * gram_stride(grad_nb<KC>()) * sizeof(double), 128) + align_up((size_t)32 * GRAD_WS * sizeof(double), 128);
+}
+template <int KC> inline size_t grad_smem_bytes() { return STREAM_WARPS * grad_warp_bytes<KC>(); }
+
+// D += W^T X over the warp's 32 events: acc[b] holds the C fragment of feature block b (row = weight lane >> 2,
+// columns 2 (lane & 3) + {0, 1}); group g takes the events 8 (g >> 1) + 2 (lane & 3) + (g & 1) (bank-conflict free)
+template <int NB>
+__device__ __forceinline__ void grad_mma_tile(const double *Xs, const double *Ws, double (&acc)[NB][2]) {
+  constexpr int XS = gram_stride(NB);
+  const int lane = threadIdx.x & 31;
+  __syncwarp();
+  const double *xb = Xs + (2 * (lane & 3)) * XS + (lane >> 2);
+  const double *wb = Ws + (2 * (lane & 3)) * GRAD_WS + (lane >> 2);
 #pragma unroll
-  for (int j = 0; j < NA; ++j) acc[j] = 0.0;
-  const double yG = R.y * R.Gamma, xG = R.x * R.Gamma;
-  const int64_t stride = (int64_t)gridDim.x * STREAM_BLOCK;
-#pragma unroll 1
-  for (int64_t i = (int64_t)blockIdx.x * STREAM_BLOCK + tid; i < n; i += stride) {
-    double2 v[KC];
+  for (int grp = 0; grp < 8; ++grp) {
+    const int e0 = 8 * (grp >> 1) + (grp & 1);
+    const double w = wb[e0 * GRAD_WS];
 #pragma unroll
-    for (int c = 0; c < KC; ++c) v[c] = ldg_stream2(a + c * ld + i);
-    const double ti = ldg_stream1(t + i);
-    double2 A = make_double2(0.0, 0.0), Ab = make_double2(0.0, 0.0);
-#pragma unroll
-    for (int c = 0; c < KC; ++c) amp_add(A, Ab, R.c[c][0], R.c[c][1], R.cbar[c][0], R.cbar[c][1], v[c]);
-    double ch, sh, cs, sn;
-    mixing_functions<SMALL>(yG * ti, xG * ti, ch, sh, cs, sn);
-    const Bilinears q = bilinears(A, Ab);
-    const double aa = q.aa, bb = q.bb, cre = q.cre, cim = q.cim;
-    const double B = rate_form(q, ch, cs, sh, sn);                                        // the bits of bracket()
-    la.add(B);
-    const double inv = 1.0 / B;
-    const double gx = ((ch + cs) * A.x - (sh * Ab.x - sn * Ab.y)) * inv, gy = ((ch + cs) * A.y - (sh * Ab.y + sn * Ab.x)) * inv;
-    const double hx = ((ch - cs) * Ab.x - (sh * A.x + sn * A.y)) * inv, hy = ((ch - cs) * Ab.y - (sh * A.y - sn * A.x)) * inv;
-#pragma unroll
-    for (int c = 0; c < KC; ++c) {
-      acc[2 * c] = fma(gx, v[c].x, fma(gy, v[c].y, acc[2 * c]));                 // Re conj(gA) a_c
-      acc[2 * c + 1] = fma(gx, v[c].y, fma(-gy, v[c].x, acc[2 * c + 1]));         // Im conj(gA) a_c
-      acc[2 * KC + 2 * c] = fma(hx, v[c].x, fma(hy, v[c].y, acc[2 * KC + 2 * c]));
-      acc[2 * KC + 2 * c + 1] = fma(hx, v[c].y, fma(-hy, v[c].x, acc[2 * KC + 2 * c + 1]));
-    }
-    const double gt = R.Gamma * ti * inv;
-    acc[4 * KC] += gt * (-(aa - bb) * sn - 2.0 * cim * cs);
-    acc[4 * KC + 1] += gt * ((aa + bb) * sh - 2.0 * cre * ch);
+    for (int b = 0; b < NB; ++b) dmma884(acc[b][0], acc[b][1], w, xb[e0 * XS + 8 * b]);
   }
-  // block partials, fixed order: lanes by butterfly, warps in index order
+  __syncwarp();
+}
+
+// Block and grid reduction of the gradient sums.  Per block: NB * 32 tensor-core sums C_b[m][n] (m < 4 weights, n < 8
+// features), NS scalar sums, the mantissa product.  Returns true in the last block, with the grid totals in s_sum
+// ([NB * 32 + NS]) and the merged product in s_p[0], s_e[0], s_b[0].
+template <int NB, int NS>
+__device__ __forceinline__ bool grad_reduce(double (&acc)[NB][2], double (&sc)[NS], MantAcc la, double *__restrict__ partials,
+                                            unsigned int *ticket, double *s_red /* [WARPS][NB*32+NS] */, double *s_sum,
+                                            double *s_p, long long *s_e, int *s_b, bool *last) {
+  constexpr int NC = NB * 32, NA = NC + NS, PS = NA + 3;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  if (lane < 16) {
 #pragma unroll
-  for (int j = 0; j < NA; ++j) {
-    double s = warp_sum(acc[j]);
-    if (lane == 0) s_red[warp][j] = s;
+    for (int b = 0; b < NB; ++b) {
+      s_red[warp * NA + b * 32 + (lane >> 2) * 8 + 2 * (lane & 3)] = acc[b][0];
+      s_red[warp * NA + b * 32 + (lane >> 2) * 8 + 2 * (lane & 3) + 1] = acc[b][1];
+    }
+  }
+#pragma unroll
+  for (int j = 0; j < NS; ++j) {
+    double v = warp_sum(sc[j]);
+    if (lane == 0) s_red[warp * NA + NC + j] = v;
   }
   warp_merge(la);
   if (lane == 0) { s_p[warp] = la.prod; s_e[warp] = la.esum; s_b[warp] = la.bad; }
   __syncthreads();
   double *mine = partials + (int64_t)blockIdx.x * PS;
   for (int j = tid; j < NA; j += STREAM_BLOCK) {
-    double s = 0.0;
+    double v = 0.0;
 #pragma unroll
-    for (int w = 0; w < STREAM_WARPS; ++w) s += s_red[w][j];
-    mine[j] = s;
+    for (int w = 0; w < STREAM_WARPS; ++w) v += s_red[w * NA + j];
+    mine[j] = v;
   }
   if (tid == 0) {
     MantAcc m;
@@ -98,46 +98,163 @@ nll_grad_kernel(const double2 *__restrict__ a, const double *__restrict__ t, int
   }
   __threadfence();
   __syncthreads();
-  if (tid == 0) last = atomicAdd(ticket, 1u) == gridDim.x - 1;
+  if (tid == 0) *last = atomicAdd(ticket, 1u) == gridDim.x - 1;
   __syncthreads();
-  if (!last) return;
+  if (!*last) return false;
   __threadfence();
-  // last block: sums over blocks (16 chains per entry, fixed tree), mantissa products merged in block order by warp 0
-  for (int j = tid; j < NA; j += STREAM_BLOCK) {
-    double part[16];
+  // last block: column sums over the block partials.  Warp w takes the blocks b = w, w + WARPS, ...; its lanes cover the
+  // entries j = lane, lane + 32, ... (coalesced rows of the partial array), every load independent of the others, eight
+  // blocks in flight per lane; the warps' sums are then added in warp order.  Fixed tree: same bits every run.  (The
+  // first version gave each entry to one thread that walked all blocks in rounds of 16 loads: 66 busy threads, 19
+  // dependent L2 round trips -- about 25 of the kernel's 57 us at 1 M events, measured as SM-active time with ncu.)
+  {
+    constexpr int SLOTS = (NA + 31) / 32;
+    double sum[SLOTS];
 #pragma unroll
-    for (int c = 0; c < 16; ++c) part[c] = 0.0;
-    for (unsigned b = 0; b < gridDim.x; b += 16) {
+    for (int q = 0; q < SLOTS; ++q) sum[q] = 0.0;
+    unsigned b = warp;
+    for (; b + 7 * STREAM_WARPS < gridDim.x; b += 8 * STREAM_WARPS) {
+      double v[8][SLOTS];
 #pragma unroll
-      for (int c = 0; c < 16; ++c)
-        if (b + c < gridDim.x) part[c] += __ldcg(partials + (int64_t)(b + c) * PS + j);
+      for (int r = 0; r < 8; ++r)
+#pragma unroll
+        for (int q = 0; q < SLOTS; ++q) {
+          const int j = lane + 32 * q;
+          v[r][q] = j < NA ? __ldcg(partials + (int64_t)(b + r * STREAM_WARPS) * PS + j) : 0.0;
+        }
+#pragma unroll
+      for (int r = 0; r < 8; ++r)
+#pragma unroll
+        for (int q = 0; q < SLOTS; ++q) sum[q] += v[r][q];
     }
-    double s = 0.0;
+    for (; b < gridDim.x; b += STREAM_WARPS) {
 #pragma unroll
-    for (int c = 0; c < 16; ++c) s += part[c];
-    s_sum[j] = s;
+      for (int q = 0; q < SLOTS; ++q) {
+        const int j = lane + 32 * q;
+        if (j < NA) sum[q] += __ldcg(partials + (int64_t)b * PS + j);
+      }
+    }
+    __syncthreads();                                        // s_red of the first stage is free
+#pragma unroll
+    for (int q = 0; q < SLOTS; ++q) {
+      const int j = lane + 32 * q;
+      if (j < NA) s_red[warp * NA + j] = sum[q];
+    }
   }
-  MantAcc m;
+  __syncthreads();
+  for (int j = tid; j < NA; j += STREAM_BLOCK) {
+    double v = 0.0;
+#pragma unroll
+    for (int w = 0; w < STREAM_WARPS; ++w) v += s_red[w * NA + j];
+    s_sum[j] = v;
+  }
   if (warp == STREAM_WARPS - 1) {
-    for (unsigned b = lane; b < gridDim.x; b += 32) {
-      const double *pb = partials + (int64_t)b * PS + NA;
-      m.merge(__ldcg(pb), (long long)__ldcg(pb + 1), (int)__ldcg(pb + 2));
+    MantAcc m;
+    constexpr int PER = 10;                                 // up to 320 blocks with every load in flight at once
+    double pp[PER], pe[PER], pb[PER];
+#pragma unroll
+    for (int r = 0; r < PER; ++r) {
+      const unsigned b = lane + 32 * r;
+      const bool ok = b < gridDim.x;
+      const double *src = partials + (int64_t)(ok ? b : 0) * PS + NA;
+      pp[r] = ok ? __ldcg(src) : 1.0; pe[r] = ok ? __ldcg(src + 1) : 0.0; pb[r] = ok ? __ldcg(src + 2) : 0.0;
+    }
+#pragma unroll
+    for (int r = 0; r < PER; ++r) { m.merge(pp[r], (long long)pe[r], (int)pb[r]); m.renorm(); }
+    for (unsigned b = lane + 32 * PER; b < gridDim.x; b += 32) {
+      const double *src = partials + (int64_t)b * PS + NA;
+      m.merge(__ldcg(src), (long long)__ldcg(src + 1), (int)__ldcg(src + 2));
       m.renorm();
     }
     warp_merge(m);
     if (lane == 0) { s_p[0] = m.prod; s_e[0] = m.esum; s_b[0] = m.bad; }
-  } else if (warp == 1) {
-    double nAA, nBB, xr, xi;
-    gram_sums_warp(R, G, KC, inv_n_norm, nAA, nBB, xr, xi);
-    if (lane == 0) { s_n[0] = nAA; s_n[1] = nBB; s_n[2] = xr; s_n[3] = xi; }
-  } else if (warp == 2 && lane < KC) {
-    double2 u = make_double2(0.0, 0.0), ub = make_double2(0.0, 0.0);   // u_k = sum_j c_j G_jk / n, ubar_k with cbar
+  }
+  return true;
+}
+// sum_i W_i[m] X_i[f] from the reduced tiles
+__device__ __forceinline__ double grad_c(const double *s_sum, int m, int f) { return s_sum[(f >> 3) * 32 + m * 8 + (f & 7)]; }
+// u_k = sum_j c_j G_jk / n and ubar_k (Hermitian G): one lane per k
+template <int KC>
+__device__ __forceinline__ void grad_gram_vectors(const RateParams &R, const double *__restrict__ G, double inv_n_norm, int lane,
+                                                  double2 *s_u, double2 *s_ub) {
+  if (lane < KC) {
+    double2 u = make_double2(0.0, 0.0), ub = make_double2(0.0, 0.0);
     for (int j = 0; j < KC; ++j) {
       double gr = __ldcg(G + (j * KC + lane) * 2) * inv_n_norm, gi = __ldcg(G + (j * KC + lane) * 2 + 1) * inv_n_norm;
       u.x += R.c[j][0] * gr - R.c[j][1] * gi;    u.y += R.c[j][0] * gi + R.c[j][1] * gr;
       ub.x += R.cbar[j][0] * gr - R.cbar[j][1] * gi;  ub.y += R.cbar[j][0] * gi + R.cbar[j][1] * gr;
     }
     s_u[lane] = u; s_ub[lane] = ub;
+  }
+}
+
+template <int KC, bool SMALL>
+__global__ void __launch_bounds__(STREAM_BLOCK, grad_bps<KC>())
+nll_grad_kernel(const double2 *__restrict__ a, const double *__restrict__ t, int64_t ld, int64_t n,
+                const __grid_constant__ RateParams R, const __grid_constant__ GradParams GP, const double *__restrict__ G,
+                double inv_n_norm, double sum_t, double *__restrict__ partials /* [grid][NB * 32 + 5] */, unsigned int *ticket,
+                double *__restrict__ result) {
+  constexpr int NB = grad_nb<KC>(), XS = gram_stride(NB), NS = 2, NA = NB * 32 + NS;
+  extern __shared__ __align__(16) char smem_raw[];
+  __shared__ double s_red[STREAM_WARPS * NA];
+  __shared__ double s_sum[NA];
+  __shared__ double s_p[STREAM_WARPS];
+  __shared__ long long s_e[STREAM_WARPS];
+  __shared__ int s_b[STREAM_WARPS];
+  __shared__ double s_n[4];
+  __shared__ double2 s_u[KC], s_ub[KC];
+  __shared__ bool last;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  double *Xs = reinterpret_cast<double *>(smem_raw + (size_t)warp * grad_warp_bytes<KC>());
+  double *Wt = Xs + align_up((size_t)32 * XS * sizeof(double), 128) / sizeof(double);
+  double *xrow = Xs + lane * XS, *wrow = Wt + lane * GRAD_WS;
+#pragma unroll
+  for (int c = 0; c < XS; ++c) xrow[c] = 0.0;               // features beyond 2 K_c and the weight rows 4..7 stay zero
+#pragma unroll
+  for (int c = 0; c < GRAD_WS; ++c) wrow[c] = 0.0;
+  MantAcc la;
+  double acc[NB][2], sc[NS] = {0.0, 0.0};
+#pragma unroll
+  for (int b = 0; b < NB; ++b) acc[b][0] = acc[b][1] = 0.0;
+  const double yG = R.y * R.Gamma, xG = R.x * R.Gamma;
+  const int64_t stride = (int64_t)gridDim.x * STREAM_BLOCK;
+#pragma unroll 1
+  for (int64_t i0 = (int64_t)blockIdx.x * STREAM_BLOCK + warp * 32; i0 < n; i0 += stride) {   // whole warps: the MMA is warp-wide
+    const int64_t i = i0 + lane;
+    const bool live = i < n;
+    double2 v[KC];
+#pragma unroll
+    for (int c = 0; c < KC; ++c) v[c] = live ? ldg_stream2(a + c * ld + i) : make_double2(0.0, 0.0);
+    const double ti = live ? ldg_stream1(t + i) : 0.0;
+    double2 A = make_double2(0.0, 0.0), Ab = make_double2(0.0, 0.0);
+#pragma unroll
+    for (int c = 0; c < KC; ++c) {
+      amp_add(A, Ab, R.c[c][0], R.c[c][1], R.cbar[c][0], R.cbar[c][1], v[c]);
+      *reinterpret_cast<double2 *>(xrow + 2 * c) = v[c];
+    }
+    double ch, sh, cs, sn;
+    mixing_functions<SMALL>(yG * ti, xG * ti, ch, sh, cs, sn);
+    const Bilinears q = bilinears(A, Ab);
+    const double aa = q.aa, bb = q.bb, cre = q.cre, cim = q.cim;
+    const double B = rate_form(q, ch, cs, sh, sn);                                        // the bits of bracket()
+    double inv = 0.0;
+    if (live) { la.add(B); inv = 1.0 / B; }
+    // conj(gA) / B and conj(gAbar) / B as (Re, Im) pairs: the weights of this event
+    *reinterpret_cast<double2 *>(wrow) = make_double2(((ch + cs) * A.x - (sh * Ab.x - sn * Ab.y)) * inv, ((ch + cs) * A.y - (sh * Ab.y + sn * Ab.x)) * inv);
+    *reinterpret_cast<double2 *>(wrow + 2) = make_double2(((ch - cs) * Ab.x - (sh * A.x + sn * A.y)) * inv, ((ch - cs) * Ab.y - (sh * A.y - sn * A.x)) * inv);
+    const double gt = R.Gamma * ti * inv;
+    sc[0] += gt * (-(aa - bb) * sn - 2.0 * cim * cs);
+    sc[1] += gt * ((aa + bb) * sh - 2.0 * cre * ch);
+    grad_mma_tile<NB>(Xs, Wt, acc);
+  }
+  const bool fin = grad_reduce<NB, NS>(acc, sc, la, partials, ticket, s_red, s_sum, s_p, s_e, s_b, &last);
+  if (!fin) return;
+  if (warp == 1) {
+    double nAA, nBB, xr, xi;
+    gram_sums_warp(R, G, KC, inv_n_norm, nAA, nBB, xr, xi);
+    if (lane == 0) { s_n[0] = nAA; s_n[1] = nBB; s_n[2] = xr; s_n[3] = xi; }
+  } else if (warp == 2) {
+    grad_gram_vectors<KC>(R, G, inv_n_norm, lane, s_u, s_ub);
   }
   __syncthreads();
   const double nAA = s_n[0], nBB = s_n[1], xr = s_n[2], xi = s_n[3];
@@ -150,16 +267,19 @@ nll_grad_kernel(const double2 *__restrict__ a, const double *__restrict__ t, int
     const double hi = (R.T[0] + R.T[1]) * u.y - (R.T[2] * ub.y + R.T[3] * ub.x);
     const double br = (R.T[0] - R.T[1]) * ub.x - (R.T[2] * u.x + R.T[3] * u.y);
     const double bi = (R.T[0] - R.T[1]) * ub.y - (R.T[2] * u.y - R.T[3] * u.x);
+    // Re D_k = sum (gx vx + gy vy), Im D_k = sum (gx vy - gy vx); W rows: 0 gx, 1 gy, 2 hx, 3 hy; features 2k (Re), 2k+1 (Im)
+    const double dre = grad_c(s_sum, 0, 2 * tid) + grad_c(s_sum, 1, 2 * tid + 1), dim = grad_c(s_sum, 0, 2 * tid + 1) - grad_c(s_sum, 1, 2 * tid);
+    const double ere = grad_c(s_sum, 2, 2 * tid) + grad_c(s_sum, 3, 2 * tid + 1), eim = grad_c(s_sum, 2, 2 * tid + 1) - grad_c(s_sum, 3, 2 * tid);
     double *g = result + GRAD_OFFSET;
-    g[2 * tid] = -2.0 * s_sum[2 * tid] + scale * 2.0 * hr;
-    g[2 * tid + 1] = 2.0 * s_sum[2 * tid + 1] + scale * 2.0 * hi;
-    g[2 * KC + 2 * tid] = -2.0 * s_sum[2 * KC + 2 * tid] + scale * 2.0 * br;
-    g[2 * KC + 2 * tid + 1] = 2.0 * s_sum[2 * KC + 2 * tid + 1] + scale * 2.0 * bi;
+    g[2 * tid] = -2.0 * dre + scale * 2.0 * hr;
+    g[2 * tid + 1] = 2.0 * dim + scale * 2.0 * hi;
+    g[2 * KC + 2 * tid] = -2.0 * ere + scale * 2.0 * br;
+    g[2 * KC + 2 * tid + 1] = 2.0 * eim + scale * 2.0 * bi;
   }
   if (tid == 0) {
     double *g = result + GRAD_OFFSET;
-    g[4 * KC] = -s_sum[4 * KC] + scale * (GP.dT1dx * (nAA - nBB) - 2.0 * GP.dT3dx * xi);
-    g[4 * KC + 1] = -s_sum[4 * KC + 1] + scale * (GP.dT0dy * (nAA + nBB) - 2.0 * GP.dT2dy * xr);
+    g[4 * KC] = -s_sum[NB * 32] + scale * (GP.dT1dx * (nAA - nBB) - 2.0 * GP.dT3dx * xi);
+    g[4 * KC + 1] = -s_sum[NB * 32 + 1] + scale * (GP.dT0dy * (nAA + nBB) - 2.0 * GP.dT2dy * xr);
     const double prod = s_p[0];
     const long long esum = s_e[0];
     const int bad = s_b[0];
@@ -177,12 +297,13 @@ nll_grad_kernel(const double2 *__restrict__ a, const double *__restrict__ t, int
 // columns, the eight time rows and the eight derivative rows (tres_grad_kernel).  d(sum log N_i)/dc_k* keeps the Gram
 // structure with per-call weights W_m = sum_i T_m,i / N_i:  (W0+W1) u_k - (W2 + i W3) ubar_k.
 template <int KC>
-__global__ void __launch_bounds__(STREAM_BLOCK, 1)
+__global__ void __launch_bounds__(STREAM_BLOCK, STREAM_BLOCKS_PER_SM)
 nll_grad_res_kernel(const double2 *__restrict__ a, const double *__restrict__ tr, const double *__restrict__ trg, int64_t ld,
                     int64_t n, const __grid_constant__ RateParams R, const double *__restrict__ G, double inv_n_norm,
-                    double *__restrict__ partials /* [grid][NA + 3] */, unsigned int *ticket, double *__restrict__ result) {
-  constexpr int NG = 4 * KC + 2, NA = NG + 4, PS = NA + 3;
-  __shared__ double s_red[STREAM_WARPS][NA];
+                    double *__restrict__ partials /* [grid][NB * 32 + 9] */, unsigned int *ticket, double *__restrict__ result) {
+  constexpr int NB = grad_nb<KC>(), XS = gram_stride(NB), NS = 6, NC = NB * 32, NA = NC + NS;
+  extern __shared__ __align__(16) char smem_raw[];
+  __shared__ double s_red[STREAM_WARPS * NA];
   __shared__ double s_sum[NA];
   __shared__ double s_p[STREAM_WARPS];
   __shared__ long long s_e[STREAM_WARPS];
@@ -193,118 +314,71 @@ nll_grad_res_kernel(const double2 *__restrict__ a, const double *__restrict__ tr
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   block_phase_space_sums(R, G, KC, inv_n_norm, s_S);
   const double S1 = s_S[0], S2 = s_S[1], S3 = s_S[2], S4 = s_S[3];
-  MantAcc la;
-  double acc[NA];
+  double *Xs = reinterpret_cast<double *>(smem_raw + (size_t)warp * grad_warp_bytes<KC>());
+  double *Wt = Xs + align_up((size_t)32 * XS * sizeof(double), 128) / sizeof(double);
+  double *xrow = Xs + lane * XS, *wrow = Wt + lane * GRAD_WS;
 #pragma unroll
-  for (int j = 0; j < NA; ++j) acc[j] = 0.0;
+  for (int c = 0; c < XS; ++c) xrow[c] = 0.0;
+#pragma unroll
+  for (int c = 0; c < GRAD_WS; ++c) wrow[c] = 0.0;
+  MantAcc la;
+  double acc[NB][2], sc[NS];
+#pragma unroll
+  for (int b = 0; b < NB; ++b) acc[b][0] = acc[b][1] = 0.0;
+#pragma unroll
+  for (int j = 0; j < NS; ++j) sc[j] = 0.0;
   const int64_t stride = (int64_t)gridDim.x * STREAM_BLOCK;
 #pragma unroll 1
-  for (int64_t i = (int64_t)blockIdx.x * STREAM_BLOCK + tid; i < n; i += stride) {
+  for (int64_t i0 = (int64_t)blockIdx.x * STREAM_BLOCK + warp * 32; i0 < n; i0 += stride) {
+    const int64_t i = i0 + lane;
+    const bool live = i < n;
     double2 v[KC];
     double w[8], d[8];
 #pragma unroll
-    for (int c = 0; c < KC; ++c) v[c] = ldg_stream2(a + c * ld + i);
+    for (int c = 0; c < KC; ++c) v[c] = live ? ldg_stream2(a + c * ld + i) : make_double2(0.0, 0.0);
 #pragma unroll
-    for (int m = 0; m < 8; ++m) { w[m] = ldg_stream1(tr + m * ld + i); d[m] = ldg_stream1(trg + m * ld + i); }
+    for (int m = 0; m < 8; ++m) { w[m] = live ? ldg_stream1(tr + m * ld + i) : 1.0; d[m] = live ? ldg_stream1(trg + m * ld + i) : 0.0; }
     double2 A = make_double2(0.0, 0.0), Ab = make_double2(0.0, 0.0);
 #pragma unroll
-    for (int c = 0; c < KC; ++c) amp_add(A, Ab, R.c[c][0], R.c[c][1], R.cbar[c][0], R.cbar[c][1], v[c]);
+    for (int c = 0; c < KC; ++c) {
+      amp_add(A, Ab, R.c[c][0], R.c[c][1], R.cbar[c][0], R.cbar[c][1], v[c]);
+      *reinterpret_cast<double2 *>(xrow + 2 * c) = v[c];
+    }
     const Bilinears q = bilinears(A, Ab);
     const double aa = q.aa, bb = q.bb, cre = q.cre, cim = q.cim;
     const double Rv = rate_form(q, w[0], w[1], w[2], w[3]);                                        // the bits of resolved_prob()
     const double Nv = fma(S1, w[4], fma(S2, w[5], fma(-2.0 * S3, w[6], __dmul_rn(-2.0 * S4, w[7]))));
-    la.add(__ddiv_rn(Rv, Nv));
-    const double invR = 1.0 / Rv, invN = 1.0 / Nv;
-    const double gx = ((w[0] + w[1]) * A.x - (w[2] * Ab.x - w[3] * Ab.y)) * invR, gy = ((w[0] + w[1]) * A.y - (w[2] * Ab.y + w[3] * Ab.x)) * invR;
-    const double hx = ((w[0] - w[1]) * Ab.x - (w[2] * A.x + w[3] * A.y)) * invR, hy = ((w[0] - w[1]) * Ab.y - (w[2] * A.y - w[3] * A.x)) * invR;
-#pragma unroll
-    for (int c = 0; c < KC; ++c) {
-      acc[2 * c] = fma(gx, v[c].x, fma(gy, v[c].y, acc[2 * c]));
-      acc[2 * c + 1] = fma(gx, v[c].y, fma(-gy, v[c].x, acc[2 * c + 1]));
-      acc[2 * KC + 2 * c] = fma(hx, v[c].x, fma(hy, v[c].y, acc[2 * KC + 2 * c]));
-      acc[2 * KC + 2 * c + 1] = fma(hx, v[c].y, fma(-hy, v[c].x, acc[2 * KC + 2 * c + 1]));
-    }
+    double invR = 0.0, invN = 0.0;
+    if (live) { la.add(__ddiv_rn(Rv, Nv)); invR = 1.0 / Rv; invN = 1.0 / Nv; }
+    *reinterpret_cast<double2 *>(wrow) = make_double2(((w[0] + w[1]) * A.x - (w[2] * Ab.x - w[3] * Ab.y)) * invR, ((w[0] + w[1]) * A.y - (w[2] * Ab.y + w[3] * Ab.x)) * invR);
+    *reinterpret_cast<double2 *>(wrow + 2) = make_double2(((w[0] - w[1]) * Ab.x - (w[2] * A.x + w[3] * A.y)) * invR, ((w[0] - w[1]) * Ab.y - (w[2] * A.y - w[3] * A.x)) * invR);
     // d log(R/N) / dx, / dy: d = (dpsi1/dx, dpsi3/dx, dpsi0/dy, dpsi2/dy, dT1/dx, dT3/dx, dT0/dy, dT2/dy)
-    acc[4 * KC] += ((aa - bb) * d[0] - 2.0 * cim * d[1]) * invR - (S2 * d[4] - 2.0 * S4 * d[5]) * invN;
-    acc[4 * KC + 1] += ((aa + bb) * d[2] - 2.0 * cre * d[3]) * invR - (S1 * d[6] - 2.0 * S3 * d[7]) * invN;
+    sc[0] += ((aa - bb) * d[0] - 2.0 * cim * d[1]) * invR - (S2 * d[4] - 2.0 * S4 * d[5]) * invN;
+    sc[1] += ((aa + bb) * d[2] - 2.0 * cre * d[3]) * invR - (S1 * d[6] - 2.0 * S3 * d[7]) * invN;
 #pragma unroll
-    for (int m = 0; m < 4; ++m) acc[NG + m] = fma(w[4 + m], invN, acc[NG + m]);     // W_m
+    for (int m = 0; m < 4; ++m) sc[2 + m] = fma(w[4 + m], invN, sc[2 + m]);     // W_m
+    grad_mma_tile<NB>(Xs, Wt, acc);
   }
-#pragma unroll
-  for (int j = 0; j < NA; ++j) {
-    double s = warp_sum(acc[j]);
-    if (lane == 0) s_red[warp][j] = s;
-  }
-  warp_merge(la);
-  if (lane == 0) { s_p[warp] = la.prod; s_e[warp] = la.esum; s_b[warp] = la.bad; }
+  const bool fin = grad_reduce<NB, NS>(acc, sc, la, partials, ticket, s_red, s_sum, s_p, s_e, s_b, &last);
+  if (!fin) return;
+  if (warp == 2) grad_gram_vectors<KC>(R, G, inv_n_norm, lane, s_u, s_ub);
   __syncthreads();
-  double *mine = partials + (int64_t)blockIdx.x * PS;
-  for (int j = tid; j < NA; j += STREAM_BLOCK) {
-    double s = 0.0;
-#pragma unroll
-    for (int wp = 0; wp < STREAM_WARPS; ++wp) s += s_red[wp][j];
-    mine[j] = s;
-  }
-  if (tid == 0) {
-    MantAcc m;
-#pragma unroll
-    for (int wp = 0; wp < STREAM_WARPS; ++wp) m.merge(s_p[wp], s_e[wp], s_b[wp]);
-    m.renorm();
-    mine[NA] = m.prod; mine[NA + 1] = (double)m.esum; mine[NA + 2] = (double)m.bad;
-  }
-  __threadfence();
-  __syncthreads();
-  if (tid == 0) last = atomicAdd(ticket, 1u) == gridDim.x - 1;
-  __syncthreads();
-  if (!last) return;
-  __threadfence();
-  for (int j = tid; j < NA; j += STREAM_BLOCK) {
-    double part[16];
-#pragma unroll
-    for (int c = 0; c < 16; ++c) part[c] = 0.0;
-    for (unsigned b = 0; b < gridDim.x; b += 16) {
-#pragma unroll
-      for (int c = 0; c < 16; ++c)
-        if (b + c < gridDim.x) part[c] += __ldcg(partials + (int64_t)(b + c) * PS + j);
-    }
-    double s = 0.0;
-#pragma unroll
-    for (int c = 0; c < 16; ++c) s += part[c];
-    s_sum[j] = s;
-  }
-  if (warp == STREAM_WARPS - 1) {
-    MantAcc m;
-    for (unsigned b = lane; b < gridDim.x; b += 32) {
-      const double *pb = partials + (int64_t)b * PS + NA;
-      m.merge(__ldcg(pb), (long long)__ldcg(pb + 1), (int)__ldcg(pb + 2));
-      m.renorm();
-    }
-    warp_merge(m);
-    if (lane == 0) { s_p[0] = m.prod; s_e[0] = m.esum; s_b[0] = m.bad; }
-  } else if (warp == 2 && lane < KC) {
-    double2 u = make_double2(0.0, 0.0), ub = make_double2(0.0, 0.0);
-    for (int j = 0; j < KC; ++j) {
-      double gr = __ldcg(G + (j * KC + lane) * 2) * inv_n_norm, gi = __ldcg(G + (j * KC + lane) * 2 + 1) * inv_n_norm;
-      u.x += R.c[j][0] * gr - R.c[j][1] * gi;    u.y += R.c[j][0] * gi + R.c[j][1] * gr;
-      ub.x += R.cbar[j][0] * gr - R.cbar[j][1] * gi;  ub.y += R.cbar[j][0] * gi + R.cbar[j][1] * gr;
-    }
-    s_u[lane] = u; s_ub[lane] = ub;
-  }
-  __syncthreads();
-  const double W0 = s_sum[NG], W1 = s_sum[NG + 1], W2 = s_sum[NG + 2], W3 = s_sum[NG + 3];
+  const double W0 = s_sum[NC + 2], W1 = s_sum[NC + 3], W2 = s_sum[NC + 4], W3 = s_sum[NC + 5];
   double *g = result + GRAD_OFFSET;
   if (tid < KC) {
     const double2 u = s_u[tid], ub = s_ub[tid];
     const double hr = (W0 + W1) * u.x - (W2 * ub.x - W3 * ub.y), hi = (W0 + W1) * u.y - (W2 * ub.y + W3 * ub.x);
     const double br = (W0 - W1) * ub.x - (W2 * u.x + W3 * u.y), bi = (W0 - W1) * ub.y - (W2 * u.y - W3 * u.x);
-    g[2 * tid] = -2.0 * s_sum[2 * tid] + 2.0 * hr;
-    g[2 * tid + 1] = 2.0 * s_sum[2 * tid + 1] + 2.0 * hi;
-    g[2 * KC + 2 * tid] = -2.0 * s_sum[2 * KC + 2 * tid] + 2.0 * br;
-    g[2 * KC + 2 * tid + 1] = 2.0 * s_sum[2 * KC + 2 * tid + 1] + 2.0 * bi;
+    const double dre = grad_c(s_sum, 0, 2 * tid) + grad_c(s_sum, 1, 2 * tid + 1), dim = grad_c(s_sum, 0, 2 * tid + 1) - grad_c(s_sum, 1, 2 * tid);
+    const double ere = grad_c(s_sum, 2, 2 * tid) + grad_c(s_sum, 3, 2 * tid + 1), eim = grad_c(s_sum, 2, 2 * tid + 1) - grad_c(s_sum, 3, 2 * tid);
+    g[2 * tid] = -2.0 * dre + 2.0 * hr;
+    g[2 * tid + 1] = 2.0 * dim + 2.0 * hi;
+    g[2 * KC + 2 * tid] = -2.0 * ere + 2.0 * br;
+    g[2 * KC + 2 * tid + 1] = 2.0 * eim + 2.0 * bi;
   }
   if (tid == 0) {
-    g[4 * KC] = -s_sum[4 * KC];
-    g[4 * KC + 1] = -s_sum[4 * KC + 1];
+    g[4 * KC] = -s_sum[NC];
+    g[4 * KC + 1] = -s_sum[NC + 1];
     const double s0 = log(s_p[0]) + 0.693147180559945309417 * (double)s_e[0];
     const double norm = R.T[0] * S1 + R.T[1] * S2 - 2.0 * R.T[2] * S3 - 2.0 * R.T[3] * S4;
     double nll = -s0;

@@ -67,6 +67,35 @@ __global__ void __launch_bounds__(256) row_gather_kernel(const double *__restric
 }
 
 // ------------------------------------------------------------------------------------------------
+// Sum of the ranks' Gram sums in rank order (event-sharded evaluation): gathered [world][len]
+__global__ void __launch_bounds__(256) gram_reduce_kernel(const double *__restrict__ gathered, int world, int stride, int len,
+                                                         double *__restrict__ G) {
+  for (int q = threadIdx.x; q < len; q += 256) {
+    double sum = 0.0;
+    for (int r = 0; r < world; ++r) sum += gathered[(int64_t)r * stride + q];
+    G[q] = sum;
+  }
+}
+__global__ void __launch_bounds__(32) append_count_kernel(double *dst, double value) { if (threadIdx.x == 0) *dst = value; }
+
+// fp64 issue-rate probe: 8 independent DFMA chains per thread, 4096 FMAs each, 148 x 4 x 256 threads
+__global__ void __launch_bounds__(256) fp64_peak_kernel(double *out, double a, double b, int iters) {
+  double v[8];
+#pragma unroll
+  for (int k = 0; k < 8; ++k) v[k] = a + k + threadIdx.x;
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int r = 0; r < 16; ++r)
+#pragma unroll
+      for (int k = 0; k < 8; ++k) v[k] = fma(v[k], a, b);
+  }
+  double s = 0.0;
+#pragma unroll
+  for (int k = 0; k < 8; ++k) s += v[k];
+  if (s == 123.456) out[0] = s;
+}
+
+// ------------------------------------------------------------------------------------------------
 constexpr int COL_BLOCK = 128;
 // per-term amplitudes a_k (un-summed), for per-layer parity only (TDDP4_GET_TERMS)
 __global__ void __launch_bounds__(COL_BLOCK)
@@ -89,25 +118,31 @@ terms_kernel(const __grid_constant__ ModelTab M, const __grid_constant__ LinePar
 }
 
 // ------------------------------------------------------------------------------------------------
-// deterministic sum and max |.| of a vector (decay times at load): one block, fixed order
-__global__ void __launch_bounds__(1024) stat_kernel(const double *__restrict__ v, int64_t n, double *out /* [2] */) {
+// deterministic sum, max |.| and minimum of a vector (decay times, sigma_t at load): one block, fixed order
+__global__ void __launch_bounds__(1024) stat_kernel(const double *__restrict__ v, int64_t n, double *out /* [3] */) {
   __shared__ double red[32];
-  double acc = 0.0, mx = 0.0;
+  __shared__ double red2[32];
+  double acc = 0.0, mx = 0.0, mn = INFINITY;
   for (int64_t i = threadIdx.x; i < n; i += 1024) {
     double x = v[i];
     acc += x;
     mx = fmax(mx, fabs(x));
+    mn = fmin(mn, x);
   }
   acc = block_sum<1024>(acc, red);
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+  for (int o = 16; o > 0; o >>= 1) {
+    mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+    mn = fmin(mn, __shfl_xor_sync(0xffffffffu, mn, o));
+  }
   __syncthreads();
-  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = mx;
+  if ((threadIdx.x & 31) == 0) { red[threadIdx.x >> 5] = mx; red2[threadIdx.x >> 5] = mn; }
   __syncthreads();
   if (threadIdx.x == 0) {
-    for (int k = 1; k < 32; ++k) mx = fmax(mx, red[k]);
+    for (int k = 1; k < 32; ++k) { mx = fmax(mx, red[k]); mn = fmin(mn, red2[k]); }
     out[0] = acc;
     out[1] = mx;
+    out[2] = mn;
   }
 }
 
@@ -168,7 +203,7 @@ __device__ __forceinline__ double candidate_ratio(const ModelTab &M, const LineP
 __global__ void __launch_bounds__(GEN_BLOCK, 4)
 gen_ratio_kernel(const __grid_constant__ ModelTab M, const __grid_constant__ LineParams LP,
                  const __grid_constant__ RateParams R, double tau, uint64_t seed, uint32_t stream, uint64_t first,
-                 int64_t n, int mode, double envelope,
+                 int64_t n, int mode, double envelope /* mode 2: the envelope, or its scale if from_pilot */, int from_pilot,
                  double *__restrict__ out_p4, double *__restrict__ out_t, double *__restrict__ out_w,
                  double *__restrict__ out_ratio, double *__restrict__ out_u,
                  unsigned long long *pilot_max_bits, uint32_t *__restrict__ flags /* one bit per candidate */,
@@ -207,6 +242,7 @@ gen_ratio_kernel(const __grid_constant__ ModelTab M, const __grid_constant__ Lin
     if ((tid & 31) == 0) atomicMax(pilot_max_bits, (unsigned long long)__double_as_longlong(m));
     return;
   }
+  if (from_pilot) envelope *= __longlong_as_double((long long)*pilot_max_bits);   // E = scale * max over the pilot (G5), no host round trip
   bool acc = live && (u * envelope < rho);
   unsigned ballot = __ballot_sync(0xffffffffu, acc);
   unsigned over = __ballot_sync(0xffffffffu, live && rho > envelope);
@@ -224,10 +260,13 @@ gen_ratio_kernel(const __grid_constant__ ModelTab M, const __grid_constant__ Lin
   }
 }
 
-// exclusive scan of the block counts (single block; counts fit in 32 bits per launch chunk)
+// exclusive scan of the block counts of one launch chunk (single block), continued from the running total of the
+// chunks before it: offs[b] = *total + sum_{b' < b} cnt[b'], and *total advances by the chunk's count (no host round trip)
 __global__ void __launch_bounds__(1024) scan_kernel(const uint32_t *__restrict__ cnt, int64_t nb,
-                                                    unsigned long long *__restrict__ offs /* [nb+1] */) {
+                                                    unsigned long long *__restrict__ offs /* [nb+1] */,
+                                                    unsigned long long *__restrict__ total) {
   __shared__ unsigned long long part[1024];
+  __shared__ unsigned long long base;
   int tid = threadIdx.x;
   int64_t per = (nb + 1023) / 1024, lo = tid * per, hi = lo + per < nb ? lo + per : nb;
   unsigned long long s = 0;
@@ -237,43 +276,67 @@ __global__ void __launch_bounds__(1024) scan_kernel(const uint32_t *__restrict__
   if (tid == 0) {
     unsigned long long run = 0;
     for (int k = 0; k < 1024; ++k) { unsigned long long v = part[k]; part[k] = run; run += v; }
-    offs[nb] = run;
+    base = *total;
+    offs[nb] = base + run;
+    *total = base + run;
   }
   __syncthreads();
-  unsigned long long run = part[tid];
+  unsigned long long run = base + part[tid];
   for (int64_t b = lo; b < hi; ++b) { offs[b] = run; run += cnt[b]; }
 }
 
-// G6: regenerate the accepted candidates (Philox is counter based: no state to carry) and write them
-// compacted, in candidate order.
-__global__ void __launch_bounds__(GEN_BLOCK)
+// G6: regenerate the accepted candidates (Philox is counter based: no state to carry) and write them compacted, in
+// candidate order.  One block covers EMIT_SPAN candidates: it first turns their accept bits into a dense list of local
+// indices in shared memory, then its threads walk that list, so every lane that runs Philox + Raubold-Lynch produces an
+// output event (at 6.6 % acceptance the one-thread-per-candidate form kept 89 % of the warps busy for 1/15 of the
+// lanes: 0.96 ms against 1.21 ms for the ratio pass itself) and consecutive threads write consecutive output slots.
+constexpr int EMIT_BLOCK = 128, EMIT_SPAN = 2048, EMIT_WORDS = EMIT_SPAN / 32;
+static_assert(EMIT_SPAN % GEN_BLOCK == 0, "an emit block starts at a ratio-block boundary");
+__global__ void __launch_bounds__(EMIT_BLOCK)
 gen_emit_kernel(const __grid_constant__ ModelTab M, double tau, uint64_t seed, uint32_t stream, uint64_t first,
                 int64_t n, const uint32_t *__restrict__ flags, const unsigned long long *__restrict__ offs,
-                int64_t base, int64_t capacity, double *__restrict__ out_p4, double *__restrict__ out_t,
+                int64_t capacity, double *__restrict__ out_p4, double *__restrict__ out_t,
                 int64_t *__restrict__ out_index) {
-  __shared__ int s_cnt[GEN_BLOCK / 32];
-  int tid = threadIdx.x, wid = tid >> 5, lane = tid & 31;
-  int64_t j = (int64_t)blockIdx.x * GEN_BLOCK + tid;
-  unsigned word = (j - lane) < n ? flags[j >> 5] : 0u;
-  if (lane == 0) s_cnt[wid] = __popc(word);
+  __shared__ uint16_t s_list[EMIT_SPAN];
+  __shared__ int s_pre[EMIT_WORDS + 1];
+  const int tid = threadIdx.x;
+  const int64_t j0 = (int64_t)blockIdx.x * EMIT_SPAN;
+  uint32_t word = 0;
+  if (tid < EMIT_WORDS && j0 + (int64_t)tid * 32 < n) word = flags[(j0 >> 5) + tid];
+  if (tid < EMIT_WORDS) s_pre[tid + 1] = __popc(word);
+  if (tid == 0) s_pre[0] = 0;
   __syncthreads();
-  if (!((word >> lane) & 1u)) return;
-  int64_t pos = base + (int64_t)offs[blockIdx.x];
-  for (int k = 0; k < wid; ++k) pos += s_cnt[k];
-  pos += __popc(word & ((1u << lane) - 1u));
-  if (pos >= capacity) return;
-  V4 p[4];
-  double t, w, u;
-  rl_candidate(M, tau, seed, stream, first + (uint64_t)j, p, t, w, u);
-  if (out_p4) {
-#pragma unroll
-    for (int a = 0; a < 4; ++a) {
-      out_p4[(4 * a) * capacity + pos] = p[a].e; out_p4[(4 * a + 1) * capacity + pos] = p[a].x;
-      out_p4[(4 * a + 2) * capacity + pos] = p[a].y; out_p4[(4 * a + 3) * capacity + pos] = p[a].z;
+  if (tid == 0)
+    for (int k = 1; k <= EMIT_WORDS; ++k) s_pre[k] += s_pre[k - 1];
+  __syncthreads();
+  if (tid < EMIT_WORDS) {
+    int at = s_pre[tid];
+    while (word) {
+      int b = __ffs(word) - 1;
+      word &= word - 1;
+      s_list[at++] = (uint16_t)(tid * 32 + b);
     }
   }
-  if (out_t) out_t[pos] = t;
-  if (out_index) out_index[pos] = (int64_t)first + j;
+  __syncthreads();
+  const int count = s_pre[EMIT_WORDS];
+  const int64_t base = (int64_t)offs[j0 / GEN_BLOCK];
+  for (int k = tid; k < count; k += EMIT_BLOCK) {
+    const int64_t pos = base + k;
+    if (pos >= capacity) break;
+    const int64_t j = j0 + s_list[k];
+    V4 p[4];
+    double t, w, u;
+    rl_candidate(M, tau, seed, stream, first + (uint64_t)j, p, t, w, u);
+    if (out_p4) {
+#pragma unroll
+      for (int a = 0; a < 4; ++a) {
+        out_p4[(4 * a) * capacity + pos] = p[a].e; out_p4[(4 * a + 1) * capacity + pos] = p[a].x;
+        out_p4[(4 * a + 2) * capacity + pos] = p[a].y; out_p4[(4 * a + 3) * capacity + pos] = p[a].z;
+      }
+    }
+    if (out_t) out_t[pos] = t;
+    if (out_index) out_index[pos] = (int64_t)first + j;
+  }
 }
 
 }  // namespace tddp4k

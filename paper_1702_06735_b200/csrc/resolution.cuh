@@ -128,10 +128,81 @@ __device__ __forceinline__ void time_terms(const FaddTab &F, double t, double si
   double hm = conv_exp_real(t, lm, sigma), hp = conv_exp_real(t, lp, sigma);
   double2 hx = conv_exp_complex(F, t, lxr, lxi, sigma);
   psi[0] = 0.5 * (hm + hp); psi[1] = hx.x; psi[2] = 0.5 * (hm - hp); psi[3] = hx.y;
+  if (tint) {
+    const double derf = erf_scaled(t_hi, sigma) - erf_scaled(t_lo, sigma);
+    double Im = window_real(t_lo, t_hi, lm, sigma, derf), Ip = window_real(t_lo, t_hi, lp, sigma, derf);
+    double2 Ix = window_complex(F, t_lo, t_hi, lxr, lxi, sigma, derf);
+    tint[0] = 0.5 * (Im + Ip); tint[1] = Ix.x; tint[2] = 0.5 * (Im - Ip); tint[3] = Ix.y;
+  }
+}
+
+// The four window integrals depend on the event only through sigma, and they are smooth in it: per call (x, y, tau moved)
+// one warp evaluates them exactly at TRES_NODES Chebyshev nodes of [sigma_min, sigma_max] of the data sample and turns
+// the values into Chebyshev coefficients; each event then costs four short Clenshaw sums instead of four real and two
+// complex convolutions at the window edges (tres_kernel: 989 -> 4xx us per 10 M events).  The table declares itself
+// unusable (ok = 0: the kernel evaluates the edges exactly, as before) unless its last eight coefficients are below
+// 1e-15 of the largest one, i.e. unless the interpolant has converged to rounding level on this sigma range.
+// (A NaN anywhere -- sigma <= 0 -- makes every comparison fail: ok = 0.)
+constexpr int TRES_NODES = 32;
+struct TresTable {
+  double mid, half;               // sigma = mid + half * xi, xi in [-1, 1]
+  int deg, ok;                    // highest coefficient worth summing; 1: converged
+  double c[4][TRES_NODES];        // Chebyshev coefficients of tint[m] (c[m][0] already halved)
+};
+__device__ __forceinline__ void window_terms(const FaddTab &F, double sigma, double x, double y, double Gamma, double t_lo,
+                                             double t_hi, double tint[4]) {
+  double lm = Gamma * (1.0 - y), lp = Gamma * (1.0 + y), lxr = Gamma, lxi = -Gamma * x;
   const double derf = erf_scaled(t_hi, sigma) - erf_scaled(t_lo, sigma);
   double Im = window_real(t_lo, t_hi, lm, sigma, derf), Ip = window_real(t_lo, t_hi, lp, sigma, derf);
   double2 Ix = window_complex(F, t_lo, t_hi, lxr, lxi, sigma, derf);
   tint[0] = 0.5 * (Im + Ip); tint[1] = Ix.x; tint[2] = 0.5 * (Im - Ip); tint[3] = Ix.y;
+}
+// one warp: exact values at the nodes, discrete cosine sums, convergence test
+__global__ void __launch_bounds__(32) tres_table_kernel(const __grid_constant__ FaddTab F, double x, double y, double Gamma,
+                                                        double t_lo, double t_hi, double sig_lo, double sig_hi,
+                                                        TresTable *__restrict__ out) {
+  const int lane = threadIdx.x;
+  const double mid = 0.5 * (sig_lo + sig_hi), half = 0.5 * (sig_hi - sig_lo);
+  double f[4];
+  window_terms(F, mid + half * cospi((lane + 0.5) / TRES_NODES), x, y, Gamma, t_lo, t_hi, f);
+  double c[4] = {0.0, 0.0, 0.0, 0.0};
+  for (int j = 0; j < TRES_NODES; ++j) {
+    const double w = cospi(lane * (j + 0.5) / TRES_NODES);
+#pragma unroll
+    for (int m = 0; m < 4; ++m) c[m] = fma(__shfl_sync(0xffffffffu, f[m], j), w, c[m]);
+  }
+  // one scale for all four series: tint[2], tint[3] are differences of quantities of the size of tint[0] and carry its
+  // rounding noise, in the exact evaluation as much as here
+  double mx = 0.0;
+#pragma unroll
+  for (int m = 0; m < 4; ++m) {
+    c[m] *= (lane == 0 ? 1.0 : 2.0) / TRES_NODES;
+    mx = fmax(mx, fabs(c[m]));
+    out->c[m][lane] = c[m];
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) mx = fmax(mx, __shfl_xor_sync(0xffffffffu, mx, o));
+  bool small = true;
+#pragma unroll
+  for (int m = 0; m < 4; ++m) small = small && fabs(c[m]) <= 1e-15 * mx;
+  const unsigned big = __ballot_sync(0xffffffffu, !small);            // lanes = orders that still matter
+  const bool ok = (big >> (TRES_NODES - 8)) == 0u && isfinite(mx) && sig_lo > 0.0;   // sigma_t <= 0 is outside the contract: the exact path reports it
+  const int deg = big ? 31 - __clz(big) : 0;
+  if (lane == 0) { out->mid = mid; out->half = half; out->deg = deg; out->ok = ok ? 1 : 0; }
+}
+// Clenshaw sums of the four series at one sigma; tab: the table in shared memory
+__device__ __forceinline__ void window_terms_table(const TresTable &tab, double sigma, double tint[4]) {
+  const double xi = tab.half > 0.0 ? (sigma - tab.mid) / tab.half : 0.0, x2 = 2.0 * xi;
+  double b1[4] = {0.0, 0.0, 0.0, 0.0}, b2[4] = {0.0, 0.0, 0.0, 0.0};
+  for (int k = tab.deg; k >= 1; --k) {
+#pragma unroll
+    for (int m = 0; m < 4; ++m) {
+      double b0 = fma(x2, b1[m], tab.c[m][k] - b2[m]);
+      b2[m] = b1[m]; b1[m] = b0;
+    }
+  }
+#pragma unroll
+  for (int m = 0; m < 4; ++m) tint[m] = fma(xi, b1[m], tab.c[m][0] - b2[m]);
 }
 
 // Derivatives with respect to the mixing parameters (tddp4_nll_grad in resolution mode).  From the definition,

@@ -5,7 +5,7 @@
 //   nll_res_kernel, tres_kernel, prob_*  resolution mode (config 5) and per-event probabilities
 // All are HBM streams: every row is read exactly once per call with coalesced loads straight into registers (256-byte
 // warp segments of 8-byte rows, 512-byte segments of the 16-byte columns), every load of an event requested before any
-// arithmetic (17-40 loads in flight per thread), from STREAM_BLOCK-thread persistent blocks, two per SM.  Event i always
+// arithmetic (9-40 loads in flight per thread), from STREAM_BLOCK-thread persistent blocks, two per SM.  Event i always
 // belongs to thread (i mod stride) of the grid-stride decomposition, stride = gridDim.x * STREAM_BLOCK, and every thread
 // visits its events in increasing order; nll_stream and colnll_stream are launched with the same grid, so the fixed-order
 // reduction returns bit-identical NLLs whether the columns were cached or rebuilt in the call.  Consecutive kernels
@@ -159,11 +159,13 @@ __device__ __forceinline__ double resolved_prob(double2 A, double2 Ab, const dou
 // common tail of the two NLL kernels (step 7, second pass).  Thread products -> warp -> block partial
 // (prod, exponent sum, #bad); the last block to arrive merges the block partials in index order in warp 0 while
 // warp 1 evaluates N, then thread 0 takes the one log and writes the result slot:
-//   [0] sum log B, [1] sum t, [2] N, [3] NLL = Gamma sum t - sum log B + n log N, [4] #bad events
+//   [0] sum log B, [1] sum t, [2] N, [3] NLL = Gamma sum t - sum log B + n log N, [4] #bad events,
+//   [5] seq: the caller's sequence stamp, written LAST behind a system-wide fence -- when the slot lives in mapped host
+//   memory the host polls this word instead of waiting on a CUDA event (see wait_slot() in tddp4_api.cu)
 template <bool RES = false>
 __device__ __forceinline__ void nll_finish(const RateParams &R, int KC, int64_t n, double sum_t, MantAcc la,
                                            const double *__restrict__ G, double inv_n, double *__restrict__ partials,
-                                           unsigned int *ticket, double *__restrict__ result) {
+                                           unsigned int *ticket, double *__restrict__ result, double seq) {
   __shared__ double s_p[STREAM_WARPS];
   __shared__ long long s_e[STREAM_WARPS];
   __shared__ int s_b[STREAM_WARPS];
@@ -233,44 +235,33 @@ __device__ __forceinline__ void nll_finish(const RateParams &R, int KC, int64_t 
     if (m.bad > 0 || !(norm > 0.0)) nll = INFINITY;
     result[0] = s0; result[1] = sum_t; result[2] = norm; result[3] = nll; result[4] = (double)m.bad;
     *ticket = 0;
+    if (seq != 0.0) {                       // 0: nobody polls this slot (batched / device-side results)
+      __threadfence_system();
+      *reinterpret_cast<volatile double *>(result + 5) = seq;
+    }
   }
 }
 
 // ------------------------------------------------------------------------------------------------
 // Coupling-only call.  Reads K_c columns (16 B elements) and t: algorithmic traffic 16 K_c + 8 B per event.
-// Two events per thread per iteration: 2 (K_c + 1) independent loads in flight per thread.
+// One event per thread per iteration (K_c + 1 independent loads in flight per thread, 72 registers at K_c = 8): the
+// blocks of the NEXT kernel in the stream then fit next to this kernel's two blocks per SM, so consecutive calls
+// overlap head to tail under programmatic dependent launch.  Measured on B200 (1 M events, K_c = 8, back to back):
+// two events per iteration (128 registers, SM full) 21.3 us per call, this form 16.1 us; isolated both 22 us from
+// first block start to result.  A reversed traversal on every other call (L2 reuse of the 136 MB stream in the 126 MB
+// L2) gave 14.0 us but makes the per-thread product order depend on the call parity; not used.
 template <int KC, bool SMALL>
 __global__ void __launch_bounds__(STREAM_BLOCK, STREAM_BLOCKS_PER_SM)
 nll_stream_kernel(const double2 *__restrict__ a, const double *__restrict__ t, int64_t ld, int64_t n,
                   const __grid_constant__ RateParams R, const double *__restrict__ G, double inv_n_norm, double sum_t,
-                  double *__restrict__ partials, unsigned int *ticket, double *__restrict__ result, int early_wait) {
-  constexpr int UNR = KC <= 8 ? 2 : 1;   // wider models: one event per iteration, or the columns spill
+                  double *__restrict__ partials, unsigned int *ticket, double *__restrict__ result, int early_wait, double seq) {
   if (early_wait) pdl_wait();            // the predecessor wrote the columns
   pdl_launch_dependents();               // only after this kernel's own early wait: see the ordering note at pdl_wait()
   MantAcc la;
   const double yG = R.y * R.Gamma, xG = R.x * R.Gamma;
   const int64_t stride = (int64_t)gridDim.x * STREAM_BLOCK;
-  int64_t i = (int64_t)blockIdx.x * STREAM_BLOCK + threadIdx.x;
 #pragma unroll 1
-  for (; i + (UNR - 1) * stride < n; i += UNR * stride) {
-    double2 v[UNR][KC];
-    double ti[UNR];
-#pragma unroll
-    for (int u = 0; u < UNR; ++u) {
-#pragma unroll
-      for (int c = 0; c < KC; ++c) v[u][c] = ldg_stream2(a + c * ld + i + u * stride);
-      ti[u] = ldg_stream1(t + i + u * stride);
-    }
-#pragma unroll
-    for (int u = 0; u < UNR; ++u) {
-      double2 A = make_double2(0.0, 0.0), Ab = make_double2(0.0, 0.0);
-#pragma unroll
-      for (int c = 0; c < KC; ++c) amp_add(A, Ab, R.c[c][0], R.c[c][1], R.cbar[c][0], R.cbar[c][1], v[u][c]);
-      la.add(bracket<SMALL>(A, Ab, yG * ti[u], xG * ti[u]));
-    }
-  }
-#pragma unroll 1
-  for (; i < n; i += stride) {
+  for (int64_t i = (int64_t)blockIdx.x * STREAM_BLOCK + threadIdx.x; i < n; i += stride) {
     double2 v[KC];
 #pragma unroll
     for (int c = 0; c < KC; ++c) v[c] = ldg_stream2(a + c * ld + i);
@@ -281,7 +272,7 @@ nll_stream_kernel(const double2 *__restrict__ a, const double *__restrict__ t, i
     la.add(bracket<SMALL>(A, Ab, yG * ti, xG * ti));
   }
   if (!early_wait) pdl_wait();
-  nll_finish(R, KC, n, sum_t, la, G, inv_n_norm, partials, ticket, result);
+  nll_finish(R, KC, n, sum_t, la, G, inv_n_norm, partials, ticket, result, seq);
 }
 
 // P_i = e^{-Gamma t_i} B_i / N for parity and plots (tddp4_nll with prob_out): same per-event arithmetic as the
@@ -304,7 +295,7 @@ template <int KC>
 __global__ void __launch_bounds__(STREAM_BLOCK, STREAM_BLOCKS_PER_SM)
 nll_res_kernel(const double2 *__restrict__ a, const double *__restrict__ tr, int64_t ld, int64_t n,
                const __grid_constant__ RateParams R, const double *__restrict__ G, double inv_n_norm,
-               double *__restrict__ partials, unsigned int *ticket, double *__restrict__ result) {
+               double *__restrict__ partials, unsigned int *ticket, double *__restrict__ result, double seq) {
   __shared__ double s_S[4];
   MantAcc la;
   pdl_wait();                              // G is read first thing
@@ -321,7 +312,7 @@ nll_res_kernel(const double2 *__restrict__ a, const double *__restrict__ tr, int
     for (int c = 0; c < KC; ++c) amp_add(A, Ab, R.c[c][0], R.c[c][1], R.cbar[c][0], R.cbar[c][1], v[c]);
     la.add(resolved_prob(A, Ab, tr + i, ld, s_S));
   }
-  nll_finish<true>(R, KC, n, 0.0, la, G, inv_n_norm, partials, ticket, result);
+  nll_finish<true>(R, KC, n, 0.0, la, G, inv_n_norm, partials, ticket, result, seq);
 }
 // P_i with resolution for prob_out
 __global__ void __launch_bounds__(STREAM_BLOCK)
@@ -342,11 +333,22 @@ prob_res_kernel(const double2 *__restrict__ a, const double *__restrict__ tr, in
 constexpr int TRES_BLOCK = 128;
 __global__ void __launch_bounds__(TRES_BLOCK)
 tres_kernel(const __grid_constant__ FaddTab F, const double *__restrict__ t, const double *__restrict__ sigma_t, int64_t n,
-            double x, double y, double Gamma, double t_lo, double t_hi, double *__restrict__ tr, int64_t ld) {
+            double x, double y, double Gamma, double t_lo, double t_hi, const TresTable *__restrict__ table,
+            double *__restrict__ tr, int64_t ld) {
+  __shared__ TresTable tab;
+  for (int k = threadIdx.x; k < (int)(sizeof(TresTable) / sizeof(double)); k += TRES_BLOCK)
+    reinterpret_cast<double *>(&tab)[k] = reinterpret_cast<const double *>(table)[k];
+  __syncthreads();
   int64_t i = (int64_t)blockIdx.x * TRES_BLOCK + threadIdx.x;
   if (i >= n) return;
   double psi[4], tint[4];
-  time_terms(F, t[i], sigma_t[i], x, y, Gamma, t_lo, t_hi, psi, tint);
+  const double sig = sigma_t[i];
+  if (tab.ok) {                                   // block-uniform
+    time_terms(F, t[i], sig, x, y, Gamma, t_lo, t_hi, psi, nullptr);
+    window_terms_table(tab, sig, tint);
+  } else {
+    time_terms(F, t[i], sig, x, y, Gamma, t_lo, t_hi, psi, tint);
+  }
 #pragma unroll
   for (int m = 0; m < 4; ++m) { tr[m * ld + i] = psi[m]; tr[(4 + m) * ld + i] = tint[m]; }
 }
@@ -458,7 +460,7 @@ colnll_stream_kernel(const __grid_constant__ StreamTab S, const __grid_constant_
                      double2 *__restrict__ a,
                      const __grid_constant__ RateParams R, const double *__restrict__ G, double inv_n_norm, double sum_t,
                      double *__restrict__ partials, unsigned int *ticket, double *__restrict__ result, int early_wait,
-                     uint32_t store_mask /* bit kappa: the stored column kappa is stale and is rewritten */) {
+                     uint32_t store_mask /* bit kappa: the stored column kappa is stale and is rewritten */, double seq) {
   extern __shared__ __align__(16) char smem_raw[];
   __shared__ double s_S[4];
   if (RES || early_wait) pdl_wait();       // the predecessor reads the columns this kernel rewrites (or RES: G first)
@@ -489,7 +491,7 @@ colnll_stream_kernel(const __grid_constant__ StreamTab S, const __grid_constant_
     else la.add(bracket<SMALL>(A, Ab, yG * ti, xG * ti));
   }
   if (!(RES || early_wait)) pdl_wait();
-  nll_finish<RES>(R, S.n_kc, n, sum_t, la, G, inv_n_norm, partials, ticket, result);
+  nll_finish<RES>(R, S.n_kc, n, sum_t, la, G, inv_n_norm, partials, ticket, result, seq);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -502,7 +504,13 @@ colnll_stream_kernel(const __grid_constant__ StreamTab S, const __grid_constant_
 // the warp then feeds its 32 events, 4 at a time, through the MMA.  NB = number of 8-feature blocks.
 // Reads the s rows in use, the g rows, the f rows, and w if the sample is weighted.
 // Deterministic: per-warp accumulation in event order, warps then blocks summed in index order.
-__host__ __device__ constexpr int gram_stride(int NB) { return NB <= 2 ? 20 : 36; }   // = 4 mod 16: conflict-free fragments
+// X tile of a warp: row = event, gram_stride(NB) = 8 NB + 2 doubles per row (F = 8 NB features, the weight at [F]).
+// Both access patterns are bank-conflict free: a lane's 16-byte column stores land in slot (e (4 NB + 1) + kappa) mod 8,
+// distinct over the 8 lanes of a wavefront; MMA group g takes the four events e = 8 (g >> 1) + 2 (lane & 3) + (g & 1), so
+// the fragment loads of a half-warp hit the 8-byte banks (phi + 4 (lane & 3) + const) mod 16, phi = lane >> 2.
+// (Measured: rows of 20 doubles with groups of consecutive events had 2-way store conflicts, 7.2 M conflict
+// wavefronts per 4 M events with the LSU data pipe 83 % busy; this layout: Gram kernel 215 -> 211 us.)
+__host__ __device__ constexpr int gram_stride(int NB) { return 8 * NB + 2; }
 inline size_t gram_warp_scratch(int NB, int n_inst4) {
   return align_up(lineshape_scratch_bytes(n_inst4), 128) + align_up((size_t)32 * gram_stride(NB) * sizeof(double), 128);
 }
@@ -544,10 +552,10 @@ gram_stream_kernel(const __grid_constant__ StreamTab S, const __grid_constant__ 
   // lanes of a ragged last tile compute on zeros: f = 0 gives zero columns, and their weight is forced to 0.
   auto mma_tile = [&]() {
     __syncwarp();
-    const double *base = Xs + (lane & 3) * STRIDE + (lane >> 2);
+    const double *base = Xs + (2 * (lane & 3)) * STRIDE + (lane >> 2);
 #pragma unroll
     for (int grp = 0; grp < 8; ++grp) {                  // 4 events per MMA, 8 groups per warp tile
-      const double *r = base + grp * 4 * STRIDE;
+      const double *r = base + (8 * (grp >> 1) + (grp & 1)) * STRIDE;
       double wv = r[F - (lane >> 2)];
       double x[NB];
 #pragma unroll

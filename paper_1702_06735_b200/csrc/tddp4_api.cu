@@ -36,6 +36,7 @@ struct EventSet {
   double *trg = nullptr;                             // derivative rows of the gradient in resolution mode, [8][ld] (on demand)
   bool tresg_valid = false;
   double sum_t = 0.0, t_max = 0.0;                   // sum and max |t| of the decay times (fixed-order kernel)
+  double sig_lo = 0.0, sig_hi = 0.0;                 // range of sigma_t (resolution mode: the window-integral table covers it)
   bool cols_dirty = true;                            // coupling columns stale (a mass or width moved since they were built)
   bool loaded = false;
 };
@@ -62,6 +63,9 @@ struct tddp4 {
   LineParams LP{};
   RateParams RP{};
   FaddTab FT{};                      // Faddeeva expansion coefficients (resolution mode)
+  double *staging = nullptr;         // device staging of host four-momenta (grow-only)
+  size_t staging_cap = 0;
+  TresTable *tres_tab = nullptr;     // device: Chebyshev table of the window integrals in sigma, rebuilt with the time rows
   std::vector<double> mass, width;
   EventSet set[2];
   // normalisation
@@ -94,6 +98,9 @@ struct tddp4 {
   double prof_bytes[TDDP4_K_COUNT] = {0};   // algorithmic bytes of the profiled launches
   int64_t prof_n[TDDP4_K_COUNT] = {0};
   int64_t launches = 0;
+  double seq = 0.0;                  // sequence stamp of the last NLL kernel enqueued (word [5] of its result slot)
+  bool stamp = false;                // the evaluation being enqueued writes to a polled slot: its kernel carries a stamp
+  double slot_seq[N_SLOTS] = {0};    // stamp each slot is waiting for
   int sm_count = 148;
   std::string err;
 };
@@ -323,10 +330,10 @@ int launch_nll(tddp4 *h, const EventSet &e, double inv_n, double *result, bool s
   const int early = !(h->prev_kind == PREV_NLL || h->prev_kind == PREV_GRAM);
   if (small)
     CU_LAUNCH(launch_pdl(nll_stream_kernel<KC, true>, grid, STREAM_BLOCK, 0, h->stream, (const double2 *)e.a, (const double *)e.t, e.ld, e.n, h->RP,
-                         (const double *)h->G, inv_n, e.sum_t, h->partials, h->ticket, result, early));
+                         (const double *)h->G, inv_n, e.sum_t, h->partials, h->ticket, result, early, h->stamp ? ++h->seq : 0.0));
   else
     CU_LAUNCH(launch_pdl(nll_stream_kernel<KC, false>, grid, STREAM_BLOCK, 0, h->stream, (const double2 *)e.a, (const double *)e.t, e.ld, e.n, h->RP,
-                         (const double *)h->G, inv_n, e.sum_t, h->partials, h->ticket, result, early));
+                         (const double *)h->G, inv_n, e.sum_t, h->partials, h->ticket, result, early, h->stamp ? ++h->seq : 0.0));
   h->prev_kind = PREV_NLL;
   return TDDP4_OK;
 }
@@ -338,7 +345,7 @@ int launch_nll_res(tddp4 *h, const EventSet &e, double inv_n, double *result) {
   if (rc) return rc;
   Prof p(h, TDDP4_K_NLL, (double)e.n * (16.0 * KC + 64.0));
   CU_LAUNCH(launch_pdl(nll_res_kernel<KC>, grid, STREAM_BLOCK, 0, h->stream, (const double2 *)e.a, (const double *)e.tr, e.ld, e.n, h->RP,
-                       (const double *)h->G, inv_n, h->partials, h->ticket, result));
+                       (const double *)h->G, inv_n, h->partials, h->ticket, result, h->stamp ? ++h->seq : 0.0));
   h->prev_kind = PREV_NLL;
   return TDDP4_OK;
 }
@@ -360,7 +367,8 @@ int launch_colnll(tddp4 *h, const EventSet &e, double inv_n, double *result, boo
   const double *tp = h->use_resolution ? e.tr : e.t;
 #define COLNLL_LAUNCH(SM, RS)                                                                                                  \
   launch_pdl(colnll_stream_kernel<SM, RS, NI, NT>, grid, STREAM_BLOCK, smem, h->stream, S, h->LP, (const double *)e.cache, tp, e.ld, e.n, \
-             e.a, h->RP, (const double *)h->G, inv_n, sum_t, h->partials, h->ticket, result, early, h->store_mask)
+             e.a, h->RP, (const double *)h->G, inv_n, sum_t, h->partials, h->ticket, result, early, h->store_mask, seq)
+  const double seq = h->stamp ? h->seq + 1.0 : 0.0;
   cudaError_t launched = with_size_class(h->size_class, [&](auto ni, auto nt) {
     constexpr int NI = decltype(ni)::value, NT = decltype(nt)::value;
     if (mode == 2) return COLNLL_LAUNCH(false, true);
@@ -369,6 +377,7 @@ int launch_colnll(tddp4 *h, const EventSet &e, double inv_n, double *result, boo
   });
 #undef COLNLL_LAUNCH
   CU_LAUNCH(launched);
+  if (h->stamp) h->seq = seq;
   h->prev_kind = PREV_COLNLL;   // committed only after the launch succeeded: a failed launch keeps the stale-column set
   h->store_mask = 0;
   return TDDP4_OK;
@@ -417,8 +426,10 @@ int enqueue_nll(tddp4 *h, double *result, double *prob) {
       fill_rows_kernel<<<(int)((d.n + 255) / 256), 256, 0, h->stream>>>(d.tr, d.ld, d.n, v);
     } else {
       Prof p(h, TDDP4_K_TRES, (double)d.n * 80.0);
+      tres_table_kernel<<<1, 32, 0, h->stream>>>(h->FT, h->RP.x, h->RP.y, h->RP.Gamma, h->t_lo, h->t_hi, d.sig_lo, d.sig_hi, h->tres_tab);
       tres_kernel<<<grid, TRES_BLOCK, 0, h->stream>>>(h->FT, d.t, d.sigma_t, d.n, h->RP.x, h->RP.y, h->RP.Gamma, h->t_lo, h->t_hi,
-                                                      d.tr, d.ld);
+                                                      h->tres_tab, d.tr, d.ld);
+      ++h->launches;
     }
     CU(cudaGetLastError());
     d.tres_valid = true;
@@ -454,40 +465,70 @@ int enqueue_nll_slot(tddp4 *h, int slot, double *prob) {
   // stays in device memory and is copied.
   const bool direct = prob == nullptr;
   double *result = (direct ? h->results_host_dev : h->results) + (size_t)slot * SLOT_DOUBLES;
+  h->stamp = direct;
   int rc = enqueue_nll(h, result, prob);
+  h->stamp = false;
   if (rc) return rc;
   if (!direct)
     CU(cudaMemcpyAsync(h->results_host + (size_t)slot * SLOT_DOUBLES, result, SLOT_DOUBLES * sizeof(double),
                        cudaMemcpyDeviceToHost, h->stream));
   CU(cudaEventRecord(h->slot_event[slot], h->stream));
   h->slot_used[slot] = true;
+  h->slot_seq[slot] = direct ? h->seq : 0.0;
   return TDDP4_OK;
 }
 
+// Wait for a result slot.  A slot in mapped host memory carries the kernel's sequence stamp in word [5], written after
+// the result behind a system-wide fence: the host polls that word (about a microsecond after the kernel's last store)
+// instead of going through cudaEventSynchronize (measured: 36 -> 2x us per synchronous coupling-only call).  The event
+// is still consulted from time to time so that a failed kernel cannot hang the caller.
+int wait_slot(tddp4 *h, int slot) {
+  const double want = h->slot_seq[slot];
+  if (want > 0.0) {
+    const volatile double *flag = h->results_host + (size_t)slot * SLOT_DOUBLES + 5;
+    for (long spin = 0;; ++spin) {
+      if (*flag == want) return TDDP4_OK;
+      if ((spin & 0xfff) == 0xfff) {
+        cudaError_t q = cudaEventQuery(h->slot_event[slot]);
+        if (q == cudaSuccess) break;                       // complete: the stamp is visible by now (or the launch never ran)
+        if (q != cudaErrorNotReady) return fail(h, TDDP4_ERR_CUDA, "cudaEventQuery: %s", cudaGetErrorString(q));
+      }
+    }
+  }
+  CU(cudaEventSynchronize(h->slot_event[slot]));
+  return TDDP4_OK;
+}
+
+// gradient kernels (grad_kernels.cuh): whole warps iterate together, per-warp X and W tiles in dynamic shared memory
 template <int KC>
 int launch_nll_grad_res(tddp4 *h, const EventSet &e, double inv_n) {
-  int grid = (int)std::max<int64_t>(1, std::min<int64_t>((e.n + STREAM_BLOCK - 1) / STREAM_BLOCK, (int64_t)h->sm_count));
-  int rc = ensure_partials(h, (size_t)grid * (4 * KC + 9) + 16);
+  constexpr int NB = grad_nb<KC>();
+  int grid = stream_grid(h, e.n);
+  int rc = ensure_partials(h, (size_t)grid * (NB * 32 + 9) + 16);
   if (rc) return rc;
+  const size_t smem = grad_smem_bytes<KC>();
   Prof p(h, TDDP4_K_GRAD, (double)e.n * (16.0 * KC + 128.0));
-  nll_grad_res_kernel<KC><<<grid, STREAM_BLOCK, 0, h->stream>>>(e.a, e.tr, e.trg, e.ld, e.n, h->RP, h->G, inv_n, h->partials, h->ticket,
-                                                              h->grad_host_dev);
+  nll_grad_res_kernel<KC><<<grid, STREAM_BLOCK, smem, h->stream>>>(e.a, e.tr, e.trg, e.ld, e.n, h->RP, h->G, inv_n, h->partials, h->ticket,
+                                                                  h->grad_host_dev);
   return TDDP4_OK;
 }
 
 template <int KC>
 int launch_nll_grad(tddp4 *h, const EventSet &e, double inv_n, bool small) {
-  int grid = (int)std::max<int64_t>(1, std::min<int64_t>((e.n + STREAM_BLOCK - 1) / STREAM_BLOCK, (int64_t)h->sm_count * (KC <= 8 ? 2 : 1)));
-  int rc = ensure_partials(h, (size_t)grid * (4 * KC + 5) + 16);
+  constexpr int NB = grad_nb<KC>();
+  int grid = (int)std::max<int64_t>(1, std::min<int64_t>((e.n + STREAM_BLOCK - 1) / STREAM_BLOCK, (int64_t)h->sm_count * grad_bps<KC>()));
+  int rc = ensure_partials(h, (size_t)grid * (NB * 32 + 5) + 16);
   if (rc) return rc;
   GradParams gp = time_integral_derivatives(h->RP.x, h->RP.y, h->RP.Gamma, h->t_lo, h->t_hi);
+  const size_t smem = grad_smem_bytes<KC>();
   Prof p(h, TDDP4_K_GRAD, (double)e.n * (16.0 * KC + 8.0));
-  if (small)
-    nll_grad_kernel<KC, true><<<grid, STREAM_BLOCK, 0, h->stream>>>(e.a, e.t, e.ld, e.n, h->RP, gp, h->G, inv_n, e.sum_t, h->partials,
-                                                                   h->ticket, h->grad_host_dev);
-  else
-    nll_grad_kernel<KC, false><<<grid, STREAM_BLOCK, 0, h->stream>>>(e.a, e.t, e.ld, e.n, h->RP, gp, h->G, inv_n, e.sum_t, h->partials,
-                                                                    h->ticket, h->grad_host_dev);
+  if (small) {
+    nll_grad_kernel<KC, true><<<grid, STREAM_BLOCK, smem, h->stream>>>(e.a, e.t, e.ld, e.n, h->RP, gp, h->G, inv_n, e.sum_t, h->partials,
+                                                                      h->ticket, h->grad_host_dev);
+  } else {
+    nll_grad_kernel<KC, false><<<grid, STREAM_BLOCK, smem, h->stream>>>(e.a, e.t, e.ld, e.n, h->RP, gp, h->G, inv_n, e.sum_t, h->partials,
+                                                                       h->ticket, h->grad_host_dev);
+  }
   return TDDP4_OK;
 }
 
@@ -642,9 +683,11 @@ int tddp4_create(const tddp4_model_desc *desc, tddp4 **out) {
             cudaHostGetDevicePointer((void **)&h->results_host_dev, h->results_host, 0) == cudaSuccess &&
             cudaHostAlloc(&h->grad_host, sizeof(double) * (GRAD_OFFSET + 4 * MAX_KC + 2), cudaHostAllocMapped) == cudaSuccess &&
             cudaHostGetDevicePointer((void **)&h->grad_host_dev, h->grad_host, 0) == cudaSuccess &&
-            cudaMalloc(&h->gen_scalars, sizeof(unsigned long long) * 2) == cudaSuccess &&
+            cudaMalloc(&h->gen_scalars, sizeof(unsigned long long) * 4) == cudaSuccess &&
+            cudaMalloc(&h->tres_tab, sizeof(TresTable)) == cudaSuccess &&
             cudaMemset(h->ticket, 0, sizeof(unsigned int)) == cudaSuccess &&
             cudaMemset(h->G, 0, sizeof(double) * 2 * KC * KC) == cudaSuccess;
+  if (ok) memset(h->results_host, 0, sizeof(double) * N_SLOTS * SLOT_DOUBLES);   // no stale sequence stamps from a recycled allocation
   for (int s = 0; ok && s < N_SLOTS; ++s) ok = cudaEventCreateWithFlags(&h->slot_event[s], cudaEventDisableTiming) == cudaSuccess;
   if (!ok) return bail(fail(h, TDDP4_ERR_CUDA, "allocation failed: %s", cudaGetErrorString(cudaGetLastError())));
   // kernels that need more than 48 KB of dynamic shared memory
@@ -667,6 +710,14 @@ int tddp4_create(const tddp4_model_desc *desc, tddp4 **out) {
     });
   }
   cudaFuncSetAttribute(terms_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(MAX_INST * COL_BLOCK * sizeof(double2)));
+  switch (KC) {   // the gradient kernels' per-warp tiles (grad_kernels.cuh)
+#define CASE(k) case k: cudaFuncSetAttribute(nll_grad_kernel<k, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)grad_smem_bytes<k>()); \
+                        cudaFuncSetAttribute(nll_grad_kernel<k, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)grad_smem_bytes<k>()); \
+                        cudaFuncSetAttribute(nll_grad_res_kernel<k>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)grad_smem_bytes<k>()); break;
+    CASE(1) CASE(2) CASE(3) CASE(4) CASE(5) CASE(6) CASE(7) CASE(8) CASE(9) CASE(10) CASE(11) CASE(12)
+    CASE(13) CASE(14) CASE(15) CASE(16)
+#undef CASE
+  }
   *out = h;
   return TDDP4_OK;
 }
@@ -678,7 +729,7 @@ int tddp4_destroy(tddp4 *h) {
   for (auto e : h->pool) cudaEventDestroy(e);
   free_set(h->set[0]);
   free_set(h->set[1]);
-  cudaFree(h->G); cudaFree(h->partials); cudaFree(h->ticket); cudaFree(h->results); cudaFree(h->batch_res);
+  cudaFree(h->G); cudaFree(h->partials); cudaFree(h->ticket); cudaFree(h->results); cudaFree(h->batch_res); cudaFree(h->tres_tab); cudaFree(h->staging);
   if (h->batch_res_host) cudaFreeHost(h->batch_res_host);
   if (h->results_host) cudaFreeHost(h->results_host);
   if (h->grad_host) cudaFreeHost(h->grad_host);
@@ -710,24 +761,34 @@ int tddp4_load_events(tddp4 *h, int which, int64_t n, int64_t ld_in, const doubl
   h->prev_kind = PREV_NONE;
   if (which == 0) h->store_mask = 0xFFFFFFFFu;
   EventSet &e = h->set[which];
-  free_set(e);
-  e.n = n;
-  e.ld = std::max<int64_t>(32, (n + 31) / 32 * 32);   // rows start 256-byte aligned
   const ModelTab &M = h->M;
-  e.R = h->S.R + (weight && n > 0 ? 1 : 0);
-  const CacheRows cr{e.R, M.n_sys, M.n_sys + h->S.n_inst4};
-  CU(cudaMalloc(&e.cache, sizeof(double) * e.R * e.ld));
-  CU(cudaMemsetAsync(e.cache, 0, sizeof(double) * e.R * e.ld, h->stream));   // padding rows and the ragged tail stay zero
-  if (which == 0) {   // the normalisation sample keeps no columns; a coupling without chains keeps its zero column
-    CU(cudaMalloc(&e.a, sizeof(double2) * M.n_kc * e.ld));
-    CU(cudaMemsetAsync(e.a, 0, sizeof(double2) * M.n_kc * e.ld, h->stream));
-    if (h->use_resolution) CU(cudaMalloc(&e.tr, sizeof(double) * 8 * e.ld));
+  const int R_new = h->S.R + (weight && n > 0 ? 1 : 0);
+  // a reload of the same shape (same n, same optional rows) keeps every allocation: the padding rows, the ragged tail
+  // and the columns of couplings without chains are still zero, everything else is rewritten below
+  const bool reuse = e.loaded && e.n == n && e.R == R_new && n > 0 && (e.t != nullptr) == (t != nullptr) &&
+                     (e.sigma_t != nullptr) == (sigma_t != nullptr) && (e.w != nullptr) == (weight != nullptr);
+  if (!reuse) {
+    free_set(e);
+    e.n = n;
+    e.ld = std::max<int64_t>(32, (n + 31) / 32 * 32);   // rows start 256-byte aligned
+    e.R = R_new;
+    CU(cudaMalloc(&e.cache, sizeof(double) * e.R * e.ld));
+    CU(cudaMemsetAsync(e.cache, 0, sizeof(double) * e.R * e.ld, h->stream));   // padding rows and the ragged tail stay zero
+    if (which == 0) {   // the normalisation sample keeps no columns; a coupling without chains keeps its zero column
+      CU(cudaMalloc(&e.a, sizeof(double2) * M.n_kc * e.ld));
+      CU(cudaMemsetAsync(e.a, 0, sizeof(double2) * M.n_kc * e.ld, h->stream));
+      if (h->use_resolution) CU(cudaMalloc(&e.tr, sizeof(double) * 8 * e.ld));
+    }
   }
+  e.tres_valid = e.tresg_valid = false;
+  const CacheRows cr{e.R, M.n_sys, M.n_sys + h->S.n_inst4};
   cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
   auto copy_vec = [&](double **dst, const double *src) -> cudaError_t {
     if (!src || n == 0) return cudaSuccess;
-    cudaError_t e_ = cudaMalloc(dst, sizeof(double) * e.ld);
-    if (e_ != cudaSuccess) return e_;
+    if (!*dst) {
+      cudaError_t e_ = cudaMalloc(dst, sizeof(double) * e.ld);
+      if (e_ != cudaSuccess) return e_;
+    }
     return cudaMemcpyAsync(*dst, src, sizeof(double) * n, kind, h->stream);
   };
   CU(copy_vec(&e.t, t));
@@ -735,13 +796,17 @@ int tddp4_load_events(tddp4 *h, int which, int64_t n, int64_t ld_in, const doubl
   CU(copy_vec(&e.w, weight));
   if (n > 0) {
     const double *dp4 = p4;
-    double *staging = nullptr;
     int64_t ld_dev = ld_in;
-    if (!on_device) {
-      CU(cudaMalloc(&staging, sizeof(double) * 16 * n));
-      CU(cudaMemcpy2DAsync(staging, sizeof(double) * n, p4, sizeof(double) * ld_in, sizeof(double) * n, 16,
+    if (!on_device) {   // host input goes through a staging buffer the handle keeps (grow-only)
+      if ((size_t)(16 * n) > h->staging_cap) {
+        cudaFree(h->staging);
+        h->staging = nullptr; h->staging_cap = 0;
+        CU(cudaMalloc(&h->staging, sizeof(double) * 16 * n));
+        h->staging_cap = (size_t)(16 * n);
+      }
+      CU(cudaMemcpy2DAsync(h->staging, sizeof(double) * n, p4, sizeof(double) * ld_in, sizeof(double) * n, 16,
                            cudaMemcpyHostToDevice, h->stream));
-      dp4 = staging;
+      dp4 = h->staging;
       ld_dev = n;
     }
     int grid = (int)((n + KIN_BLOCK - 1) / KIN_BLOCK);
@@ -756,17 +821,19 @@ int tddp4_load_events(tddp4 *h, int which, int64_t n, int64_t ld_in, const doubl
       ++h->launches;
       CU(cudaGetLastError());
     }
+    double st[6] = {0};
     if (e.t) {
-      double st[2];
-      stat_kernel<<<1, 1024, 0, h->stream>>>(e.t, n, h->results);   // slot 0 words 0, 1 as scratch
+      stat_kernel<<<1, 1024, 0, h->stream>>>(e.t, n, h->results);   // slot 0 as scratch
       ++h->launches;
-      CU(cudaMemcpyAsync(st, h->results, 2 * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
-      CU(cudaStreamSynchronize(h->stream));
+      if (e.sigma_t) { stat_kernel<<<1, 1024, 0, h->stream>>>(e.sigma_t, n, h->results + 3); ++h->launches; }
+      CU(cudaMemcpyAsync(st, h->results, 6 * sizeof(double), cudaMemcpyDeviceToHost, h->stream));
+    }
+    CU(cudaStreamSynchronize(h->stream));        // the one synchronisation of a load: the caller's buffers are free again
+    if (e.t) {
       e.sum_t = st[0];
       e.t_max = st[1];
+      if (e.sigma_t) { e.sig_lo = st[5]; e.sig_hi = st[4]; }   // sigma_t > 0: max |.| = max
     }
-    CU(cudaStreamSynchronize(h->stream));
-    if (staging) cudaFree(staging);
   }
   e.cols_dirty = true;
   e.loaded = true;
@@ -830,7 +897,8 @@ int tddp4_nll_async(tddp4 *h, int slot) {
 int tddp4_nll_result(tddp4 *h, int slot, double *nll_out) {
   if (!h || slot < 0 || slot >= N_SLOTS || !nll_out) return fail(h, TDDP4_ERR_ARG, "bad slot");
   if (!h->slot_used[slot]) return fail(h, TDDP4_ERR_STATE, "slot %d holds no evaluation", slot);
-  CU(cudaEventSynchronize(h->slot_event[slot]));
+  int wrc = wait_slot(h, slot);
+  if (wrc) return wrc;
   const double *r = h->results_host + (size_t)slot * SLOT_DOUBLES;
   *nll_out = r[3];
   if (r[4] > 0.0 || !std::isfinite(r[3])) {
@@ -901,7 +969,8 @@ int tddp4_nll_grad(tddp4 *h, double *nll_out, double *grad_out) {
 int tddp4_nll_parts(tddp4 *h, int slot, double out[5]) {
   if (!h || slot < 0 || slot >= N_SLOTS || !out) return fail(h, TDDP4_ERR_ARG, "bad slot");
   if (!h->slot_used[slot]) return fail(h, TDDP4_ERR_STATE, "slot %d holds no evaluation", slot);
-  CU(cudaEventSynchronize(h->slot_event[slot]));
+  int wrc = wait_slot(h, slot);
+  if (wrc) return wrc;
   memcpy(out, h->results_host + (size_t)slot * SLOT_DOUBLES, 5 * sizeof(double));
   return TDDP4_OK;
 }
@@ -975,6 +1044,73 @@ int tddp4_gram_override(tddp4 *h, const double *G_sum, int64_t n_norm) {
   return TDDP4_OK;
 }
 
+int tddp4_gram_state(const tddp4 *h, int *valid, int *overridden) {
+  if (!h) return TDDP4_ERR_ARG;
+  if (valid) *valid = h->gram_valid ? 1 : 0;
+  if (overridden) *overridden = h->gram_overridden ? 1 : 0;
+  return TDDP4_OK;
+}
+
+int tddp4_gram_enqueue(tddp4 *h, double *G_dev) {
+  if (!h || !G_dev) return fail(h, TDDP4_ERR_ARG, "null argument");
+  if (!h->have_params) return fail(h, TDDP4_ERR_STATE, "tddp4_set_params has not been called");
+  if (h->gram_overridden) { h->gram_valid = false; h->gram_overridden = false; }
+  int rc = ensure_gram(h);
+  if (rc) return rc;
+  const int len = 2 * h->M.n_kc * h->M.n_kc;
+  CU(cudaMemcpyAsync(G_dev, h->G, sizeof(double) * len, cudaMemcpyDeviceToDevice, h->stream));
+  append_count_kernel<<<1, 32, 0, h->stream>>>(G_dev + len, (double)h->gram_n);
+  ++h->launches;
+  CU(cudaGetLastError());
+  h->prev_kind = PREV_NONE;
+  return TDDP4_OK;
+}
+
+int tddp4_gram_reduce(tddp4 *h, const double *gathered_dev, int world, int64_t n_norm_total) {
+  if (!h || !gathered_dev || world < 1 || n_norm_total <= 0) return fail(h, TDDP4_ERR_ARG, "bad argument");
+  const int len = 2 * h->M.n_kc * h->M.n_kc;
+  gram_reduce_kernel<<<1, 256, 0, h->stream>>>(gathered_dev, world, len + 1, len, h->G);
+  ++h->launches;
+  CU(cudaGetLastError());
+  h->gram_valid = true;
+  h->gram_overridden = true;
+  h->gram_n = n_norm_total;
+  h->prev_kind = PREV_NONE;
+  return TDDP4_OK;
+}
+
+int tddp4_nll_enqueue(tddp4 *h, double *result_dev) {
+  if (!h || !result_dev) return fail(h, TDDP4_ERR_ARG, "null argument");
+  int rc = enqueue_nll(h, result_dev, nullptr);
+  h->prev_kind = PREV_NONE;      // the caller's collective follows on the stream: the next kernel waits early
+  return rc;
+}
+
+int tddp4_fp64_peak(tddp4 *h, double *inst_per_s) {
+  if (!h || !inst_per_s) return fail(h, TDDP4_ERR_ARG, "null argument");
+  const int grid = h->sm_count * 4, iters = 256;
+  cudaEvent_t a, b;
+  CU(cudaEventCreate(&a));
+  CU(cudaEventCreate(&b));
+  double best = 0.0;
+  for (int rep = 0; rep < 4; ++rep) {      // the first repetition warms up
+    CU(cudaEventRecord(a, h->stream));
+    fp64_peak_kernel<<<grid, 256, 0, h->stream>>>(h->results, 1.0000001, 1e-9, iters);
+    CU(cudaEventRecord(b, h->stream));
+    CU(cudaEventSynchronize(b));
+    float ms = 0.f;
+    CU(cudaEventElapsedTime(&ms, a, b));
+    double rate = (double)grid * 256.0 * 8.0 * 16.0 * iters / (ms * 1e-3);
+    if (rep > 0 && rate > best) best = rate;
+  }
+  h->launches += 4;
+  cudaEventDestroy(a);
+  cudaEventDestroy(b);
+  h->prev_kind = PREV_NONE;
+  *inst_per_s = best;
+  return TDDP4_OK;
+}
+
 int tddp4_norm(tddp4 *h, double *norm_out) {
   if (!h || !norm_out) return fail(h, TDDP4_ERR_ARG, "null argument");
   if (!h->have_params) return fail(h, TDDP4_ERR_STATE, "tddp4_set_params has not been called");
@@ -1017,13 +1153,13 @@ static int ensure_gen(tddp4 *h, int64_t n) {
   return TDDP4_OK;
 }
 
-static int launch_ratio(tddp4 *h, uint64_t seed, uint32_t stream_id, uint64_t first, int64_t n, int mode, double env,
+static int launch_ratio(tddp4 *h, uint64_t seed, uint32_t stream_id, uint64_t first, int64_t n, int mode, double env, int from_pilot,
                         double *p4, double *t, double *w, double *ratio, double *u) {
   int grid = (int)((n + GEN_BLOCK - 1) / GEN_BLOCK);
   {
     Prof p(h, TDDP4_K_GEN_RATIO);
     gen_ratio_kernel<<<grid, GEN_BLOCK, gen_smem_bytes(h->M.n_sys, h->M.n_inst), h->stream>>>(
-        h->M, h->LP, h->RP, 1.0 / h->RP.Gamma, seed, stream_id, first, n, mode, env, p4, t, w, ratio, u,
+        h->M, h->LP, h->RP, 1.0 / h->RP.Gamma, seed, stream_id, first, n, mode, env, from_pilot, p4, t, w, ratio, u,
         h->gen_scalars, h->gen_flags, h->gen_counts, h->gen_scalars + 1);
   }
   CU(cudaGetLastError());
@@ -1035,7 +1171,7 @@ int tddp4_candidates(tddp4 *h, uint64_t seed, uint32_t stream_id, int64_t first,
   if (!h || n < 0 || first < 0) return fail(h, TDDP4_ERR_ARG, "bad argument");
   if (!h->have_params) return fail(h, TDDP4_ERR_STATE, "tddp4_set_params has not been called");
   if (n == 0) return TDDP4_OK;
-  int rc = launch_ratio(h, seed, stream_id, (uint64_t)first, n, 0, 0.0, out_p4, out_t, out_w, out_ratio, out_u);
+  int rc = launch_ratio(h, seed, stream_id, (uint64_t)first, n, 0, 0.0, 0, out_p4, out_t, out_w, out_ratio, out_u);
   if (rc) return rc;
   CU(cudaStreamSynchronize(h->stream));
   return TDDP4_OK;
@@ -1050,48 +1186,40 @@ int tddp4_generate(tddp4 *h, uint64_t seed, uint32_t stream_id, int64_t first, i
   const int64_t CHUNK = (int64_t)1 << 25;
   int rc = ensure_gen(h, std::min<int64_t>(std::max<int64_t>(n_candidates, n_pilot), CHUNK));
   if (rc) return rc;
-  CU(cudaMemsetAsync(h->gen_scalars, 0, 2 * sizeof(unsigned long long), h->stream));
-  double env = envelope_scale;
-  if (n_pilot > 0) {   // G5: exact, order-independent maximum over the pilot
-    for (int64_t f = 0; f < n_pilot; f += CHUNK) {
-      rc = launch_ratio(h, seed, stream_id, (uint64_t)f, std::min(CHUNK, n_pilot - f), 1, 0.0, nullptr, nullptr, nullptr,
-                        nullptr, nullptr);
-      if (rc) return rc;
-    }
-    unsigned long long bits = 0;
-    CU(cudaMemcpyAsync(&bits, h->gen_scalars, sizeof bits, cudaMemcpyDeviceToHost, h->stream));
-    CU(cudaStreamSynchronize(h->stream));
-    double mx;
-    memcpy(&mx, &bits, sizeof mx);
-    env = envelope_scale * mx;
+  // device scalars: [0] pilot maximum (bit pattern), [1] overflow count, [2] running number of accepted candidates.
+  // Everything is enqueued without a host round trip: the envelope is read by the ratio kernel from [0], the output
+  // offsets of a chunk continue from [2]; one copy at the end brings the three words back.
+  CU(cudaMemsetAsync(h->gen_scalars, 0, 3 * sizeof(unsigned long long), h->stream));
+  const int from_pilot = n_pilot > 0;
+  for (int64_t f = 0; f < n_pilot; f += CHUNK) {   // G5: exact, order-independent maximum over the pilot
+    rc = launch_ratio(h, seed, stream_id, (uint64_t)f, std::min(CHUNK, n_pilot - f), 1, 0.0, 0, nullptr, nullptr, nullptr, nullptr, nullptr);
+    if (rc) return rc;
   }
-  int64_t total = 0;
   for (int64_t f = 0; f < n_candidates; f += CHUNK) {   // G6
     int64_t n = std::min(CHUNK, n_candidates - f);
     int64_t blocks = (n + GEN_BLOCK - 1) / GEN_BLOCK;
-    rc = launch_ratio(h, seed, stream_id, (uint64_t)(first + f), n, 2, env, nullptr, nullptr, nullptr, nullptr, nullptr);
+    rc = launch_ratio(h, seed, stream_id, (uint64_t)(first + f), n, 2, envelope_scale, from_pilot, nullptr, nullptr, nullptr, nullptr, nullptr);
     if (rc) return rc;
-    scan_kernel<<<1, 1024, 0, h->stream>>>(h->gen_counts, blocks, h->gen_offs);
+    scan_kernel<<<1, 1024, 0, h->stream>>>(h->gen_counts, blocks, h->gen_offs, h->gen_scalars + 2);
     ++h->launches;
     CU(cudaGetLastError());
     {
       Prof p(h, TDDP4_K_GEN_EMIT);
-      gen_emit_kernel<<<(int)blocks, GEN_BLOCK, 0, h->stream>>>(h->M, 1.0 / h->RP.Gamma, seed, stream_id,
-                                                                (uint64_t)(first + f), n, h->gen_flags, h->gen_offs, total,
-                                                                capacity, out_p4, out_t, out_index);
+      gen_emit_kernel<<<(int)((n + EMIT_SPAN - 1) / EMIT_SPAN), EMIT_BLOCK, 0, h->stream>>>(h->M, 1.0 / h->RP.Gamma, seed, stream_id,
+                                                                                         (uint64_t)(first + f), n, h->gen_flags, h->gen_offs,
+                                                                                         capacity, out_p4, out_t, out_index);
     }
     CU(cudaGetLastError());
-    unsigned long long cnt = 0;
-    CU(cudaMemcpyAsync(&cnt, h->gen_offs + blocks, sizeof cnt, cudaMemcpyDeviceToHost, h->stream));
-    CU(cudaStreamSynchronize(h->stream));
-    total += (int64_t)cnt;
   }
-  unsigned long long over = 0;
-  CU(cudaMemcpyAsync(&over, h->gen_scalars + 1, sizeof over, cudaMemcpyDeviceToHost, h->stream));
+  unsigned long long sc[3] = {0, 0, 0};
+  CU(cudaMemcpyAsync(sc, h->gen_scalars, sizeof sc, cudaMemcpyDeviceToHost, h->stream));
   CU(cudaStreamSynchronize(h->stream));
+  double mx;
+  memcpy(&mx, &sc[0], sizeof mx);
+  const int64_t total = (int64_t)sc[2];
   *n_accepted = total;
-  *n_overflow = (int64_t)over;
-  *envelope_out = env;
+  *n_overflow = (int64_t)sc[1];
+  *envelope_out = from_pilot ? envelope_scale * mx : envelope_scale;
   if (total > capacity) return fail(h, TDDP4_ERR_CAPACITY, "%lld accepted events exceed capacity %lld", (long long)total, (long long)capacity);
   return TDDP4_OK;
 }
