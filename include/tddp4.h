@@ -170,7 +170,7 @@ int tddp4_norm(tddp4 *h, double *norm_out);
  *   added in rank order by one kernel (same bits on every rank), normalised by n_norm_total.  Stays in force
  *   until the masses/widths change or the normalisation sample is reloaded.
  * tddp4_nll_enqueue: result_dev device [8]: words 0..4 as tddp4_nll_parts ([3] = this rank's NLL term
- *   Gamma sum t - sum log B + n log N with the Gram matrix in force), [5] = sequence stamp, [6..7] unused.
+ *   Gamma sum t - sum log B + n log N with the Gram matrix in force), [5..7] unused.
  * tddp4_gram_state: *valid = the matrix in force matches the current masses/widths; *overridden = it came from
  *   tddp4_gram_override / tddp4_gram_reduce.                                                           */
 int tddp4_gram_enqueue(tddp4 *h, double *G_dev);
@@ -197,6 +197,17 @@ int tddp4_weight_bound(const tddp4 *h, double *bound_out);
  * weight), out_ratio [n] (w B), out_u [n] (accept uniform); any may be NULL.                          */
 int tddp4_candidates(tddp4 *h, uint64_t seed, uint32_t stream_id, int64_t first, int64_t n, double *out_p4,
                      double *out_t, double *out_w, double *out_ratio, double *out_u);
+
+/* ---- validation projections (Fig. 3) ---------------------------------------- */
+/* The five observables the paper projects its generated samples on: m12, m34 (invariant masses of the pi+ pi- pair =
+ * particles (2,3) and of the K+ pi- pair = particles (0,1)), cos12, cos34 (helicity cosines of the pi+ and of the K+ in
+ * their pair's rest frame, with respect to the pair's flight direction in the D rest frame) and phi (angle between the
+ * two decay planes in the D rest frame, in (-pi, pi]); the paper does not define them, DESIGN.md 3 gives the reading.
+ * p4: device [16][ld] SoA, any frame.  ranges: host [5][2] (lo, hi) per observable; bin = floor((v - lo)/(hi - lo) *
+ * n_bins), v == hi counts in the last bin, values outside are dropped.  hist_out: host [5][n_bins] counts.
+ * values_dev: device [5][n] or NULL, the per-event observables.  n_bins <= 512.  Synchronous.           */
+int tddp4_project(tddp4 *h, int64_t n, int64_t ld, const double *p4, int n_bins, const double *ranges, int64_t *hist_out,
+                  double *values_dev);
 
 /* ---- inspection (per-layer parity, profiling) ---------------------------------------------------- */
 enum {

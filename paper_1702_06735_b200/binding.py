@@ -26,7 +26,7 @@ SYMBOLS = ["tddp4_create", "tddp4_destroy", "tddp4_set_stream", "tddp4_last_erro
            "tddp4_nll_parts", "tddp4_nll_grad", "tddp4_param_stride", "tddp4_nll_batch", "tddp4_gram", "tddp4_gram_override", "tddp4_norm", "tddp4_generate", "tddp4_weight_bound",
            "tddp4_candidates", "tddp4_get", "tddp4_layout", "tddp4_profile", "tddp4_profile_read",
            "tddp4_profile_reset", "tddp4_launch_count", "tddp4_gram_enqueue", "tddp4_gram_reduce", "tddp4_nll_enqueue",
-           "tddp4_gram_state", "tddp4_fp64_peak"]
+           "tddp4_gram_state", "tddp4_fp64_peak", "tddp4_project"]
 
 
 class Tddp4Error(RuntimeError):
@@ -97,6 +97,7 @@ def load_library():
     L.tddp4_nll_enqueue.argtypes = [vp, vp]
     L.tddp4_gram_state.argtypes = [vp, C.POINTER(C.c_int), C.POINTER(C.c_int)]
     L.tddp4_fp64_peak.argtypes = [vp, dp]
+    L.tddp4_project.argtypes = [vp, i64, i64, vp, C.c_int, vp, vp, vp]
     _lib = L
     return L
 
@@ -361,6 +362,18 @@ class Tddp4:
         self._check(self.lib.tddp4_candidates(self._h, seed, stream_id, first, n, _ptr(p4), _ptr(t), _ptr(w), _ptr(r),
                                               _ptr(u)))
         return p4, t, w, r, u
+
+    # -- tddp4_project ----------------------------------------------------------------------------
+    def project(self, p4, n_bins, ranges, want_values=False):
+        """p4: CUDA tensor [16][n].  Returns (hist int64 [5][n_bins], values CUDA [5][n] or None)."""
+        assert p4.is_cuda and p4.dim() == 2 and p4.shape[0] == 16 and p4.stride(1) == 1
+        n, ld = p4.shape[1], (p4.stride(0) if p4.shape[1] > 1 else max(1, p4.shape[1]))
+        self._torch.cuda.current_stream(self.device).synchronize()
+        rng = np.ascontiguousarray(ranges, dtype=np.float64)
+        hist = np.zeros((5, n_bins), dtype=np.int64)
+        values = self.empty(5, max(1, n)) if want_values else None
+        self._check(self.lib.tddp4_project(self._h, n, ld, _ptr(p4), n_bins, rng.ctypes.data, hist.ctypes.data, _ptr(values)))
+        return hist, (values[:, :n] if want_values else None)
 
     # -- inspection -------------------------------------------------------------------------------
     def layout(self):

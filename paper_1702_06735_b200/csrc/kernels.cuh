@@ -67,6 +67,60 @@ __global__ void __launch_bounds__(256) row_gather_kernel(const double *__restric
 }
 
 // ------------------------------------------------------------------------------------------------
+// Validation observables of the paper's Fig. 3: m12, m34, cos12, cos34, phi with 12 = (pi+ pi-) =
+// particles (2,3) and 34 = (K+ pi-) = (0,1).  Frame-independent forms, no boosts: with P the pair, a its
+// first daughter, S the other pair,  cos = -[(a.P)(S.P)/P^2 - a.S] / sqrt{[(a.P)^2/P^2 - a^2] [(S.P)^2/P^2 - S^2]};
+// with a = p2, b = p0 projected orthogonally to the plane spanned by D = P12 + P34 and P12 (Gram form),
+// cos phi = a_perp.b_perp / sqrt(a_perp^2 b_perp^2),  sin phi = -eps4(D, P12, a, b) / sqrt{[(D.P12)^2 - D^2 P12^2] a_perp^2 b_perp^2}.
+// One thread per event; integer histogram counts (exact, order-independent) through shared-memory atomics.
+constexpr int PROJ_BLOCK = 256, PROJ_MAX_BINS = 512;
+struct ProjRanges { double lo[5], inv_width[5], hi[5]; };
+__device__ __forceinline__ double helicity_cos(V4 a, V4 P, V4 S, double sP, double sS) {
+  double aP = dot(a, P), SP = dot(S, P);
+  double num = aP * SP / sP - dot(a, S);
+  double ka2 = aP * aP / sP - dot(a, a), ks2 = SP * SP / sP - sS;
+  return -num / sqrt(ka2 * ks2);
+}
+__global__ void __launch_bounds__(PROJ_BLOCK)
+project_kernel(const double *__restrict__ p4, int64_t ld, int64_t n, int n_bins, const __grid_constant__ ProjRanges R,
+               unsigned long long *__restrict__ hist /* [5][n_bins] */, double *__restrict__ values /* [5][n] or NULL */) {
+  __shared__ unsigned int s_h[5 * PROJ_MAX_BINS];
+  for (int k = threadIdx.x; k < 5 * n_bins; k += PROJ_BLOCK) s_h[k] = 0u;
+  __syncthreads();
+  const int64_t stride = (int64_t)gridDim.x * PROJ_BLOCK;
+  for (int64_t i = (int64_t)blockIdx.x * PROJ_BLOCK + threadIdx.x; i < n; i += stride) {
+    V4 p[4];
+#pragma unroll
+    for (int a = 0; a < 4; ++a) p[a] = {p4[(4 * a) * ld + i], p4[(4 * a + 1) * ld + i], p4[(4 * a + 2) * ld + i], p4[(4 * a + 3) * ld + i]};
+    const V4 P12 = p[2] + p[3], P34 = p[0] + p[1], D = P12 + P34;
+    const double s12 = dot(P12, P12), s34 = dot(P34, P34), sD = dot(D, D), DP = dot(D, P12);
+    double v[5];
+    v[0] = sqrt(s12);
+    v[1] = sqrt(s34);
+    v[2] = helicity_cos(p[2], P12, P34, s12, s34);
+    v[3] = helicity_cos(p[0], P34, P12, s34, s12);
+    const double den = sD * s12 - DP * DP;                       // < 0: -(M_D |P12 vec|)^2 in the D rest frame
+    auto perp = [&](V4 a, V4 b) {
+      double aD = dot(a, D), bD = dot(b, D), aP = dot(a, P12), bP = dot(b, P12);
+      return dot(a, b) - (aD * bD * s12 - aD * bP * DP - aP * bD * DP + aP * bP * sD) / den;
+    };
+    const double aa = perp(p[2], p[2]), bb = perp(p[0], p[0]), ab = perp(p[2], p[0]);
+    const double nrm = sqrt(aa * bb);
+    v[4] = atan2(-eps4(D, P12, p[2], p[0]) / (sqrt(-den) * nrm), ab / nrm);
+#pragma unroll
+    for (int k = 0; k < 5; ++k) {
+      if (values) values[(int64_t)k * n + i] = v[k];
+      int b = (int)floor((v[k] - R.lo[k]) * R.inv_width[k] * n_bins);
+      if (v[k] == R.hi[k]) b = n_bins - 1;
+      if (b >= 0 && b < n_bins) atomicAdd(&s_h[k * n_bins + b], 1u);
+    }
+  }
+  __syncthreads();
+  for (int k = threadIdx.x; k < 5 * n_bins; k += PROJ_BLOCK)
+    if (s_h[k]) atomicAdd(&hist[k], (unsigned long long)s_h[k]);
+}
+
+// ------------------------------------------------------------------------------------------------
 // Sum of the ranks' Gram sums in rank order (event-sharded evaluation): gathered [world][len]
 __global__ void __launch_bounds__(256) gram_reduce_kernel(const double *__restrict__ gathered, int world, int stride, int len,
                                                          double *__restrict__ G) {

@@ -1233,6 +1233,33 @@ int tddp4_weight_bound(const tddp4 *h, double *bound_out) {
   return TDDP4_OK;
 }
 
+// ---- validation projections ----------------------------------------------------------------------------
+int tddp4_project(tddp4 *h, int64_t n, int64_t ld, const double *p4, int n_bins, const double *ranges, int64_t *hist_out,
+                  double *values_dev) {
+  if (!h || n < 0 || ld < n || (n > 0 && !p4) || n_bins < 1 || n_bins > PROJ_MAX_BINS || !ranges || !hist_out)
+    return fail(h, TDDP4_ERR_ARG, "bad tddp4_project argument");
+  ProjRanges R;
+  for (int k = 0; k < 5; ++k) {
+    if (!(ranges[2 * k + 1] > ranges[2 * k])) return fail(h, TDDP4_ERR_ARG, "empty histogram range %d", k);
+    R.lo[k] = ranges[2 * k]; R.hi[k] = ranges[2 * k + 1]; R.inv_width[k] = 1.0 / (ranges[2 * k + 1] - ranges[2 * k]);
+  }
+  unsigned long long *hist = nullptr;
+  CU(cudaMalloc(&hist, sizeof(unsigned long long) * 5 * n_bins));
+  CU(cudaMemsetAsync(hist, 0, sizeof(unsigned long long) * 5 * n_bins, h->stream));
+  if (n > 0) {
+    int grid = (int)std::min<int64_t>((n + PROJ_BLOCK - 1) / PROJ_BLOCK, (int64_t)h->sm_count * 8);
+    project_kernel<<<grid, PROJ_BLOCK, 0, h->stream>>>(p4, ld, n, n_bins, R, hist, values_dev);
+    ++h->launches;
+  }
+  cudaError_t e1 = cudaGetLastError();
+  cudaError_t e2 = cudaMemcpyAsync(hist_out, hist, sizeof(unsigned long long) * 5 * n_bins, cudaMemcpyDeviceToHost, h->stream);
+  cudaError_t e3 = cudaStreamSynchronize(h->stream);
+  cudaFree(hist);
+  h->prev_kind = PREV_NONE;
+  CU(e1); CU(e2); CU(e3);
+  return TDDP4_OK;
+}
+
 // ---- inspection ---------------------------------------------------------------------------------------
 int tddp4_get(tddp4 *h, int which, int what, double *out) {
   if (!h || which < 0 || which > 1 || !out) return fail(h, TDDP4_ERR_ARG, "bad argument");

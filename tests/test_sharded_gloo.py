@@ -29,6 +29,12 @@ class OracleEvaluator:
     def set_params(self, par):
         self.par = par
 
+    def load_events(self, which, p4, t=None):
+        if which == 0:
+            self.p4, self.t, self.n_data = p4, t, p4.shape[1]
+        else:
+            self.p4n = p4
+
     def _columns(self, p4):
         if p4.shape[1] == 0:
             return np.zeros((self.mdl.n_couplings, 0), complex)
@@ -94,7 +100,13 @@ def _worker(rank, world, port, n_data, n_norm, out):
         p3 = p2.copy(); p3.mass[0] *= 1.001                      # mass step: Gram exchange
         sh.set_params(p3)
         vals.append(sh.nll())
-        out[rank] = (vals, ev.gram_calls, sh.exchanges)
+        counts = (ev.gram_calls, sh.exchanges)
+        # a reloaded normalisation shard with unchanged masses/widths must trigger a new exchange
+        half = (hn - ln) // 2
+        sh.load_events(1, p4n[:, ln:ln + half].copy())
+        sh.set_params(p3)
+        vals.append(sh.nll())
+        out[rank] = (vals, counts[0], counts[1], ev.gram_calls, (ln, ln + half))
     finally:
         dist.destroy_process_group()
 
@@ -112,12 +124,16 @@ def test_world_size_2_matches_single_process(n_data, n_norm):
     p2 = par.copy(); p2.c[0] *= 1.01; p2.x *= 1.1
     p3 = p2.copy(); p3.mass[0] *= 1.001
     ref = [oracle.nll(mdl, p, p4, t, p4n, want_prob=False)[0] for p in (par, p2, p3)]
+    keep = np.concatenate([np.arange(*out[r][4]) for r in range(world)])      # the halved normalisation shards
+    if len(keep):
+        ref.append(oracle.nll(mdl, p3, p4, t, np.ascontiguousarray(p4n[:, keep]), want_prob=False)[0])
     assert out[0][0] == out[1][0]                                # same bits on both ranks
     for got, want in zip(out[0][0], ref):
         assert abs(got - want) <= 1e-11 * max(abs(want), 1.0)
     for r in range(world):
         assert out[r][1] == 2                                    # Gram rebuilt at the first call and at the mass step only
         assert out[r][2] == 2 + 3                                # 2 Gram exchanges + 3 scalar exchanges
+        assert out[r][3] == 3                                    # ... and once more after the reload
 
 
 def test_shard_ranges_partition_the_events():
