@@ -38,7 +38,7 @@ class _Model(C.Structure):
                 ("n_res", C.c_int), ("res_L", C.c_int * MAX_RES), ("n_terms", C.c_int),
                 ("term_sf", C.c_int * MAX_TERMS), ("term_res", (C.c_int * 2) * MAX_TERMS),
                 ("term_perm", (C.c_int * 4) * MAX_TERMS), ("term_coupling", C.c_int * MAX_TERMS),
-                ("n_couplings", C.c_int)]
+                ("n_couplings", C.c_int), ("res_r", C.c_double * MAX_RES), ("res_kind", C.c_int * MAX_RES)]
 
 
 class _Params(C.Structure):
@@ -104,6 +104,10 @@ def c_model(mdl) -> _Model:
     m.n_res = mdl.n_res
     for i, L in enumerate(mdl.res_L):
         m.res_L[i] = L
+    for i, r in enumerate(getattr(mdl, "res_r", []) or []):
+        m.res_r[i] = r
+    for i, k in enumerate(getattr(mdl, "res_lineshape", []) or []):
+        m.res_kind[i] = k
     m.n_terms = mdl.n_terms
     for k in range(mdl.n_terms):
         m.term_sf[k] = mdl.term_sf[k]
@@ -168,6 +172,12 @@ def breit_wigner(m0, gamma0, L, r, s, ma, mb, ma0=None, mb0=None):
                                 mb if mb0 is None else mb0, out)
     if st:
         raise ValueError("pole below threshold")
+    return complex(out[0], out[1])
+
+
+def breit_wigner_constant(m0, gamma0, s):
+    out = (C.c_double * 2)()
+    lib().orc_breit_wigner_constant(C.c_double(m0), C.c_double(gamma0), C.c_double(s), out)
     return complex(out[0], out[1])
 
 

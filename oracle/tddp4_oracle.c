@@ -41,7 +41,11 @@
 #define ORC_MAX_COUPLINGS 32
 
 /* spin-factor kinds, O-4 */
-enum { ORC_SF_NONRES = 0, ORC_SF_VV_S = 1, ORC_SF_VV_P = 2, ORC_SF_VV_D = 3, ORC_SF_AP_S = 4, ORC_SF_TP_D = 5 };
+enum { ORC_SF_NONRES = 0, ORC_SF_VV_S = 1, ORC_SF_VV_P = 2, ORC_SF_VV_D = 3, ORC_SF_AP_S = 4, ORC_SF_TP_D = 5,
+       ORC_SF_AP_D = 6 };
+/* lineshape kinds ("resonance lineshapes" is a class of building blocks; the paper names none) */
+enum { ORC_LS_RUNNING = 0,   /* O-6: relativistic Breit-Wigner with mass-dependent width          */
+       ORC_LS_CONSTANT = 1 };/* relativistic Breit-Wigner with constant width: 1/(m0^2 - s - i m0 Gamma0) */
 
 typedef struct {
   double m_parent;            /* nominal D0 mass (used by the generator only)           */
@@ -57,6 +61,9 @@ typedef struct {
   int term_perm[ORC_MAX_TERMS][4];   /* role r -> final-state index                      */
   int term_coupling[ORC_MAX_TERMS];  /* kappa(k): index of the coupling, O-2             */
   int n_couplings;
+  double res_r[ORC_MAX_RES];  /* Blatt-Weisskopf radius of this resonance's own decay vertex; 0: r_res (O-5:    */
+                              /* "per-resonance radii")                                     */
+  int res_kind[ORC_MAX_RES];  /* ORC_LS_*                                                                       */
 } orc_model;
 
 typedef struct {
@@ -236,6 +243,13 @@ double orc_spin_factor_event(int sf, const int perm[4], const double p[4][4]) {
       for (int nu = 0; nu < 4; ++nu) s += (G4[mu] * d[mu]) * P[mu][nu] * (G4[nu] * v[nu]);
     return -s;
   }
+  if (sf == ORC_SF_AP_D) {                                         /* d_mu L2^{mu nu}(pX,qX) v_nu: axial -> V P in D-wave */
+    double L2X[4][4], s = 0.0;
+    orc_L2(pX, qX, L2X);
+    for (int mu = 0; mu < 4; ++mu)
+      for (int nu = 0; nu < 4; ++nu) s += (G4[mu] * d[mu]) * L2X[mu][nu] * (G4[nu] * v[nu]);
+    return s;
+  }
   if (sf == ORC_SF_TP_D) {
     /* L2^{rho sg}(pD,qD) eps_{rho al be ga} L2(pX,qX)_sg^al pX^be v^ga */
     double L2D[4][4], L2T[4][4], s = 0.0;
@@ -280,12 +294,25 @@ int orc_breit_wigner(double m0, double gamma0, int L, double r, double s, double
   return 0;
 }
 
+/* Breit-Wigner with constant width (lineshape kind 1): T(s) = 1 / (m0^2 - s - i m0 Gamma0).  No threshold enters. */
+void orc_breit_wigner_constant(double m0, double gamma0, double s, double out[2]) {
+  double complex T = 1.0 / ((m0 * m0 - s) - I * (m0 * gamma0));
+  out[0] = creal(T); out[1] = cimag(T);
+}
+
 /* L of the D vertex for each spin-factor kind (O-5) */
 static int parent_L(int sf) {
   switch (sf) {
     case ORC_SF_VV_S: return 0; case ORC_SF_VV_P: return 1; case ORC_SF_VV_D: return 2;
-    case ORC_SF_AP_S: return 1; case ORC_SF_TP_D: return 2; default: return 0;
+    case ORC_SF_AP_S: return 1; case ORC_SF_TP_D: return 2; case ORC_SF_AP_D: return 1; default: return 0;
   }
+}
+/* radius of resonance R's own decay vertex, and its lineshape by kind */
+static double res_radius(const orc_model *m, int R) { return m->res_r[R] > 0.0 ? m->res_r[R] : m->r_res; }
+static int lineshape(const orc_model *m, const orc_params *par, int R, double s, double ma, double mb, double ma0,
+                     double mb0, double out[2]) {
+  if (m->res_kind[R] == ORC_LS_CONSTANT) { orc_breit_wigner_constant(par->mass[R], par->width[R], s, out); return 0; }
+  return orc_breit_wigner(par->mass[R], par->width[R], m->res_L[R], res_radius(m, R), s, ma, mb, ma0, mb0, out);
 }
 
 /* O-2: one decay-chain amplitude a_k = S_k F_{L_D}(z_D) prod_R [F_{L_R}(z_R) T_R]. */
@@ -314,11 +341,11 @@ int orc_term_event(const orc_model *m, const orc_params *par, int k, const doubl
       double qD = orc_breakup(mD, sqrt(s1), sqrt(s2));
       double q1 = orc_breakup(sqrt(s1), ma, mb), q2 = orc_breakup(sqrt(s2), mc, md);
       F *= orc_barrier(parent_L(sf), (qD * m->r_parent) * (qD * m->r_parent));
-      F *= orc_barrier(m->res_L[R0], (q1 * m->r_res) * (q1 * m->r_res));
-      F *= orc_barrier(m->res_L[R1], (q2 * m->r_res) * (q2 * m->r_res));
-      status |= orc_breit_wigner(par->mass[R0], par->width[R0], m->res_L[R0], m->r_res, s1, ma, mb, ma, mb, bw);
+      F *= orc_barrier(m->res_L[R0], (q1 * res_radius(m, R0)) * (q1 * res_radius(m, R0)));
+      F *= orc_barrier(m->res_L[R1], (q2 * res_radius(m, R1)) * (q2 * res_radius(m, R1)));
+      status |= lineshape(m, par, R0, s1, ma, mb, ma, mb, bw);
       T *= bw[0] + I * bw[1];
-      status |= orc_breit_wigner(par->mass[R1], par->width[R1], m->res_L[R1], m->r_res, s2, mc, md, mc, md, bw);
+      status |= lineshape(m, par, R1, s2, mc, md, mc, md, bw);
       T *= bw[0] + I * bw[1];
     } else {
       double pV[4], pX[4];
@@ -330,13 +357,12 @@ int orc_term_event(const orc_model *m, const orc_params *par, int k, const doubl
       double qX = orc_breakup(sqrt(sX), sqrt(sV), mc);
       double qV = orc_breakup(sqrt(sV), ma, mb);
       F *= orc_barrier(parent_L(sf), (qD * m->r_parent) * (qD * m->r_parent));
-      F *= orc_barrier(m->res_L[R0], (qX * m->r_res) * (qX * m->r_res));
-      F *= orc_barrier(m->res_L[R1], (qV * m->r_res) * (qV * m->r_res));
+      F *= orc_barrier(m->res_L[R0], (qX * res_radius(m, R0)) * (qX * res_radius(m, R0)));
+      F *= orc_barrier(m->res_L[R1], (qV * res_radius(m, R1)) * (qV * res_radius(m, R1)));
       /* X -> V c: running daughter mass at s, the daughter's current m0 at the pole (O-6) */
-      status |= orc_breit_wigner(par->mass[R0], par->width[R0], m->res_L[R0], m->r_res, sX, sqrt(sV), mc,
-                                 par->mass[R1], mc, bw);
+      status |= lineshape(m, par, R0, sX, sqrt(sV), mc, par->mass[R1], mc, bw);
       T *= bw[0] + I * bw[1];
-      status |= orc_breit_wigner(par->mass[R1], par->width[R1], m->res_L[R1], m->r_res, sV, ma, mb, ma, mb, bw);
+      status |= lineshape(m, par, R1, sV, ma, mb, ma, mb, bw);
       T *= bw[0] + I * bw[1];
     }
   }

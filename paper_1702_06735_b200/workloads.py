@@ -20,7 +20,9 @@ from dataclasses import dataclass, field
 import numpy as np
 
 # spin-factor kinds (O-4).  Plain labels; each side maps them onto its own enum.
-SF_NONRES, SF_VV_S, SF_VV_P, SF_VV_D, SF_AP_S, SF_TP_D = range(6)
+SF_NONRES, SF_VV_S, SF_VV_P, SF_VV_D, SF_AP_S, SF_TP_D, SF_AP_D = range(7)
+# lineshape kinds: 0 relativistic Breit-Wigner with mass-dependent width (O-6), 1 with constant width
+LS_RUNNING, LS_CONSTANT = 0, 1
 
 # final-state order 0 = K+, 1 = pi-, 2 = pi+, 3 = pi- (O-3); masses from BJ:configs[0]
 M_D0 = 1.86484
@@ -42,6 +44,7 @@ RESONANCES = {
     "K1(1270)": (1.272, 0.09, 0),
     "K2*(1430)": (1.4324, 0.109, 2),
     "K1(1400)": (1.403, 0.174, 0),
+    "K1(1400)[D]": (1.403, 0.174, 2),      # the same state decaying to K* pi in D-wave (its own entry: L is per entry)
 }
 
 # decay chains, ordering A (O-7): (spin factor, (res0, res1), perm).  perm maps role -> particle:
@@ -56,6 +59,7 @@ CHAINS = {
     6: (SF_VV_P, ("K*(892)0", "rho(770)0"), (0, 1, 2, 3)),
     7: (SF_VV_D, ("K*(892)0", "rho(770)0"), (0, 1, 2, 3)),
     8: (SF_NONRES, (None, None), (0, 1, 2, 3)),
+    9: (SF_AP_D, ("K1(1400)[D]", "K*(892)0"), (0, 1, 2, 3)),       # further building block, in no config
 }
 
 
@@ -73,6 +77,8 @@ class Model:
     res_L: list = field(default_factory=list)
     res_mass: list = field(default_factory=list)    # nominal m0 (initial parameter values)
     res_width: list = field(default_factory=list)   # nominal Gamma0
+    res_r: list = field(default_factory=list)       # per-resonance Blatt-Weisskopf radius, 0 = r_res
+    res_lineshape: list = field(default_factory=list)   # LS_* per resonance
     term_sf: list = field(default_factory=list)
     term_res: list = field(default_factory=list)    # [(r0, r1)] indices, -1 = none
     term_perm: list = field(default_factory=list)
@@ -109,6 +115,8 @@ def build_model(chain_ids, bose=False, **kw) -> Model:
                 mdl.res_L.append(L)
                 mdl.res_mass.append(m0)
                 mdl.res_width.append(g0)
+                mdl.res_r.append(0.0)
+                mdl.res_lineshape.append(LS_RUNNING)
             idx.append(mdl.res_names.index(nm))
         kappa = mdl.n_couplings
         mdl.n_couplings += 1

@@ -76,6 +76,8 @@ def closed_spin_factor(sf, perm, p):
     if sf == 5:
         mD2 = dot(pD, pD)
         return dot(d, t) * eps4(d, t, pX, v) + dot(d, d) / 3.0 * dot(pD, t) / mD2 * eps4(pD, t, pX, v)
+    if sf == 6:     # d_mu L2^{mu nu}(pX, qX) v_nu = (d.t)(t.v) - (t.t)/3 [d.v - (pX.d)(pX.v)/sX]
+        return dot(d, t) * dot(t, v) - dot(t, t) / 3.0 * (dot(d, v) - dot(pX, d) * dot(pX, v) / dot(pX, pX))
     raise ValueError(sf)
 
 

@@ -49,7 +49,20 @@ def bw(m0, g0, L, r, s, sa, sb, sa0, sb0):
     return 1 / mp.mpc(m0 * m0 - s, -m0 * gam)
 
 
-LD = {0: 0, 1: 0, 2: 1, 3: 2, 4: 1, 5: 2}
+LD = {0: 0, 1: 0, 2: 1, 3: 2, 4: 1, 5: 2, 6: 1}
+
+
+def radius(mdl, R):
+    r = (getattr(mdl, "res_r", None) or [0.0] * mdl.n_res)[R]
+    return mp.mpf(r if r > 0 else mdl.r_res)
+
+
+def lineshape(mdl, R, m0, g0, s, sa, sb, sa0, sb0):
+    """Kind 0: running-width Breit-Wigner with the resonance's own radius; kind 1: constant width."""
+    kind = (getattr(mdl, "res_lineshape", None) or [0] * mdl.n_res)[R]
+    if kind == 1:
+        return 1 / mp.mpc(m0[R] * m0[R] - s, -m0[R] * g0[R])
+    return bw(m0[R], g0[R], mdl.res_L[R], radius(mdl, R), s, sa, sb, sa0, sb0)
 
 
 def term(mdl, par, k, p):
@@ -61,7 +74,8 @@ def term(mdl, par, k, p):
     R0, R1 = mdl.term_res[k]
     m0 = [mp.mpf(float(v)) for v in par.mass]
     g0 = [mp.mpf(float(v)) for v in par.width]
-    rr, rp = mp.mpf(mdl.r_res), mp.mpf(mdl.r_parent)
+    rp = mp.mpf(mdl.r_parent)
+    r0, r1 = radius(mdl, R0), radius(mdl, R1)
     if sf in (W.SF_VV_S, W.SF_VV_P, W.SF_VV_D):
         p1, q1, p2, q2 = madd(r[0], r[1]), msub(r[0], r[1]), madd(r[2], r[3]), msub(r[2], r[3])
         pD, qD = madd(p1, p2), msub(p1, p2)
@@ -73,10 +87,10 @@ def term(mdl, par, k, p):
             S = meps(pD, qD, v1, v2)
         else:
             S = mdot(d, v1) * mdot(d, v2) - mdot(d, d) / 3 * (mdot(v1, v2) - mdot(pD, v1) * mdot(pD, v2) / sD)
-        Fp = (F(LD[sf], (kallen_q(sD, s1, s2) * rp) ** 2) * F(mdl.res_L[R0], (kallen_q(s1, mf2[0], mf2[1]) * rr) ** 2)
-              * F(mdl.res_L[R1], (kallen_q(s2, mf2[2], mf2[3]) * rr) ** 2))
-        T = (bw(m0[R0], g0[R0], mdl.res_L[R0], rr, s1, mf2[0], mf2[1], mf2[0], mf2[1])
-             * bw(m0[R1], g0[R1], mdl.res_L[R1], rr, s2, mf2[2], mf2[3], mf2[2], mf2[3]))
+        Fp = (F(LD[sf], (kallen_q(sD, s1, s2) * rp) ** 2) * F(mdl.res_L[R0], (kallen_q(s1, mf2[0], mf2[1]) * r0) ** 2)
+              * F(mdl.res_L[R1], (kallen_q(s2, mf2[2], mf2[3]) * r1) ** 2))
+        T = (lineshape(mdl, R0, m0, g0, s1, mf2[0], mf2[1], mf2[0], mf2[1])
+             * lineshape(mdl, R1, m0, g0, s2, mf2[2], mf2[3], mf2[2], mf2[3]))
         return S * Fp * T
     pV, qV = madd(r[0], r[1]), msub(r[0], r[1])
     pX, qX = madd(pV, r[2]), msub(pV, r[2])
@@ -85,12 +99,14 @@ def term(mdl, par, k, p):
     sV, sX, sD = mdot(pV, pV), mdot(pX, pX), mdot(pD, pD)
     if sf == W.SF_AP_S:
         S = -(mdot(d, v) - mdot(pX, d) * mdot(pX, v) / sX)
+    elif sf == W.SF_AP_D:
+        S = mdot(d, t) * mdot(t, v) - mdot(t, t) / 3 * (mdot(d, v) - mdot(pX, d) * mdot(pX, v) / sX)
     else:
         S = mdot(d, t) * meps(d, t, pX, v) + mdot(d, d) / 3 * mdot(pD, t) / sD * meps(pD, t, pX, v)
-    Fp = (F(LD[sf], (kallen_q(sD, sX, mf2[3]) * rp) ** 2) * F(mdl.res_L[R0], (kallen_q(sX, sV, mf2[2]) * rr) ** 2)
-          * F(mdl.res_L[R1], (kallen_q(sV, mf2[0], mf2[1]) * rr) ** 2))
-    T = (bw(m0[R0], g0[R0], mdl.res_L[R0], rr, sX, sV, mf2[2], m0[R1] ** 2, mf2[2])
-         * bw(m0[R1], g0[R1], mdl.res_L[R1], rr, sV, mf2[0], mf2[1], mf2[0], mf2[1]))
+    Fp = (F(LD[sf], (kallen_q(sD, sX, mf2[3]) * rp) ** 2) * F(mdl.res_L[R0], (kallen_q(sX, sV, mf2[2]) * r0) ** 2)
+          * F(mdl.res_L[R1], (kallen_q(sV, mf2[0], mf2[1]) * r1) ** 2))
+    T = (lineshape(mdl, R0, m0, g0, sX, sV, mf2[2], m0[R1] ** 2, mf2[2])
+         * lineshape(mdl, R1, m0, g0, sV, mf2[0], mf2[1], mf2[0], mf2[1]))
     return S * Fp * T
 
 
@@ -146,6 +162,38 @@ def test_ten_event_brute_force(cfg):
     for po, pb in zip(P_o, P_b):
         assert float(abs(po - pb) / pb) < 1e-11
     assert float(abs(nll_o - nll_b)) < 1e-11 * max(1.0, float(abs(nll_b)))
+
+
+def blocks_model():
+    """Every further building block of SURVEY.md 8(f) NEXT-2 in one model: the axial D-wave cascade (chain 9), a
+    constant-width lineshape, resonance radii different from the model's."""
+    mdl = W.build_model([1, 3, 9, 2], bose=True)
+    mdl.res_r[mdl.res_names.index("K*(892)0")] = 3.0
+    mdl.res_r[mdl.res_names.index("K1(1400)[D]")] = 2.2
+    mdl.res_lineshape[mdl.res_names.index("a1(1260)")] = W.LS_CONSTANT
+    return mdl
+
+
+def test_ten_event_brute_force_further_building_blocks():
+    mdl = blocks_model()
+    par = W.initial_params(mdl)
+    par.x, par.y = 0.31, 0.12
+    p4, t, w, _ = oracle.candidates(mdl, par.tau, 4321, 0, 0, 35)
+    data, td = p4[:, :10].copy(), t[:10] * 3.0
+    nrm, wn = p4[:, 10:].copy(), w[10:] * 30.0
+    nll_o, N_o, P_o, st = oracle.nll(mdl, par, data, td, nrm, wn)
+    assert st == 0
+    nll_b, N_b, P_b = brute_nll(mdl, par, data, td, nrm, wn)
+    assert float(abs(N_o - N_b) / N_b) < 1e-12
+    for po, pb in zip(P_o, P_b):
+        assert float(abs(po - pb) / pb) < 1e-11
+    assert float(abs(nll_o - nll_b)) < 1e-11 * max(1.0, float(abs(nll_b)))
+    S, Fb, a = oracle.terms(mdl, par, data)
+    for i in range(5):
+        p = [[mp.mpf(float(data[4 * b + c, i])) for c in range(4)] for b in range(4)]
+        for k in range(mdl.n_terms):
+            ref = complex(term(mdl, par, k, p))
+            assert abs(a[k, i] - ref) <= 1e-11 * abs(ref)
 
 
 def test_brute_force_per_term():

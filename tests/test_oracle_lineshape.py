@@ -86,3 +86,50 @@ def test_breakup_momentum():
     assert oracle.breakup(2.0, 0.3, 0.7) == pytest.approx(
         math.sqrt((4 - 1.0) * (4 - 0.16)) / 4, rel=4e-16)             # sqrt(lambda(M^2,a^2,b^2)) / 2M
     assert oracle.breakup(2.0, 0.3, 0.7) == pytest.approx(oracle.breakup(2.0, 0.7, 0.3), rel=1e-15)
+
+
+def test_constant_width_breit_wigner():
+    """Lineshape kind 1 ("further lineshapes"): T = 1 / (m0^2 - s - i m0 Gamma0).  Pole value
+    i / (m0 Gamma0); |T|^2 is a Lorentzian in s with half maximum exactly at s = m0^2 +- m0 Gamma0; the phase goes
+    through 90 degrees at the pole and T(s) -> -1/s far above it; it equals the running-width form where Gamma(s) = Gamma0."""
+    m0, g0 = 1.403, 0.174
+    T0 = oracle.breit_wigner_constant(m0, g0, m0 * m0)
+    assert abs(T0.real) < 1e-15 and T0.imag == pytest.approx(1.0 / (m0 * g0), rel=1e-15)
+    for sgn in (1.0, -1.0):
+        T = oracle.breit_wigner_constant(m0, g0, m0 * m0 + sgn * m0 * g0)
+        assert abs(T) ** 2 == pytest.approx(0.5 * abs(T0) ** 2, rel=1e-14)
+        assert math.degrees(math.atan2(T.imag, T.real)) == pytest.approx(90.0 + sgn * 45.0, abs=1e-10)   # the phase rises through 90 degrees
+    assert oracle.breit_wigner_constant(m0, g0, 1e6) == pytest.approx(-1e-6, rel=1e-5)
+    assert oracle.breit_wigner_constant(m0, g0, m0 * m0) == pytest.approx(
+        oracle.breit_wigner(m0, g0, 0, 1.5, m0 * m0, 0.8955, MPI), rel=1e-14)
+
+
+def test_per_resonance_radius_and_lineshape_kind_reach_the_term_amplitude():
+    """The radius of a resonance enters its own barrier factor and its running width, nothing else; a constant-width
+    entry replaces only that resonance's lineshape.  Checked on whole term amplitudes against products rebuilt here from
+    the scalar building blocks (breakup momenta from the event's invariant masses)."""
+    import samples
+    from helpers import dot, event
+    p4, _ = samples.flat_sample(40)
+    base = W.build_model([1, 3])                       # K* rho (VV S-wave) and K1(1270) -> K* pi
+    par = W.initial_params(base)
+    iK, iR, iK1 = (base.res_names.index(n) for n in ("K*(892)0", "rho(770)0", "K1(1270)"))
+    S0, F0, a0 = oracle.terms(base, par, p4)
+    mod = W.build_model([1, 3])
+    mod.res_r[iK] = 3.0                                # K* vertex radius 3 GeV^-1, everything else 1.5
+    mod.res_lineshape[iK1] = W.LS_CONSTANT
+    S1, F1, a1 = oracle.terms(mod, par, p4)
+    assert np.array_equal(S0, S1)                      # spin factors do not know about radii or lineshapes
+    for i in range(p4.shape[1]):
+        ev = event(p4, i)
+        sK = dot(ev[0] + ev[1], ev[0] + ev[1]); sR = dot(ev[2] + ev[3], ev[2] + ev[3])
+        sX = dot(ev[0] + ev[1] + ev[2], ev[0] + ev[1] + ev[2])
+        qK = breakup(math.sqrt(sK), MK, MPI)
+        ratio = oracle.barrier(1, (qK * 3.0) ** 2) / oracle.barrier(1, (qK * 1.5) ** 2)
+        for k in (0, 1):                               # both chains contain the K* vertex
+            assert F1[k, i] == pytest.approx(F0[k, i] * ratio, rel=1e-13)
+        TK3 = oracle.breit_wigner(par.mass[iK], par.width[iK], 1, 3.0, sK, MK, MPI)
+        TR = oracle.breit_wigner(par.mass[iR], par.width[iR], 1, 1.5, sR, MPI, MPI)
+        assert a1[0, i] == pytest.approx(S1[0, i] * F1[0, i] * TK3 * TR, rel=1e-12)
+        TK1c = oracle.breit_wigner_constant(par.mass[iK1], par.width[iK1], sX)
+        assert a1[1, i] == pytest.approx(S1[1, i] * F1[1, i] * TK1c * TK3, rel=1e-12)

@@ -11,7 +11,7 @@ from paper_1702_06735_b200 import workloads as W
 from helpers import (L1, boost_matrix, boost_to_rest, breakup, closed_spin_factor, dot, eps4, event, rotation)
 
 PERMS = [(0, 1, 2, 3), (2, 3, 1, 0), (0, 3, 2, 1), (2, 1, 3, 0), (3, 0, 1, 2)]
-KINDS = [1, 2, 3, 4, 5]
+KINDS = [1, 2, 3, 4, 5, 6]
 
 
 @pytest.fixture(scope="module")
@@ -43,7 +43,7 @@ def test_lorentz_invariance(events, sf):
             assert oracle.spin_factor(sf, PERMS[0], q) == pytest.approx(ref, rel=1e-9, abs=1e-12)
 
 
-@pytest.mark.parametrize("sf,odd", [(1, False), (2, True), (3, False), (4, False), (5, True)])
+@pytest.mark.parametrize("sf,odd", [(1, False), (2, True), (3, False), (4, False), (5, True), (6, False)])
 def test_parity(events, sf, odd):
     flip = np.diag([1.0, -1.0, -1.0, -1.0])
     for p in events[:16]:
@@ -107,6 +107,25 @@ def test_rest_frame_reduction_tensor(events):
             pstar = breakup(math.sqrt(mD2), math.sqrt(sX), math.sqrt(dot(r[3], r[3])))
             ref = -math.sqrt(sX) * (kappa ** 2 - 4 * pstar ** 2 / (3 * mD2)) * (p1 @ t) * (p1 @ np.cross(t, v))
             assert oracle.spin_factor(5, perm, p) == pytest.approx(ref, rel=1e-9, abs=1e-13)
+
+
+def test_rest_frame_reduction_axial_d_wave(events):
+    """S_{AP-D} (axial -> V P in D-wave) in the rest frame of X: the l = 2 tensor of the X decay
+    momentum contracted with the bachelor direction and the V polarisation,
+    S = -kappa [ (p.t)(t.v) - |t|^2 (p.v) / 3 ], same kappa as the S-wave reduction, all 3-vectors by explicit boosts."""
+    for p in events[:24]:
+        for perm in PERMS[:4]:
+            r = [p[perm[i]] for i in range(4)]
+            pV, qV = r[0] + r[1], r[0] - r[1]
+            pX, qX = pV + r[2], pV - r[2]
+            pD = pX + r[3]
+            B = boost_to_rest(pX)
+            v = (B @ L1(pV, qV))[1:]
+            t = (B @ L1(pX, qX))[1:]
+            p1 = (B @ r[3])[1:]
+            kappa = (dot(pD, pD) + dot(pX, pX) - dot(r[3], r[3])) / dot(pD, pD)
+            ref = -kappa * ((p1 @ t) * (t @ v) - (t @ t) * (p1 @ v) / 3.0)
+            assert oracle.spin_factor(6, perm, p) == pytest.approx(ref, rel=1e-9, abs=1e-13)
 
 
 def test_vv_s_wave_in_rest_frames(events):
