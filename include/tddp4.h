@@ -57,12 +57,21 @@ typedef enum {
  *   NONRES : constant amplitude 1;                                           res = {-1, -1}          */
 enum {
   TDDP4_SF_NONRES = 0, TDDP4_SF_VV_S = 1, TDDP4_SF_VV_P = 2, TDDP4_SF_VV_D = 3,
-  TDDP4_SF_AP_S = 4, TDDP4_SF_TP_D = 5
+  TDDP4_SF_AP_S = 4, TDDP4_SF_TP_D = 5,
+  TDDP4_SF_AP_D = 6   /* the AP_S cascade with X -> V perm[2] in D-wave: d_mu L2^{mu nu}(p_X, q_X) v_nu (the resonance
+                       * entry of X then has L = 2); further building block in the sense of PAPER.md line 51          */
 };
+/* Lineshape kinds ("resonance lineshapes" are a class of building blocks; the paper names none):
+ * 0 relativistic Breit-Wigner with mass-dependent width and Blatt-Weisskopf ratio (O-6);
+ * 1 relativistic Breit-Wigner with constant width, T = 1 / (m0^2 - s - i m0 Gamma0).                               */
+enum { TDDP4_LS_RUNNING = 0, TDDP4_LS_CONSTANT = 1 };
 
 typedef struct {
-  int L; /* orbital angular momentum of the resonance's own decay: exponent 2L+1 of the running width
-            and order of its Blatt-Weisskopf factor (O-5, O-6).  m0, Gamma0 come via tddp4_set_params. */
+  int L;         /* orbital angular momentum of the resonance's own decay: exponent 2L+1 of the running width
+                    and order of its Blatt-Weisskopf factor (O-5, O-6).  m0, Gamma0 come via tddp4_set_params.
+                    A state that decays in two partial waves is listed twice (one entry per L).              */
+  int lineshape; /* TDDP4_LS_*                                                                                 */
+  double r;      /* Blatt-Weisskopf radius of this resonance's own vertex, GeV^-1; 0: the model's r_res        */
 } tddp4_res;
 
 typedef struct {

@@ -36,7 +36,7 @@ class Tddp4Error(RuntimeError):
 
 
 class _Res(C.Structure):
-    _fields_ = [("L", C.c_int)]
+    _fields_ = [("L", C.c_int), ("lineshape", C.c_int), ("r", C.c_double)]
 
 
 class _Term(C.Structure):
@@ -128,8 +128,10 @@ class Tddp4:
         self.model = model
         self.n_res, self.n_terms, self.kc = model.n_res, model.n_terms, model.n_couplings
         res = (_Res * max(1, model.n_res))()
+        radii = getattr(model, "res_r", None) or [0.0] * model.n_res
+        kinds = getattr(model, "res_lineshape", None) or [0] * model.n_res
         for r, L in enumerate(model.res_L):
-            res[r].L = L
+            res[r].L, res[r].lineshape, res[r].r = L, kinds[r], radii[r]
         terms = (_Term * model.n_terms)()
         for k in range(model.n_terms):
             terms[k].spin_factor = model.term_sf[k]

@@ -81,6 +81,8 @@ __device__ __forceinline__ double spin_factor(int sf, V4 r0, V4 r1, V4 r2, V4 r3
   V4 d = L1(pD, qD, sD);
   if (sf == SF_AP_S) return -(dot(d, v) - dot(pX, d) * dot(pX, v) / sX);
   V4 t = L1(pX, qX, sX);
+  // axial -> V P in D-wave: d_mu L2^{mu nu}(pX, qX) v_nu
+  if (sf == SF_AP_D) return dot(d, t) * dot(t, v) - dot(t, t) * (1.0 / 3.0) * (dot(d, v) - dot(pX, d) * dot(pX, v) / sX);
   return dot(d, t) * eps4(d, t, pX, v) + dot(d, d) * (1.0 / 3.0) * (dot(pD, t) / sD) * eps4(pD, t, pX, v);
 }
 
@@ -119,7 +121,7 @@ __device__ __forceinline__ void kinematics(const ModelTab &M, const Scratch &sc,
     double ma = in.sub >= 0 ? sqrt(sc.S(in.sub, tid)) : in.ma;
     double q2 = breakup2(Mr, s, ma, in.mb);
     sc.Q(i, tid) = q2;
-    sink.g(i, width_shape(in.L, q2, q2 * M.r_res2, Mr));
+    sink.g(i, in.kind == LS_CONSTANT ? 1.0 : width_shape(in.L, q2, q2 * in.r2, Mr));
   }
   double sD = sc.S(M.sysD, tid);
   double mD = sqrt(sD);
@@ -136,8 +138,8 @@ __device__ __forceinline__ void kinematics(const ModelTab &M, const Scratch &sc,
       double m2 = tm.sf <= SF_VV_D ? sqrt(sc.S(i1.sys, tid)) : M.m_final[tm.perm[3]];
       double qD2 = breakup2(mD, sD, m1, m2);
       f *= barrier(tm.LD, qD2 * M.r_parent2);
-      f *= barrier(i0.L, sc.Q(tm.inst0, tid) * M.r_res2);
-      f *= barrier(i1.L, sc.Q(tm.inst1, tid) * M.r_res2);
+      f *= barrier(i0.L, sc.Q(tm.inst0, tid) * i0.r2);
+      f *= barrier(i1.L, sc.Q(tm.inst1, tid) * i1.r2);
     }
     sink.f(k, f);
   }

@@ -31,8 +31,8 @@ constexpr int GRAD_OFFSET = 8;
 
 // shared-memory tiles of one warp: X [32][gram_stride(NB)] (event-major, as the Gram kernel), W [32][GRAD_WS] (rows 4..7 zero)
 constexpr int GRAD_WS = 10;
-// resident blocks per SM (the kernel is latency-bound on its 9 loads per event: 24 warps per SM where the registers allow it)
-template <int KC> __host__ __device__ constexpr int grad_bps() { return KC <= 8 ? 3 : 2; }
+// resident blocks per SM
+template <int KC> __host__ __device__ constexpr int grad_bps() { return 2; }
 template <int KC> __host__ __device__ constexpr int grad_nb() { return (KC + 3) / 4; }
 template <int KC> __host__ __device__ constexpr size_t grad_warp_bytes() {
   return align_up((size_t)32 * gram_stride(grad_nb<KC>()) * sizeof(double), 128) + align_up((size_t)32 * GRAD_WS * sizeof(double), 128);
@@ -218,14 +218,24 @@ nll_grad_kernel(const double2 *__restrict__ a, const double *__restrict__ t, int
   for (int b = 0; b < NB; ++b) acc[b][0] = acc[b][1] = 0.0;
   const double yG = R.y * R.Gamma, xG = R.x * R.Gamma;
   const int64_t stride = (int64_t)gridDim.x * STREAM_BLOCK;
-#pragma unroll 1
-  for (int64_t i0 = (int64_t)blockIdx.x * STREAM_BLOCK + warp * 32; i0 < n; i0 += stride) {   // whole warps: the MMA is warp-wide
-    const int64_t i = i0 + lane;
+  // Whole warps iterate together (the MMA is warp-wide); the loads of the next tile are issued at the end of an
+  // iteration, behind the tensor-core phase.  Measured at K_c = 8, 1 M events (ncu): this form 38 us; three blocks per SM
+  // at 80 registers 41 us; columns brought in by cp.async, double buffered, straight into the X tile 50 us.
+  double2 v[KC];
+  double ti = 0.0;
+  int64_t i0 = (int64_t)blockIdx.x * STREAM_BLOCK + warp * 32;
+  auto load_tile = [&](int64_t first) {
+    const int64_t i = first + lane;
     const bool live = i < n;
-    double2 v[KC];
 #pragma unroll
     for (int c = 0; c < KC; ++c) v[c] = live ? ldg_stream2(a + c * ld + i) : make_double2(0.0, 0.0);
-    const double ti = live ? ldg_stream1(t + i) : 0.0;
+    ti = live ? ldg_stream1(t + i) : 0.0;
+  };
+  if (i0 < n) load_tile(i0);
+#pragma unroll 1
+  for (; i0 < n; i0 += stride) {
+    const bool live = i0 + lane < n;
+    const double tcur = ti;
     double2 A = make_double2(0.0, 0.0), Ab = make_double2(0.0, 0.0);
 #pragma unroll
     for (int c = 0; c < KC; ++c) {
@@ -233,7 +243,7 @@ nll_grad_kernel(const double2 *__restrict__ a, const double *__restrict__ t, int
       *reinterpret_cast<double2 *>(xrow + 2 * c) = v[c];
     }
     double ch, sh, cs, sn;
-    mixing_functions<SMALL>(yG * ti, xG * ti, ch, sh, cs, sn);
+    mixing_functions<SMALL>(yG * tcur, xG * tcur, ch, sh, cs, sn);
     const Bilinears q = bilinears(A, Ab);
     const double aa = q.aa, bb = q.bb, cre = q.cre, cim = q.cim;
     const double B = rate_form(q, ch, cs, sh, sn);                                        // the bits of bracket()
@@ -242,10 +252,11 @@ nll_grad_kernel(const double2 *__restrict__ a, const double *__restrict__ t, int
     // conj(gA) / B and conj(gAbar) / B as (Re, Im) pairs: the weights of this event
     *reinterpret_cast<double2 *>(wrow) = make_double2(((ch + cs) * A.x - (sh * Ab.x - sn * Ab.y)) * inv, ((ch + cs) * A.y - (sh * Ab.y + sn * Ab.x)) * inv);
     *reinterpret_cast<double2 *>(wrow + 2) = make_double2(((ch - cs) * Ab.x - (sh * A.x + sn * A.y)) * inv, ((ch - cs) * Ab.y - (sh * A.y - sn * A.x)) * inv);
-    const double gt = R.Gamma * ti * inv;
+    const double gt = R.Gamma * tcur * inv;
     sc[0] += gt * (-(aa - bb) * sn - 2.0 * cim * cs);
     sc[1] += gt * ((aa + bb) * sh - 2.0 * cre * ch);
     grad_mma_tile<NB>(Xs, Wt, acc);
+    if (i0 + stride < n) load_tile(i0 + stride);
   }
   const bool fin = grad_reduce<NB, NS>(acc, sc, la, partials, ticket, s_red, s_sum, s_p, s_e, s_b, &last);
   if (!fin) return;

@@ -11,7 +11,8 @@ constexpr int MAX_TERMS = 32;
 constexpr int MAX_KC = 16;
 constexpr int MAX_RES = 16;
 
-enum { SF_NONRES = 0, SF_VV_S = 1, SF_VV_P = 2, SF_VV_D = 3, SF_AP_S = 4, SF_TP_D = 5 };
+enum { SF_NONRES = 0, SF_VV_S = 1, SF_VV_P = 2, SF_VV_D = 3, SF_AP_S = 4, SF_TP_D = 5, SF_AP_D = 6 };
+enum { LS_RUNNING = 0, LS_CONSTANT = 1 };   // lineshape kinds: mass-dependent width (O-6), constant width
 
 struct InstTab {     // one lineshape instance = (resonance, system it sits on, running daughter)
   int8_t res;        // resonance index
@@ -19,8 +20,10 @@ struct InstTab {     // one lineshape instance = (resonance, system it sits on, 
   int8_t sub;        // system index of the running daughter (cascade X -> V c), -1: two stable daughters
   int8_t L;          // L of the resonance's decay vertex
   int8_t dres;       // daughter resonance (its current m0 enters q0), -1 none
-  int8_t pad[3];
+  int8_t kind;       // LS_*: a constant-width instance has the shape g = 1 and gam = m0 Gamma0
+  int8_t pad[2];
   double ma, mb;     // fixed daughter masses (ma unused when sub >= 0)
+  double r2;         // Blatt-Weisskopf radius squared of this resonance's own vertex, GeV^-2
 };
 
 struct TermTab {     // one decay chain (one Bose ordering)
@@ -42,7 +45,7 @@ struct ModelTab {
   TermTab term[MAX_TERMS];
   double m_final[4];
   double m_parent;
-  double r_res2, r_parent2;        // radii squared, GeV^-2
+  double r_res2, r_parent2;        // default resonance radius and parent radius, squared, GeV^-2
 };
 
 // The per-call kernels' view of the model and of the static cache.  The cache of one event set is ONE tile-major array:

@@ -9,6 +9,7 @@
 #include <cstdarg>
 #include <cstdio>
 #include <cstring>
+#include <cstdlib>
 #include <limits>
 #include <string>
 #include <type_traits>
@@ -158,7 +159,7 @@ void drain_profile(tddp4 *h) {
 int parent_L(int sf) {
   switch (sf) {
     case SF_VV_S: return 0; case SF_VV_P: return 1; case SF_VV_D: return 2;
-    case SF_AP_S: return 1; case SF_TP_D: return 2; default: return 0;
+    case SF_AP_S: return 1; case SF_TP_D: return 2; case SF_AP_D: return 1; default: return 0;
   }
 }
 
@@ -173,7 +174,7 @@ int find_or_add_sys(ModelTab &M, unsigned mask) {
 int find_or_add_inst(ModelTab &M, const InstTab &in) {
   for (int i = 0; i < M.n_inst; ++i) {
     const InstTab &o = M.inst[i];
-    if (o.res == in.res && o.sys == in.sys && o.sub == in.sub && o.dres == in.dres && o.ma == in.ma && o.mb == in.mb)
+    if (o.res == in.res && o.sys == in.sys && o.sub == in.sub && o.dres == in.dres && o.ma == in.ma && o.mb == in.mb && o.L == in.L)
       return i;
   }
   if (M.n_inst >= MAX_INST) return -1;
@@ -522,13 +523,12 @@ int launch_nll_grad(tddp4 *h, const EventSet &e, double inv_n, bool small) {
   GradParams gp = time_integral_derivatives(h->RP.x, h->RP.y, h->RP.Gamma, h->t_lo, h->t_hi);
   const size_t smem = grad_smem_bytes<KC>();
   Prof p(h, TDDP4_K_GRAD, (double)e.n * (16.0 * KC + 8.0));
-  if (small) {
+  if (small)
     nll_grad_kernel<KC, true><<<grid, STREAM_BLOCK, smem, h->stream>>>(e.a, e.t, e.ld, e.n, h->RP, gp, h->G, inv_n, e.sum_t, h->partials,
                                                                       h->ticket, h->grad_host_dev);
-  } else {
+  else
     nll_grad_kernel<KC, false><<<grid, STREAM_BLOCK, smem, h->stream>>>(e.a, e.t, e.ld, e.n, h->RP, gp, h->G, inv_n, e.sum_t, h->partials,
                                                                        h->ticket, h->grad_host_dev);
-  }
   return TDDP4_OK;
 }
 
@@ -567,7 +567,9 @@ int tddp4_create(const tddp4_model_desc *desc, tddp4 **out) {
   for (int k = 0; k < desc->n_terms; ++k) order[k] = k;
   std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return desc->terms[a].coupling < desc->terms[b].coupling; });
   for (int r = 0; r < desc->n_res; ++r)
-    if (desc->res[r].L < 0 || desc->res[r].L > 2) return bail(fail(h, TDDP4_ERR_ARG, "resonance %d: L must be 0, 1 or 2", r));
+    if (desc->res[r].L < 0 || desc->res[r].L > 2 || desc->res[r].lineshape < 0 || desc->res[r].lineshape > LS_CONSTANT ||
+        !(desc->res[r].r >= 0.0))
+      return bail(fail(h, TDDP4_ERR_ARG, "resonance %d: L must be 0, 1 or 2, lineshape 0 or 1, r >= 0", r));
   int pos = 0;
   for (int kap = 0; kap <= M.n_kc; ++kap) {
     M.col_begin[kap] = (int8_t)pos;
@@ -586,7 +588,7 @@ int tddp4_create(const tddp4_model_desc *desc, tddp4 **out) {
       tm.perm[r] = (int8_t)t.perm[r];
     }
     if (seen != 0xF) return bail(fail(h, TDDP4_ERR_ARG, "term %d: perm is not a permutation", order[k]));
-    if (t.spin_factor < SF_NONRES || t.spin_factor > SF_TP_D)
+    if (t.spin_factor < SF_NONRES || t.spin_factor > SF_AP_D)
       return bail(fail(h, TDDP4_ERR_ARG, "term %d: unknown spin factor", order[k]));
     tm.sf = (int8_t)t.spin_factor;
     tm.LD = (int8_t)parent_L(t.spin_factor);
@@ -610,6 +612,10 @@ int tddp4_create(const tddp4_model_desc *desc, tddp4 **out) {
     }
     a.L = (int8_t)desc->res[a.res].L;
     b.L = (int8_t)desc->res[b.res].L;
+    a.kind = (int8_t)desc->res[a.res].lineshape;
+    b.kind = (int8_t)desc->res[b.res].lineshape;
+    a.r2 = desc->res[a.res].r > 0.0 ? desc->res[a.res].r * desc->res[a.res].r : M.r_res2;
+    b.r2 = desc->res[b.res].r > 0.0 ? desc->res[b.res].r * desc->res[b.res].r : M.r_res2;
     if (a.sys < 0 || b.sys < 0) return bail(fail(h, TDDP4_ERR_ARG, "too many particle systems"));
     int ia = find_or_add_inst(M, a), ib = find_or_add_inst(M, b);
     if (ia < 0 || ib < 0) return bail(fail(h, TDDP4_ERR_ARG, "too many lineshape instances"));
@@ -853,12 +859,17 @@ int tddp4_set_params(tddp4 *h, const double *c, const double *cbar, const double
     const InstTab &in = M.inst[j];
     double m0 = mass_width[2 * in.res], g0 = mass_width[2 * in.res + 1];
     double ma0 = in.dres >= 0 ? mass_width[2 * in.dres] : in.ma;
+    lp.m0sq[j] = m0 * m0;
+    if (in.kind == LS_CONSTANT) {                       // constant width: shape row g = 1, m0 Gamma = m0 Gamma0
+      if (!(m0 > 0.0) || !(g0 > 0.0)) return fail(h, TDDP4_ERR_DOMAIN, "resonance %d: mass and width must be positive", (int)in.res);
+      lp.gam[j] = m0 * g0;
+      continue;
+    }
     if (!(m0 > ma0 + in.mb) || !(g0 > 0.0))
       return fail(h, TDDP4_ERR_DOMAIN, "resonance %d: pole mass %.6g below its decay threshold %.6g (or width <= 0)",
                   (int)in.res, m0, ma0 + in.mb);
     double q0 = host_breakup(m0, ma0, in.mb);
-    double z0 = q0 * q0 * M.r_res2;
-    lp.m0sq[j] = m0 * m0;
+    double z0 = q0 * q0 * in.r2;
     lp.gam[j] = m0 * m0 * g0 / (std::pow(q0, 2 * in.L + 1) * host_barrier2(in.L, z0));
   }
   bool dirty = !h->have_params;                       // any lineshape constant moved: columns and Gram are stale

@@ -109,3 +109,46 @@ def fit(handle, par0, free_couplings="all_but_first", free_xy=True, hesse=True, 
         out.n_calls = calls[0]
         handle.set_params(best)
     return out
+
+
+def sensitivity_study(binding, model, par, sizes=(20_000, 50_000, 70_000), n_toys=50, n_norm=1_000_000, device="cuda:0",
+                      seed=4242, flat_model=None, flat_par=None, n_pilot=100_000, envelope_scale=1.2):
+    """The shape of the paper's Table 1 (statistical sensitivity to x and y against the number of
+    events, model fixed, no resolution, no background): for every sample size an ensemble of `n_toys` independent
+    pseudo-experiments, each generated with tddp4_generate from `model` at `par` (own Philox seed) and fitted for x and
+    y with `fit` (couplings fixed).  Orchestration only: generation, kinematics, NLL and gradient run behind the C-ABI.
+
+    Returns one dict per size: mean Hessian errors, the ensemble RMS of the fitted values and the mean pulls."""
+    import numpy as _np
+    stream_norm, stream_data = 2, 0
+    if flat_model is not None:
+        hf = binding.Tddp4(flat_model, device)
+        hf.set_params(flat_par)
+        p4n, _, _, _ = hf.generate_n(seed, stream_norm, n_norm, 0, 2.0 * hf.weight_bound(), chunk=1 << 24)
+        hf.close()
+    else:
+        raise ValueError("a constant-amplitude model is needed to un-weight the normalisation sample")
+    gen = binding.Tddp4(model, device)
+    gen.set_params(par)
+    h = binding.Tddp4(model, device)
+    h.load_events(1, p4n)
+    rows, toy = [], 0
+    for n in sizes:
+        xs, ys, sx, sy, calls = [], [], [], [], 0
+        for _ in range(n_toys):
+            toy += 1
+            p4, t, _, _ = gen.generate_n(seed + toy, stream_data, n, n_pilot, envelope_scale, chunk=1 << 23)
+            h.load_events(0, p4, t)
+            res = fit(h, par, free_couplings=None, free_xy=True)
+            calls += res.n_calls
+            if res.success and "x" in res.errors and "y" in res.errors:
+                xs.append(res.par.x); ys.append(res.par.y); sx.append(res.errors["x"]); sy.append(res.errors["y"])
+        xs, ys, sx, sy = map(_np.asarray, (xs, ys, sx, sy))
+        rows.append({"n_events": int(n), "n_toys": int(len(xs)), "sigma_x_hesse": float(sx.mean()), "sigma_y_hesse": float(sy.mean()),
+                     "rms_x": float(xs.std(ddof=1)), "rms_y": float(ys.std(ddof=1)),
+                     "pull_mean_x": float(((xs - par.x) / sx).mean()), "pull_mean_y": float(((ys - par.y) / sy).mean()),
+                     "pull_rms_x": float(((xs - par.x) / sx).std(ddof=1)), "pull_rms_y": float(((ys - par.y) / sy).std(ddof=1)),
+                     "nll_grad_calls_per_fit": calls / max(1, n_toys)})
+    gen.close()
+    h.close()
+    return rows

@@ -117,6 +117,40 @@ def test_layers(B):
     assert np.max(np.abs(col - ref_col) / scale) < TOL_LAYER
 
 
+def test_further_building_blocks(B):
+    """SURVEY.md 8(f) NEXT-2 / PAPER.md line 51: the axial D-wave cascade, per-resonance radii and a constant-width
+    lineshape in one Bose-symmetrised model: static factors, per-term amplitudes, P_i, N, the NLL, the gradient, and a
+    mass/width step on the constant-width and on the re-sized resonance (dirty tracking through the new code paths)."""
+    from test_oracle_bruteforce import blocks_model
+    from oracle import gradient as OG
+    mdl = blocks_model()
+    par = W.initial_params(mdl)
+    p4, _, _, _ = oracle.candidates(mdl, par.tau, 42, 5, 0, 1_555)      # raw candidates: whole phase space
+    t = np.random.default_rng(3).exponential(par.tau, p4.shape[1])
+    p4n, _ = samples.flat_sample(4_001)
+    h = check_against_oracle(B, mdl, par, p4, t, p4n)
+    S, F, a = oracle.terms(mdl, par, p4)
+    f_gpu = h.get(0, B.GET_STATIC).cpu().numpy()
+    assert np.max(np.abs(f_gpu - S * F) / np.abs(S * F).max(axis=1, keepdims=True)) < TOL_LAYER
+    a_gpu = h.get(0, B.GET_TERMS).cpu().numpy()
+    assert np.max(np.abs(a_gpu - a) / np.abs(a).max(axis=1, keepdims=True)) < TOL_LAYER
+    ref, _ = OG.nll_gradient(mdl, par, p4, t, p4n)
+    _, g = h.nll_grad()
+    assert np.max(np.abs(g - ref)) <= 1e-10 * np.abs(ref).max()
+    for name in ("a1(1260)", "K*(892)0", "K1(1400)[D]"):
+        step = par.copy()
+        r = mdl.res_names.index(name)
+        step.mass[r] *= 1.003; step.width[r] *= 0.98
+        h.set_params(step)
+        ref = oracle.nll(mdl, step, p4, t, p4n)
+        assert nll_close(h.nll(), ref[0], np.log(ref[2]))
+    # generation with the same blocks: candidate ratios against the oracle
+    h.set_params(par)
+    _, _, _, rho, _ = h.candidates(77, 0, 0, 3_000)
+    rho_ref, _ = oracle.candidate_ratio(mdl, par, 77, 0, 0, 3_000)
+    assert samples.rel_err(rho.cpu().numpy(), rho_ref, floor=np.abs(rho_ref).max() * 1e-12) < 1e-10
+
+
 def test_trajectory_dirty_tracking(B):
     """Parameter steps as the minimiser would make them: every call is checked against a from-scratch oracle
     evaluation, so stale caches (lineshapes not refreshed, Gram matrix not rebuilt) cannot hide."""
@@ -415,11 +449,13 @@ def many_instance_model():
     """24 de-duplicated lineshape instances on 10 particle systems (the limits of the tables are 24 and 12): two copies of
     the resonance list under different names, the second copy's K* rho chain on the systems (0,2), (1,3)."""
     mdl = W.Model()
+    names = ["K*(892)0", "rho(770)0", "a1(1260)", "K1(1270)", "K2*(1430)", "K1(1400)"]
     for copy in (0, 1):
-        for nm, (m0, g0, L) in W.RESONANCES.items():
+        for nm in names:
+            m0, g0, L = W.RESONANCES[nm]
             mdl.res_names.append(f"{nm}#{copy}"); mdl.res_L.append(L)
             mdl.res_mass.append(m0 * (1.0 + 0.01 * copy)); mdl.res_width.append(g0 * (1.0 + 0.1 * copy))
-    names = list(W.RESONANCES)
+            mdl.res_r.append(0.0); mdl.res_lineshape.append(W.LS_RUNNING)
     for copy, chains in ((0, (1, 2, 3, 4, 5)), (1, (1, 2, 3, 4))):
         for cid in chains:
             sf, res, perm = W.CHAINS[cid]
