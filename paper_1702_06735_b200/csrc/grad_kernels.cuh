@@ -218,24 +218,13 @@ nll_grad_kernel(const double2 *__restrict__ a, const double *__restrict__ t, int
   for (int b = 0; b < NB; ++b) acc[b][0] = acc[b][1] = 0.0;
   const double yG = R.y * R.Gamma, xG = R.x * R.Gamma;
   const int64_t stride = (int64_t)gridDim.x * STREAM_BLOCK;
-  // Whole warps iterate together (the MMA is warp-wide); the loads of the next tile are issued at the end of an
-  // iteration, behind the tensor-core phase.  Measured at K_c = 8, 1 M events (ncu): this form 38 us; three blocks per SM
-  // at 80 registers 41 us; columns brought in by cp.async, double buffered, straight into the X tile 50 us.
-  double2 v[KC];
-  double ti = 0.0;
-  int64_t i0 = (int64_t)blockIdx.x * STREAM_BLOCK + warp * 32;
-  auto load_tile = [&](int64_t first) {
-    const int64_t i = first + lane;
-    const bool live = i < n;
-#pragma unroll
-    for (int c = 0; c < KC; ++c) v[c] = live ? ldg_stream2(a + c * ld + i) : make_double2(0.0, 0.0);
-    ti = live ? ldg_stream1(t + i) : 0.0;
-  };
-  if (i0 < n) load_tile(i0);
-#pragma unroll 1
-  for (; i0 < n; i0 += stride) {
-    const bool live = i0 + lane < n;
-    const double tcur = ti;
+  // Whole warps iterate together (the MMA is warp-wide), one tile per iteration.  Measured at K_c = 8, 1 M events (ncu
+  // gpu__time_duration): this form 38 us; two tiles per iteration (their loads issued together) 40 us; three blocks per
+  // SM at 80 registers 41 us; columns brought in by cp.async, double buffered, straight into the X tile 50 us.  The
+  // kernel issues ~440 warp instructions per 32 events, ~300 of them on the fp64 pipe (2 cycles each) plus 16 DMMA: about
+  // 16 us of fp64-pipe time per million events on B200's 64 lanes per clock per SM -- it is bound by that pipe and by the
+  // serial dependency chain of one event, not by the 136 B per event it streams.
+  auto process = [&](const double2 (&v)[KC], double tcur, bool live) {
     double2 A = make_double2(0.0, 0.0), Ab = make_double2(0.0, 0.0);
 #pragma unroll
     for (int c = 0; c < KC; ++c) {
@@ -256,7 +245,28 @@ nll_grad_kernel(const double2 *__restrict__ a, const double *__restrict__ t, int
     sc[0] += gt * (-(aa - bb) * sn - 2.0 * cim * cs);
     sc[1] += gt * ((aa + bb) * sh - 2.0 * cre * ch);
     grad_mma_tile<NB>(Xs, Wt, acc);
-    if (i0 + stride < n) load_tile(i0 + stride);
+  };
+  auto load_tile = [&](double2 (&v)[KC], double &tt, int64_t first) {
+    const int64_t i = first + lane;
+    const bool live = i < n;
+#pragma unroll
+    for (int c = 0; c < KC; ++c) v[c] = live ? ldg_stream2(a + c * ld + i) : make_double2(0.0, 0.0);
+    tt = live ? ldg_stream1(t + i) : 0.0;
+  };
+  constexpr bool TWO = false;                             // two tiles per iteration: measured slower (40 against 38 us)
+#pragma unroll 1
+  for (int64_t i0 = (int64_t)blockIdx.x * STREAM_BLOCK + warp * 32; i0 < n; i0 += (TWO ? 2 : 1) * stride) {
+    double2 va[KC], vb[TWO ? KC : 1];
+    double ta, tb = 0.0;
+    const bool second = TWO && i0 + stride < n;            // warp-uniform
+    load_tile(va, ta, i0);
+    if (TWO) {
+      if (second) load_tile(reinterpret_cast<double2 (&)[KC]>(vb), tb, i0 + stride);
+    }
+    process(va, ta, i0 + lane < n);
+    if (TWO) {
+      if (second) process(reinterpret_cast<const double2 (&)[KC]>(vb), tb, i0 + stride + lane < n);
+    }
   }
   const bool fin = grad_reduce<NB, NS>(acc, sc, la, partials, ticket, s_red, s_sum, s_p, s_e, s_b, &last);
   if (!fin) return;

@@ -331,26 +331,46 @@ prob_res_kernel(const double2 *__restrict__ a, const double *__restrict__ tr, in
 // The time rows of the data sample: psi[4], tint[4] per event (resolution.cuh).  Re-run when x, y, tau or the sample
 // change; one thread per event; reads t and sigma_t (16 B), writes 64 B.  ALU-bound (3 exp, 6 erfcx, 3 Faddeeva).
 constexpr int TRES_BLOCK = 128;
+// parts: bit 0 = the real-lambda rows (psi_0, psi_2, T_0, T_2: they depend on y and tau), bit 1 = the complex-lambda rows
+// (psi_1, psi_3, T_1, T_3: x and tau).  A step that moved only x (only y) rewrites only its half of the rows.
 __global__ void __launch_bounds__(TRES_BLOCK)
 tres_kernel(const __grid_constant__ FaddTab F, const double *__restrict__ t, const double *__restrict__ sigma_t, int64_t n,
             double x, double y, double Gamma, double t_lo, double t_hi, const TresTable *__restrict__ table,
-            double *__restrict__ tr, int64_t ld) {
+            double *__restrict__ tr, int64_t ld, int parts) {
   __shared__ TresTable tab;
   for (int k = threadIdx.x; k < (int)(sizeof(TresTable) / sizeof(double)); k += TRES_BLOCK)
     reinterpret_cast<double *>(&tab)[k] = reinterpret_cast<const double *>(table)[k];
   __syncthreads();
   int64_t i = (int64_t)blockIdx.x * TRES_BLOCK + threadIdx.x;
   if (i >= n) return;
-  double psi[4], tint[4];
-  const double sig = sigma_t[i];
-  if (tab.ok) {                                   // block-uniform
-    time_terms(F, t[i], sig, x, y, Gamma, t_lo, t_hi, psi, nullptr);
-    window_terms_table(tab, sig, tint);
-  } else {
-    time_terms(F, t[i], sig, x, y, Gamma, t_lo, t_hi, psi, tint);
+  const double ti = t[i], sig = sigma_t[i];
+  const bool table_ok = tab.ok != 0;              // block-uniform
+  double tint[4];
+  if (table_ok) window_terms_table(tab, sig, tint);
+  const double derf = table_ok ? 0.0 : erf_scaled(t_hi, sig) - erf_scaled(t_lo, sig);
+  if (parts & 1) {
+    const double lm = Gamma * (1.0 - y), lp = Gamma * (1.0 + y);
+    const double hm = conv_exp_real(ti, lm, sig), hp = conv_exp_real(ti, lp, sig);
+    tr[0 * ld + i] = 0.5 * (hm + hp);
+    tr[2 * ld + i] = 0.5 * (hm - hp);
+    if (!table_ok) {
+      const double Im = window_real(t_lo, t_hi, lm, sig, derf), Ip = window_real(t_lo, t_hi, lp, sig, derf);
+      tint[0] = 0.5 * (Im + Ip); tint[2] = 0.5 * (Im - Ip);
+    }
+    tr[4 * ld + i] = tint[0];
+    tr[6 * ld + i] = tint[2];
   }
-#pragma unroll
-  for (int m = 0; m < 4; ++m) { tr[m * ld + i] = psi[m]; tr[(4 + m) * ld + i] = tint[m]; }
+  if (parts & 2) {
+    const double2 hx = conv_exp_complex(F, ti, Gamma, -Gamma * x, sig);
+    tr[1 * ld + i] = hx.x;
+    tr[3 * ld + i] = hx.y;
+    if (!table_ok) {
+      const double2 Ix = window_complex(F, t_lo, t_hi, Gamma, -Gamma * x, sig, derf);
+      tint[1] = Ix.x; tint[3] = Ix.y;
+    }
+    tr[5 * ld + i] = tint[1];
+    tr[7 * ld + i] = tint[3];
+  }
 }
 
 // Time-integrated mode (use_resolution = 2): every event has the same eight "time quantities", the window integrals
@@ -511,6 +531,8 @@ colnll_stream_kernel(const __grid_constant__ StreamTab S, const __grid_constant_
 // (Measured: rows of 20 doubles with groups of consecutive events had 2-way store conflicts, 7.2 M conflict
 // wavefronts per 4 M events with the LSU data pipe 83 % busy; this layout: Gram kernel 215 -> 211 us.)
 __host__ __device__ constexpr int gram_stride(int NB) { return 8 * NB + 2; }
+constexpr int GRAM_GROUP = 16;        // blocks per group of the two-level grid reduction
+constexpr int MAX_TICKETS = 1 + 256;  // grid ticket + group tickets (grids up to 4096 blocks)
 inline size_t gram_warp_scratch(int NB, int n_inst4) {
   return align_up(lineshape_scratch_bytes(n_inst4), 128) + align_up((size_t)32 * gram_stride(NB) * sizeof(double), 128);
 }
@@ -609,33 +631,50 @@ gram_stream_kernel(const __grid_constant__ StreamTab S, const __grid_constant__ 
     for (int wp = 0; wp < WARPS; ++wp) sum += Ws[wp * NB * NB * 64 + e];
     partials[(int64_t)blockIdx.x * NB * NB * 64 + e] = sum;
   }
+  // Two-level, fixed-order reduction over the grid.  Blocks form groups of GRAM_GROUP consecutive blocks; the last block
+  // of a group to arrive (group ticket) adds the group's partials in block order, the last group to finish (grid ticket)
+  // adds the group sums in group order.  Every level is one round of independent loads: two L2 round trips after the
+  // last block partial instead of one block pulling all gridDim.x partials (455 KB at K_c = 8) through a single SM.
+  const unsigned n_groups = (gridDim.x + GRAM_GROUP - 1) / GRAM_GROUP, grp = blockIdx.x / GRAM_GROUP;
+  const unsigned g_first = grp * GRAM_GROUP, g_size = min((unsigned)GRAM_GROUP, gridDim.x - g_first);
   __threadfence();
   __syncthreads();
-  if (tid == 0) last = atomicAdd(ticket, 1u) == gridDim.x - 1;
+  if (tid == 0) last = atomicAdd(ticket + 1 + grp, 1u) == g_size - 1;
   __syncthreads();
   if (!last) return;
   __threadfence();
-  // final pass: upper blocks summed over blocks in index order, staged in shared memory, then G
+  double *gsum = partials + (int64_t)gridDim.x * NB * NB * 64;        // [n_groups][NB*NB*64]
+  for (int e = tid; e < NB * NB * 64; e += STREAM_BLOCK) {
+    int bi = e / (NB * 64), bj = (e / 64) % NB;
+    if (bi > bj) continue;
+    double v[GRAM_GROUP];
+#pragma unroll
+    for (int c = 0; c < GRAM_GROUP; ++c) v[c] = (unsigned)c < g_size ? __ldcg(partials + (int64_t)(g_first + c) * NB * NB * 64 + e) : 0.0;
+    double sum = 0.0;
+#pragma unroll
+    for (int c = 0; c < GRAM_GROUP; ++c) sum += v[c];
+    gsum[(int64_t)grp * NB * NB * 64 + e] = sum;
+  }
+  __threadfence();
+  __syncthreads();
+  if (tid == 0) { ticket[1 + grp] = 0; last = atomicAdd(ticket, 1u) == n_groups - 1; }
+  __syncthreads();
+  if (!last) return;
+  __threadfence();
   double *XtX = Ws;                                      // [NB][NB][64], reused
   for (int e = tid; e < NB * NB * 64; e += STREAM_BLOCK) {
     int bi = e / (NB * 64), bj = (e / 64) % NB;
     if (bi > bj) continue;
-    // 16 independent chains (block b goes to chain b mod 16), chains added in index order: a fixed summation tree with
-    // 16 loads in flight instead of gridDim.x dependent L2 round trips at the tail of the kernel
-    double part[16];
-#pragma unroll
-    for (int c = 0; c < 16; ++c) part[c] = 0.0;
-    unsigned b = 0;
-    for (; b + 16 <= gridDim.x; b += 16) {
-#pragma unroll
-      for (int c = 0; c < 16; ++c) part[c] += __ldcg(partials + (int64_t)(b + c) * NB * NB * 64 + e);
-    }
-#pragma unroll
-    for (int c = 0; c < 16; ++c)
-      if (b + c < gridDim.x) part[c] += __ldcg(partials + (int64_t)(b + c) * NB * NB * 64 + e);
     double sum = 0.0;
+    unsigned g = 0;
+    for (; g + 8 <= n_groups; g += 8) {
+      double v[8];
 #pragma unroll
-    for (int c = 0; c < 16; ++c) sum += part[c];
+      for (int c = 0; c < 8; ++c) v[c] = __ldcg(gsum + (int64_t)(g + c) * NB * NB * 64 + e);
+#pragma unroll
+      for (int c = 0; c < 8; ++c) sum += v[c];
+    }
+    for (; g < n_groups; ++g) sum += __ldcg(gsum + (int64_t)g * NB * NB * 64 + e);
     XtX[e] = sum;
   }
   __syncthreads();

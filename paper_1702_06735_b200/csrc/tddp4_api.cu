@@ -34,6 +34,7 @@ struct EventSet {
   double *t = nullptr, *sigma_t = nullptr, *w = nullptr;
   double *tr = nullptr;                              // resolution mode: time rows psi[4], tint[4], [8][ld]
   bool tres_valid = false;                           // tr matches the current x, y, tau
+  int tres_parts = 3;                                // which halves of tr are stale: bit 0 real-lambda rows (y, tau), bit 1 complex (x, tau)
   double *trg = nullptr;                             // derivative rows of the gradient in resolution mode, [8][ld] (on demand)
   bool tresg_valid = false;
   double sum_t = 0.0, t_max = 0.0;                   // sum and max |t| of the decay times (fixed-order kernel)
@@ -289,7 +290,7 @@ template <int NB>
 int launch_gram(tddp4 *h, const EventSet &e) {
   const ModelTab &M = h->M;
   int grid = stream_grid(h, e.n);
-  int rc = ensure_partials(h, (size_t)grid * 64 * NB * NB + 16);
+  int rc = ensure_partials(h, (size_t)(grid + (grid + GRAM_GROUP - 1) / GRAM_GROUP) * 64 * NB * NB + 16);
   if (rc) return rc;
   StreamTab S = h->S;
   S.R = e.R;
@@ -429,11 +430,12 @@ int enqueue_nll(tddp4 *h, double *result, double *prob) {
       Prof p(h, TDDP4_K_TRES, (double)d.n * 80.0);
       tres_table_kernel<<<1, 32, 0, h->stream>>>(h->FT, h->RP.x, h->RP.y, h->RP.Gamma, h->t_lo, h->t_hi, d.sig_lo, d.sig_hi, h->tres_tab);
       tres_kernel<<<grid, TRES_BLOCK, 0, h->stream>>>(h->FT, d.t, d.sigma_t, d.n, h->RP.x, h->RP.y, h->RP.Gamma, h->t_lo, h->t_hi,
-                                                      h->tres_tab, d.tr, d.ld);
+                                                      h->tres_tab, d.tr, d.ld, d.tres_parts);
       ++h->launches;
     }
     CU(cudaGetLastError());
     d.tres_valid = true;
+    d.tres_parts = 0;
   }
   double inv_n = h->gram_n > 0 ? 1.0 / (double)h->gram_n : 0.0;
   // Taylor forms of the four time functions are valid when both mixing phases stay below 1/4 on this sample
@@ -683,7 +685,7 @@ int tddp4_create(const tddp4_model_desc *desc, tddp4 **out) {
   h->own_stream = true;
   int KC = M.n_kc;
   bool ok = cudaMalloc(&h->G, sizeof(double) * 2 * KC * KC) == cudaSuccess &&
-            cudaMalloc(&h->ticket, sizeof(unsigned int)) == cudaSuccess &&
+            cudaMalloc(&h->ticket, sizeof(unsigned int) * MAX_TICKETS) == cudaSuccess &&
             cudaMalloc(&h->results, sizeof(double) * (N_SLOTS + 1) * SLOT_DOUBLES) == cudaSuccess &&
             cudaHostAlloc(&h->results_host, sizeof(double) * N_SLOTS * SLOT_DOUBLES, cudaHostAllocMapped) == cudaSuccess &&
             cudaHostGetDevicePointer((void **)&h->results_host_dev, h->results_host, 0) == cudaSuccess &&
@@ -691,7 +693,7 @@ int tddp4_create(const tddp4_model_desc *desc, tddp4 **out) {
             cudaHostGetDevicePointer((void **)&h->grad_host_dev, h->grad_host, 0) == cudaSuccess &&
             cudaMalloc(&h->gen_scalars, sizeof(unsigned long long) * 4) == cudaSuccess &&
             cudaMalloc(&h->tres_tab, sizeof(TresTable)) == cudaSuccess &&
-            cudaMemset(h->ticket, 0, sizeof(unsigned int)) == cudaSuccess &&
+            cudaMemset(h->ticket, 0, sizeof(unsigned int) * MAX_TICKETS) == cudaSuccess &&
             cudaMemset(h->G, 0, sizeof(double) * 2 * KC * KC) == cudaSuccess;
   if (ok) memset(h->results_host, 0, sizeof(double) * N_SLOTS * SLOT_DOUBLES);   // no stale sequence stamps from a recycled allocation
   for (int s = 0; ok && s < N_SLOTS; ++s) ok = cudaEventCreateWithFlags(&h->slot_event[s], cudaEventDisableTiming) == cudaSuccess;
@@ -787,6 +789,7 @@ int tddp4_load_events(tddp4 *h, int which, int64_t n, int64_t ld_in, const doubl
     }
   }
   e.tres_valid = e.tresg_valid = false;
+  e.tres_parts = 3;
   const CacheRows cr{e.R, M.n_sys, M.n_sys + h->S.n_inst4};
   cudaMemcpyKind kind = on_device ? cudaMemcpyDeviceToDevice : cudaMemcpyHostToDevice;
   auto copy_vec = [&](double **dst, const double *src) -> cudaError_t {
@@ -887,7 +890,12 @@ int tddp4_set_params(tddp4 *h, const double *c, const double *cbar, const double
     R.c[k][0] = c[2 * k]; R.c[k][1] = c[2 * k + 1];
     R.cbar[k][0] = cbar[2 * k]; R.cbar[k][1] = cbar[2 * k + 1];
   }
-  if (R.x != x || R.y != y || R.Gamma != 1.0 / tau || !h->have_params) h->set[0].tres_valid = h->set[0].tresg_valid = false;
+  if (R.x != x || R.y != y || R.Gamma != 1.0 / tau || !h->have_params) {
+    h->set[0].tres_valid = h->set[0].tresg_valid = false;
+    if (R.Gamma != 1.0 / tau || !h->have_params) h->set[0].tres_parts = 3;
+    if (R.y != y) h->set[0].tres_parts |= 1;
+    if (R.x != x) h->set[0].tres_parts |= 2;
+  }
   R.x = x; R.y = y; R.Gamma = 1.0 / tau;
   R.t_lo = h->t_lo; R.t_hi = h->t_hi; R.use_resolution = h->use_resolution;
   time_integrals(x, y, R.Gamma, h->t_lo, h->t_hi, R.T);
