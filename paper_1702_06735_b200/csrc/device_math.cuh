@@ -49,17 +49,6 @@ __device__ __forceinline__ double width_shape(int L, double q2, double z, double
   return q * q2 * q2 / ((9.0 + 3.0 * z + z * z) * M);
 }
 
-// T = 1 / (m0sq - s - i gam g)   (O-6)
-__device__ __forceinline__ double2 breit_wigner(double m0sq, double gam, double s, double g) {
-  double re = m0sq - s, im = gam * g;
-  double inv = 1.0 / (re * re + im * im);
-  return make_double2(re * inv, im * inv);
-}
-
-__device__ __forceinline__ double2 cmul(double2 a, double2 b) {
-  return make_double2(a.x * b.x - a.y * b.y, a.x * b.y + a.y * b.x);
-}
-
 // closed-form spin factors (O-4), role vectors r0..r3 already gathered
 __device__ __forceinline__ double spin_factor(int sf, V4 r0, V4 r1, V4 r2, V4 r3) {
   if (sf == SF_NONRES) return 1.0;

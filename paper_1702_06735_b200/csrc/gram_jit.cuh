@@ -1,0 +1,107 @@
+// gram_jit.cuh -- step 6 (the normalisation "from several million phase space
+// points"), fused with steps 2+3 over the static cache of the normalisation sample:
+//     G_kl = sum_j w_j a_k(p_j) conj(a_l(p_j))        (K_c x K_c Hermitian; O-8: N is a contraction of G with the couplings)
+// The columns of the normalisation sample are never stored.  With x_j = (Re a_0, Im a_0, Re a_1, ...) the real matrix
+// X^T diag(w) X holds every Re/Im piece of G, and it is a dense contraction over events: it runs on the fp64 tensor cores
+// (mma.sync m8n8k4, SASS DMMA), the only place of the path where they apply (north_star):
+//   G_kl.re = XtX[2k][2l] + XtX[2k+1][2l+1],   G_kl.im = XtX[2k+1][2l] - XtX[2k][2l+1].
+//
+// This file is NOT compiled by nvcc.  The library compiles it at run time with NVRTC (jit.h), once per model, behind a
+// generated prelude that states the model as compile-time constants:
+//   J_NB, J_KC, J_NINST, J_NTERMS, J_NSU, J_R, J_SKIP, J_GOFF, J_FOFF, J_WOFF (element offsets in a tile, -1: unweighted),
+//   J_SROW[J_NINST]  index (0 .. J_NSU-1) of the s row instance j reads, rows counted from J_SKIP,
+//   J_T0[J_NTERMS], J_T1[J_NTERMS]  lineshape instances of term k (-1: none),  J_COL[J_NTERMS]  its coupling column,
+//   J_LAST[J_NTERMS]  1: term k closes its column (terms are sorted by column).
+// Why: PAPER.md line 51 builds the amplitude from tables of shared lineshape / spin-factor instances.  A table-driven
+// kernel has to park the lineshapes T_R of an event in shared memory, because the terms index them at run time: per
+// 32-event tile that was 13 STS.128 + 32 LDS.128 of lineshapes next to the loads themselves, the X tile and the MMA
+// fragments -- 342 wavefronts of the LSU data pipe per tile, and ncu showed that pipe 80-82 % busy with no other unit
+// above 45 %: the kernel sat at 0.82-0.85 of the HBM roofline on the shared-memory pipe, not on bytes.  With the tables
+// compile-time constants every index below is an immediate: the lineshapes stay in registers (no scratch at all), every
+// load carries an immediate offset, and the per-term table lookups, address arithmetic and flush branches disappear.
+// Deterministic: per-warp accumulation in event order, warps, blocks and block groups summed in index order.
+#include "jit_shared.cuh"
+
+namespace tddp4k {
+
+constexpr int JG_BLOCK = 256, JG_WARPS = JG_BLOCK / 32;
+
+extern "C" __global__ void __launch_bounds__(JG_BLOCK, J_BPS)
+gram_jit(const __grid_constant__ LineParams LP, const double *__restrict__ cache, long long n,
+         double *__restrict__ partials /* [grid + groups][64 NB NB] */, unsigned int *ticket,
+         double *__restrict__ G /* [KC][KC][2] sums, Hermitian, full */) {
+  constexpr int NB = J_NB, F = 8 * NB, STRIDE = gram_stride(NB), NP = NB * (NB + 1) / 2;
+  constexpr bool WEIGHTED = J_WOFF >= 0;
+  extern __shared__ __align__(16) char smem_raw[];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  double *Xs = reinterpret_cast<double *>(smem_raw) + (size_t)warp * 32 * STRIDE;   // [32][STRIDE]: row = event
+  double *row = Xs + lane * STRIDE;
+#pragma unroll
+  for (int c = 0; c < STRIDE; ++c) row[c] = 0.0;                // features beyond 2 K_c stay zero
+  double acc[NP][2];
+#pragma unroll
+  for (int q = 0; q < NP; ++q) acc[q][0] = acc[q][1] = 0.0;
+  const long long stride = (long long)gridDim.x * JG_BLOCK;
+  // whole warps iterate together (the MMA is warp-wide).  The cache is allocated and zero-filled in whole tiles, so the
+  // lanes of a ragged last tile compute on zeros: f = 0 gives zero columns, and their weight is forced to 0.
+  long long i0 = (long long)blockIdx.x * JG_BLOCK + warp * 32;
+#pragma unroll 1
+  for (; i0 < n; i0 += stride) {
+    if (PF_DIST > 0 && lane == 0 && i0 + PF_DIST * stride < n)
+      prefetch_l2_bulk(tile_event(cache, J_R, i0 + PF_DIST * stride) + J_SKIP, (unsigned)(J_R * 32 - J_SKIP) * 8u);
+    const double *ev = tile_event(cache, J_R, i0 + lane);
+    double sv[J_NSU + 1], gv[J_NINST + 1], fv[J_NTERMS];   // + 1: a model without resonances has no instance
+#pragma unroll
+    for (int r = 0; r < J_NSU; ++r) sv[r] = ldg_stream1(ev + J_SKIP + r * 32);
+#pragma unroll
+    for (int j = 0; j < J_NINST; ++j) gv[j] = ldg_stream1(ev + J_GOFF + j * 32);
+#pragma unroll
+    for (int k = 0; k < J_NTERMS; ++k) fv[k] = ldg_stream1(ev + J_FOFF + k * 32);
+    double wj = 1.0;
+    if (WEIGHTED) wj = ldg_stream1(ev + J_WOFF);
+    double2 T[J_NINST + 1];
+#pragma unroll
+    for (int j = 0; j < J_NINST; ++j) T[j] = breit_wigner(LP.m0sq[j], LP.gam[j], sv[J_SROW[j]], gv[j]);
+    double2 a = make_double2(0.0, 0.0);
+#pragma unroll
+    for (int k = 0; k < J_NTERMS; ++k) {
+      double2 P;
+      if (J_T0[k] >= 0 && J_T1[k] >= 0) P = cmul(T[J_T0[k] >= 0 ? J_T0[k] : 0], T[J_T1[k] >= 0 ? J_T1[k] : 0]);
+      else if (J_T0[k] >= 0) P = T[J_T0[k] >= 0 ? J_T0[k] : 0];
+      else if (J_T1[k] >= 0) P = T[J_T1[k] >= 0 ? J_T1[k] : 0];
+      else P = make_double2(1.0, 0.0);
+      a.x = fma(fv[k], P.x, a.x);
+      a.y = fma(fv[k], P.y, a.y);
+      if (J_LAST[k]) {
+        *reinterpret_cast<double2 *>(row + 2 * J_COL[k]) = a;
+        a = make_double2(0.0, 0.0);
+      }
+    }
+    if (WEIGHTED) row[F] = i0 + lane < n ? wj : 0.0;
+    __syncwarp();
+    {
+      const double *base = Xs + (2 * (lane & 3)) * STRIDE + (lane >> 2);
+#pragma unroll
+      for (int grp = 0; grp < 8; ++grp) {                  // 4 events per MMA, 8 groups per warp tile
+        const double *r = base + (8 * (grp >> 1) + (grp & 1)) * STRIDE;
+        double x[NB];
+#pragma unroll
+        for (int b = 0; b < NB; ++b) x[b] = r[8 * b];
+        double wv = 1.0;
+        if (WEIGHTED) wv = r[F - (lane >> 2)];
+        int q = 0;
+#pragma unroll
+        for (int bi = 0; bi < NB; ++bi) {
+          const double aw = WEIGHTED ? wv * x[bi] : x[bi];
+#pragma unroll
+          for (int bj = bi; bj < NB; ++bj, ++q) dmma884(acc[q][0], acc[q][1], aw, x[bj]);
+        }
+      }
+    }
+    __syncwarp();                                          // the X tile is free again
+  }
+  __syncthreads();                                         // the X tiles are free: the reduction reuses the memory
+  gram_reduce_tail<NB, JG_BLOCK>(acc, reinterpret_cast<double *>(smem_raw), J_KC, partials, ticket, G);
+}
+
+}  // namespace tddp4k

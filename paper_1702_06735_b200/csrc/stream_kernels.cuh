@@ -1,7 +1,7 @@
 // stream_kernels.cuh -- the per-call kernels of the NLL path:
 //   nll_stream_kernel     steps 4+5+7   over cached coupling columns             (coupling / x / y / tau-only call)
 //   colnll_stream_kernel  steps 2..5+7  over the static cache of the data set    (call after a mass or width moved)
-//   gram_stream_kernel    steps 2+3+6   over the static cache of the normalisation set (fp64 tensor-core Gram)
+//   (gram_kernel.cuh:     steps 2+3+6   over the static cache of the normalisation set, fp64 tensor-core Gram)
 //   nll_res_kernel, tres_kernel, prob_*  resolution mode (config 5) and per-event probabilities
 // All are HBM streams: every row is read exactly once per call with coalesced loads straight into registers (256-byte
 // warp segments of 8-byte rows, 512-byte segments of the 16-byte columns), every load of an event requested before any
@@ -20,40 +20,6 @@ namespace tddp4k {
 constexpr int STREAM_BLOCK = 256;
 constexpr int STREAM_WARPS = STREAM_BLOCK / 32;
 constexpr int STREAM_BLOCKS_PER_SM = 2;
-
-__host__ __device__ constexpr size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
-
-// read-once loads: no L1 allocation
-__device__ __forceinline__ double2 ldg_stream2(const double2 *p) {
-  double2 v;
-  asm volatile("ld.global.nc.L1::no_allocate.v2.f64 {%0,%1}, [%2];" : "=d"(v.x), "=d"(v.y) : "l"(p));
-  return v;
-}
-__device__ __forceinline__ double ldg_stream1(const double *p) {
-  double v;
-  asm volatile("ld.global.nc.L1::no_allocate.f64 %0, [%1];" : "=d"(v) : "l"(p));
-  return v;
-}
-
-// Programmatic dependent launch (the host launches the per-call kernels with programmatic stream serialization): a kernel
-// lets its successor's blocks become resident as soon as its own blocks exit, so the successor's launch latency, ramp-up
-// and read-only streaming overlap this kernel's tail and final reduction.  pdl_wait() blocks until the predecessor grid
-// has completed and its memory is visible; it sits in front of the first access to anything the predecessor may read or
-// write (partials, ticket, G, result slots; the columns when the predecessor or this kernel writes them).
-// Ordering rule: a successor may become resident as soon as every block of this kernel has executed
-// launch_dependents -- possibly while this kernel's own predecessor is still running.  A successor that skips its early
-// wait must therefore never conflict with that older kernel: (i) a kernel that has an early wait triggers only after it,
-// (ii) the Gram kernel, after which the column-writing kernel skips its early wait, triggers only after its late wait,
-// (iii) an NLL kernel without early wait may trigger at once: whatever follows it either waits early or only reads what
-// no kernel before it writes.
-__device__ __forceinline__ void pdl_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;"); }
-__device__ __forceinline__ void pdl_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
-
-// One lane asks the memory system to bring a whole contiguous region into L2 (no destination, no register, no scoreboard):
-// the tile-major cache makes the NEXT tile of a warp one such region, so its loads later hit L2 instead of HBM.
-__device__ __forceinline__ void prefetch_l2_bulk(const void *p, uint32_t bytes) {
-  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(p), "r"(bytes) : "memory");
-}
 
 // ------------------------------------------------------------------------------------------------
 // sum_i log B_i without a log per event: B = m 2^e with m in [1,2); the mantissas are multiplied up and the
@@ -447,26 +413,31 @@ __device__ __forceinline__ void columns_from_scratch(const StreamTab &S, const d
 #pragma unroll
         for (int u = 0; u < GT; ++u) fv[u] = ldg_stream1(f_ev + (k0 + u) * 32);
       }
+      // Two phases per sub-batch of TB terms: first every lineshape product (shared-memory reads only), then the sums and
+      // the flushes.  A flush stores to shared memory (the Gram kernel's X tile) at a run-time address, which the compiler
+      // must assume to alias the lineshape slots: with one loop it kept every term's two LDS behind the previous term's
+      // store, sixteen serial LDS -> DMUL -> DFMA chains per event (34 % of the Gram kernel's warp samples).
+      constexpr int TB = GT < 8 ? GT : 8;
 #pragma unroll
-      for (int u = 0; u < GT; ++u) {
-        const int k = k0 + u;
-        double2 T = cmul(sTl[S.term_t0[k]], sTl[S.term_t1[k]]);
-        acc.x = fma(fv[u], T.x, acc.x);
-        acc.y = fma(fv[u], T.y, acc.y);
-        if (S.term_last[k]) {
-          flush((int)S.term_col[k], acc);
-          acc = make_double2(0.0, 0.0);
+      for (int u0 = 0; u0 < GT; u0 += TB) {
+        double2 TT[TB];
+#pragma unroll
+        for (int u = 0; u < TB; ++u) TT[u] = cmul(sTl[S.term_t0[k0 + u0 + u]], sTl[S.term_t1[k0 + u0 + u]]);
+#pragma unroll
+        for (int u = 0; u < TB; ++u) {
+          const int k = k0 + u0 + u;
+          acc.x = fma(fv[u0 + u], TT[u].x, acc.x);
+          acc.y = fma(fv[u0 + u], TT[u].y, acc.y);
+          if (S.term_last[k]) {
+            flush((int)S.term_col[k], acc);
+            acc = make_double2(0.0, 0.0);
+          }
         }
       }
     }
   }
 }
 __host__ __device__ inline size_t lineshape_scratch_bytes(int n_inst4) { return (size_t)(n_inst4 + 1) * 32 * sizeof(double2); }
-// address of (row 0, event i) in a tile-major cache of R rows
-__device__ __forceinline__ const double *tile_event(const double *__restrict__ cache, int R, int64_t i) {
-  return cache + ((i >> 5) * R) * 32 + (i & 31);
-}
-
 // ------------------------------------------------------------------------------------------------
 // Call after a mass or width moved, data set.  Reads the s rows in use, the g rows, the f rows and t; writes every
 // coupling column back (for the coupling-only calls that follow) and finishes the NLL in the same pass.
@@ -493,9 +464,12 @@ colnll_stream_kernel(const __grid_constant__ StreamTab S, const __grid_constant_
   const int64_t stride = (int64_t)gridDim.x * STREAM_BLOCK;
   if (RES) block_phase_space_sums(R, G, S.n_kc, inv_n_norm, s_S);
   int64_t i = (int64_t)blockIdx.x * STREAM_BLOCK + threadIdx.x;
+#pragma unroll
+  for (int d = 1; d < PF_DIST; ++d)
+    if (lane == 0 && i + d * stride < n) prefetch_l2_bulk(tile_event(cache, S.R, i + d * stride) + S.skip, (uint32_t)(S.R * 32 - S.skip) * 8u);
 #pragma unroll 1
   for (; i < n; i += stride) {
-    if (lane == 0 && i + stride < n) prefetch_l2_bulk(tile_event(cache, S.R, i + stride) + S.skip, (uint32_t)(S.R * 32 - S.skip) * 8u);
+    if (PF_DIST > 0 && lane == 0 && i + PF_DIST * stride < n) prefetch_l2_bulk(tile_event(cache, S.R, i + PF_DIST * stride) + S.skip, (uint32_t)(S.R * 32 - S.skip) * 8u);
     double ti = RES ? 0.0 : ldg_stream1(t + i);            // RES: t points at the time rows [8][ld]
     const double *ev = tile_event(cache, S.R, i);
     double fv[GT];
@@ -512,185 +486,6 @@ colnll_stream_kernel(const __grid_constant__ StreamTab S, const __grid_constant_
   }
   if (!(RES || early_wait)) pdl_wait();
   nll_finish<RES>(R, S.n_kc, n, sum_t, la, G, inv_n_norm, partials, ticket, result, seq);
-}
-
-// ------------------------------------------------------------------------------------------------
-// step 6: Hermitian Gram matrix G_kl = sum_j w_j a_k(p_j) conj(a_l(p_j)) over the normalisation sample, fused with
-// steps 2+3: the columns of the normalisation sample are never stored.  With x_j = (Re a_0, Im a_0, Re a_1, ...)
-// the real matrix X^T diag(w) X holds every Re/Im piece of G, and it is a dense contraction over events: it runs on
-// the fp64 tensor cores (mma.sync m8n8k4, SASS DMMA), the only place of the path where they apply (north_star).
-//   G_kl.re = XtX[2k][2l] + XtX[2k+1][2l+1],   G_kl.im = XtX[2k+1][2l] - XtX[2k][2l+1].
-// One thread per event computes the columns into its row of the warp's X tile (padded, conflict-free fragments);
-// the warp then feeds its 32 events, 4 at a time, through the MMA.  NB = number of 8-feature blocks.
-// Reads the s rows in use, the g rows, the f rows, and w if the sample is weighted.
-// Deterministic: per-warp accumulation in event order, warps then blocks summed in index order.
-// X tile of a warp: row = event, gram_stride(NB) = 8 NB + 2 doubles per row (F = 8 NB features, the weight at [F]).
-// Both access patterns are bank-conflict free: a lane's 16-byte column stores land in slot (e (4 NB + 1) + kappa) mod 8,
-// distinct over the 8 lanes of a wavefront; MMA group g takes the four events e = 8 (g >> 1) + 2 (lane & 3) + (g & 1), so
-// the fragment loads of a half-warp hit the 8-byte banks (phi + 4 (lane & 3) + const) mod 16, phi = lane >> 2.
-// (Measured: rows of 20 doubles with groups of consecutive events had 2-way store conflicts, 7.2 M conflict
-// wavefronts per 4 M events with the LSU data pipe 83 % busy; this layout: Gram kernel 215 -> 211 us.)
-__host__ __device__ constexpr int gram_stride(int NB) { return 8 * NB + 2; }
-constexpr int GRAM_GROUP = 16;        // blocks per group of the two-level grid reduction
-constexpr int MAX_TICKETS = 1 + 256;  // grid ticket + group tickets (grids up to 4096 blocks)
-inline size_t gram_warp_scratch(int NB, int n_inst4) {
-  return align_up(lineshape_scratch_bytes(n_inst4), 128) + align_up((size_t)32 * gram_stride(NB) * sizeof(double), 128);
-}
-inline size_t gram_smem_bytes(int NB, int n_inst4) {
-  size_t work = STREAM_WARPS * gram_warp_scratch(NB, n_inst4), red = (size_t)STREAM_WARPS * NB * NB * 64 * sizeof(double);
-  return work > red ? work : red;
-}
-
-__device__ __forceinline__ void dmma884(double &c0, double &c1, double a, double b) {
-  asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
-               : "+d"(c0), "+d"(c1) : "d"(a), "d"(b));
-}
-
-template <int NB, int GI, int GT>
-__global__ void __launch_bounds__(STREAM_BLOCK, STREAM_BLOCKS_PER_SM)
-gram_stream_kernel(const __grid_constant__ StreamTab S, const __grid_constant__ LineParams LP,
-                   const double *__restrict__ cache, int64_t n,
-                   double *__restrict__ partials /* [grid][64 NB NB] */, unsigned int *ticket,
-                   double *__restrict__ G /* [KC][KC][2] sums, Hermitian, full */) {
-  constexpr int F = 8 * NB, STRIDE = gram_stride(NB), NP = NB * (NB + 1) / 2, WARPS = STREAM_WARPS;
-  extern __shared__ __align__(16) char smem_raw[];
-  __shared__ bool last;
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  const int KC = S.n_kc;
-  const size_t t_bytes = align_up(lineshape_scratch_bytes(S.n_inst4), 128);
-  const size_t x_bytes = align_up((size_t)32 * STRIDE * sizeof(double), 128);
-  char *scratch = smem_raw + (size_t)warp * (t_bytes + x_bytes);
-  double2 *sTl = reinterpret_cast<double2 *>(scratch) + lane;  // [n_inst][32], this lane's slots
-  double *Xs = reinterpret_cast<double *>(scratch + t_bytes);  // [32][STRIDE]: row = event, F features + weight
-  double *row = Xs + lane * STRIDE;
-  sTl[S.n_inst4 * 32] = make_double2(1.0, 0.0);                // unit lineshape slot
-#pragma unroll
-  for (int c = 0; c < STRIDE; ++c) row[c] = 0.0;                // features beyond 2 K_c stay zero
-  double acc[NP][2];
-#pragma unroll
-  for (int q = 0; q < NP; ++q) acc[q][0] = acc[q][1] = 0.0;
-  const int64_t stride = (int64_t)gridDim.x * STREAM_BLOCK;
-  // whole warps iterate together (the MMA is warp-wide).  The cache is allocated and zero-filled in whole tiles, so the
-  // lanes of a ragged last tile compute on zeros: f = 0 gives zero columns, and their weight is forced to 0.
-  auto mma_tile = [&]() {
-    __syncwarp();
-    const double *base = Xs + (2 * (lane & 3)) * STRIDE + (lane >> 2);
-#pragma unroll
-    for (int grp = 0; grp < 8; ++grp) {                  // 4 events per MMA, 8 groups per warp tile
-      const double *r = base + (8 * (grp >> 1) + (grp & 1)) * STRIDE;
-      double wv = r[F - (lane >> 2)];
-      double x[NB];
-#pragma unroll
-      for (int b = 0; b < NB; ++b) x[b] = r[8 * b];
-      int q = 0;
-#pragma unroll
-      for (int bi = 0; bi < NB; ++bi) {
-        double aw = wv * x[bi];
-#pragma unroll
-        for (int bj = bi; bj < NB; ++bj, ++q) dmma884(acc[q][0], acc[q][1], aw, x[bj]);
-      }
-    }
-    __syncwarp();                                        // the X tile is free again
-  };
-  int64_t i0 = (int64_t)blockIdx.x * STREAM_BLOCK + warp * 32;
-#pragma unroll 1
-  for (; i0 < n; i0 += stride) {
-    if (lane == 0 && i0 + stride < n) prefetch_l2_bulk(tile_event(cache, S.R, i0 + stride) + S.skip, (uint32_t)(S.R * 32 - S.skip) * 8u);
-    const double *ev = tile_event(cache, S.R, i0 + lane);
-    double wj = S.w_off >= 0 ? ldg_stream1(ev + S.w_off) : 1.0;
-    double fv[GT];
-    prefetch_f<GT>(S, ev, fv);
-    lineshapes_to_scratch<GI>(S, LP, ev, sTl);
-    columns_from_scratch<GT>(S, ev, sTl, fv, [&](int kap, double2 col) { *reinterpret_cast<double2 *>(row + 2 * kap) = col; });
-    row[F] = i0 + lane < n ? wj : 0.0;
-    mma_tile();
-  }
-  __syncthreads();                                       // all scratch is free
-  // block reduction in warp order, block partial = upper 8x8 blocks of X^T W X
-  double *Ws = reinterpret_cast<double *>(smem_raw);     // [WARPS][NB*NB][64]
-  {
-    int q = 0;
-#pragma unroll
-    for (int bi = 0; bi < NB; ++bi)
-#pragma unroll
-      for (int bj = bi; bj < NB; ++bj, ++q) {
-        double *dst = Ws + ((warp * NB + bi) * NB + bj) * 64;
-        dst[(lane >> 2) * 8 + 2 * (lane & 3)] = acc[q][0];      // C fragment: row lane/4, cols 2 (lane%4) + {0,1}
-        dst[(lane >> 2) * 8 + 2 * (lane & 3) + 1] = acc[q][1];
-      }
-  }
-  __syncthreads();
-  pdl_wait();                              // partials, ticket and G may still be in use by the predecessor
-  pdl_launch_dependents();                 // not earlier: a successor that skips its early wait relies on this kernel's
-                                           // predecessors being complete once it becomes resident
-  for (int e = tid; e < NB * NB * 64; e += STREAM_BLOCK) {
-    int bi = e / (NB * 64), bj = (e / 64) % NB;
-    if (bi > bj) continue;
-    double sum = 0.0;
-#pragma unroll
-    for (int wp = 0; wp < WARPS; ++wp) sum += Ws[wp * NB * NB * 64 + e];
-    partials[(int64_t)blockIdx.x * NB * NB * 64 + e] = sum;
-  }
-  // Two-level, fixed-order reduction over the grid.  Blocks form groups of GRAM_GROUP consecutive blocks; the last block
-  // of a group to arrive (group ticket) adds the group's partials in block order, the last group to finish (grid ticket)
-  // adds the group sums in group order.  Every level is one round of independent loads: two L2 round trips after the
-  // last block partial instead of one block pulling all gridDim.x partials (455 KB at K_c = 8) through a single SM.
-  const unsigned n_groups = (gridDim.x + GRAM_GROUP - 1) / GRAM_GROUP, grp = blockIdx.x / GRAM_GROUP;
-  const unsigned g_first = grp * GRAM_GROUP, g_size = min((unsigned)GRAM_GROUP, gridDim.x - g_first);
-  __threadfence();
-  __syncthreads();
-  if (tid == 0) last = atomicAdd(ticket + 1 + grp, 1u) == g_size - 1;
-  __syncthreads();
-  if (!last) return;
-  __threadfence();
-  double *gsum = partials + (int64_t)gridDim.x * NB * NB * 64;        // [n_groups][NB*NB*64]
-  for (int e = tid; e < NB * NB * 64; e += STREAM_BLOCK) {
-    int bi = e / (NB * 64), bj = (e / 64) % NB;
-    if (bi > bj) continue;
-    double v[GRAM_GROUP];
-#pragma unroll
-    for (int c = 0; c < GRAM_GROUP; ++c) v[c] = (unsigned)c < g_size ? __ldcg(partials + (int64_t)(g_first + c) * NB * NB * 64 + e) : 0.0;
-    double sum = 0.0;
-#pragma unroll
-    for (int c = 0; c < GRAM_GROUP; ++c) sum += v[c];
-    gsum[(int64_t)grp * NB * NB * 64 + e] = sum;
-  }
-  __threadfence();
-  __syncthreads();
-  if (tid == 0) { ticket[1 + grp] = 0; last = atomicAdd(ticket, 1u) == n_groups - 1; }
-  __syncthreads();
-  if (!last) return;
-  __threadfence();
-  double *XtX = Ws;                                      // [NB][NB][64], reused
-  for (int e = tid; e < NB * NB * 64; e += STREAM_BLOCK) {
-    int bi = e / (NB * 64), bj = (e / 64) % NB;
-    if (bi > bj) continue;
-    double sum = 0.0;
-    unsigned g = 0;
-    for (; g + 8 <= n_groups; g += 8) {
-      double v[8];
-#pragma unroll
-      for (int c = 0; c < 8; ++c) v[c] = __ldcg(gsum + (int64_t)(g + c) * NB * NB * 64 + e);
-#pragma unroll
-      for (int c = 0; c < 8; ++c) sum += v[c];
-    }
-    for (; g < n_groups; ++g) sum += __ldcg(gsum + (int64_t)g * NB * NB * 64 + e);
-    XtX[e] = sum;
-  }
-  __syncthreads();
-  auto xtx = [&](int m, int nn) {                        // symmetric: only the upper triangle is ever read
-    if (m > nn) { int tmp = m; m = nn; nn = tmp; }
-    return XtX[((m >> 3) * NB + (nn >> 3)) * 64 + (m & 7) * 8 + (nn & 7)];
-  };
-  for (int q = tid; q < KC * KC; q += STREAM_BLOCK) {
-    int kk = q / KC, l = q % KC;
-    double re = xtx(2 * kk, 2 * l) + xtx(2 * kk + 1, 2 * l + 1);
-    double im = xtx(2 * kk + 1, 2 * l) - xtx(2 * kk, 2 * l + 1);
-    if (kk == l) im = 0.0;
-    G[q * 2] = re;
-    G[q * 2 + 1] = im;
-  }
-  if (tid == 0) *ticket = 0;
 }
 
 }  // namespace tddp4k

@@ -2,11 +2,13 @@
 // Internal to csrc/; the public boundary is include/tddp4.h.
 #pragma once
 #include <stdint.h>
+#include "jit_shared.cuh"
 
 namespace tddp4k {
 
 constexpr int MAX_SYS = 12;    // distinct particle systems (2-, 3- and the 4-body one)
 constexpr int MAX_INST = 24;   // de-duplicated lineshape instances
+static_assert(MAX_INST == TDDP4_MAX_INST, "jit_shared.cuh");
 constexpr int MAX_TERMS = 32;
 constexpr int MAX_KC = 16;
 constexpr int MAX_RES = 16;
@@ -66,11 +68,6 @@ struct StreamTab {
   uint32_t term_t1[MAX_TERMS];     // ... of T_R2
   uint32_t term_col[MAX_TERMS];    // coupling column of term k (terms are sorted by coupling)
   uint32_t term_last[MAX_TERMS];   // 1: term k closes its column
-};
-
-struct LineParams {                // per set_params: T = 1 / (m0sq - s - i gam g(s)),  O-6
-  double m0sq[MAX_INST];
-  double gam[MAX_INST];            // m0^2 Gamma0 / (q0^(2L+1) F_L(z0)^2)
 };
 
 struct RateParams {                // eq. (1) and O-8
