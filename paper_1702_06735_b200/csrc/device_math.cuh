@@ -204,48 +204,4 @@ __device__ __forceinline__ void rl_candidate(const ModelTab &M, double tau, uint
   t = -tau * log(1.0 - ut);
 }
 
-// eq. (1): bracket B from A, Abar and the mixing phases u = y Gamma t, v = x Gamma t.
-// SMALL (|u|, |v| < 1/4, guaranteed by the host): cosh, sinh, cos, sin as Taylor polynomials up to u^12 / u^13;
-// the first omitted term is below 4e-20 of the leading one.
-// the four time functions of eq. (1) at mixing phases u = y Gamma t, v = x Gamma t
-template <bool SMALL>
-__device__ __forceinline__ void mixing_functions(double u, double v, double &ch, double &sh, double &cs, double &sn) {
-  if (SMALL) {
-    const double c2 = 1.0 / 2, c4 = 1.0 / 24, c6 = 1.0 / 720, c8 = 1.0 / 40320, c10 = 1.0 / 3628800, c12 = 1.0 / 479001600;
-    const double s3 = 1.0 / 6, s5 = 1.0 / 120, s7 = 1.0 / 5040, s9 = 1.0 / 362880, s11 = 1.0 / 39916800, s13 = 1.0 / 6227020800.0;
-    double u2 = u * u, v2 = v * v;
-    ch = fma(u2, fma(u2, fma(u2, fma(u2, fma(u2, fma(u2, c12, c10), c8), c6), c4), c2), 1.0);
-    sh = u * fma(u2, fma(u2, fma(u2, fma(u2, fma(u2, fma(u2, s13, s11), s9), s7), s5), s3), 1.0);
-    cs = fma(v2, fma(v2, fma(v2, fma(v2, fma(v2, fma(v2, c12, -c10), c8), -c6), c4), -c2), 1.0);
-    sn = v * fma(v2, fma(v2, fma(v2, fma(v2, fma(v2, fma(v2, s13, -s11), s9), -s7), s5), -s3), 1.0);
-  } else {
-    double e = exp(u), ei = 1.0 / e;
-    ch = 0.5 * (e + ei);
-    sh = 0.5 * (e - ei);
-    sincos(v, &sn, &cs);
-  }
-}
-// |A|^2, |Abar|^2, Re(A conj(Abar)), Im(A conj(Abar)) and the bracket itself with every contraction written out
-// (fma / __dmul_rn): the NLL, column-rebuilding and gradient kernels must produce the same bits for the same event, and
-// nvcc's default -fmad=true would otherwise be free to contract the sums differently per template instantiation.
-struct Bilinears { double aa, bb, cre, cim; };
-__device__ __forceinline__ Bilinears bilinears(double2 A, double2 Ab) {
-  Bilinears q;
-  q.aa = fma(A.x, A.x, __dmul_rn(A.y, A.y));
-  q.bb = fma(Ab.x, Ab.x, __dmul_rn(Ab.y, Ab.y));
-  q.cre = fma(A.x, Ab.x, __dmul_rn(A.y, Ab.y));
-  q.cim = fma(A.y, Ab.x, -__dmul_rn(A.x, Ab.y));
-  return q;
-}
-// (aa + bb) f0 + (aa - bb) f1 - 2 cre f2 - 2 cim f3: eq. (1) with f = (cosh, cos, sinh, sin), or its convolved / integrated forms
-__device__ __forceinline__ double rate_form(const Bilinears &q, double f0, double f1, double f2, double f3) {
-  return fma(__dadd_rn(q.aa, q.bb), f0, fma(__dsub_rn(q.aa, q.bb), f1, fma(-2.0 * q.cre, f2, __dmul_rn(-2.0 * q.cim, f3))));
-}
-template <bool SMALL>
-__device__ __forceinline__ double bracket(double2 A, double2 Ab, double u, double v) {
-  double ch, sh, sn, cs;
-  mixing_functions<SMALL>(u, v, ch, sh, cs, sn);
-  return rate_form(bilinears(A, Ab), ch, cs, sh, sn);
-}
-
 }  // namespace tddp4k

@@ -24,7 +24,7 @@
 
 namespace tddp4k {
 
-constexpr int JG_BLOCK = 256, JG_WARPS = JG_BLOCK / 32;
+constexpr int JG_BLOCK = 256;
 
 extern "C" __global__ void __launch_bounds__(JG_BLOCK, J_BPS)
 gram_jit(const __grid_constant__ LineParams LP, const double *__restrict__ cache, long long n,

@@ -8,11 +8,6 @@ namespace tddp4k {
 
 // ------------------------------------------------------------------------------------------------
 // deterministic block reductions (fixed shuffle tree, then warp 0 over the warp partials)
-__device__ __forceinline__ double warp_sum(double v) {
-#pragma unroll
-  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
-  return v;
-}
 template <int BLOCK>
 __device__ __forceinline__ double block_sum(double v, double *red /* [BLOCK/32] shared */) {
   v = warp_sum(v);

@@ -2,7 +2,7 @@
 // Internal to csrc/; the public boundary is include/tddp4.h.
 #pragma once
 #include <stdint.h>
-#include "jit_shared.cuh"
+#include "nll_shared.cuh"
 
 namespace tddp4k {
 
@@ -11,6 +11,7 @@ constexpr int MAX_INST = 24;   // de-duplicated lineshape instances (PAPER.md li
 static_assert(MAX_INST == TDDP4_MAX_INST, "jit_shared.cuh");
 constexpr int MAX_TERMS = 32;
 constexpr int MAX_KC = 16;
+static_assert(MAX_KC == TDDP4_MAX_KC, "nll_shared.cuh");
 constexpr int MAX_RES = 16;
 
 enum { SF_NONRES = 0, SF_VV_S = 1, SF_VV_P = 2, SF_VV_D = 3, SF_AP_S = 4, SF_TP_D = 5, SF_AP_D = 6 };
@@ -68,15 +69,6 @@ struct StreamTab {
   uint32_t term_t1[MAX_TERMS];     // ... of T_R2
   uint32_t term_col[MAX_TERMS];    // coupling column of term k (terms are sorted by coupling)
   uint32_t term_last[MAX_TERMS];   // 1: term k closes its column
-};
-
-struct RateParams {                // eq. (1) and O-8
-  double c[MAX_KC][2];
-  double cbar[MAX_KC][2];
-  double x, y, Gamma;
-  double T[4];                     // time integrals of cosh, cos, sinh, sin terms over the window
-  double t_lo, t_hi;
-  int use_resolution;
 };
 
 }  // namespace tddp4k
