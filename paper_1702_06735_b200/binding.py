@@ -26,7 +26,7 @@ SYMBOLS = ["tddp4_create", "tddp4_destroy", "tddp4_set_stream", "tddp4_last_erro
            "tddp4_nll_parts", "tddp4_nll_grad", "tddp4_param_stride", "tddp4_nll_batch", "tddp4_gram", "tddp4_gram_override", "tddp4_norm", "tddp4_generate", "tddp4_weight_bound",
            "tddp4_candidates", "tddp4_get", "tddp4_layout", "tddp4_profile", "tddp4_profile_read",
            "tddp4_profile_reset", "tddp4_launch_count", "tddp4_gram_enqueue", "tddp4_gram_reduce", "tddp4_nll_enqueue",
-           "tddp4_gram_state", "tddp4_fp64_peak", "tddp4_project"]
+           "tddp4_gram_state", "tddp4_fp64_peak", "tddp4_project", "tddp4_jit_source"]
 
 
 class Tddp4Error(RuntimeError):
@@ -97,6 +97,8 @@ def load_library():
     L.tddp4_nll_enqueue.argtypes = [vp, vp]
     L.tddp4_gram_state.argtypes = [vp, C.POINTER(C.c_int), C.POINTER(C.c_int)]
     L.tddp4_fp64_peak.argtypes = [vp, dp]
+    L.tddp4_jit_source.argtypes = [C.POINTER(_Desc), C.c_int, C.c_int, C.c_int, C.c_char_p, i64]
+    L.tddp4_jit_source.restype = i64
     L.tddp4_project.argtypes = [vp, i64, i64, vp, C.c_int, vp, vp, vp]
     _lib = L
     return L
@@ -109,6 +111,43 @@ def _ptr(t):
     if isinstance(t, np.ndarray):
         return t.ctypes.data
     return t.data_ptr()
+
+
+def _make_desc(model):
+    """workloads.Model-like object -> (tddp4_model_desc, the ctypes arrays it points to)."""
+    res = (_Res * max(1, model.n_res))()
+    radii = getattr(model, "res_r", None) or [0.0] * model.n_res
+    kinds = getattr(model, "res_lineshape", None) or [0] * model.n_res
+    for r, L in enumerate(model.res_L):
+        res[r].L, res[r].lineshape, res[r].r = L, kinds[r], radii[r]
+    terms = (_Term * model.n_terms)()
+    for k in range(model.n_terms):
+        terms[k].spin_factor = model.term_sf[k]
+        terms[k].res[0], terms[k].res[1] = model.term_res[k]
+        for r in range(4):
+            terms[k].perm[r] = model.term_perm[k][r]
+        terms[k].coupling = model.term_coupling[k]
+    d = _Desc()
+    d.m_parent = model.m_parent
+    for i in range(4):
+        d.m_final[i] = model.m_final[i]
+    d.r_res, d.r_parent = model.r_res, model.r_parent
+    d.n_res, d.res, d.n_terms, d.terms = model.n_res, res, model.n_terms, terms
+    d.n_couplings, d.t_lo, d.t_hi, d.use_resolution = model.n_couplings, model.t_lo, model.t_hi, model.use_resolution
+    return d, (res, terms)
+
+
+def jit_source(model, what, weighted=False, mode=1):
+    """tddp4_jit_source: the CUDA text the library hands to NVRTC for this model (what = 0 Gram pass, 1 data pass) or one
+    of the headers it includes (2 jit_shared.cuh, 3 nll_shared.cuh).  Needs no GPU."""
+    lib = load_library()
+    d, keep = _make_desc(model)
+    need = lib.tddp4_jit_source(C.byref(d), what, int(weighted), mode, None, 0)
+    if need < 0:
+        raise Tddp4Error(int(need), "tddp4_jit_source")
+    buf = C.create_string_buffer(int(need))
+    lib.tddp4_jit_source(C.byref(d), what, int(weighted), mode, buf, need)
+    return buf.value.decode()
 
 
 class Tddp4:
@@ -127,25 +166,7 @@ class Tddp4:
         torch.zeros(1, device=self.device)           # make sure the primary context exists
         self.model = model
         self.n_res, self.n_terms, self.kc = model.n_res, model.n_terms, model.n_couplings
-        res = (_Res * max(1, model.n_res))()
-        radii = getattr(model, "res_r", None) or [0.0] * model.n_res
-        kinds = getattr(model, "res_lineshape", None) or [0] * model.n_res
-        for r, L in enumerate(model.res_L):
-            res[r].L, res[r].lineshape, res[r].r = L, kinds[r], radii[r]
-        terms = (_Term * model.n_terms)()
-        for k in range(model.n_terms):
-            terms[k].spin_factor = model.term_sf[k]
-            terms[k].res[0], terms[k].res[1] = model.term_res[k]
-            for r in range(4):
-                terms[k].perm[r] = model.term_perm[k][r]
-            terms[k].coupling = model.term_coupling[k]
-        d = _Desc()
-        d.m_parent = model.m_parent
-        for i in range(4):
-            d.m_final[i] = model.m_final[i]
-        d.r_res, d.r_parent = model.r_res, model.r_parent
-        d.n_res, d.res, d.n_terms, d.terms = model.n_res, res, model.n_terms, terms
-        d.n_couplings, d.t_lo, d.t_hi, d.use_resolution = model.n_couplings, model.t_lo, model.t_hi, model.use_resolution
+        d, self._desc_keep = _make_desc(model)
         self._h = C.c_void_p()
         rc = self.lib.tddp4_create(C.byref(d), C.byref(self._h))
         if rc != OK:

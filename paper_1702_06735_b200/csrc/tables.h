@@ -51,24 +51,16 @@ struct ModelTab {
   double r_res2, r_parent2;        // default resonance radius and parent radius, squared, GeV^-2
 };
 
-// The per-call kernels' view of the model and of the static cache.  The cache of one event set is ONE tile-major array:
-// tile = 32 consecutive events, R rows of 32 doubles each (256 B per row per tile), rows ordered
-//   [ s: n_sys | g: n_inst4 | f: n_terms4 | w (if weighted) ],
+// The static cache of one event set is ONE tile-major array: tile = 32 consecutive events, R rows of 32 doubles each
+// (256 B per row per tile), rows ordered
+//   [ s: n_sys | g: n_inst | f: n_terms | w (if weighted) ],
 // element (row r, event i) at ((i >> 5) * R + r) * 32 + (i & 31).  A warp working on one tile therefore addresses every
-// row as tile base + lane + CONSTANT, and the whole tile is one contiguous R * 256-byte region of HBM.
-// Every table entry is a 32-bit word so that an unrolled loop uses it as an immediate-indexed constant-bank operand.
-// Instances and terms are padded to multiples of the size class's load-batch sizes (GI, GT) (group-level guards only) with all-zero rows: a padded instance
-// reads s row 0 and m0sq = -1, gam = 0 (finite, unused); a padded term has f = 0 and the unit lineshape slot.
-struct StreamTab {
-  int n_inst4, n_terms4, n_kc;     // padded counts
-  int R;                           // rows per tile
-  int g_off, f_off, w_off;         // element offsets (row * 32) of the first g row, first f row, weight row (-1: none)
-  int skip;                        // element offset of the first row the kernels read (unused s rows come first)
-  uint32_t inst_soff[MAX_INST];    // element offset of the s row lineshape instance j reads
-  uint32_t term_t0[MAX_TERMS];     // element offset (slot * 32) of T_R1 in the warp's lineshape scratch; unit slot if none
-  uint32_t term_t1[MAX_TERMS];     // ... of T_R2
-  uint32_t term_col[MAX_TERMS];    // coupling column of term k (terms are sorted by coupling)
-  uint32_t term_last[MAX_TERMS];   // 1: term k closes its column
+// row as tile base + lane + CONSTANT, and the whole tile is one contiguous R * 256-byte region of HBM.  The fused
+// per-call kernels get these offsets (and the model tables) as compile-time constants (jit_prelude in tddp4_api.cu).
+struct CacheLayout {
+  int R;                           // rows per tile of an unweighted event set (+ 1 with weights)
+  int g_off, f_off;                // element offsets (row * 32) of the first g row and the first f row
+  int skip;                        // element offset of the first row the per-call kernels read (unused s rows come first)
 };
 
 }  // namespace tddp4k
