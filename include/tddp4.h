@@ -260,8 +260,8 @@ int tddp4_fp64_peak(tddp4 *h, double *inst_per_s);
 /* The CUDA source of a kernel the library specialises to a model and compiles at run time with NVRTC (the two fused
  * passes over the static caches: what = 0 the Gram pass, 8(a) rows 2+3+6; what = 1 the data pass after a mass/width move,
  * rows 2..5+7; the model's table of shared lineshape / spin-factor instances becomes compile-time
- * constants), or of a header these include (what = 2 "jit_shared.cuh", 3 "nll_shared.cuh"; desc may then be any valid
- * model).  weighted: the event set carries a weight row; mode (what = 1): 0 full-range time functions, 1 small mixing
+ * constants; what = 4 the candidate kernel of the generator, G1-G5), or of a header these include (what = 2
+ * "jit_shared.cuh", 3 "nll_shared.cuh", 5 "tables.h", 6 "device_math.cuh"; desc may then be any valid model).  weighted: the event set carries a weight row; mode (what = 1): 0 full-range time functions, 1 small mixing
  * phases, 2 resolution / time-integrated rows.  Needs NO device: it is what tddp4_create hands to NVRTC, exposed so that
  * a build check can compile it.  Host buf of cap bytes (may be NULL with cap = 0); returns the size needed including the
  * terminating NUL (the text is written only if it fits), or a negative tddp4_status.                              */

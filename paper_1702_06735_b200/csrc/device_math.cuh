@@ -2,7 +2,6 @@
 // Philox4x32-10 and Raubold-Lynch generation as __device__ functions (sm_100a).
 // Formulas: SURVEY.md 8(c) O-3 .. O-9 (the paper prints none of them).
 #pragma once
-#include <stdint.h>
 #include "tables.h"
 
 namespace tddp4k {
@@ -36,20 +35,24 @@ __device__ __forceinline__ double breakup2(double M, double s, double ma, double
 // un-normalised Blatt-Weisskopf factor F_L(z) (O-5)
 __device__ __forceinline__ double barrier(int L, double z) {
   if (L == 0) return 1.0;
-  if (L == 1) return 1.0 / sqrt(1.0 + z);
-  return 1.0 / sqrt(9.0 + 3.0 * z + z * z);
+  if (L == 1) return rsqrt_pos(1.0 + z);
+  return rsqrt_pos(9.0 + 3.0 * z + z * z);
 }
 
 // parameter-free shape of the running width: g = q^(2L+1) F_L(z)^2 / sqrt(s), so that
 // m0 Gamma(s) = gam * g with gam = m0^2 Gamma0 / (q0^(2L+1) F_L(z0)^2)   (O-6)
 __device__ __forceinline__ double width_shape(int L, double q2, double z, double M) {
-  double q = sqrt(q2);
-  if (L == 0) return q / M;
-  if (L == 1) return q * q2 / ((1.0 + z) * M);
-  return q * q2 * q2 / ((9.0 + 3.0 * z + z * z) * M);
+  double q = sqrt_pos(q2);
+  if (L == 0) return q * rcp_normal(M);
+  if (L == 1) return q * q2 * rcp_normal((1.0 + z) * M);
+  return q * q2 * q2 * rcp_normal((9.0 + 3.0 * z + z * z) * M);
 }
 
-// closed-form spin factors (O-4), role vectors r0..r3 already gathered
+// closed-form spin factors (O-4), role vectors r0..r3 already gathered.  IEEE divisions and square roots here, in L1, in
+// breakup2 and for the invariant-mass roots: these quantities are differences of nearly equal terms for events next to a
+// threshold, and the full-size parity (1e-10 on every P_i of 10 M events) has no room for a second ulp there.  The
+// branch-free forms (jit_shared.cuh) are used where the result only multiplies: barrier factors, width shape, the
+// boosts and two-body decays of the generator.
 __device__ __forceinline__ double spin_factor(int sf, V4 r0, V4 r1, V4 r2, V4 r3) {
   if (sf == SF_NONRES) return 1.0;
   if (sf <= SF_VV_D) {
@@ -159,26 +162,27 @@ __device__ __forceinline__ void uniform_pair(uint64_t seed, uint64_t index, uint
 
 __device__ __forceinline__ double breakup_excess(double excess, double M, double ma, double mb) {
   double rad = excess * (M + ma + mb) * (M + ma - mb) * (M - ma + mb);
-  return rad > 0.0 ? sqrt(rad) / (2.0 * M) : 0.0;
+  return rad > 0.0 ? div_normal(sqrt_pos(rad), 2.0 * M) : 0.0;
 }
 // E' = (E_P E + P.p)/M ; p' = p + P [ (P.p)/(M (E_P + M)) + E/M ]   (O-9)
 __device__ __forceinline__ V4 boost(V4 P, double M, V4 p) {
   double Pp = P.x * p.x + P.y * p.y + P.z * p.z;
-  double f = Pp / (M * (P.e + M)) + p.e / M;
-  return {(P.e * p.e + Pp) / M, p.x + P.x * f, p.y + P.y * f, p.z + P.z * f};
+  const double iM = rcp_normal(M);
+  double f = div_normal(Pp, M * (P.e + M)) + div_by(p.e, iM, M);
+  return {div_by(P.e * p.e + Pp, iM, M), p.x + P.x * f, p.y + P.y * f, p.z + P.z * f};
 }
 __device__ __forceinline__ void two_body(double m_first, double m_second, double ps, double u_cos, double u_phi,
                                          V4 &first, V4 &second) {
   double ct = 2.0 * u_cos - 1.0;
-  double st = sqrt(1.0 - ct * ct);
+  double st = sqrt_pos(1.0 - ct * ct);
   double sphi, cphi;
   sincospi(2.0 * u_phi, &sphi, &cphi);   // phi = 2 pi u: exact argument reduction, no multiple-of-pi rounding
   double nx = st * cphi, ny = st * sphi, nz = ct;
-  first = {sqrt(m_first * m_first + ps * ps), ps * nx, ps * ny, ps * nz};
-  second = {sqrt(m_second * m_second + ps * ps), -ps * nx, -ps * ny, -ps * nz};
+  first = {sqrt_pos(m_first * m_first + ps * ps), ps * nx, ps * ny, ps * nz};
+  second = {sqrt_pos(m_second * m_second + ps * ps), -ps * nx, -ps * ny, -ps * nz};
 }
 // G2/G3: one Raubold-Lynch candidate (O-9).  p[0..3]: final-state momenta in the D rest frame.
-__device__ __forceinline__ void rl_candidate(const ModelTab &M, double tau, uint64_t seed, uint32_t stream,
+__device__ __forceinline__ void rl_candidate(const double (&mf)[4], double m_parent, double tau, uint64_t seed, uint32_t stream,
                                              uint64_t i, V4 p[4], double &t, double &w, double &u_acc) {
   double ra, rb, c1, f1, c2, f2, c3, f3, ut;
   uniform_pair(seed, i, 0, stream, ra, rb);
@@ -186,10 +190,9 @@ __device__ __forceinline__ void rl_candidate(const ModelTab &M, double tau, uint
   uniform_pair(seed, i, 2, stream, c2, f2);
   uniform_pair(seed, i, 3, stream, c3, f3);
   uniform_pair(seed, i, 4, stream, ut, u_acc);
-  const double *mf = M.m_final;
   double r1 = fmin(ra, rb), r2 = fmax(ra, rb);
-  double Tk = M.m_parent - (mf[0] + mf[1] + mf[2] + mf[3]);
-  double M2 = mf[0] + mf[1] + r1 * Tk, M3 = mf[0] + mf[1] + mf[2] + r2 * Tk, M4 = M.m_parent;
+  double Tk = m_parent - (mf[0] + mf[1] + mf[2] + mf[3]);
+  double M2 = mf[0] + mf[1] + r1 * Tk, M3 = mf[0] + mf[1] + mf[2] + r2 * Tk, M4 = m_parent;
   double ps1 = breakup_excess((1.0 - r2) * Tk, M4, M3, mf[3]);
   double ps2 = breakup_excess((r2 - r1) * Tk, M3, M2, mf[2]);
   double ps3 = breakup_excess(r1 * Tk, M2, mf[0], mf[1]);

@@ -200,114 +200,9 @@ __global__ void __launch_bounds__(1024) stat_kernel(const double *__restrict__ v
 namespace tddp4k {
 
 // ------------------------------------------------------------------------------------------------
-// G1-G4: candidate generation and rate on the fly (no caches).  One thread per candidate.
+// G1-G5: candidate generation with the rate evaluated on the fly is the run-time specialised kernel of gen_jit.cuh
+// (one thread per candidate, GEN_BLOCK candidates per block: flags and block counts below are laid out for it).
 constexpr int GEN_BLOCK = 128;
-// The sink turns each shape function into T_R at once and folds each static factor into the coupling
-// column it belongs to, so only p, s, q^2 and T_R live in shared memory (terms are sorted by coupling).
-struct GenSink {
-  const ModelTab &M; const LineParams &LP; const RateParams &R; const Scratch &sc;
-  double2 *sT;
-  int tid, kap;
-  double2 A, Ab, col;
-  __device__ __forceinline__ void s(int, double) {}
-  __device__ __forceinline__ void g(int j, double gv) {
-    sT[j * GEN_BLOCK + tid] = breit_wigner(LP.m0sq[j], LP.gam[j], sc.S(M.inst[j].sys, tid), gv);
-  }
-  __device__ __forceinline__ void flush() {
-    A.x += R.c[kap][0] * col.x - R.c[kap][1] * col.y;
-    A.y += R.c[kap][0] * col.y + R.c[kap][1] * col.x;
-    Ab.x += R.cbar[kap][0] * col.x - R.cbar[kap][1] * col.y;
-    Ab.y += R.cbar[kap][0] * col.y + R.cbar[kap][1] * col.x;
-    col = make_double2(0.0, 0.0);
-    ++kap;
-  }
-  __device__ __forceinline__ void f(int k, double fv) {
-    while (k >= M.col_begin[kap + 1]) flush();
-    const TermTab &tm = M.term[k];
-    double2 T = make_double2(1.0, 0.0);
-    if (tm.inst0 >= 0) T = cmul(sT[tm.inst0 * GEN_BLOCK + tid], sT[tm.inst1 * GEN_BLOCK + tid]);
-    col.x += fv * T.x; col.y += fv * T.y;
-  }
-};
-// shared memory per block: p[16], s[n_sys], q2[n_inst] (double rows), T[n_inst] (double2 rows)
-__host__ __device__ inline size_t gen_smem_bytes(int n_sys, int n_inst) {
-  return sizeof(double) * (size_t)(16 + n_sys + 3 * n_inst) * GEN_BLOCK;
-}
-
-__device__ __forceinline__ double candidate_ratio(const ModelTab &M, const LineParams &LP, const RateParams &R,
-                                                  double *smem, int tid, const V4 p[4], double t, double w) {
-  Scratch sc{smem, smem + 16 * GEN_BLOCK, smem + (16 + M.n_sys) * GEN_BLOCK, GEN_BLOCK};
-  double2 *sT = reinterpret_cast<double2 *>(smem + (16 + M.n_sys + M.n_inst) * GEN_BLOCK);
-#pragma unroll
-  for (int a = 0; a < 4; ++a) {
-    sc.P(4 * a, tid) = p[a].e; sc.P(4 * a + 1, tid) = p[a].x; sc.P(4 * a + 2, tid) = p[a].y; sc.P(4 * a + 3, tid) = p[a].z;
-  }
-  GenSink sink{M, LP, R, sc, sT, tid, 0, make_double2(0.0, 0.0), make_double2(0.0, 0.0), make_double2(0.0, 0.0)};
-  kinematics(M, sc, tid, sink);
-  sink.flush();
-  return w * bracket<false>(sink.A, sink.Ab, R.y * R.Gamma * t, R.x * R.Gamma * t);
-}
-
-// mode 0: raw candidate dump (parity); mode 1: pilot maximum (G5); mode 2: accept flags + block counts (G6)
-__global__ void __launch_bounds__(GEN_BLOCK, 4)
-gen_ratio_kernel(const __grid_constant__ ModelTab M, const __grid_constant__ LineParams LP,
-                 const __grid_constant__ RateParams R, double tau, uint64_t seed, uint32_t stream, uint64_t first,
-                 int64_t n, int mode, double envelope /* mode 2: the envelope, or its scale if from_pilot */, int from_pilot,
-                 double *__restrict__ out_p4, double *__restrict__ out_t, double *__restrict__ out_w,
-                 double *__restrict__ out_ratio, double *__restrict__ out_u,
-                 unsigned long long *pilot_max_bits, uint32_t *__restrict__ flags /* one bit per candidate */,
-                 uint32_t *__restrict__ block_count, unsigned long long *overflow) {
-  extern __shared__ double smem[];
-  __shared__ int s_cnt[GEN_BLOCK / 32];
-  int tid = threadIdx.x;
-  int64_t j = (int64_t)blockIdx.x * GEN_BLOCK + tid;
-  bool live = j < n;
-  V4 p[4];
-  double t = 0.0, w = 0.0, u = 1.0, rho = 0.0;
-  if (live) {
-    rl_candidate(M, tau, seed, stream, first + (uint64_t)j, p, t, w, u);
-    rho = candidate_ratio(M, LP, R, smem, tid, p, t, w);
-  }
-  if (mode == 0) {
-    if (!live) return;
-    if (out_p4) {
-#pragma unroll
-      for (int a = 0; a < 4; ++a) {
-        out_p4[(4 * a) * n + j] = p[a].e; out_p4[(4 * a + 1) * n + j] = p[a].x;
-        out_p4[(4 * a + 2) * n + j] = p[a].y; out_p4[(4 * a + 3) * n + j] = p[a].z;
-      }
-    }
-    if (out_t) out_t[j] = t;
-    if (out_w) out_w[j] = w;
-    if (out_ratio) out_ratio[j] = rho;
-    if (out_u) out_u[j] = u;
-    return;
-  }
-  if (mode == 1) {
-    // rho >= 0: the IEEE bit pattern is monotone, so an integer max is the exact fp64 max
-    double m = live && rho > 0.0 ? rho : 0.0;
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) m = fmax(m, __shfl_xor_sync(0xffffffffu, m, o));
-    if ((tid & 31) == 0) atomicMax(pilot_max_bits, (unsigned long long)__double_as_longlong(m));
-    return;
-  }
-  if (from_pilot) envelope *= __longlong_as_double((long long)*pilot_max_bits);   // E = scale * max over the pilot (G5), no host round trip
-  bool acc = live && (u * envelope < rho);
-  unsigned ballot = __ballot_sync(0xffffffffu, acc);
-  unsigned over = __ballot_sync(0xffffffffu, live && rho > envelope);
-  if ((tid & 31) == 0) {
-    flags[j >> 5] = ballot;
-    s_cnt[tid >> 5] = __popc(ballot);
-    if (over) atomicAdd(overflow, (unsigned long long)__popc(over));
-  }
-  __syncthreads();
-  if (tid == 0) {
-    int c = 0;
-#pragma unroll
-    for (int k = 0; k < GEN_BLOCK / 32; ++k) c += s_cnt[k];
-    block_count[blockIdx.x] = c;
-  }
-}
 
 // exclusive scan of the block counts of one launch chunk (single block), continued from the running total of the
 // chunks before it: offs[b] = *total + sum_{b' < b} cnt[b'], and *total advances by the chunk's count (no host round trip)
@@ -375,7 +270,7 @@ gen_emit_kernel(const __grid_constant__ ModelTab M, double tau, uint64_t seed, u
     const int64_t j = j0 + s_list[k];
     V4 p[4];
     double t, w, u;
-    rl_candidate(M, tau, seed, stream, first + (uint64_t)j, p, t, w, u);
+    rl_candidate(M.m_final, M.m_parent, tau, seed, stream, first + (uint64_t)j, p, t, w, u);
     if (out_p4) {
 #pragma unroll
       for (int a = 0; a < 4; ++a) {

@@ -1,7 +1,12 @@
 // tables.h -- plain-data tables handed to the kernels by value (they live in the constant bank).
 // Internal to csrc/; the public boundary is include/tddp4.h.
 #pragma once
+#ifdef __CUDACC_RTC__       // NVRTC has no system headers (this file is also part of run-time compiled programs, jit.h)
+typedef signed char int8_t; typedef unsigned char uint8_t; typedef int int32_t; typedef unsigned int uint32_t;
+typedef long long int64_t; typedef unsigned long long uint64_t;
+#else
 #include <stdint.h>
+#endif
 #include "nll_shared.cuh"
 
 namespace tddp4k {

@@ -1,4 +1,4 @@
-"""CPU-side build check of the run-time specialised kernels (gram_jit.cuh, colnll_jit.cuh): the text tddp4_create hands
+"""CPU-side build check of the run-time specialised kernels (gram_jit.cuh, colnll_jit.cuh, gen_jit.cuh): the text tddp4_create hands
 to NVRTC -- the generated prelude of model tables + the kernel file -- is obtained through the C-ABI
 (tddp4_jit_source, no device needed) for every workload model and compiled here for sm_100a with NVRTC.  The cubins must
 keep the lineshapes in registers (no local memory), and the Gram pass must contain fp64 tensor-core instructions."""
@@ -19,9 +19,9 @@ def _lib():
 
 
 def compile_sm100a(source, name, tmp_path):
-    headers = [binding.jit_source(W.config(1).model, 2).encode(), binding.jit_source(W.config(1).model, 3).encode()]
-    names = [b"jit_shared.cuh", b"nll_shared.cuh"]
-    err, prog = nvrtc.nvrtcCreateProgram(source.encode(), name.encode(), 2, headers, names)
+    names = {b"jit_shared.cuh": 2, b"nll_shared.cuh": 3, b"tables.h": 5, b"device_math.cuh": 6}
+    headers = [binding.jit_source(W.config(1).model, what).encode() for what in names.values()]
+    err, prog = nvrtc.nvrtcCreateProgram(source.encode(), name.encode(), len(names), headers, list(names))
     assert err == nvrtc.nvrtcResult.NVRTC_SUCCESS
     opts = [b"--gpu-architecture=sm_100a", b"--std=c++17", b"-lineinfo"]
     (res,) = nvrtc.nvrtcCompileProgram(prog, len(opts), opts)
@@ -68,6 +68,14 @@ def test_data_pass_compiles_for_sm100a(name, tmp_path):
         assert m and int(m.group(1)) <= 128, usage
         if mode != 0:          # mode 0 calls sincos, whose large-argument path keeps a table on the stack
             assert int(m.group(2)) == 0 and "LDL" not in sass and "STL" not in sass, usage
+
+
+@pytest.mark.parametrize("name", ["C1", "C3", "flat"])
+def test_generator_kernel_compiles_for_sm100a(name, tmp_path):
+    usage, sass = compile_sm100a(binding.jit_source(models()[name], 4), f"gen_{name}", str(tmp_path))
+    m = re.search(r"REG:(\d+) STACK:(\d+)", usage)
+    assert m and int(m.group(1)) <= 80, usage          # six blocks of 128 threads per SM
+    assert "MUFU.RSQ64H" in sass and "MUFU.RCP64H" in sass
 
 
 def test_prelude_states_the_model_tables():
