@@ -96,73 +96,61 @@ __device__ __forceinline__ bool grad_reduce(double (&acc)[NB][2], double (&sc)[N
     m.renorm();
     mine[NA] = m.prod; mine[NA + 1] = (double)m.esum; mine[NA + 2] = (double)m.bad;
   }
+  // Two-level, fixed-order reduction over the grid (as the Gram kernel's, jit_shared.cuh): blocks form groups of GRAM_GROUP
+  // consecutive blocks; the last block of a group to arrive adds the group's partials in block order, the last group to
+  // finish adds the group sums in group order.  Every level is one round of independent loads.  (The single-level form --
+  // one block pulling gridDim.x x PS doubles, 163 KB at K_c = 8, through one SM in five rounds -- left the SMs idle for a
+  // third of the launch: ncu sm__cycles_active 61 k of 91 k elapsed cycles at 1 M events.)
+  const unsigned n_groups = (gridDim.x + GRAM_GROUP - 1) / GRAM_GROUP, grp = blockIdx.x / GRAM_GROUP;
+  const unsigned g_first = grp * GRAM_GROUP, g_size = min((unsigned)GRAM_GROUP, gridDim.x - g_first);
+  double *gsum = partials + (int64_t)gridDim.x * PS;               // [n_groups][PS]
   __threadfence();
   __syncthreads();
-  if (tid == 0) *last = atomicAdd(ticket, 1u) == gridDim.x - 1;
+  if (tid == 0) *last = atomicAdd(ticket + 1 + grp, 1u) == g_size - 1;
   __syncthreads();
   if (!*last) return false;
   __threadfence();
-  // last block: column sums over the block partials.  Warp w takes the blocks b = w, w + WARPS, ...; its lanes cover the
-  // entries j = lane, lane + 32, ... (coalesced rows of the partial array), every load independent of the others, eight
-  // blocks in flight per lane; the warps' sums are then added in warp order.  Fixed tree: same bits every run.  (The
-  // first version gave each entry to one thread that walked all blocks in rounds of 16 loads: 66 busy threads, 19
-  // dependent L2 round trips -- about 25 of the kernel's 57 us at 1 M events, measured as SM-active time with ncu.)
-  {
-    constexpr int SLOTS = (NA + 31) / 32;
-    double sum[SLOTS];
-#pragma unroll
-    for (int q = 0; q < SLOTS; ++q) sum[q] = 0.0;
-    unsigned b = warp;
-    for (; b + 7 * STREAM_WARPS < gridDim.x; b += 8 * STREAM_WARPS) {
-      double v[8][SLOTS];
-#pragma unroll
-      for (int r = 0; r < 8; ++r)
-#pragma unroll
-        for (int q = 0; q < SLOTS; ++q) {
-          const int j = lane + 32 * q;
-          v[r][q] = j < NA ? __ldcg(partials + (int64_t)(b + r * STREAM_WARPS) * PS + j) : 0.0;
-        }
-#pragma unroll
-      for (int r = 0; r < 8; ++r)
-#pragma unroll
-        for (int q = 0; q < SLOTS; ++q) sum[q] += v[r][q];
-    }
-    for (; b < gridDim.x; b += STREAM_WARPS) {
-#pragma unroll
-      for (int q = 0; q < SLOTS; ++q) {
-        const int j = lane + 32 * q;
-        if (j < NA) sum[q] += __ldcg(partials + (int64_t)b * PS + j);
-      }
-    }
-    __syncthreads();                                        // s_red of the first stage is free
-#pragma unroll
-    for (int q = 0; q < SLOTS; ++q) {
-      const int j = lane + 32 * q;
-      if (j < NA) s_red[warp * NA + j] = sum[q];
-    }
-  }
-  __syncthreads();
   for (int j = tid; j < NA; j += STREAM_BLOCK) {
-    double v = 0.0;
+    double v[GRAM_GROUP];
 #pragma unroll
-    for (int w = 0; w < STREAM_WARPS; ++w) v += s_red[w * NA + j];
-    s_sum[j] = v;
+    for (int c = 0; c < GRAM_GROUP; ++c) v[c] = (unsigned)c < g_size ? __ldcg(partials + (int64_t)(g_first + c) * PS + j) : 0.0;
+    double sum = 0.0;
+#pragma unroll
+    for (int c = 0; c < GRAM_GROUP; ++c) sum += v[c];
+    gsum[(int64_t)grp * PS + j] = sum;
+  }
+  if (warp == STREAM_WARPS - 1) {                                  // the group's mantissa product: one lane per block
+    MantAcc m;
+    if ((unsigned)lane < g_size) {
+      const double *src = partials + (int64_t)(g_first + lane) * PS + NA;
+      m.merge(__ldcg(src), (long long)__ldcg(src + 1), (int)__ldcg(src + 2));
+    }
+    warp_merge(m);
+    if (lane == 0) { double *dst = gsum + (int64_t)grp * PS + NA; dst[0] = m.prod; dst[1] = (double)m.esum; dst[2] = (double)m.bad; }
+  }
+  __threadfence();
+  __syncthreads();
+  if (tid == 0) { ticket[1 + grp] = 0; *last = atomicAdd(ticket, 1u) == n_groups - 1; }
+  __syncthreads();
+  if (!*last) return false;
+  __threadfence();
+  for (int j = tid; j < NA; j += STREAM_BLOCK) {
+    double sum = 0.0;
+    unsigned g = 0;
+    for (; g + 8 <= n_groups; g += 8) {
+      double v[8];
+#pragma unroll
+      for (int c = 0; c < 8; ++c) v[c] = __ldcg(gsum + (int64_t)(g + c) * PS + j);
+#pragma unroll
+      for (int c = 0; c < 8; ++c) sum += v[c];
+    }
+    for (; g < n_groups; ++g) sum += __ldcg(gsum + (int64_t)g * PS + j);
+    s_sum[j] = sum;
   }
   if (warp == STREAM_WARPS - 1) {
     MantAcc m;
-    constexpr int PER = 10;                                 // up to 320 blocks with every load in flight at once
-    double pp[PER], pe[PER], pb[PER];
-#pragma unroll
-    for (int r = 0; r < PER; ++r) {
-      const unsigned b = lane + 32 * r;
-      const bool ok = b < gridDim.x;
-      const double *src = partials + (int64_t)(ok ? b : 0) * PS + NA;
-      pp[r] = ok ? __ldcg(src) : 1.0; pe[r] = ok ? __ldcg(src + 1) : 0.0; pb[r] = ok ? __ldcg(src + 2) : 0.0;
-    }
-#pragma unroll
-    for (int r = 0; r < PER; ++r) { m.merge(pp[r], (long long)pe[r], (int)pb[r]); m.renorm(); }
-    for (unsigned b = lane + 32 * PER; b < gridDim.x; b += 32) {
-      const double *src = partials + (int64_t)b * PS + NA;
+    for (unsigned g = lane; g < n_groups; g += 32) {
+      const double *src = gsum + (int64_t)g * PS + NA;
       m.merge(__ldcg(src), (long long)__ldcg(src + 1), (int)__ldcg(src + 2));
       m.renorm();
     }
@@ -220,7 +208,8 @@ nll_grad_kernel(const double2 *__restrict__ a, const double *__restrict__ t, int
   const int64_t stride = (int64_t)gridDim.x * STREAM_BLOCK;
   // Whole warps iterate together (the MMA is warp-wide), one tile per iteration.  Measured at K_c = 8, 1 M events (ncu
   // gpu__time_duration): this form 38 us; two tiles per iteration (their loads issued together) 40 us; three blocks per
-  // SM at 80 registers 41 us; columns brought in by cp.async, double buffered, straight into the X tile 50 us.  The
+  // SM at 80 registers 41 us; columns brought in by cp.async, double buffered, straight into the X tile 50 us; bulk L2
+  // prefetch of the warp's next tile (nine UBLKPF per tile): memory stalls 43 -> 27 % of the warp samples, duration unchanged.  The
   // kernel issues ~440 warp instructions per 32 events, ~300 of them on the fp64 pipe (2 cycles each) plus 16 DMMA: about
   // 16 us of fp64-pipe time per million events on B200's 64 lanes per clock per SM -- it is bound by that pipe and by the
   // serial dependency chain of one event, not by the 136 B per event it streams.
