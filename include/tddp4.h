@@ -257,6 +257,11 @@ int64_t tddp4_launch_count(const tddp4 *h);
  * denominator of the "alu"-bound fractions of the generator, kinematics and time-row kernels).  Host out:
  * fp64 instructions per second (one per lane; an FMA counts once).  Synchronous, ~1 ms.              */
 int tddp4_fp64_peak(tddp4 *h, double *inst_per_s);
+/* The branch-free fp64 primitives the kernels use where an IEEE division or square root would put a divergent slow path
+ * into a hot loop (Breit-Wigner reciprocal, barrier factors, generator boosts; csrc/jit_shared.cuh), evaluated on arrays
+ * for accuracy tests: what = 0 1/x, 1 sqrt(x), 2 1/sqrt(x), 3 x/y.  x, y (what = 3 only), out: device [n]; inputs must
+ * be normal numbers (x > 0 for the roots).  Synchronous.                                                        */
+int tddp4_math_probe(tddp4 *h, int what, int64_t n, const double *x, const double *y, double *out);
 /* The CUDA source of a kernel the library specialises to a model and compiles at run time with NVRTC (the two fused
  * passes over the static caches: what = 0 the Gram pass, 8(a) rows 2+3+6; what = 1 the data pass after a mass/width move,
  * rows 2..5+7; the model's table of shared lineshape / spin-factor instances becomes compile-time

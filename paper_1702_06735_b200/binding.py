@@ -26,7 +26,7 @@ SYMBOLS = ["tddp4_create", "tddp4_destroy", "tddp4_set_stream", "tddp4_last_erro
            "tddp4_nll_parts", "tddp4_nll_grad", "tddp4_param_stride", "tddp4_nll_batch", "tddp4_gram", "tddp4_gram_override", "tddp4_norm", "tddp4_generate", "tddp4_weight_bound",
            "tddp4_candidates", "tddp4_get", "tddp4_layout", "tddp4_profile", "tddp4_profile_read",
            "tddp4_profile_reset", "tddp4_launch_count", "tddp4_gram_enqueue", "tddp4_gram_reduce", "tddp4_nll_enqueue",
-           "tddp4_gram_state", "tddp4_fp64_peak", "tddp4_project", "tddp4_jit_source"]
+           "tddp4_gram_state", "tddp4_fp64_peak", "tddp4_project", "tddp4_jit_source", "tddp4_math_probe"]
 
 
 class Tddp4Error(RuntimeError):
@@ -99,6 +99,7 @@ def load_library():
     L.tddp4_fp64_peak.argtypes = [vp, dp]
     L.tddp4_jit_source.argtypes = [C.POINTER(_Desc), C.c_int, C.c_int, C.c_int, C.c_char_p, i64]
     L.tddp4_jit_source.restype = i64
+    L.tddp4_math_probe.argtypes = [vp, C.c_int, i64, vp, vp, vp]
     L.tddp4_project.argtypes = [vp, i64, i64, vp, C.c_int, vp, vp, vp]
     _lib = L
     return L
@@ -330,6 +331,12 @@ class Tddp4:
         out = C.c_double()
         self._check(self.lib.tddp4_fp64_peak(self._h, C.byref(out)))
         return out.value
+
+    def math_probe(self, what, x, y=None):
+        """tddp4_math_probe: 0 1/x, 1 sqrt(x), 2 1/sqrt(x), 3 x/y with the kernels' branch-free primitives; device tensors."""
+        out = self._torch.empty_like(x)
+        self._check(self.lib.tddp4_math_probe(self._h, what, x.numel(), _ptr(x), _ptr(y), _ptr(out)))
+        return out
 
     def norm(self):
         out = C.c_double()

@@ -128,6 +128,16 @@ __global__ void __launch_bounds__(256) gram_reduce_kernel(const double *__restri
 __global__ void __launch_bounds__(32) append_count_kernel(double *dst, double value) { if (threadIdx.x == 0) *dst = value; }
 
 // fp64 issue-rate probe: 8 independent DFMA chains per thread, 4096 FMAs each, 148 x 4 x 256 threads
+// The branch-free fp64 primitives of jit_shared.cuh on arrays (tddp4_math_probe): what = 0 rcp_normal(x), 1 sqrt_pos(x),
+// 2 rsqrt_pos(x), 3 div_normal(x, y).  For the accuracy tests only.
+__global__ void __launch_bounds__(256) math_probe_kernel(int what, int64_t n, const double *__restrict__ x,
+                                                         const double *__restrict__ y, double *__restrict__ out) {
+  int64_t i = (int64_t)blockIdx.x * 256 + threadIdx.x;
+  if (i >= n) return;
+  double v = x[i];
+  out[i] = what == 0 ? rcp_normal(v) : what == 1 ? sqrt_pos(v) : what == 2 ? rsqrt_pos(v) : div_normal(v, y[i]);
+}
+
 __global__ void __launch_bounds__(256) fp64_peak_kernel(double *out, double a, double b, int iters) {
   double v[8];
 #pragma unroll
