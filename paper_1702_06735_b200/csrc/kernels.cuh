@@ -214,29 +214,65 @@ namespace tddp4k {
 // (one thread per candidate, GEN_BLOCK candidates per block: flags and block counts below are laid out for it).
 constexpr int GEN_BLOCK = 128;
 
-// exclusive scan of the block counts of one launch chunk (single block), continued from the running total of the
-// chunks before it: offs[b] = *total + sum_{b' < b} cnt[b'], and *total advances by the chunk's count (no host round trip)
-__global__ void __launch_bounds__(1024) scan_kernel(const uint32_t *__restrict__ cnt, int64_t nb,
-                                                    unsigned long long *__restrict__ offs /* [nb+1] */,
-                                                    unsigned long long *__restrict__ total) {
-  __shared__ unsigned long long part[1024];
-  __shared__ unsigned long long base;
-  int tid = threadIdx.x;
-  int64_t per = (nb + 1023) / 1024, lo = tid * per, hi = lo + per < nb ? lo + per : nb;
-  unsigned long long s = 0;
-  for (int64_t b = lo; b < hi; ++b) s += cnt[b];
-  part[tid] = s;
-  __syncthreads();
-  if (tid == 0) {
-    unsigned long long run = 0;
-    for (int k = 0; k < 1024; ++k) { unsigned long long v = part[k]; part[k] = run; run += v; }
-    base = *total;
-    offs[nb] = base + run;
-    *total = base + run;
+// Output offsets of one launch chunk, one per span of EMIT_SPAN candidates (= SCAN_PER ratio blocks; an emit block covers
+// one span), continued from the running total of the chunks before it: offs[s] = *total + number of accepted candidates in
+// the spans before s; *total advances by the chunk's count (no host round trip).  Single block: a thread sums the
+// SCAN_PER counts of its span (four 16-byte loads), the block scans the span sums with warp shuffles in tiles of 1024 spans
+// and carries the running total from tile to tile; the next tile's counts are loaded before the current tile is scanned.
+// Integer arithmetic: the same result in any order.  (The first version scanned every block count, each thread one
+// contiguous stretch and thread 0 the 1024 stretch sums serially: 63 us for the 78 125 counts of config 4, 234 us for a
+// 16 M-candidate chunk -- a tenth of the generation time.)
+constexpr int EMIT_BLOCK = 128, EMIT_SPAN = 2048, EMIT_WORDS = EMIT_SPAN / 32;
+static_assert(EMIT_SPAN % GEN_BLOCK == 0, "an emit block starts at a ratio-block boundary");
+constexpr int SCAN_BLOCK = 1024, SCAN_PER = EMIT_SPAN / GEN_BLOCK;
+static_assert(SCAN_PER % 4 == 0, "a span's counts are loaded as uint4");
+__global__ void __launch_bounds__(SCAN_BLOCK) scan_kernel(const uint32_t *__restrict__ cnt /* allocated in whole spans */, int64_t n_blocks,
+                                                          unsigned long long *__restrict__ offs /* [n_spans] */,
+                                                          unsigned long long *__restrict__ total) {
+  __shared__ uint32_t s_warp[SCAN_BLOCK / 32];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  unsigned long long carry = *total;
+  const int64_t n_spans = (n_blocks + SCAN_PER - 1) / SCAN_PER;
+  auto span_sum = [&](int64_t sp) -> uint32_t {
+    if (sp >= n_spans) return 0u;
+    const int64_t b = sp * SCAN_PER;
+    const uint4 *src = reinterpret_cast<const uint4 *>(cnt + b);
+    uint32_t acc = 0;
+#pragma unroll
+    for (int k = 0; k < SCAN_PER / 4; ++k) {               // counts beyond this chunk's blocks are leftovers of a larger chunk
+      uint4 q = src[k];
+      const int64_t r = n_blocks - (b + 4 * k);            // blocks left from this quad on
+      acc += (r > 0 ? q.x : 0u) + (r > 1 ? q.y : 0u) + (r > 2 ? q.z : 0u) + (r > 3 ? q.w : 0u);
+    }
+    return acc;
+  };
+  uint32_t next = span_sum(tid);
+  for (int64_t s0 = 0; s0 < n_spans; s0 += SCAN_BLOCK) {
+    const uint32_t mine = next;
+    next = span_sum(s0 + SCAN_BLOCK + tid);                 // in flight while this tile is scanned
+    uint32_t incl = mine;                                   // inclusive scan over the warp
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      uint32_t y = __shfl_up_sync(0xffffffffu, incl, o);
+      if (lane >= o) incl += y;
+    }
+    if (lane == 31) s_warp[warp] = incl;
+    __syncthreads();
+    if (warp == 0) {                                        // inclusive scan of the 32 warp totals
+      uint32_t w = s_warp[lane];
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        uint32_t y = __shfl_up_sync(0xffffffffu, w, o);
+        if (lane >= o) w += y;
+      }
+      s_warp[lane] = w;
+    }
+    __syncthreads();
+    if (s0 + tid < n_spans) offs[s0 + tid] = carry + (warp ? s_warp[warp - 1] : 0u) + (incl - mine);
+    carry += s_warp[SCAN_BLOCK / 32 - 1];
+    __syncthreads();                                        // s_warp is reused by the next tile
   }
-  __syncthreads();
-  unsigned long long run = base + part[tid];
-  for (int64_t b = lo; b < hi; ++b) { offs[b] = run; run += cnt[b]; }
+  if (tid == 0) *total = carry;
 }
 
 // G6: regenerate the accepted candidates (Philox is counter based: no state to carry) and write them compacted, in
@@ -244,8 +280,6 @@ __global__ void __launch_bounds__(1024) scan_kernel(const uint32_t *__restrict__
 // indices in shared memory, then its threads walk that list, so every lane that runs Philox + Raubold-Lynch produces an
 // output event (at 6.6 % acceptance the one-thread-per-candidate form kept 89 % of the warps busy for 1/15 of the
 // lanes: 0.96 ms against 1.21 ms for the ratio pass itself) and consecutive threads write consecutive output slots.
-constexpr int EMIT_BLOCK = 128, EMIT_SPAN = 2048, EMIT_WORDS = EMIT_SPAN / 32;
-static_assert(EMIT_SPAN % GEN_BLOCK == 0, "an emit block starts at a ratio-block boundary");
 __global__ void __launch_bounds__(EMIT_BLOCK)
 gen_emit_kernel(const __grid_constant__ ModelTab M, double tau, uint64_t seed, uint32_t stream, uint64_t first,
                 int64_t n, const uint32_t *__restrict__ flags, const unsigned long long *__restrict__ offs,
@@ -273,7 +307,7 @@ gen_emit_kernel(const __grid_constant__ ModelTab M, double tau, uint64_t seed, u
   }
   __syncthreads();
   const int count = s_pre[EMIT_WORDS];
-  const int64_t base = (int64_t)offs[j0 / GEN_BLOCK];
+  const int64_t base = (int64_t)offs[blockIdx.x];
   for (int k = tid; k < count; k += EMIT_BLOCK) {
     const int64_t pos = base + k;
     if (pos >= capacity) break;
