@@ -155,7 +155,7 @@ def run_ours(args):
 
     rank, world = int(os.environ.get("RANK", 0)), int(os.environ.get("WORLD_SIZE", 1))
     local = int(os.environ.get("LOCAL_RANK", 0))
-    if world > 1:
+    if world > 1 or (args.sharded and "RANK" in os.environ):
         return run_sharded(args)
     device = f"cuda:{local}"
     torch.cuda.set_device(device)
@@ -800,6 +800,9 @@ def main():
     ap.add_argument("--warmup", type=int, default=10)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--headline-only", action="store_true", help="skip the C2/C4/C5 extras (profiling runs)")
+    ap.add_argument("--sharded", action="store_true",
+                    help="run the event-sharded path (the N > 1 mode) even with one rank: a single-GPU check of that code path, "
+                         "launched under torch.distributed.run --nproc-per-node 1")
     ap.add_argument("--validation-events", type=int, default=100_000,
                     help="events per sample of the Fig. 3 comparison (the paper: 500 000; the oracle generates ~0.9 %% of its candidates)")
     args = ap.parse_args()

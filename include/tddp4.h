@@ -91,7 +91,7 @@ typedef struct {
   const tddp4_res *res;    /* host [n_res]                                                           */
   int n_terms;
   const tddp4_term *terms; /* host [n_terms]                                                         */
-  int n_couplings;         /* K_c                                                                    */
+  int n_couplings;         /* K_c; every coupling 0 .. K_c-1 must be used by at least one term               */
   double t_lo, t_hi;       /* decay-time window of the normalisation; t_hi = +INFINITY allowed       */
   int use_resolution;      /* 0: eq. (1) as printed; 1: per-event Gaussian sigma_t (O-8): the data *
                             * sample must be loaded with sigma_t > 0; P_i = R_i(t_i, sigma_i) / N_i(sigma_i);   *

@@ -89,9 +89,12 @@ def test_prelude_states_the_model_tables():
     t0 = [int(v) for v in re.search(r"J_T0\[\] = \{([^}]*)\}", src).group(1).split(",")]
     n_inst = int(re.search(r"#define J_NINST (\d+)", src).group(1))
     assert all(-1 <= v < n_inst for v in t0[:-1])
+    import copy
     with pytest.raises(binding.Tddp4Error):
-        bad = W.config(1).model
-        import copy
-        bad = copy.deepcopy(bad)
+        bad = copy.deepcopy(W.config(1).model)
         bad.term_coupling = [99] * bad.n_terms
+        binding.jit_source(bad, 0)
+    with pytest.raises(binding.Tddp4Error):            # a coupling without a term: its column would never be written
+        bad = copy.deepcopy(W.config(1).model)
+        bad.term_coupling = [0] * bad.n_terms
         binding.jit_source(bad, 0)
