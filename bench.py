@@ -671,7 +671,7 @@ def run_sharded(args):
         stream = torch.cuda.Stream(device)
         h = binding.Tddp4(mdl, device)
         h.set_stream(stream)
-        sh = sharded.ShardedNLL(h)
+        sh = sharded.ShardedNLL(h, always_collective=args.sharded)
         sh.load_events(0, p4, t)
         sh.load_events(1, p4n)
         timed(sh, stream, traj[:args.warmup])

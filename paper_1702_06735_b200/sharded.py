@@ -36,7 +36,9 @@ def shard_range(n: int, rank: int, world: int):
 
 
 class ShardedNLL:
-    def __init__(self, evaluator, group=None):
+    def __init__(self, evaluator, group=None, always_collective=False):
+        """always_collective: issue the collectives even at world size 1 (a one-rank process group): the single-GPU check
+        of the NCCL calls of the device path (tests, `bench.py --sharded`)."""
         import torch.distributed as dist
         self.ev = evaluator
         self.dist = dist
@@ -47,6 +49,7 @@ class ShardedNLL:
         self._mw = None          # host path: masses/widths the global Gram matrix in force was built for
         self._n_norm_total = None
         self.device_path = hasattr(evaluator, "nll_enqueue") and (self.world == 1 or self.backend == "nccl")
+        self.always_collective = bool(always_collective) and dist.is_initialized() and self.backend == "nccl"
         if self.device_path:
             import torch
             self.torch = torch
@@ -76,7 +79,7 @@ class ShardedNLL:
 
     def _all_gather_device(self, out, mine):
         """Enqueued on the current (= the handle's) stream; world size 1 needs no collective."""
-        if self.world == 1:
+        if self.world == 1 and not self.always_collective:
             out[0].copy_(mine)
         else:
             self.dist.all_gather_into_tensor(out, mine, group=self.group)
@@ -86,7 +89,7 @@ class ShardedNLL:
         """Sum of the ranks' normalisation sample sizes; exchanged once per loaded sample (host integers)."""
         if self._n_norm_total is None:
             n = float(self.ev.n[1])
-            if self.world == 1:
+            if self.world == 1 and not self.always_collective:
                 self._n_norm_total = int(n)
             else:
                 t = self.torch.tensor([n], dtype=self.torch.float64, device=self.ev.device)

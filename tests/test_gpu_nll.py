@@ -424,6 +424,47 @@ def test_sharded_wrapper_on_one_rank(B):
     assert abs(sh.nll() - direct2) <= 1e-13 * abs(direct2)
 
 
+def test_sharded_device_path_issues_nccl_collectives(B):
+    """The NCCL calls of the sharded device path on ONE rank (the pool has one GPU per box): a one-rank NCCL process group,
+    collectives forced, every exchange runs on the handle's stream -- same NLL as the handle alone, exchanges counted."""
+    import socket
+    import torch
+    import torch.distributed as dist
+    from paper_1702_06735_b200 import sharded
+    if dist.is_initialized():
+        pytest.skip("a process group exists already")
+    with socket.socket() as sk:
+        sk.bind(("127.0.0.1", 0))
+        port = sk.getsockname()[1]
+    dist.init_process_group("nccl", init_method=f"tcp://127.0.0.1:{port}", rank=0, world_size=1,
+                            device_id=torch.device("cuda:0"))
+    try:
+        mdl = samples.model_of(("C", 2))
+        par = W.initial_params(mdl)
+        p4, t, _ = samples.data_sample(("C", 2), 2_049)
+        p4n, _ = samples.flat_sample(10_001)
+        h = B.Tddp4(mdl)
+        h.load_events(0, p4, t); h.load_events(1, p4n)
+        h.set_params(par)
+        direct = h.nll()
+        sh = sharded.ShardedNLL(h, always_collective=True)
+        sh.set_params(par)
+        assert abs(sh.nll() - direct) <= 1e-13 * abs(direct)
+        assert sh.exchanges == 2                              # Gram sums + result words (the count exchange is not counted)
+        p2 = par.copy(); p2.c[0] *= 1.01
+        h.set_params(p2); direct2 = h.nll()
+        sh.set_params(p2)                                     # couplings only: the global Gram matrix stays in force
+        assert abs(sh.nll() - direct2) <= 1e-13 * abs(direct2)
+        assert sh.exchanges == 3
+        p3 = par.copy(); p3.mass[1] *= 1.0005
+        h.set_params(p3); direct3 = h.nll()
+        sh.set_params(p3)
+        assert abs(sh.nll() - direct3) <= 1e-13 * abs(direct3)
+        assert sh.exchanges == 5
+    finally:
+        dist.destroy_process_group()
+
+
 def test_maximum_model_size(B):
     """The limits of include/tddp4.h: 16 couplings, 32 terms (all eight chains twice, both Bose orderings), and a model
     whose instance/term counts fall between the load-batch size classes (5 instances, 5 terms -> padded rows)."""
