@@ -161,6 +161,14 @@ int tddp4_nll_batch(tddp4 *h, int64_t n_points, const double *params, double *nl
 /* G_sum[k][l] = sum_j w_j a_k(p_j) conj(a_l(p_j)) over THIS handle's normalisation sample for the
  * current masses/widths (recomputed if dirty); host [K_c][K_c][2]; *n_norm = its event count.         */
 int tddp4_gram(tddp4 *h, double *G_sum, int64_t *n_norm);
+/* How the Gram matrix is refreshed after a mass or width moved (the
+ * normalisation pass dominates a fit).  mode 0 (default): one full pass over the static cache of the normalisation
+ * sample, nothing of it stored.  mode 1: the library also keeps the sample's coupling columns (16 K_c bytes per event)
+ * and, when the columns made stale since the last pass are few enough that reading the clean ones back (16 B each) and
+ * rebuilding only the stale ones moves fewer bytes than a full pass, runs an incremental pass; otherwise a full pass that
+ * re-stores the stale columns.  Either way G has the bits of a full pass.  mode -1 only queries.  incremental_passes
+ * (host, may be NULL): number of incremental passes run so far.  Synchronises when the mode changes.              */
+int tddp4_set_gram_mode(tddp4 *h, int mode, int64_t *incremental_passes);
 /* Replace the Gram matrix used for N by G_sum / n_norm given by the caller (e.g. the all-reduced sum of
  * all ranks' matrices).  Stays in force until the masses/widths change again.                         */
 int tddp4_gram_override(tddp4 *h, const double *G_sum, int64_t n_norm);
@@ -267,7 +275,8 @@ int tddp4_math_probe(tddp4 *h, int what, int64_t n, const double *x, const doubl
  * rows 2..5+7; the model's table of shared lineshape / spin-factor instances becomes compile-time
  * constants; what = 4 the candidate kernel of the generator, G1-G5), or of a header these include (what = 2
  * "jit_shared.cuh", 3 "nll_shared.cuh", 5 "tables.h", 6 "device_math.cuh"; desc may then be any valid model).  weighted: the event set carries a weight row; mode (what = 1): 0 full-range time functions, 1 small mixing
- * phases, 2 resolution / time-integrated rows.  Needs NO device: it is what tddp4_create hands to NVRTC, exposed so that
+ * phases, 2 resolution / time-integrated rows; mode (what = 0): 0 plain pass, 1 pass that stores the columns, 2
+ * incremental pass (tddp4_set_gram_mode).  Needs NO device: it is what tddp4_create hands to NVRTC, exposed so that
  * a build check can compile it.  Host buf of cap bytes (may be NULL with cap = 0); returns the size needed including the
  * terminating NUL (the text is written only if it fits), or a negative tddp4_status.                              */
 int64_t tddp4_jit_source(const tddp4_model_desc *desc, int what, int weighted, int mode, char *buf, int64_t cap);

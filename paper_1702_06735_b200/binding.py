@@ -26,7 +26,7 @@ SYMBOLS = ["tddp4_create", "tddp4_destroy", "tddp4_set_stream", "tddp4_last_erro
            "tddp4_nll_parts", "tddp4_nll_grad", "tddp4_param_stride", "tddp4_nll_batch", "tddp4_gram", "tddp4_gram_override", "tddp4_norm", "tddp4_generate", "tddp4_weight_bound",
            "tddp4_candidates", "tddp4_get", "tddp4_layout", "tddp4_profile", "tddp4_profile_read",
            "tddp4_profile_reset", "tddp4_launch_count", "tddp4_gram_enqueue", "tddp4_gram_reduce", "tddp4_nll_enqueue",
-           "tddp4_gram_state", "tddp4_fp64_peak", "tddp4_project", "tddp4_jit_source", "tddp4_math_probe"]
+           "tddp4_gram_state", "tddp4_fp64_peak", "tddp4_project", "tddp4_jit_source", "tddp4_math_probe", "tddp4_set_gram_mode"]
 
 
 class Tddp4Error(RuntimeError):
@@ -100,6 +100,7 @@ def load_library():
     L.tddp4_jit_source.argtypes = [C.POINTER(_Desc), C.c_int, C.c_int, C.c_int, C.c_char_p, i64]
     L.tddp4_jit_source.restype = i64
     L.tddp4_math_probe.argtypes = [vp, C.c_int, i64, vp, vp, vp]
+    L.tddp4_set_gram_mode.argtypes = [vp, C.c_int, C.POINTER(i64)]
     L.tddp4_project.argtypes = [vp, i64, i64, vp, C.c_int, vp, vp, vp]
     _lib = L
     return L
@@ -138,7 +139,7 @@ def _make_desc(model):
     return d, (res, terms)
 
 
-def jit_source(model, what, weighted=False, mode=1):
+def jit_source(model, what, weighted=False, mode=0):
     """tddp4_jit_source: the CUDA text the library hands to NVRTC for this model (what = 0 Gram pass, 1 data pass) or one
     of the headers it includes (2 jit_shared.cuh, 3 nll_shared.cuh).  Needs no GPU."""
     lib = load_library()
@@ -330,6 +331,13 @@ class Tddp4:
     def fp64_peak(self):
         out = C.c_double()
         self._check(self.lib.tddp4_fp64_peak(self._h, C.byref(out)))
+        return out.value
+
+    def set_gram_mode(self, mode):
+        """tddp4_set_gram_mode: 0 full Gram passes (default), 1 stored normalisation columns + incremental passes, -1 query;
+        returns the number of incremental passes run so far."""
+        out = C.c_int64()
+        self._check(self.lib.tddp4_set_gram_mode(self._h, mode, C.byref(out)))
         return out.value
 
     def math_probe(self, what, x, y=None):

@@ -20,6 +20,13 @@
 // compile-time constants every index below is an immediate: the lineshapes stay in registers (no scratch at all), every
 // load carries an immediate offset, and the per-term table lookups, address arithmetic and flush branches disappear.
 // Deterministic: per-warp accumulation in event order, warps, blocks and block groups summed in index order.
+//
+// J_GMODE (the incremental update of G; tddp4_set_gram_mode):
+//   0  plain pass: nothing of the normalisation sample is stored (the default);
+//   1  full pass that also stores the coupling columns whose bit is set in `mask` into an[K_c][ld];
+//   2  incremental pass: columns whose bit is clear in `mask` are READ from an (16 B), only the masked ones are rebuilt
+//      from the rows of their terms (J_INSTCOLS / J_SROWCOLS: the columns each lineshape instance / s row feeds) and
+//      written back.  Same tiles, same arithmetic, same accumulation order: G has the bits of a full pass.
 #include "jit_shared.cuh"
 
 namespace tddp4k {
@@ -29,7 +36,9 @@ constexpr int JG_BLOCK = 256;
 extern "C" __global__ void __launch_bounds__(JG_BLOCK, J_BPS)
 gram_jit(const __grid_constant__ LineParams LP, const double *__restrict__ cache, long long n,
          double *__restrict__ partials /* [grid + groups][64 NB NB] */, unsigned int *ticket,
-         double *__restrict__ G /* [KC][KC][2] sums, Hermitian, full */) {
+         double *__restrict__ G /* [KC][KC][2] sums, Hermitian, full */,
+         double2 *__restrict__ an /* J_GMODE > 0: stored columns [KC][ld] */, long long ld, unsigned int mask) {
+  constexpr int GMODE = J_GMODE;
   constexpr int NB = J_NB, F = 8 * NB, STRIDE = gram_stride(NB), NP = NB * (NB + 1) / 2;
   constexpr bool WEIGHTED = J_WOFF >= 0;
   extern __shared__ __align__(16) char smem_raw[];
@@ -47,21 +56,35 @@ gram_jit(const __grid_constant__ LineParams LP, const double *__restrict__ cache
   long long i0 = (long long)blockIdx.x * JG_BLOCK + warp * 32;
 #pragma unroll 1
   for (; i0 < n; i0 += stride) {
-    if (PF_DIST > 0 && lane == 0 && i0 + PF_DIST * stride < n)
+    if (GMODE != 2 && PF_DIST > 0 && lane == 0 && i0 + PF_DIST * stride < n)     // (an incremental pass reads part of a tile only)
       prefetch_l2_bulk(tile_event(cache, J_R, i0 + PF_DIST * stride) + J_SKIP, (unsigned)(J_R * 32 - J_SKIP) * 8u);
     const double *ev = tile_event(cache, J_R, i0 + lane);
     double sv[J_NSU + 1], gv[J_NINST + 1], fv[J_NTERMS];   // + 1: a model without resonances has no instance
+    double2 kept[J_KC];                                    // GMODE 2: the clean columns, read back
+    if (GMODE == 2) {                                      // only the rows the masked columns need (warp-uniform guards)
 #pragma unroll
-    for (int r = 0; r < J_NSU; ++r) sv[r] = ldg_stream1(ev + J_SKIP + r * 32);
+      for (int c = 0; c < J_KC; ++c) kept[c] = (mask >> c) & 1u ? make_double2(0.0, 0.0) : ldg_stream2(an + c * ld + i0 + lane);
 #pragma unroll
-    for (int j = 0; j < J_NINST; ++j) gv[j] = ldg_stream1(ev + J_GOFF + j * 32);
+      for (int r = 0; r < J_NSU; ++r) sv[r] = (mask & J_SROWCOLS[r]) ? ldg_stream1(ev + J_SKIP + r * 32) : 0.0;
 #pragma unroll
-    for (int k = 0; k < J_NTERMS; ++k) fv[k] = ldg_stream1(ev + J_FOFF + k * 32);
+      for (int j = 0; j < J_NINST; ++j) gv[j] = (mask & J_INSTCOLS[j]) ? ldg_stream1(ev + J_GOFF + j * 32) : 0.0;
+#pragma unroll
+      for (int k = 0; k < J_NTERMS; ++k) fv[k] = (mask >> J_COL[k]) & 1u ? ldg_stream1(ev + J_FOFF + k * 32) : 0.0;
+    } else {
+#pragma unroll
+      for (int r = 0; r < J_NSU; ++r) sv[r] = ldg_stream1(ev + J_SKIP + r * 32);
+#pragma unroll
+      for (int j = 0; j < J_NINST; ++j) gv[j] = ldg_stream1(ev + J_GOFF + j * 32);
+#pragma unroll
+      for (int k = 0; k < J_NTERMS; ++k) fv[k] = ldg_stream1(ev + J_FOFF + k * 32);
+    }
     double wj = 1.0;
     if (WEIGHTED) wj = ldg_stream1(ev + J_WOFF);
     double2 T[J_NINST + 1];
 #pragma unroll
-    for (int j = 0; j < J_NINST; ++j) T[j] = breit_wigner(LP.m0sq[j], LP.gam[j], sv[J_SROW[j]], gv[j]);
+    for (int j = 0; j < J_NINST; ++j)
+      if (GMODE != 2 || (mask & J_INSTCOLS[j])) T[j] = breit_wigner(LP.m0sq[j], LP.gam[j], sv[J_SROW[j]], gv[j]);
+      else T[j] = make_double2(0.0, 0.0);
     double2 a = make_double2(0.0, 0.0);
 #pragma unroll
     for (int k = 0; k < J_NTERMS; ++k) {
@@ -73,6 +96,8 @@ gram_jit(const __grid_constant__ LineParams LP, const double *__restrict__ cache
       a.x = fma(fv[k], P.x, a.x);
       a.y = fma(fv[k], P.y, a.y);
       if (J_LAST[k]) {
+        if (GMODE == 2 && !((mask >> J_COL[k]) & 1u)) a = kept[J_COL[k]];
+        if (GMODE != 0 && ((mask >> J_COL[k]) & 1u)) an[J_COL[k] * ld + i0 + lane] = a;
         *reinterpret_cast<double2 *>(row + 2 * J_COL[k]) = a;
         a = make_double2(0.0, 0.0);
       }

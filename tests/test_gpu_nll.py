@@ -424,6 +424,36 @@ def test_sharded_wrapper_on_one_rank(B):
     assert abs(sh.nll() - direct2) <= 1e-13 * abs(direct2)
 
 
+def test_incremental_gram_has_the_bits_of_a_full_pass(B):
+    """with tddp4_set_gram_mode(1) the normalisation columns are kept and a move of few columns
+    rebuilds only those; along a trajectory of single-resonance, all-parameter and coupling-only moves G and the NLL must
+    be bit-identical to a handle that runs full passes, and incremental passes must actually have happened."""
+    mdl = samples.model_of(("C", 3))
+    p4, t, _ = samples.data_sample(("C", 3), 1_031)
+    p4n, _ = samples.flat_sample(20_011)
+    par = W.initial_params(mdl)
+    full, inc = B.Tddp4(mdl), B.Tddp4(mdl)
+    assert inc.set_gram_mode(1) == 0
+    for h in (full, inc):
+        h.load_events(0, p4, t); h.load_events(1, p4n)
+    traj = W.trajectory(mdl, par, 60, "minuit", seed=77)
+    for k, p in enumerate(traj):
+        full.set_params(p); inc.set_params(p)
+        assert full.nll() == inc.nll(), k
+        if k % 7 == 0:
+            Gf, nf = full.gram(); Gi, ni = inc.gram()
+            assert nf == ni and np.array_equal(Gf, Gi), k
+    n_inc = inc.set_gram_mode(-1)
+    assert 0 < n_inc < 60
+    # a reload drops the stored columns' validity; switching the mode off frees them
+    inc.load_events(1, p4n)
+    inc.set_params(traj[3]); full.set_params(traj[3])
+    assert inc.nll() == full.nll()
+    inc.set_gram_mode(0)
+    inc.set_params(traj[5]); full.set_params(traj[5])
+    assert inc.nll() == full.nll()
+
+
 def test_sharded_device_path_issues_nccl_collectives(B):
     """The NCCL calls of the sharded device path on ONE rank (the pool has one GPU per box): a one-rank NCCL process group,
     collectives forced, every exchange runs on the handle's stream -- same NLL as the handle alone, exchanges counted."""

@@ -49,14 +49,17 @@ def models():
 @pytest.mark.parametrize("name", ["C1", "C2", "C3", "C5", "flat"])
 def test_gram_pass_compiles_for_sm100a(name, tmp_path):
     mdl = models()[name]
-    for weighted in (False, True):
-        usage, sass = compile_sm100a(binding.jit_source(mdl, 0, weighted), f"gram_{name}_{int(weighted)}", str(tmp_path))
+    for weighted, gmode in ((False, 0), (True, 0), (False, 1), (False, 2)):
+        usage, sass = compile_sm100a(binding.jit_source(mdl, 0, weighted, gmode), f"gram_{name}_{int(weighted)}{gmode}", str(tmp_path))
         assert "sm_100a" in sass
         m = re.search(r"REG:(\d+) STACK:(\d+)", usage)
-        assert m and int(m.group(2)) == 0 and int(m.group(1)) <= 128, usage      # no spills, two blocks per SM
+        assert m and int(m.group(1)) <= 128, usage                               # two blocks per SM
+        if gmode != 2:                                                           # (the incremental pass also holds the kept columns)
+            assert int(m.group(2)) == 0 and "LDL" not in sass and "STL" not in sass, usage
+        else:
+            assert int(m.group(2)) <= 128, usage
         assert "DMMA" in sass                                                    # fp64 tensor cores
-        assert "UBLKPF" in sass                                                  # bulk L2 prefetch of the next tile
-        assert "LDL" not in sass and "STL" not in sass
+        assert ("UBLKPF" in sass) == (gmode != 2)                                # bulk L2 prefetch of the next tile
 
 
 @pytest.mark.parametrize("name", ["C1", "C2", "C3", "C5", "flat"])
