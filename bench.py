@@ -372,6 +372,21 @@ def run_ours(args):
                "gram_launches": pg[1], "incremental_passes": n_inc,
                "gram_us_per_launch": round(1e3 * pg[0] / max(1, pg[1]), 2), "gram_alg_MB_per_launch": round(pg[2] / max(1, pg[1]) / 1e6, 1),
                "stored_columns_MB": round(16.0 * KC * Nn / 1e6, 1), "bit_identical_nll": bool(np.array_equal(nll_inc, nll_vals))}
+        # where it pays: a trajectory of one-column moves (mass or width of a1, K1(1270), K2*, K1(1400), each in ONE column)
+        one = h.pack_params(W.trajectory(mdl, p0, args.warmup + 200, "one_resonance", resonances=[2, 3, 4, 5]))
+        for mode, key in ((1, "ms_per_step"), (0, "ms_per_step_full_passes")):
+            h.set_gram_mode(mode)
+            h.set_params(p0)
+            h.nll_batch(one[:args.warmup])
+            torch.cuda.synchronize()
+            a.record(stream)
+            v, _ = h.nll_batch(one[args.warmup:])
+            b.record(stream)
+            torch.cuda.synchronize()
+            inc.setdefault("one_column_moves", {"steps": 200})[key] = round(a.elapsed_time(b) / 200, 5)
+            inc["one_column_moves"].setdefault("nll", []).append(float(v[-1]))
+        nl = inc["one_column_moves"].pop("nll")
+        inc["one_column_moves"]["bit_identical_nll"] = nl[0] == nl[1]
         h.set_gram_mode(0)
     except Exception as e:
         inc = {"error": repr(e)}

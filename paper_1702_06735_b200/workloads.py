@@ -166,15 +166,16 @@ def flat_params(mdl: Model) -> Params:
                   x=0.0, y=0.0, tau=TAU_D0)
 
 
-def trajectory(mdl: Model, p0: Params, n_calls, kind, seed=BASE_SEED, rel=1e-3):
+def trajectory(mdl: Model, p0: Params, n_calls, kind, seed=BASE_SEED, rel=1e-3, resonances=None):
     """Parameter steps standing in for the host minimiser.
 
     kind: 'couplings_xy' - every call perturbs couplings, x, y; masses/widths fixed (config 2)
           'minuit'       - p=0.8 one random floating parameter moves, p=0.2 all move (configs 3, 5)
           'coupling_only'- one coupling component moves per call (best case)
           'all'          - every parameter moves on every call (worst case)
+          'one_resonance'- the mass or the width of ONE resonance (drawn from `resonances`, default all) moves per call
     Steps are relative Gaussian perturbations of size `rel` around the start point p0."""
-    kinds = {"couplings_xy": 0, "minuit": 1, "coupling_only": 2, "all": 3}
+    kinds = {"couplings_xy": 0, "minuit": 1, "coupling_only": 2, "all": 3, "one_resonance": 4}
     rng = np.random.default_rng([seed, STREAM_PARAMS, n_calls, kinds[kind]])
     kc, nr = mdl.n_couplings, mdl.n_res
     n_float = 4 * kc + 2 * nr + 2
@@ -216,6 +217,10 @@ def trajectory(mdl: Model, p0: Params, n_calls, kind, seed=BASE_SEED, rel=1e-3):
         elif kind == "all":
             for j in range(n_float):
                 move(nxt, j)
+        elif kind == "one_resonance":
+            pool = list(range(nr)) if resonances is None else list(resonances)
+            r = pool[int(rng.integers(len(pool)))]
+            move(nxt, 4 * kc + r + (nr if rng.uniform() < 0.5 else 0))
         else:
             raise ValueError(kind)
         out.append(nxt)
