@@ -497,7 +497,7 @@ def test_sharded_device_path_issues_nccl_collectives(B):
 
 def test_maximum_model_size(B):
     """The limits of include/tddp4.h: 16 couplings, 32 terms (all eight chains twice, both Bose orderings), and a model
-    whose instance/term counts fall between the load-batch size classes (5 instances, 5 terms -> padded rows)."""
+    with odd instance and term counts (5 instances, 5 terms)."""
     mdl = W.build_model(list(range(1, 9)) * 2, bose=True)
     assert mdl.n_couplings == 16 and mdl.n_terms == 32
     par = W.initial_params(mdl)
