@@ -31,9 +31,10 @@ constexpr int GRAD_OFFSET = 8;
 
 // shared-memory tiles of one warp: X [32][gram_stride(NB)] (event-major, as the Gram kernel), W [32][GRAD_WS] (rows 4..7 zero)
 constexpr int GRAD_WS = 10;
-// resident blocks per SM
-template <int KC> __host__ __device__ constexpr int grad_bps() { return 2; }
+// resident blocks per SM: three (24 warps, 80 registers, no spills once the grid reduction went two-level) where the
+// per-warp tiles leave room, else two.  Measured at K_c = 8, 1 M events: 47 us at two blocks, 44 us at three.
 template <int KC> __host__ __device__ constexpr int grad_nb() { return (KC + 3) / 4; }
+template <int KC> __host__ __device__ constexpr int grad_bps() { return grad_nb<KC>() <= 2 ? 3 : 2; }
 template <int KC> __host__ __device__ constexpr size_t grad_warp_bytes() {
   return align_up((size_t)32 * gram_stride(grad_nb<KC>()) * sizeof(double), 128) + align_up((size_t)32 * GRAD_WS * sizeof(double), 128);
 }
@@ -207,8 +208,8 @@ nll_grad_kernel(const double2 *__restrict__ a, const double *__restrict__ t, int
   const double yG = R.y * R.Gamma, xG = R.x * R.Gamma;
   const int64_t stride = (int64_t)gridDim.x * STREAM_BLOCK;
   // Whole warps iterate together (the MMA is warp-wide), one tile per iteration.  Measured at K_c = 8, 1 M events (ncu
-  // gpu__time_duration): this form 38 us; two tiles per iteration (their loads issued together) 40 us; three blocks per
-  // SM at 80 registers 41 us; columns brought in by cp.async, double buffered, straight into the X tile 50 us; bulk L2
+  // gpu__time_duration, before the two-level grid reduction): this form 38 us; two tiles per iteration (their loads issued
+  // together) 40 us; columns brought in by cp.async, double buffered, straight into the X tile 50 us; bulk L2
   // prefetch of the warp's next tile (nine UBLKPF per tile): memory stalls 43 -> 27 % of the warp samples, duration unchanged.  The
   // kernel issues ~440 warp instructions per 32 events, ~300 of them on the fp64 pipe (2 cycles each) plus 16 DMMA: about
   // 16 us of fp64-pipe time per million events on B200's 64 lanes per clock per SM -- it is bound by that pipe and by the
