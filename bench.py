@@ -225,6 +225,7 @@ def run_ours(args):
     torch.cuda.synchronize()
     ms_prof = ev2.elapsed_time(ev3)
     prof = h.profile_read()
+    in_us, in_n = h.profile_in_kernel()      # the coupling-only kernel on the GPU's own clock (earliest block start -> result written)
     h.profile(False)
     assert np.array_equal(nll_prof, nll_vals), "profiled and unprofiled passes differ"
 
@@ -323,6 +324,15 @@ def run_ours(args):
             # context, not a bench value: the same kernel's gpu__time_duration in the committed ncu capture (one cold launch, no
             # launch gap between CUDA events).  For the data pass the captured launch rewrote one column, not the mixture's mean.
             ktab[k]["ncu_us_per_launch_committed"] = float(tr[k]["ncu_us_per_launch"])
+
+    if "nll" in ktab and in_n:
+        us = in_us / in_n
+        ktab["nll"].update({"in_kernel_us_per_launch": round(us, 2), "in_kernel_launches": in_n,
+                            "in_kernel_GBs": round(N * (16.0 * KC + 8.0) / (us * 1e-6) / 1e9, 1),
+                            "in_kernel_frac": round(N * (16.0 * KC + 8.0) / (us * 1e-6) / 1e9 / hbm, 4),
+                            "in_kernel_frac_of_8TBs_nominal": round(N * (16.0 * KC + 8.0) / (us * 1e-6) / 1e9 / 8000.0, 4),
+                            "in_kernel_note": "%globaltimer from the earliest block start to the result written, same launches as "
+                                              "us_per_launch: the CUDA-event figure also contains the launch gap of an isolated launch"})
 
     # ---- analytic gradient: one pass against the 2 (4 K_c + 2) NLL calls of a numerical gradient ----
     grad = {}

@@ -259,6 +259,11 @@ int tddp4_profile(tddp4 *h, int enable);
  * for one kernel id; synchronises.                                                                     */
 int tddp4_profile_read(tddp4 *h, int kernel_id, double *total_ms, int64_t *launches, double *alg_bytes);
 int tddp4_profile_reset(tddp4 *h);
+/* In-kernel duration of the coupling-only NLL kernel (8(a) rows 4+5+7) while profiling is on: per launch, the time on the
+ * GPU's %globaltimer from the start of its earliest block to the moment its last block has written the result -- what the
+ * kernel itself takes, without the launch gap a pair of CUDA events around an isolated launch also measures.  Host out:
+ * the sum over launches since the last tddp4_profile_reset in microseconds and their number; synchronises.      */
+int tddp4_profile_in_kernel(tddp4 *h, double *total_us, int64_t *launches);
 /* Number of kernels this handle has launched since creation (all kinds).                            */
 int64_t tddp4_launch_count(const tddp4 *h);
 /* Measured fp64 issue rate of this GPU: a dependent-free chain of DFMA instructions on every SM (the

@@ -26,7 +26,7 @@ SYMBOLS = ["tddp4_create", "tddp4_destroy", "tddp4_set_stream", "tddp4_last_erro
            "tddp4_nll_parts", "tddp4_nll_grad", "tddp4_param_stride", "tddp4_nll_batch", "tddp4_gram", "tddp4_gram_override", "tddp4_norm", "tddp4_generate", "tddp4_weight_bound",
            "tddp4_candidates", "tddp4_get", "tddp4_layout", "tddp4_profile", "tddp4_profile_read",
            "tddp4_profile_reset", "tddp4_launch_count", "tddp4_gram_enqueue", "tddp4_gram_reduce", "tddp4_nll_enqueue",
-           "tddp4_gram_state", "tddp4_fp64_peak", "tddp4_project", "tddp4_jit_source", "tddp4_math_probe", "tddp4_set_gram_mode"]
+           "tddp4_gram_state", "tddp4_fp64_peak", "tddp4_project", "tddp4_jit_source", "tddp4_math_probe", "tddp4_set_gram_mode", "tddp4_profile_in_kernel"]
 
 
 class Tddp4Error(RuntimeError):
@@ -101,6 +101,7 @@ def load_library():
     L.tddp4_jit_source.restype = i64
     L.tddp4_math_probe.argtypes = [vp, C.c_int, i64, vp, vp, vp]
     L.tddp4_set_gram_mode.argtypes = [vp, C.c_int, C.POINTER(i64)]
+    L.tddp4_profile_in_kernel.argtypes = [vp, dp, C.POINTER(i64)]
     L.tddp4_project.argtypes = [vp, i64, i64, vp, C.c_int, vp, vp, vp]
     _lib = L
     return L
@@ -446,6 +447,12 @@ class Tddp4:
             self._check(self.lib.tddp4_profile_read(self._h, k, C.byref(ms), C.byref(n), C.byref(by)))
             out[name] = (ms.value, n.value, by.value)
         return out
+
+    def profile_in_kernel(self):
+        """tddp4_profile_in_kernel: (sum of in-kernel durations of the coupling-only NLL kernel in us, launches)."""
+        us, n = C.c_double(), C.c_int64()
+        self._check(self.lib.tddp4_profile_in_kernel(self._h, C.byref(us), C.byref(n)))
+        return us.value, n.value
 
     def launch_count(self):
         return int(self.lib.tddp4_launch_count(self._h))

@@ -183,10 +183,19 @@ __device__ __forceinline__ double resolved_prob(double2 A, double2 Ab, const dou
 //   [0] sum log B, [1] sum t, [2] N, [3] NLL = Gamma sum t - sum log B + n log N, [4] #bad events,
 //   [5] seq: the caller's sequence stamp, written LAST behind a system-wide fence -- when the slot lives in mapped host
 //   memory the host polls this word instead of waiting on a CUDA event (see wait_slot() in tddp4_api.cu)
+// %globaltimer: nanoseconds on one clock for the whole GPU (in-kernel timing of tddp4_profile, below)
+__device__ __forceinline__ unsigned long long global_ns() {
+  unsigned long long t;
+  asm volatile("mov.u64 %0, %%globaltimer;" : "=l"(t));
+  return t;
+}
+// stamps (profiling only, else NULL): [0] earliest block start of this launch (atomicMin by the kernel's blocks), [1] sum
+// over launches of (result written - earliest start) in ns, [2] launches counted.
 template <bool RES = false>
 __device__ __forceinline__ void nll_finish(const RateParams &R, int KC, long long n, double sum_t, MantAcc la,
                                            const double *__restrict__ G, double inv_n, double *__restrict__ partials,
-                                           unsigned int *ticket, double *__restrict__ result, double seq) {
+                                           unsigned int *ticket, double *__restrict__ result, double seq,
+                                           unsigned long long *stamps = nullptr) {
   __shared__ double s_p[STREAM_WARPS];
   __shared__ long long s_e[STREAM_WARPS];
   __shared__ int s_b[STREAM_WARPS];
@@ -259,6 +268,12 @@ __device__ __forceinline__ void nll_finish(const RateParams &R, int KC, long lon
     if (seq != 0.0) {                       // 0: nobody polls this slot (batched / device-side results)
       __threadfence_system();
       *reinterpret_cast<volatile double *>(result + 5) = seq;
+    }
+    if (stamps) {
+      const unsigned long long t1 = global_ns(), t0 = *reinterpret_cast<volatile unsigned long long *>(stamps);
+      atomicAdd(stamps + 1, t1 - t0);
+      atomicAdd(stamps + 2, 1ull);
+      *reinterpret_cast<volatile unsigned long long *>(stamps) = ~0ull;
     }
   }
 }

@@ -30,7 +30,9 @@ template <int KC, bool SMALL>
 __global__ void __launch_bounds__(STREAM_BLOCK, STREAM_BLOCKS_PER_SM)
 nll_stream_kernel(const double2 *__restrict__ a, const double *__restrict__ t, int64_t ld, int64_t n,
                   const __grid_constant__ RateParams R, const double *__restrict__ G, double inv_n_norm, double sum_t,
-                  double *__restrict__ partials, unsigned int *ticket, double *__restrict__ result, int early_wait, double seq) {
+                  double *__restrict__ partials, unsigned int *ticket, double *__restrict__ result, int early_wait, double seq,
+                  unsigned long long *stamps /* in-kernel timing while profiling, else NULL */) {
+  if (stamps && threadIdx.x == 0) atomicMin(stamps, global_ns());
   if (early_wait) pdl_wait();            // the predecessor wrote the columns
   pdl_launch_dependents();               // only after this kernel's own early wait: see the ordering note at pdl_wait()
   MantAcc la;
@@ -48,7 +50,7 @@ nll_stream_kernel(const double2 *__restrict__ a, const double *__restrict__ t, i
     la.add(bracket<SMALL>(A, Ab, yG * ti, xG * ti));
   }
   if (!early_wait) pdl_wait();
-  nll_finish(R, KC, n, sum_t, la, G, inv_n_norm, partials, ticket, result, seq);
+  nll_finish(R, KC, n, sum_t, la, G, inv_n_norm, partials, ticket, result, seq, stamps);
 }
 
 // P_i = e^{-Gamma t_i} B_i / N for parity and plots (tddp4_nll with prob_out): same per-event arithmetic as the

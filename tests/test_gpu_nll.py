@@ -424,6 +424,30 @@ def test_sharded_wrapper_on_one_rank(B):
     assert abs(sh.nll() - direct2) <= 1e-13 * abs(direct2)
 
 
+def test_in_kernel_timing_of_the_coupling_only_kernel(B):
+    """tddp4_profile_in_kernel: counted once per coupling-only launch while profiling, positive, below the CUDA-event
+    duration of the same launches, and off (no count) when profiling is off; the NLL bits do not depend on it."""
+    mdl = samples.model_of(("C", 2))
+    par = W.initial_params(mdl)
+    p4, t, _ = samples.data_sample(("C", 2), 4_133)
+    p4n, _ = samples.flat_sample(10_001)
+    h = B.Tddp4(mdl)
+    h.load_events(0, p4, t); h.load_events(1, p4n)
+    h.set_params(par)
+    ref = h.nll()
+    plain = [h.nll() for _ in range(3)]
+    assert h.profile_in_kernel() == (0.0, 0)
+    h.profile(True); h.profile_reset()
+    timed = [h.nll() for _ in range(5)]
+    us, n = h.profile_in_kernel()
+    ev_ms, ev_n, _ = h.profile_read()["nll"]
+    h.profile(False)
+    assert plain == [ref] * 3 and timed == [ref] * 5
+    assert n == 5 and ev_n == 5 and 0.0 < us < 1e3 * ev_ms
+    h.profile_reset()
+    assert h.profile_in_kernel() == (0.0, 0)
+
+
 def test_incremental_gram_has_the_bits_of_a_full_pass(B):
     """with tddp4_set_gram_mode(1) the normalisation columns are kept and a move of few columns
     rebuilds only those; along a trajectory of single-resonance, all-parameter and coupling-only moves G and the NLL must
