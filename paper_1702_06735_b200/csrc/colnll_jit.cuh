@@ -37,16 +37,16 @@ colnll_jit(const __grid_constant__ LineParams LP, const double *__restrict__ cac
       prefetch_l2_bulk(tile_event(cache, J_R, i + PF_DIST * stride) + J_SKIP, (unsigned)(J_R * 32 - J_SKIP) * 8u);
     const double ti = RES ? 0.0 : ldg_stream1(t + i);            // RES: t points at the time rows [8][ld]
     const double *ev = tile_event(cache, J_R, i);
-    double sv[J_NSU + 1], gv[J_NINST + 1], fv[J_NTERMS];        // + 1: a model without resonances has no instance
+    double sv[J_NSU + 1], gv[J_NG + 1], fv[J_NF];               // + 1: a model without resonances has no instance
 #pragma unroll
     for (int r = 0; r < J_NSU; ++r) sv[r] = ldg_stream1(ev + J_SKIP + r * 32);
 #pragma unroll
-    for (int j = 0; j < J_NINST; ++j) gv[j] = ldg_stream1(ev + J_GOFF + j * 32);
+    for (int r = 0; r < J_NG; ++r) gv[r] = ldg_stream1(ev + J_GOFF + r * 32);
 #pragma unroll
-    for (int k = 0; k < J_NTERMS; ++k) fv[k] = ldg_stream1(ev + J_FOFF + k * 32);
+    for (int r = 0; r < J_NF; ++r) fv[r] = ldg_stream1(ev + J_FOFF + r * 32);
     double2 T[J_NINST + 1];
 #pragma unroll
-    for (int j = 0; j < J_NINST; ++j) T[j] = breit_wigner(LP.m0sq[j], LP.gam[j], sv[J_SROW[j]], gv[j]);
+    for (int j = 0; j < J_NINST; ++j) T[j] = breit_wigner(LP.m0sq[j], LP.gam[j], sv[J_SROW[j]], gv[J_GROW[j]]);
     double2 A = make_double2(0.0, 0.0), Ab = make_double2(0.0, 0.0);
     double2 col = make_double2(0.0, 0.0);
 #pragma unroll
@@ -56,8 +56,8 @@ colnll_jit(const __grid_constant__ LineParams LP, const double *__restrict__ cac
       else if (J_T0[k] >= 0) P = T[J_T0[k] >= 0 ? J_T0[k] : 0];
       else if (J_T1[k] >= 0) P = T[J_T1[k] >= 0 ? J_T1[k] : 0];
       else P = make_double2(1.0, 0.0);
-      col.x = fma(fv[k], P.x, col.x);
-      col.y = fma(fv[k], P.y, col.y);
+      col.x = fma(fv[J_FROW[k]], P.x, col.x);
+      col.y = fma(fv[J_FROW[k]], P.y, col.y);
       if (J_LAST[k]) {
         // a column none of whose lineshapes moved is recomputed to the bits already stored: skip its 16-byte store
         if ((store_mask >> J_COL[k]) & 1u) a[(long long)J_COL[k] * ld + i] = col;

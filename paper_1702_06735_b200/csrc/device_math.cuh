@@ -94,7 +94,7 @@ struct Scratch {
 };
 
 // step 1 for one event whose momenta sit in scratch: invariant masses, shape functions, static factors.
-// sink.s(i, v), sink.g(i, v), sink.f(k, v) receive the results (global rows or registers).
+// sink.s(i, v), sink.g(row, v), sink.f(row, v) receive the results (rows of the cache: InstTab::grow, TermTab::frow).
 template <class Sink>
 __device__ __forceinline__ void kinematics(const ModelTab &M, const Scratch &sc, int tid, Sink &sink) {
   for (int i = 0; i < M.n_sys; ++i) {
@@ -113,7 +113,7 @@ __device__ __forceinline__ void kinematics(const ModelTab &M, const Scratch &sc,
     double ma = in.sub >= 0 ? sqrt(sc.S(in.sub, tid)) : in.ma;
     double q2 = breakup2(Mr, s, ma, in.mb);
     sc.Q(i, tid) = q2;
-    sink.g(i, in.kind == LS_CONSTANT ? 1.0 : width_shape(in.L, q2, q2 * in.r2, Mr));
+    sink.g(in.grow, in.kind == LS_CONSTANT ? 1.0 : width_shape(in.L, q2, q2 * in.r2, Mr));   // shared rows: same value again
   }
   double sD = sc.S(M.sysD, tid);
   double mD = sqrt(sD);
@@ -133,7 +133,7 @@ __device__ __forceinline__ void kinematics(const ModelTab &M, const Scratch &sc,
       f *= barrier(i0.L, sc.Q(tm.inst0, tid) * i0.r2);
       f *= barrier(i1.L, sc.Q(tm.inst1, tid) * i1.r2);
     }
-    sink.f(k, f);
+    sink.f(tm.frow, f);
   }
 }
 

@@ -8,7 +8,8 @@
 //
 // This file is NOT compiled by nvcc.  The library compiles it at run time with NVRTC (jit.h), once per model, behind a
 // generated prelude that states the model as compile-time constants:
-//   J_NB, J_KC, J_NINST, J_NTERMS, J_NSU, J_R, J_SKIP, J_GOFF, J_FOFF, J_WOFF (element offsets in a tile, -1: unweighted),
+//   J_NB, J_KC, J_NINST, J_NTERMS, J_NSU, J_NG, J_NF (s, g, f rows streamed), J_R, J_SKIP, J_GOFF, J_FOFF, J_WOFF (element
+//   offsets in a tile, -1: unweighted), J_GROW[J_NINST], J_FROW[J_NTERMS]  the (shared) g row of instance j / f row of term k,
 //   J_SROW[J_NINST]  index (0 .. J_NSU-1) of the s row instance j reads, rows counted from J_SKIP,
 //   J_T0[J_NTERMS], J_T1[J_NTERMS]  lineshape instances of term k (-1: none),  J_COL[J_NTERMS]  its coupling column,
 //   J_LAST[J_NTERMS]  1: term k closes its column (terms are sorted by column).
@@ -59,7 +60,7 @@ gram_jit(const __grid_constant__ LineParams LP, const double *__restrict__ cache
     if (GMODE != 2 && PF_DIST > 0 && lane == 0 && i0 + PF_DIST * stride < n)     // (an incremental pass reads part of a tile only)
       prefetch_l2_bulk(tile_event(cache, J_R, i0 + PF_DIST * stride) + J_SKIP, (unsigned)(J_R * 32 - J_SKIP) * 8u);
     const double *ev = tile_event(cache, J_R, i0 + lane);
-    double sv[J_NSU + 1], gv[J_NINST + 1], fv[J_NTERMS];   // + 1: a model without resonances has no instance
+    double sv[J_NSU + 1], gv[J_NG + 1], fv[J_NF];          // + 1: a model without resonances has no instance
     double2 kept[J_KC];                                    // GMODE 2: the clean columns, read back
     if (GMODE == 2) {                                      // only the rows the masked columns need (warp-uniform guards)
 #pragma unroll
@@ -67,23 +68,23 @@ gram_jit(const __grid_constant__ LineParams LP, const double *__restrict__ cache
 #pragma unroll
       for (int r = 0; r < J_NSU; ++r) sv[r] = (mask & J_SROWCOLS[r]) ? ldg_stream1(ev + J_SKIP + r * 32) : 0.0;
 #pragma unroll
-      for (int j = 0; j < J_NINST; ++j) gv[j] = (mask & J_INSTCOLS[j]) ? ldg_stream1(ev + J_GOFF + j * 32) : 0.0;
+      for (int r = 0; r < J_NG; ++r) gv[r] = (mask & J_GROWCOLS[r]) ? ldg_stream1(ev + J_GOFF + r * 32) : 0.0;
 #pragma unroll
-      for (int k = 0; k < J_NTERMS; ++k) fv[k] = (mask >> J_COL[k]) & 1u ? ldg_stream1(ev + J_FOFF + k * 32) : 0.0;
+      for (int r = 0; r < J_NF; ++r) fv[r] = (mask & J_FROWCOLS[r]) ? ldg_stream1(ev + J_FOFF + r * 32) : 0.0;
     } else {
 #pragma unroll
       for (int r = 0; r < J_NSU; ++r) sv[r] = ldg_stream1(ev + J_SKIP + r * 32);
 #pragma unroll
-      for (int j = 0; j < J_NINST; ++j) gv[j] = ldg_stream1(ev + J_GOFF + j * 32);
+      for (int r = 0; r < J_NG; ++r) gv[r] = ldg_stream1(ev + J_GOFF + r * 32);
 #pragma unroll
-      for (int k = 0; k < J_NTERMS; ++k) fv[k] = ldg_stream1(ev + J_FOFF + k * 32);
+      for (int r = 0; r < J_NF; ++r) fv[r] = ldg_stream1(ev + J_FOFF + r * 32);
     }
     double wj = 1.0;
     if (WEIGHTED) wj = ldg_stream1(ev + J_WOFF);
     double2 T[J_NINST + 1];
 #pragma unroll
     for (int j = 0; j < J_NINST; ++j)
-      if (GMODE != 2 || (mask & J_INSTCOLS[j])) T[j] = breit_wigner(LP.m0sq[j], LP.gam[j], sv[J_SROW[j]], gv[j]);
+      if (GMODE != 2 || (mask & J_INSTCOLS[j])) T[j] = breit_wigner(LP.m0sq[j], LP.gam[j], sv[J_SROW[j]], gv[J_GROW[j]]);
       else T[j] = make_double2(0.0, 0.0);
     double2 a = make_double2(0.0, 0.0);
 #pragma unroll
@@ -93,8 +94,8 @@ gram_jit(const __grid_constant__ LineParams LP, const double *__restrict__ cache
       else if (J_T0[k] >= 0) P = T[J_T0[k] >= 0 ? J_T0[k] : 0];
       else if (J_T1[k] >= 0) P = T[J_T1[k] >= 0 ? J_T1[k] : 0];
       else P = make_double2(1.0, 0.0);
-      a.x = fma(fv[k], P.x, a.x);
-      a.y = fma(fv[k], P.y, a.y);
+      a.x = fma(fv[J_FROW[k]], P.x, a.x);
+      a.y = fma(fv[J_FROW[k]], P.y, a.y);
       if (J_LAST[k]) {
         if (GMODE == 2 && !((mask >> J_COL[k]) & 1u)) a = kept[J_COL[k]];
         if (GMODE != 0 && ((mask >> J_COL[k]) & 1u)) an[J_COL[k] * ld + i0 + lane] = a;

@@ -166,10 +166,10 @@ terms_kernel(const __grid_constant__ ModelTab M, const __grid_constant__ LinePar
   if (i >= n) return;
   for (int j = 0; j < M.n_inst; ++j)
     sT[j * COL_BLOCK + tid] = breit_wigner(LP.m0sq[j], LP.gam[j], cache[tile_index(cr.R, M.inst[j].sys, i)],
-                                           cache[tile_index(cr.R, cr.g_row0 + j, i)]);
+                                           cache[tile_index(cr.R, cr.g_row0 + M.inst[j].grow, i)]);
   for (int k = 0; k < M.n_terms; ++k) {
     const TermTab &tm = M.term[k];
-    double fv = cache[tile_index(cr.R, cr.f_row0 + k, i)];
+    double fv = cache[tile_index(cr.R, cr.f_row0 + M.term[k].frow, i)];
     double2 T = make_double2(1.0, 0.0);
     if (tm.inst0 >= 0) T = cmul(sT[tm.inst0 * COL_BLOCK + tid], sT[tm.inst1 * COL_BLOCK + tid]);
     out[(int64_t)M.user_term[k] * n + i] = make_double2(fv * T.x, fv * T.y);

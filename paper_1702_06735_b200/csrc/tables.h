@@ -29,7 +29,8 @@ struct InstTab {     // one lineshape instance = (resonance, system it sits on, 
   int8_t L;          // L of the resonance's decay vertex
   int8_t dres;       // daughter resonance (its current m0 enters q0), -1 none
   int8_t kind;       // LS_*: a constant-width instance has the shape g = 1 and gam = m0 Gamma0
-  int8_t pad[2];
+  int8_t grow;       // row of its shape g among the g rows of the cache: instances that differ only in the resonance share one
+  int8_t pad[1];
   double ma, mb;     // fixed daughter masses (ma unused when sub >= 0)
   double r2;         // Blatt-Weisskopf radius squared of this resonance's own vertex, GeV^-2
 };
@@ -40,10 +41,12 @@ struct TermTab {     // one decay chain (one Bose ordering)
   int8_t inst0;      // VV: R1; cascade: X.  -1 none
   int8_t inst1;      // VV: R2; cascade: V.  -1 none
   int8_t perm[4];    // role -> particle
+  int8_t frow;       // row of its static factor f among the f rows of the cache (shared by chains that differ only in the resonances)
 };
 
 struct ModelTab {
   int n_sys, n_inst, n_terms, n_kc;
+  int n_g, n_f;                    // distinct shape rows (<= n_inst) and static-factor rows (<= n_terms) of the cache
   int sysD;                        // index of the four-body system
   uint8_t sys_mask[MAX_SYS];
   int n_su;                        // systems whose s some lineshape instance reads (they are numbered last)
@@ -58,7 +61,7 @@ struct ModelTab {
 
 // The static cache of one event set is ONE tile-major array: tile = 32 consecutive events, R rows of 32 doubles each
 // (256 B per row per tile), rows ordered
-//   [ s: n_sys | g: n_inst | f: n_terms | w (if weighted) ],
+//   [ s: n_sys | g: n_g | f: n_f | w (if weighted) ]   (n_g, n_f: distinct rows, ModelTab),
 // element (row r, event i) at ((i >> 5) * R + r) * 32 + (i & 31).  A warp working on one tile therefore addresses every
 // row as tile base + lane + CONSTANT, and the whole tile is one contiguous R * 256-byte region of HBM.  The fused
 // per-call kernels get these offsets (and the model tables) as compile-time constants (jit_prelude in tddp4_api.cu).
