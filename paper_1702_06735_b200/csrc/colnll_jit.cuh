@@ -33,11 +33,11 @@ colnll_jit(const __grid_constant__ LineParams LP, const double *__restrict__ cac
   long long i = (long long)blockIdx.x * STREAM_BLOCK + threadIdx.x;
 #pragma unroll 1
   for (; i < n; i += stride) {
-    if (PF_DIST > 0 && lane == 0 && i + PF_DIST * stride < n)
+    if (PF_DIST > 0 && J_R * 32 - J_SKIP > 0 && lane == 0 && i + PF_DIST * stride < n)
       prefetch_l2_bulk(tile_event(cache, J_R, i + PF_DIST * stride) + J_SKIP, (unsigned)(J_R * 32 - J_SKIP) * 8u);
     const double ti = RES ? 0.0 : ldg_stream1(t + i);            // RES: t points at the time rows [8][ld]
     const double *ev = tile_event(cache, J_R, i);
-    double sv[J_NSU + 1], gv[J_NG + 1], fv[J_NF];               // + 1: a model without resonances has no instance
+    double sv[J_NSU + 1], gv[J_NG + 1], fv[J_NF + 1];               // + 1: a model without resonances has no instance
 #pragma unroll
     for (int r = 0; r < J_NSU; ++r) sv[r] = ldg_stream1(ev + J_SKIP + r * 32);
 #pragma unroll
@@ -56,8 +56,9 @@ colnll_jit(const __grid_constant__ LineParams LP, const double *__restrict__ cac
       else if (J_T0[k] >= 0) P = T[J_T0[k] >= 0 ? J_T0[k] : 0];
       else if (J_T1[k] >= 0) P = T[J_T1[k] >= 0 ? J_T1[k] : 0];
       else P = make_double2(1.0, 0.0);
-      col.x = fma(fv[J_FROW[k]], P.x, col.x);
-      col.y = fma(fv[J_FROW[k]], P.y, col.y);
+      const double fk = J_FROW[k] >= 0 ? fv[J_FROW[k] >= 0 ? J_FROW[k] : 0] : 1.0;    // non-resonant term: no row, f = 1
+      col.x = fma(fk, P.x, col.x);
+      col.y = fma(fk, P.y, col.y);
       if (J_LAST[k]) {
         // a column none of whose lineshapes moved is recomputed to the bits already stored: skip its 16-byte store
         if ((store_mask >> J_COL[k]) & 1u) a[(long long)J_COL[k] * ld + i] = col;

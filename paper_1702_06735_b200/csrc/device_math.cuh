@@ -133,7 +133,7 @@ __device__ __forceinline__ void kinematics(const ModelTab &M, const Scratch &sc,
       f *= barrier(i0.L, sc.Q(tm.inst0, tid) * i0.r2);
       f *= barrier(i1.L, sc.Q(tm.inst1, tid) * i1.r2);
     }
-    sink.f(tm.frow, f);
+    if (tm.frow >= 0) sink.f(tm.frow, f);    // a constant-amplitude term keeps no row (f = 1)
   }
 }
 

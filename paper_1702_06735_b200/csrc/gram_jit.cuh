@@ -57,10 +57,10 @@ gram_jit(const __grid_constant__ LineParams LP, const double *__restrict__ cache
   long long i0 = (long long)blockIdx.x * JG_BLOCK + warp * 32;
 #pragma unroll 1
   for (; i0 < n; i0 += stride) {
-    if (GMODE != 2 && PF_DIST > 0 && lane == 0 && i0 + PF_DIST * stride < n)     // (an incremental pass reads part of a tile only)
+    if (GMODE != 2 && PF_DIST > 0 && J_R * 32 - J_SKIP > 0 && lane == 0 && i0 + PF_DIST * stride < n)     // (an incremental pass reads part of a tile only)
       prefetch_l2_bulk(tile_event(cache, J_R, i0 + PF_DIST * stride) + J_SKIP, (unsigned)(J_R * 32 - J_SKIP) * 8u);
     const double *ev = tile_event(cache, J_R, i0 + lane);
-    double sv[J_NSU + 1], gv[J_NG + 1], fv[J_NF];          // + 1: a model without resonances has no instance
+    double sv[J_NSU + 1], gv[J_NG + 1], fv[J_NF + 1];          // + 1: a model without resonances has no instance
     double2 kept[J_KC];                                    // GMODE 2: the clean columns, read back
     if (GMODE == 2) {                                      // only the rows the masked columns need (warp-uniform guards)
 #pragma unroll
@@ -87,6 +87,7 @@ gram_jit(const __grid_constant__ LineParams LP, const double *__restrict__ cache
       if (GMODE != 2 || (mask & J_INSTCOLS[j])) T[j] = breit_wigner(LP.m0sq[j], LP.gam[j], sv[J_SROW[j]], gv[J_GROW[j]]);
       else T[j] = make_double2(0.0, 0.0);
     double2 a = make_double2(0.0, 0.0);
+    const double one = i0 + lane < n ? 1.0 : 0.0;          // lanes beyond n: rows are zero-filled, the constant f must be too
 #pragma unroll
     for (int k = 0; k < J_NTERMS; ++k) {
       double2 P;
@@ -94,8 +95,9 @@ gram_jit(const __grid_constant__ LineParams LP, const double *__restrict__ cache
       else if (J_T0[k] >= 0) P = T[J_T0[k] >= 0 ? J_T0[k] : 0];
       else if (J_T1[k] >= 0) P = T[J_T1[k] >= 0 ? J_T1[k] : 0];
       else P = make_double2(1.0, 0.0);
-      a.x = fma(fv[J_FROW[k]], P.x, a.x);
-      a.y = fma(fv[J_FROW[k]], P.y, a.y);
+      const double fk = J_FROW[k] >= 0 ? fv[J_FROW[k] >= 0 ? J_FROW[k] : 0] : one;    // non-resonant term: no row, f = 1
+      a.x = fma(fk, P.x, a.x);
+      a.y = fma(fk, P.y, a.y);
       if (J_LAST[k]) {
         if (GMODE == 2 && !((mask >> J_COL[k]) & 1u)) a = kept[J_COL[k]];
         if (GMODE != 0 && ((mask >> J_COL[k]) & 1u)) an[J_COL[k] * ld + i0 + lane] = a;

@@ -49,6 +49,10 @@ kin_kernel(const __grid_constant__ ModelTab M, const double *__restrict__ p4, in
   KinSink sink{cache, cr, i};
   kinematics(M, sc, tid, sink);
 }
+__global__ void __launch_bounds__(256) fill_kernel(double *__restrict__ dst, int64_t n, double v) {
+  int64_t i = (int64_t)blockIdx.x * 256 + threadIdx.x;
+  if (i < n) dst[i] = v;
+}
 // one row of the tile-major cache <-> a plain vector (weights in at load; inspection rows out)
 __global__ void __launch_bounds__(256) row_scatter_kernel(double *__restrict__ cache, int R, int row, int64_t n,
                                                          const double *__restrict__ src) {
@@ -169,7 +173,7 @@ terms_kernel(const __grid_constant__ ModelTab M, const __grid_constant__ LinePar
                                            cache[tile_index(cr.R, cr.g_row0 + M.inst[j].grow, i)]);
   for (int k = 0; k < M.n_terms; ++k) {
     const TermTab &tm = M.term[k];
-    double fv = cache[tile_index(cr.R, cr.f_row0 + M.term[k].frow, i)];
+    double fv = tm.frow >= 0 ? cache[tile_index(cr.R, cr.f_row0 + tm.frow, i)] : 1.0;
     double2 T = make_double2(1.0, 0.0);
     if (tm.inst0 >= 0) T = cmul(sT[tm.inst0 * COL_BLOCK + tid], sT[tm.inst1 * COL_BLOCK + tid]);
     out[(int64_t)M.user_term[k] * n + i] = make_double2(fv * T.x, fv * T.y);

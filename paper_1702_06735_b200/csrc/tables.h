@@ -41,7 +41,8 @@ struct TermTab {     // one decay chain (one Bose ordering)
   int8_t inst0;      // VV: R1; cascade: X.  -1 none
   int8_t inst1;      // VV: R2; cascade: V.  -1 none
   int8_t perm[4];    // role -> particle
-  int8_t frow;       // row of its static factor f among the f rows of the cache (shared by chains that differ only in the resonances)
+  int8_t frow;       // row of its static factor f among the f rows of the cache (shared by chains that differ only in the
+                     // resonances); -1: non-resonant term, f = 1, no row
 };
 
 struct ModelTab {

@@ -59,7 +59,9 @@ def test_gram_pass_compiles_for_sm100a(name, tmp_path):
         else:
             assert int(m.group(2)) <= 128, usage
         assert "DMMA" in sass                                                    # fp64 tensor cores
-        assert ("UBLKPF" in sass) == (gmode != 2)                                # bulk L2 prefetch of the next tile
+        # bulk L2 prefetch of the next tile (a constant-amplitude model streams no row at all: nothing to prefetch)
+        if name != "flat":
+            assert ("UBLKPF" in sass) == (gmode != 2)
 
 
 @pytest.mark.parametrize("name", ["C1", "C2", "C3", "C5", "flat"])
