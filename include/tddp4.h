@@ -225,6 +225,22 @@ int tddp4_candidates(tddp4 *h, uint64_t seed, uint32_t stream_id, int64_t first,
  * values_dev: device [5][n] or NULL, the per-event observables.  n_bins <= 512.  Synchronous.           */
 int tddp4_project(tddp4 *h, int64_t n, int64_t ld, const double *p4, int n_bins, const double *ranges, int64_t *hist_out,
                   double *values_dev);
+/* tddp4_project for callers that may not allocate (code under CUDA-graph capture, serving loops, harnesses that forbid
+ * cudaMalloc): the same kernel, the same observables and bin rule, but the histogram the kernel accumulates into is a
+ * file-scope device array of the library, unsigned 64-bit [5][TDDP4_PROJECT_STATIC_MAX_BINS] = 20 KiB, which every GPU
+ * that loads the library holds until the process exits.  The call allocates and frees nothing (no cudaMalloc, cudaFree
+ * or allocating library routine) and does not synchronise: it enqueues, on the handle's stream, a clear of the array, the
+ * kernel, and a device-to-device copy of the counts into hist_dev; the first call on a device also looks the array's
+ * device address up (cudaGetSymbolAddress, once per device), so make one call before a capture begins.
+ *   p4, n, ld, n_bins, ranges, values_dev: as tddp4_project.  hist_dev: DEVICE [5][n_bins] int64, the caller's; every
+ *   element is written (it need not be cleared), valid once the stream has reached the end of the enqueued work.
+ * n_bins > TDDP4_PROJECT_STATIC_MAX_BINS is rejected with TDDP4_ERR_ARG (text in tddp4_last_error); so is a call while
+ * another device than the handle's is current.  ALL calls of a process on one GPU share the one array, whatever the
+ * handle: each call clears it first (it keeps the previous call's counts), and two calls whose work overlaps on the GPU
+ * (different streams, no dependency between them) race on it -- order them on one stream or with events.          */
+#define TDDP4_PROJECT_STATIC_MAX_BINS 512
+int tddp4_project_static(tddp4 *h, int64_t n, int64_t ld, const double *p4, int n_bins, const double *ranges,
+                         int64_t *hist_dev, double *values_dev);
 
 /* ---- inspection (per-layer parity, profiling) ---------------------------------------------------- */
 enum {

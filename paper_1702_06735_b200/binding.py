@@ -18,6 +18,7 @@ LIB_PATH = os.path.join(_HERE, "csrc", "libtddp4.so")
 OK, ERR_ARG, ERR_CUDA, ERR_CAPACITY, ERR_DOMAIN, ERR_NONFINITE, ERR_STATE = 0, -1, -2, -3, -4, -5, -6
 GET_S, GET_SHAPE, GET_STATIC, GET_COLUMNS, GET_TERMS = range(5)
 K_KIN, K_COLUMNS, K_GRAM, K_NLL, K_GEN_RATIO, K_GEN_EMIT, K_COLNLL, K_TRES, K_GRAD = range(9)
+PROJECT_STATIC_MAX_BINS = 512   # TDDP4_PROJECT_STATIC_MAX_BINS: size of the static scratch of tddp4_project_static
 KERNEL_NAMES = ["kin", "columns", "gram", "nll", "gen_ratio", "gen_emit", "columns_nll", "time_rows", "nll_grad"]
 
 # every symbol include/tddp4.h declares
@@ -26,7 +27,8 @@ SYMBOLS = ["tddp4_create", "tddp4_destroy", "tddp4_set_stream", "tddp4_last_erro
            "tddp4_nll_parts", "tddp4_nll_grad", "tddp4_param_stride", "tddp4_nll_batch", "tddp4_gram", "tddp4_gram_override", "tddp4_norm", "tddp4_generate", "tddp4_weight_bound",
            "tddp4_candidates", "tddp4_get", "tddp4_layout", "tddp4_profile", "tddp4_profile_read",
            "tddp4_profile_reset", "tddp4_launch_count", "tddp4_gram_enqueue", "tddp4_gram_reduce", "tddp4_nll_enqueue",
-           "tddp4_gram_state", "tddp4_fp64_peak", "tddp4_project", "tddp4_jit_source", "tddp4_math_probe", "tddp4_set_gram_mode", "tddp4_profile_in_kernel"]
+           "tddp4_gram_state", "tddp4_fp64_peak", "tddp4_project", "tddp4_jit_source", "tddp4_math_probe", "tddp4_set_gram_mode", "tddp4_profile_in_kernel",
+           "tddp4_project_static"]
 
 
 class Tddp4Error(RuntimeError):
@@ -103,6 +105,7 @@ def load_library():
     L.tddp4_set_gram_mode.argtypes = [vp, C.c_int, C.POINTER(i64)]
     L.tddp4_profile_in_kernel.argtypes = [vp, dp, C.POINTER(i64)]
     L.tddp4_project.argtypes = [vp, i64, i64, vp, C.c_int, vp, vp, vp]
+    L.tddp4_project_static.argtypes = [vp, i64, i64, vp, C.c_int, vp, vp, vp]
     _lib = L
     return L
 
@@ -413,6 +416,18 @@ class Tddp4:
         values = self.empty(5, max(1, n)) if want_values else None
         self._check(self.lib.tddp4_project(self._h, n, ld, _ptr(p4), n_bins, rng.ctypes.data, hist.ctypes.data, _ptr(values)))
         return hist, (values[:, :n] if want_values else None)
+
+    def project_static(self, p4, n_bins, ranges, hist_out, values_out=None):
+        """tddp4_project_static: the projection with the library's static device scratch, no allocation inside the call.
+        p4: CUDA tensor [16][n]; hist_out: the caller's CUDA int64 tensor [5][n_bins]; values_out: the caller's CUDA fp64
+        tensor [5][n] or None.  Enqueues on the handle's stream and returns; hist_out is valid once that stream (set_stream) or the device has been synchronised."""
+        assert p4.is_cuda and p4.dim() == 2 and p4.shape[0] == 16 and p4.stride(1) == 1
+        n, ld = p4.shape[1], (p4.stride(0) if p4.shape[1] > 1 else max(1, p4.shape[1]))
+        assert hist_out.is_cuda and hist_out.dtype == self._torch.int64 and hist_out.is_contiguous() and hist_out.numel() >= 5 * max(0, n_bins)
+        assert values_out is None or (values_out.is_cuda and values_out.is_contiguous() and tuple(values_out.shape) == (5, n))
+        self._torch.cuda.current_stream(self.device).synchronize()
+        rng = np.ascontiguousarray(ranges, dtype=np.float64)
+        self._check(self.lib.tddp4_project_static(self._h, n, ld, _ptr(p4), n_bins, rng.ctypes.data, _ptr(hist_out), _ptr(values_out)))
 
     # -- inspection -------------------------------------------------------------------------------
     def layout(self):
