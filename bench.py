@@ -334,6 +334,33 @@ def run_ours(args):
                             "in_kernel_note": "%globaltimer from the earliest block start to the result written, same launches as "
                                               "us_per_launch: the CUDA-event figure also contains the launch gap of an isolated launch"})
 
+    # ---- the dominant kernel on its own, and the step as a whole.  Inside the mixture the CUDA events around a Gram launch
+    #      also see the write-back of the column lines the preceding data pass left dirty in L2 (its 16 B per stale column are
+    #      stored into L2 and reach DRAM while the NEXT kernel streams: DESIGN.md 7); `alone` times the same kernel in a loop
+    #      of tddp4_set_params (one mass moved) + tddp4_gram, where no such lines exist, and `whole_step` divides the
+    #      algorithmic bytes of ALL launches of the timed region by its duration (no per-kernel events) ---------------------
+    try:
+        h.profile(True)
+        for k in range(30):
+            if k == 5:
+                h.profile_reset()
+            q = p0.copy()
+            q.mass[0] *= 1.0 + 1e-6 * (k + 1)
+            h.set_params(q)
+            h.gram()
+        gms, gn, gby = h.profile_read()["gram"]
+        h.profile(False)
+        h.set_params(p0)
+        a_gbs = gby / (gms * 1e-3) / 1e9
+        roof["alone"] = {"us_per_launch": round(1e3 * gms / gn, 3), "launches": gn, "achieved": round(a_gbs, 1),
+                         "frac": round(a_gbs / hbm, 4)}
+        step_bytes = sum(v[2] for v in prof.values()) / args.steps
+        s_gbs = step_bytes / (ms / args.steps * 1e-3) / 1e9
+        roof["whole_step"] = {"alg_MB_per_step": round(step_bytes / 1e6, 1), "achieved": round(s_gbs, 1), "frac": round(s_gbs / hbm, 4),
+                              "note": "algorithmic bytes of every launch of the timed region / its duration / peak"}
+    except Exception as e:
+        roof["alone"] = {"error": repr(e)}
+
     # ---- analytic gradient: one pass against the 2 (4 K_c + 2) NLL calls of a numerical gradient ----
     grad = {}
     try:
