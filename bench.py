@@ -334,6 +334,29 @@ def run_ours(args):
                             "in_kernel_note": "%globaltimer from the earliest block start to the result written, same launches as "
                                               "us_per_launch: the CUDA-event figure also contains the launch gap of an isolated launch"})
 
+    # ---- what a pair of CUDA events costs around a kernel that does nothing (a one-element torch add on the same stream):
+    #      the floor under every per-launch figure of `kernels`, and under any "isolated call" figure on this machine ----
+    try:
+        tiny = torch.zeros(32, device=device)
+        floor = {}
+        with torch.cuda.stream(stream):
+            for key, sync_each in (("back_to_back", False), ("after_host_sync", True)):
+                pairs = []
+                for k in range(120):
+                    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                    a.record(stream); tiny.add_(1.0); b.record(stream)
+                    if sync_each:
+                        stream.synchronize()
+                    if k >= 20:
+                        pairs.append((a, b))
+                stream.synchronize()
+                floor[key] = round(1e3 * sum(a.elapsed_time(b) for a, b in pairs) / len(pairs), 2)
+        floor["note"] = ("us between two CUDA events around a one-element kernel: launch + completion latency that every "
+                         "event-bracketed launch above contains; tddp4_profile_in_kernel (kernels.nll.in_kernel_*) excludes it")
+        roof["event_floor_us"] = floor
+    except Exception as e:
+        roof["event_floor_us"] = {"error": repr(e)}
+
     # ---- the dominant kernel on its own, and the step as a whole.  Inside the mixture the CUDA events around a Gram launch
     #      also see the write-back of the column lines the preceding data pass left dirty in L2 (its 16 B per stale column are
     #      stored into L2 and reach DRAM while the NEXT kernel streams: DESIGN.md 7); `alone` times the same kernel in a loop
