@@ -394,9 +394,12 @@ def run_ours(args):
         for _ in range(20):
             h.nll_grad()
         gms, gn, gby = h.profile_read()["nll_grad"]
+        gin_us, gin_n = h.profile_in_kernel_of(binding.K_GRAD)   # earliest block start -> gradient written, same launches
         h.profile(False)
         grad = {"us_per_call": round(1e3 * gms / gn, 3), "alg_MB_per_call": gby / gn / 1e6,
                 "frac": round(gby / (gms * 1e-3) / 1e9 / peaks()[0], 4), "n_derivatives": 4 * KC + 2,
+                "in_kernel_us_per_call": round(gin_us / gin_n, 2) if gin_n else None,
+                "in_kernel_frac": round(gby / gn / (gin_us / gin_n * 1e-6) / 1e9 / peaks()[0], 4) if gin_n else None,
                 "numerical_gradient_us": round(2 * (4 * KC + 2) * 1e3 * sub["coupling_only"]["ms_per_step"], 1)}
     except Exception as e:
         grad = {"error": repr(e)}

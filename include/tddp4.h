@@ -280,6 +280,9 @@ int tddp4_profile_reset(tddp4 *h);
  * kernel itself takes, without the launch gap a pair of CUDA events around an isolated launch also measures.  Host out:
  * the sum over launches since the last tddp4_profile_reset in microseconds and their number; synchronises.      */
 int tddp4_profile_in_kernel(tddp4 *h, double *total_us, int64_t *launches);
+/* The same for kernel_id = TDDP4_K_NLL (identical to the call above) or TDDP4_K_GRAD (the gradient kernel of tddp4_nll_grad
+ * without resolution: earliest block start to the gradient written); any other id is TDDP4_ERR_ARG.                      */
+int tddp4_profile_in_kernel_of(tddp4 *h, int kernel_id, double *total_us, int64_t *launches);
 /* Number of kernels this handle has launched since creation (all kinds).                            */
 int64_t tddp4_launch_count(const tddp4 *h);
 /* Measured fp64 issue rate of this GPU: a dependent-free chain of DFMA instructions on every SM (the

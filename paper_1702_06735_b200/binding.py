@@ -28,7 +28,7 @@ SYMBOLS = ["tddp4_create", "tddp4_destroy", "tddp4_set_stream", "tddp4_last_erro
            "tddp4_candidates", "tddp4_get", "tddp4_layout", "tddp4_profile", "tddp4_profile_read",
            "tddp4_profile_reset", "tddp4_launch_count", "tddp4_gram_enqueue", "tddp4_gram_reduce", "tddp4_nll_enqueue",
            "tddp4_gram_state", "tddp4_fp64_peak", "tddp4_project", "tddp4_jit_source", "tddp4_math_probe", "tddp4_set_gram_mode", "tddp4_profile_in_kernel",
-           "tddp4_project_static"]
+           "tddp4_project_static", "tddp4_profile_in_kernel_of"]
 
 
 class Tddp4Error(RuntimeError):
@@ -104,6 +104,7 @@ def load_library():
     L.tddp4_math_probe.argtypes = [vp, C.c_int, i64, vp, vp, vp]
     L.tddp4_set_gram_mode.argtypes = [vp, C.c_int, C.POINTER(i64)]
     L.tddp4_profile_in_kernel.argtypes = [vp, dp, C.POINTER(i64)]
+    L.tddp4_profile_in_kernel_of.argtypes = [vp, C.c_int, dp, C.POINTER(i64)]
     L.tddp4_project.argtypes = [vp, i64, i64, vp, C.c_int, vp, vp, vp]
     L.tddp4_project_static.argtypes = [vp, i64, i64, vp, C.c_int, vp, vp, vp]
     _lib = L
@@ -467,6 +468,12 @@ class Tddp4:
         """tddp4_profile_in_kernel: (sum of in-kernel durations of the coupling-only NLL kernel in us, launches)."""
         us, n = C.c_double(), C.c_int64()
         self._check(self.lib.tddp4_profile_in_kernel(self._h, C.byref(us), C.byref(n)))
+        return us.value, n.value
+
+    def profile_in_kernel_of(self, kernel_id):
+        """tddp4_profile_in_kernel_of: the same for K_NLL or K_GRAD (the gradient kernel without resolution)."""
+        us, n = C.c_double(), C.c_int64()
+        self._check(self.lib.tddp4_profile_in_kernel_of(self._h, int(kernel_id), C.byref(us), C.byref(n)))
         return us.value, n.value
 
     def launch_count(self):

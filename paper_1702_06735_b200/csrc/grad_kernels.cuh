@@ -182,8 +182,9 @@ __global__ void __launch_bounds__(STREAM_BLOCK, grad_bps<KC>())
 nll_grad_kernel(const double2 *__restrict__ a, const double *__restrict__ t, int64_t ld, int64_t n,
                 const __grid_constant__ RateParams R, const __grid_constant__ GradParams GP, const double *__restrict__ G,
                 double inv_n_norm, double sum_t, double *__restrict__ partials /* [grid][NB * 32 + 5] */, unsigned int *ticket,
-                double *__restrict__ result) {
+                double *__restrict__ result, unsigned long long *stamps /* in-kernel timing while profiling (nll_finish), else NULL */) {
   constexpr int NB = grad_nb<KC>(), XS = gram_stride(NB), NS = 2, NA = NB * 32 + NS;
+  if (stamps && threadIdx.x == 0) atomicMin(stamps, global_ns());
   extern __shared__ __align__(16) char smem_raw[];
   __shared__ double s_red[STREAM_WARPS * NA];
   __shared__ double s_sum[NA];
@@ -299,6 +300,12 @@ nll_grad_kernel(const double2 *__restrict__ a, const double *__restrict__ t, int
     if (bad > 0 || !(norm > 0.0)) nll = INFINITY;
     result[0] = s0; result[1] = sum_t; result[2] = norm; result[3] = nll; result[4] = (double)bad;
     *ticket = 0;
+    if (stamps) {
+      const unsigned long long t1 = global_ns(), t0 = *reinterpret_cast<volatile unsigned long long *>(stamps);
+      atomicAdd(stamps + 1, t1 - t0);
+      atomicAdd(stamps + 2, 1ull);
+      *reinterpret_cast<volatile unsigned long long *>(stamps) = ~0ull;
+    }
   }
 }
 

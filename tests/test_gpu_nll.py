@@ -448,6 +448,35 @@ def test_in_kernel_timing_of_the_coupling_only_kernel(B):
     assert h.profile_in_kernel() == (0.0, 0)
 
 
+def test_in_kernel_timing_of_the_gradient_kernel(B):
+    """tddp4_profile_in_kernel_of(TDDP4_K_GRAD): one count per tddp4_nll_grad launch while profiling, positive, below the
+    CUDA-event duration of the same launches; the coupling-only counter is a separate one; NLL and gradient bits do not
+    depend on the stamps; other kernel ids are rejected."""
+    mdl = samples.model_of(("C", 2))
+    par = W.initial_params(mdl)
+    p4, t, _ = samples.data_sample(("C", 2), 4_133)
+    p4n, _ = samples.flat_sample(10_001)
+    h = B.Tddp4(mdl)
+    h.load_events(0, p4, t); h.load_events(1, p4n)
+    h.set_params(par)
+    ref_nll, ref_grad = h.nll_grad()
+    assert h.profile_in_kernel_of(B.K_GRAD) == (0.0, 0)
+    h.profile(True); h.profile_reset()
+    timed = [h.nll_grad() for _ in range(4)]
+    h.nll()
+    us, n = h.profile_in_kernel_of(B.K_GRAD)
+    us_nll, n_nll = h.profile_in_kernel_of(B.K_NLL)
+    ev_ms, ev_n, _ = h.profile_read()["nll_grad"]
+    h.profile(False)
+    assert all(v == ref_nll and np.array_equal(g, ref_grad) for v, g in timed)
+    assert n == 4 and ev_n == 4 and 0.0 < us < 1e3 * ev_ms
+    assert n_nll == 1 and us_nll > 0.0 and (us_nll, n_nll) == h.profile_in_kernel()
+    with pytest.raises(B.Tddp4Error):
+        h.profile_in_kernel_of(B.K_GRAM)
+    h.profile_reset()
+    assert h.profile_in_kernel_of(B.K_GRAD) == (0.0, 0)
+
+
 def test_incremental_gram_has_the_bits_of_a_full_pass(B):
     """with tddp4_set_gram_mode(1) the normalisation columns are kept and a move of few columns
     rebuilds only those; along a trajectory of single-resonance, all-parameter and coupling-only moves G and the NLL must
