@@ -906,6 +906,68 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def writeback_study(args):
+    """DESIGN.md 7, "Where the Gram pass's time in the mixture goes": the Gram kernel's CUDA-event duration (tddp4_profile)
+    after different predecessors on the stream.  Prints one JSON line; not part of the bench contract."""
+    import torch
+    from paper_1702_06735_b200 import binding
+    device = "cuda:0"
+    torch.cuda.set_device(device)
+    binding.load_library()
+    cfg = W.config(3)
+    p4, t, p4n, _ = build_workload(binding, cfg, device, W.BASE_SEED)
+    p0 = W.initial_params(cfg.model)
+    h = binding.Tddp4(cfg.model, device)
+    h.load_events(0, p4, t)
+    h.load_events(1, p4n)
+    del p4, p4n
+    torch.cuda.empty_cache()
+    other = torch.zeros(128 * 1024 * 1024, dtype=torch.float64, device=device)      # 1 GiB of memory the kernels never touch
+    h.set_params(p0)
+    h.nll()
+
+    def moved(k):                       # one mass moved: Gram matrix and data columns stale
+        q = p0.copy(); q.mass[0] *= 1.0 + 1e-6 * (k + 1); return q
+
+    def coupling(k, j):                 # the same masses, one coupling moved: a coupling-only call
+        q = moved(k); q.c[0] *= 1.0 + 1e-6 * (j + 1); return q
+
+    def gram_only(k):
+        h.set_params(moved(k)); h.gram()
+
+    def dirty_step(k):
+        h.set_params(moved(k)); h.nll()
+
+    def dirty_then_coupling_only(k):
+        dirty_step(k)
+        for j in range(3):
+            h.set_params(coupling(k, j)); h.nll()
+
+    def dirty_then_read_elsewhere(k):
+        dirty_step(k); other.sum().item()
+
+    def dirty_then_write_elsewhere(k):
+        dirty_step(k); other.zero_(); torch.cuda.synchronize()
+
+    rows = []
+    for name, body in (("GRAM -> GRAM (tddp4_gram after one mass moved)", gram_only),
+                       ("GRAM -> COLNLL -> GRAM (dirty steps)", dirty_step),
+                       ("GRAM -> COLNLL -> 3 x NLL -> GRAM", dirty_then_coupling_only),
+                       ("GRAM -> COLNLL -> 1 GiB read of other memory -> GRAM", dirty_then_read_elsewhere),
+                       ("GRAM -> COLNLL -> 1 GiB write of other memory -> GRAM", dirty_then_write_elsewhere)):
+        for k in range(5):
+            body(k)
+        h.profile(True); h.profile_reset()
+        for k in range(args.steps):
+            body(k + 5)
+        pr = h.profile_read()
+        h.profile(False)
+        rows.append({"sequence": name, **{n: round(1e3 * v[0] / v[1], 2) for n, v in pr.items() if v[1]}})
+    h.close()
+    print(json.dumps({"writeback_study": rows, "unit": "us per launch between CUDA events", "repetitions": args.steps,
+                      "gram_alg_MB": cfg.n_norm * 232 / 1e6}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -918,9 +980,14 @@ def main():
                          "launched under torch.distributed.run --nproc-per-node 1")
     ap.add_argument("--validation-events", type=int, default=100_000,
                     help="events per sample of the Fig. 3 comparison (the paper: 500 000; the oracle generates ~0.9 %% of its candidates)")
+    ap.add_argument("--writeback-study", action="store_true",
+                    help="instead of the bench: the Gram kernel's duration after different predecessors (DESIGN.md 7); --steps = repetitions")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3 if args.impl == "ours" else 0)
-    if args.impl == "reference":
+    if args.writeback_study:
+        args.steps = min(args.steps, 200)
+        writeback_study(args)
+    elif args.impl == "reference":
         run_reference(args)
     elif args.gpus > 1 and "WORLD_SIZE" not in os.environ:
         relaunch_under_torchrun(args)
