@@ -37,13 +37,23 @@ colnll_jit(const __grid_constant__ LineParams LP, const double *__restrict__ cac
       prefetch_l2_bulk(tile_event(cache, J_R, i + PF_DIST * stride) + J_SKIP, (unsigned)(J_R * 32 - J_SKIP) * 8u);
     const double ti = RES ? 0.0 : ldg_stream1(t + i);            // RES: t points at the time rows [8][ld]
     const double *ev = tile_event(cache, J_R, i);
-    double sv[J_NSU + 1], gv[J_NG + 1], fv[J_NF + 1];               // + 1: a model without resonances has no instance
+    double sv[J_NSU + 2], gv[J_NG + 1], fv[J_NF + 1];               // + 1: a model without resonances has no instance
 #pragma unroll
     for (int r = 0; r < J_NSU; ++r) sv[r] = ldg_stream1(ev + J_SKIP + r * 32);
 #pragma unroll
     for (int r = 0; r < J_NG; ++r) gv[r] = ldg_stream1(ev + J_GOFF + r * 32);
 #pragma unroll
     for (int r = 0; r < J_NF; ++r) fv[r] = ldg_stream1(ev + J_FOFF + r * 32);
+#if J_NSD
+    {                                                      // the s that is not streamed: a fixed combination of streamed rows
+      double d = J_SDCONST;
+#pragma unroll
+      for (int r = 0; r < J_NSU; ++r)
+        if (J_SDCOEF[r] > 0) d += sv[r];
+        else if (J_SDCOEF[r] < 0) d -= sv[r];
+      sv[J_NSU] = d;
+    }
+#endif
     double2 T[J_NINST + 1];
 #pragma unroll
     for (int j = 0; j < J_NINST; ++j) T[j] = breit_wigner(LP.m0sq[j], LP.gam[j], sv[J_SROW[j]], gv[J_GROW[j]]);

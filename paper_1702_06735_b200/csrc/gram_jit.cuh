@@ -60,7 +60,7 @@ gram_jit(const __grid_constant__ LineParams LP, const double *__restrict__ cache
     if (GMODE != 2 && PF_DIST > 0 && J_R * 32 - J_SKIP > 0 && lane == 0 && i0 + PF_DIST * stride < n)     // (an incremental pass reads part of a tile only)
       prefetch_l2_bulk(tile_event(cache, J_R, i0 + PF_DIST * stride) + J_SKIP, (unsigned)(J_R * 32 - J_SKIP) * 8u);
     const double *ev = tile_event(cache, J_R, i0 + lane);
-    double sv[J_NSU + 1], gv[J_NG + 1], fv[J_NF + 1];          // + 1: a model without resonances has no instance
+    double sv[J_NSU + 2], gv[J_NG + 1], fv[J_NF + 1];          // + 1: a model without resonances has no instance
     double2 kept[J_KC];                                    // GMODE 2: the clean columns, read back
     if (GMODE == 2) {                                      // only the rows the masked columns need (warp-uniform guards)
 #pragma unroll
@@ -79,6 +79,16 @@ gram_jit(const __grid_constant__ LineParams LP, const double *__restrict__ cache
 #pragma unroll
       for (int r = 0; r < J_NF; ++r) fv[r] = ldg_stream1(ev + J_FOFF + r * 32);
     }
+#if J_NSD
+    {                                                      // the s that is not streamed: a fixed combination of streamed rows
+      double d = J_SDCONST;
+#pragma unroll
+      for (int r = 0; r < J_NSU; ++r)
+        if (J_SDCOEF[r] > 0) d += sv[r];
+        else if (J_SDCOEF[r] < 0) d -= sv[r];
+      sv[J_NSU] = d;
+    }
+#endif
     double wj = 1.0;
     if (WEIGHTED) wj = ldg_stream1(ev + J_WOFF);
     double2 T[J_NINST + 1];

@@ -51,6 +51,13 @@ struct ModelTab {
   int sysD;                        // index of the four-body system
   uint8_t sys_mask[MAX_SYS];
   int n_su;                        // systems whose s some lineshape instance reads (they are numbered last)
+  // One three-body system whose s is a combination of streamed s rows is not streamed itself (n_sd = 1; it is numbered just
+  // before the streamed ones, so its stored row sits in the part of the tile the per-call kernels skip):
+  //   s_{pqy} = s_{pqx} - s_{px} - s_{qx} + s_{py} + s_{qy} + m_x^2 - m_y^2      (the pair pq and its masses cancel), or
+  //   s_{abc} = s_{ab} + s_{ac} + s_{bc} - m_a^2 - m_b^2 - m_c^2
+  int n_sd;                        // 0 or 1
+  int8_t sd_coef[MAX_SYS];         // coefficient (-1, 0, +1) of streamed row r (0 .. n_su-1) in the derived s
+  double sd_const;                 // the mass terms
   int8_t col_begin[MAX_KC + 1];    // terms (sorted by coupling) of column kappa: [col_begin[k], col_begin[k+1])
   int8_t user_term[MAX_TERMS];     // sorted position -> caller's term index
   InstTab inst[MAX_INST];
