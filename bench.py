@@ -963,9 +963,10 @@ def writeback_study(args):
         pr = h.profile_read()
         h.profile(False)
         rows.append({"sequence": name, **{n: round(1e3 * v[0] / v[1], 2) for n, v in pr.items() if v[1]}})
+        gram_mb = pr["gram"][2] / pr["gram"][1] / 1e6
     h.close()
     print(json.dumps({"writeback_study": rows, "unit": "us per launch between CUDA events", "repetitions": args.steps,
-                      "gram_alg_MB": cfg.n_norm * 232 / 1e6}))
+                      "gram_alg_MB": gram_mb}))
 
 
 def main():

@@ -103,3 +103,46 @@ def test_prelude_states_the_model_tables():
         bad = copy.deepcopy(W.config(1).model)
         bad.term_coupling = [0] * bad.n_terms
         binding.jit_source(bad, 0)
+
+
+def _table(src, name):
+    m = re.search(r"constexpr (?:int|double) " + name + r"\[\] = \{([^}]*)\}", src)
+    return [float.fromhex(x) if "x" in x else float(x) for x in m.group(1).replace(" ", "").rstrip(",").split(",")][:-1]
+
+
+def _define(src, name):
+    return int(re.search(r"#define " + name + r" (-?\d+)", src).group(1))
+
+
+@pytest.mark.parametrize("cfg", [1, 2, 3, 5])
+def test_derived_invariant_mass_row(cfg):
+    """A three-body s the other streamed s rows determine is derived in the fused kernels.  The tables the
+    library writes for it (J_NSD, J_SDCOEF, J_SDCONST; J_SROW = J_NSU for its instances) are checked on momenta drawn here:
+    sum_r coef_r s_r + const must be the invariant mass squared of the derived system, which is the system numbered just
+    before the streamed ones; the small models have nothing to derive."""
+    import numpy as np
+    mdl = W.config(cfg).model
+    src = binding.jit_source(mdl, 4)                       # the generator's prelude also lists the particle systems
+    n_su, n_sd, n_sys = _define(src, "J_NSU"), _define(src, "J_NSD"), _define(src, "J_NSYS")
+    masks = [int(m) for m in _table(src, "J_SYSMASK")]
+    coef, srow = _table(src, "J_SDCOEF"), _table(src, "J_SROW")
+    const = float.fromhex(re.search(r"J_SDCONST = ([^;]+);", src).group(1))
+    assert len(masks) == n_sys and len(coef) == n_su
+    if cfg in (1, 2):
+        assert n_sd == 0 and not any(coef) and max(srow, default=0) < n_su
+        return
+    assert n_sd == 1 and max(srow) == n_su and _define(src, "J_SKIP") == 32 * (n_sys - n_su)
+    rng = np.random.default_rng(5)
+    m = np.array([W.M_K, W.M_PI, W.M_PI, W.M_PI])
+    p3 = rng.normal(0.0, 0.4, (4, 3, 1000))                 # any momenta on their mass shells: the relation is an identity
+    p4 = np.concatenate([np.sqrt(m[:, None, None] ** 2 + (p3 ** 2).sum(axis=1, keepdims=True)), p3], axis=1)
+
+    def s_of(mask):
+        P = sum(p4[a] for a in range(4) if mask >> a & 1)
+        return P[0] ** 2 - (P[1:] ** 2).sum(axis=0)
+
+    streamed = masks[n_sys - n_su:]
+    derived = masks[n_sys - n_su - 1]
+    assert bin(derived).count("1") == 3
+    got = const + sum(c * s_of(mk) for c, mk in zip(coef, streamed))
+    assert np.max(np.abs(got - s_of(derived))) < 1e-12
